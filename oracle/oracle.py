@@ -1,0 +1,152 @@
+"""ctypes front end of the CPU oracle (TEST INFRASTRUCTURE ONLY).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import this.
+The product package never does. Array conventions as in include/rex_trex.h: momenta SoA [npar][4][n].
+"""
+import ctypes
+import math
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(_build.build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int)
+        L.oracle_npar.argtypes = [ctypes.c_int]
+        L.oracle_me2.argtypes = [ctypes.c_int, dp, ctypes.c_long, dp, dp, ctypes.c_int]
+        L.oracle_abd.argtypes = [ctypes.c_int, ctypes.c_int, dp, ctypes.c_long, dp, ctypes.c_int, ctypes.c_int, dp, ctypes.c_int]
+        L.oracle_reweight.argtypes = [ctypes.c_int, dp, ctypes.c_long, dp, dp, dp, dp, dp, dp, ctypes.c_int]
+        L.oracle_ttng_amps.argtypes = [ctypes.c_int, dp, dp, ctypes.c_int, ctypes.c_int, dp]
+        L.oracle_colour_matrix.argtypes = [ctypes.c_int, dp]
+        L.oracle_colour_entry.argtypes = [ctypes.c_int, ip, ip]
+        L.oracle_colour_entry.restype = ctypes.c_double
+        L.oracle_wavefunction.argtypes = [ctypes.c_int, dp, ctypes.c_int, ctypes.c_int, dp]
+        L.oracle_gamma.argtypes = [ctypes.c_int, dp]
+        _lib = L
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _mom(sid, momenta):
+    npar = lib().oracle_npar(sid)
+    m = np.ascontiguousarray(momenta, dtype=np.float64)
+    assert m.ndim == 3 and m.shape[0] == npar and m.shape[1] == 4, (m.shape, npar)
+    return m, m.shape[2]
+
+
+def me2(sid, momenta, theta, long_double=False):
+    """Helicity/colour-summed, averaged |M|^2 per event at parameters theta."""
+    m, n = _mom(sid, momenta)
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    out = np.empty(n)
+    rc = lib().oracle_me2(sid, _dp(m), n, _dp(th), _dp(out), int(long_double))
+    assert rc == 0, rc
+    return out
+
+
+def abd(sid, momenta, theta, engine=1, gauge_gluon=-1, hel_only=-1, long_double=False):
+    """(A,B,D) with me2 = A + kappa B + kappa^2 D; engine 1 = colour-ordered E1, 2 = explicit-colour E2."""
+    m, n = _mom(sid, momenta)
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    out = np.empty((n, 3))
+    rc = lib().oracle_abd(sid, engine, _dp(m), n, _dp(th), gauge_gluon, hel_only, _dp(out), int(long_double))
+    assert rc == 0, rc
+    return out
+
+
+def kappa(theta):
+    return theta[7] * theta[9] / (math.sqrt(2.0) * theta[8] ** 2)
+
+
+def reweight(sid, momenta, theta_old, theta_new, w_in, long_double=False):
+    """Returns (w_out, me2_old, me2_new): eq.(5) PAPER.md:714 with the zero guard of PAPER.md:789-799."""
+    m, n = _mom(sid, momenta)
+    to = np.ascontiguousarray(theta_old, dtype=np.float64)
+    tn = np.ascontiguousarray(theta_new, dtype=np.float64)
+    w = np.ascontiguousarray(w_in, dtype=np.float64)
+    w_out, mo, mn = np.empty(n), np.empty(n), np.empty(n)
+    rc = lib().oracle_reweight(sid, _dp(m), n, _dp(to), _dp(tn), _dp(w), _dp(w_out), _dp(mo), _dp(mn), int(long_double))
+    assert rc == 0, rc
+    return w_out, mo, mn
+
+
+def ttng_amps(sid, momenta_one, theta, hel, gauge_gluon=-1):
+    """Colour-flow amplitudes A_sigma (order 0 and order 1 in kappa) of one event and one helicity index.
+    Returns complex array [n!, 2]; orderings lexicographic."""
+    m, n = _mom(sid, momenta_one)
+    assert n == 1
+    npar = m.shape[0]
+    nperm = math.factorial(npar - 2)
+    out = np.empty((nperm, 4))
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    rc = lib().oracle_ttng_amps(sid, _dp(m), _dp(th), hel, gauge_gluon, _dp(out))
+    assert rc == 0, rc
+    return out[:, 0::2] + 1j * out[:, 1::2]
+
+
+def colour_matrix(n):
+    k = math.factorial(n)
+    out = np.empty((k, k))
+    assert lib().oracle_colour_matrix(n, _dp(out)) == 0
+    return out
+
+
+def colour_entry(sigma, sigma_p):
+    n = len(sigma)
+    a = (ctypes.c_int * n)(*sigma)
+    b = (ctypes.c_int * n)(*sigma_p)
+    return lib().oracle_colour_entry(n, a, b)
+
+
+def wavefunction(kind, p, lam, massless=False):
+    """kind: 'u','v','ubar','vbar','eps' -> complex[4]. massless=True: E := |p| (R-2)."""
+    k = {"u": 0, "v": 1, "ubar": 2, "vbar": 3, "eps": 4}[kind]
+    pp = np.ascontiguousarray(p, dtype=np.float64)
+    out = np.empty(8)
+    assert lib().oracle_wavefunction(k, _dp(pp), lam, int(massless), _dp(out)) == 0
+    return out[0::2] + 1j * out[1::2]
+
+
+def gamma(mu):
+    out = np.empty(32)
+    assert lib().oracle_gamma(mu, _dp(out)) == 0
+    return (out[0::2] + 1j * out[1::2]).reshape(4, 4)
+
+
+# ---------------------------------------------------------------- bucketing oracle (R-10)
+def bucket(keys):
+    """Stable categorisation: buckets ordered by first appearance of their key, REX_NPOS forced last.
+    Returns (perm int32[n], offsets int64[nb+1], bucket_keys uint64[nb])."""
+    keys = np.asarray(keys, dtype=np.uint64)
+    npos = np.uint64(0xFFFFFFFFFFFFFFFF)
+    order = []
+    seen = {}
+    for k in keys.tolist():
+        if k not in seen and k != int(npos):
+            seen[k] = len(order)
+            order.append(k)
+    has_npos = bool(np.any(keys == npos))
+    if has_npos:
+        seen[int(npos)] = len(order)
+        order.append(int(npos))
+    bid = np.array([seen[k] for k in keys.tolist()], dtype=np.int64)
+    perm = np.argsort(bid, kind="stable").astype(np.int32)
+    counts = np.bincount(bid, minlength=len(order)) if len(order) else np.zeros(0, dtype=np.int64)
+    offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    return perm, offsets, np.array(order, dtype=np.uint64)
+
+
+def gather(src, perm):
+    """dst[r, j] = src[r, perm[j]] (the SoA 'transpose' of PAPER.md:100, 691)."""
+    src = np.asarray(src)
+    return np.ascontiguousarray(src.reshape(-1, src.shape[-1])[:, perm]).reshape(src.shape[:-1] + (len(perm),))

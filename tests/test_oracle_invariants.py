@@ -1,0 +1,107 @@
+"""Invariance pins of the oracle: Ward identity, Lorentz invariance,
+exact quadratic c_tG dependence, unit ratio at theta_new = theta_old, zero guard."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from trex_inputs import default_theta, make_config, TH_CTG, TH_GAMMAT
+
+from helpers import random_lorentz, apply_lorentz, relclose
+
+# (sid, config to take momenta from, events)
+TTNG = [(1, 2, 4), (2, 3, 3), (3, 4, 2), (4, 5, 1)]
+QCH = [(5, 3, 2), (7, 3, 2), (8, 3, 2)]
+
+
+@pytest.mark.parametrize("sid,cfg,nev", TTNG)
+def test_ward_identity_colour_ordered(sid, cfg, nev):
+    """eps_k -> K_k kills every order in kappa (Gamma_t = 0; with a fixed width it is violated, R-9)."""
+    w = make_config(cfg, n=8)
+    th = default_theta()
+    mom = w.momenta[:, :, :nev]
+    full = O.abd(sid, mom, th)
+    ngl = mom.shape[0] - 2
+    for g in ([0, ngl - 1] if sid == 4 else range(ngl)):
+        z = O.abd(sid, mom, th, gauge_gluon=g)
+        assert np.all(np.abs(z) < 1e-20 * np.abs(full)), (g, z / full)
+    # fixed-width scheme: violated (not a bug), so the probe really is sensitive
+    th_w = th.copy()
+    th_w[TH_GAMMAT] = 1.5
+    z = O.abd(sid, mom, th_w, gauge_gluon=0)
+    assert np.all(np.abs(z[:, 0]) > 1e-16 * np.abs(full[:, 0]))
+
+
+@pytest.mark.parametrize("sid,cfg,nev", QCH)
+def test_ward_identity_quark_channels_explicit_colour(sid, cfg, nev):
+    w = make_config(cfg, n=8)
+    th = default_theta()
+    mom = w.momenta[:, :, :nev]
+    full = O.abd(sid, mom, th, engine=2)
+    z = O.abd(sid, mom, th, engine=2, gauge_gluon=0)
+    assert np.all(np.abs(z) < 1e-20 * np.abs(full))
+
+
+@pytest.mark.parametrize("sid,cfg,nev", [(0, 1, 8)] + TTNG[:3] + QCH)
+def test_lorentz_invariance(sid, cfg, nev):
+    rng = np.random.default_rng(5)
+    w = make_config(cfg, n=8)
+    mom = w.momenta[:, :, :nev]
+    th = w.theta_new.copy()
+    # a fixed top width breaks the Ward identity (R-9) and with it the frame independence of the polarisation
+    # sum at the 1e-6 level; the invariance is a property of the Gamma_t = 0 amplitude
+    th[TH_GAMMAT] = 0.0
+    ref = O.me2(sid, mom, th)
+    for _ in range(2):
+        L = random_lorentz(rng)
+        got = O.me2(sid, apply_lorentz(L, mom), th)
+        assert relclose(got, ref, rtol=5e-12), got / ref - 1
+
+
+@pytest.mark.parametrize("sid,cfg,nev", TTNG[:3] + QCH[:1])
+def test_me2_is_exactly_quadratic_in_ctg(sid, cfg, nev):
+    """At most one dim-6 insertion per amplitude (R-4): a cubic through 4 points has no cubic term, and the
+    public me2 entry agrees with A + kappa B + kappa^2 D."""
+    w = make_config(cfg, n=8)
+    mom = w.momenta[:, :, :nev]
+    cs = np.array([0.0, 0.7, 1.9, -2.6, 4.0])
+    vals = []
+    for c in cs:
+        th = default_theta()
+        th[TH_CTG] = c
+        vals.append(O.me2(sid, mom, th))
+    vals = np.array(vals)                       # [5, nev]
+    for e in range(nev):
+        coef = np.polyfit(cs, vals[:, e], 4)    # exact interpolation through 5 points
+        assert abs(coef[0]) < 1e-11 * abs(vals[0, e]) and abs(coef[1]) < 1e-11 * abs(vals[0, e])
+    th = default_theta()
+    abd = O.abd(sid, mom, th, engine=1 if sid <= 4 else 2)
+    th[TH_CTG] = 1.9
+    k = O.kappa(th)
+    assert relclose(vals[2], abd[:, 0] + k * abd[:, 1] + k * k * abd[:, 2], rtol=1e-13)
+    assert np.all(abd[:, 0] > 0) and np.all(abd[:, 2] > 0)
+    assert np.all(abd[:, 1] ** 2 <= 4 * abd[:, 0] * abd[:, 2] * (1 + 1e-12))   # |M|^2 >= 0 for every kappa
+
+
+def test_reweight_definition_unit_ratio_and_zero_guard():
+    w = make_config(2, n=64)
+    w_out, mo, mn = O.reweight(1, w.momenta, w.theta_old, w.theta_new, w.w_in)
+    assert relclose(w_out, w.w_in * O.me2(1, w.momenta, w.theta_new) / O.me2(1, w.momenta, w.theta_old), rtol=1e-15)
+    same, _, _ = O.reweight(1, w.momenta, w.theta_old, w.theta_old, w.w_in)
+    assert np.allclose(same, w.w_in, rtol=4e-16, atol=0)
+    # zero guard: alpha_s = 0 makes me2_old exactly 0 -> weight 0, not NaN/Inf
+    th0 = w.theta_old.copy()
+    th0[0] = 0.0
+    z, mo0, _ = O.reweight(1, w.momenta[:, :, :4], th0, w.theta_new, w.w_in[:4])
+    assert np.all(mo0 == 0) and np.all(z == 0)
+
+
+def test_top_width_enters_continuously_and_double_matches_long_double():
+    w = make_config(4, n=4)
+    th = w.theta_old.copy()
+    a = O.me2(3, w.momenta, th)
+    b = O.me2(3, w.momenta, th, long_double=True)
+    assert np.allclose(a, b, rtol=1e-12, atol=0)
+    th0 = th.copy(); th0[TH_GAMMAT] = 0.0
+    th1 = th.copy(); th1[TH_GAMMAT] = 1e-6
+    assert np.allclose(O.me2(3, w.momenta, th0), O.me2(3, w.momenta, th1), rtol=1e-6, atol=0)
+    assert not np.allclose(a, O.me2(3, w.momenta, th0), rtol=1e-9, atol=0)     # Gamma_t = 1.5 really changes the value
