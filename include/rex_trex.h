@@ -1,0 +1,121 @@
+/* rex_trex.h -- C ABI of the B200-native reweighting hot path (paper arxiv 2510.05100: Rex / teaRex / MadtRex).
+ *
+ * What the library computes (citations are PAPER.md line numbers):
+ *   - rex_bucket : the stable categorisation of events into per-subprocess blocks that lhe::transpose() performs
+ *                  before any reweighting (PAPER.md:354 ordering rule, :362 npos rule, :675-694 sort + transpose,
+ *                  eq.(1) :691).
+ *   - rex_gather / rex_scatter : the "transposition" into and out of the per-subprocess SoA blocks
+ *                  (PAPER.md:100-104 process object, :877 "transpose weights from processes to events").
+ *   - trex_reweight : eq.(5),  w' = w |M(p;theta_new)|^2 / |M(p;theta_old)|^2 , with the normalisation
+ *                  and zero guard of procReweightor::initialise / evaluate; |M|^2 is the LO,
+ *                  helicity- and colour-summed, initial-state averaged matrix element, the only
+ *                  input being the momenta.
+ *
+ * Conventions
+ *   - Every array pointer is a DEVICE pointer unless the comment says HOST. The caller owns every buffer; the library
+ *     only allocates internal scratch that it caches in a process-global context (freed by trex_shutdown).
+ *   - All device work is enqueued on the stream given to trex_set_stream (default: the legacy default stream).
+ *     trex_reweight, rex_gather and rex_scatter are asynchronous; rex_bucket synchronises that stream before it
+ *     returns because it hands bucket sizes back to the host.
+ *   - Return value: >= 0 success, < 0 error code below. No C++ exception crosses this boundary; the text of the last
+ *     error is available from trex_last_error().
+ *   - Not thread-safe: one caller thread per process (one process per GPU).
+ */
+#ifndef REX_TREX_H
+#define REX_TREX_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TREX_OK                0
+#define TREX_EINVAL           -1   /* null pointer, negative size, bad mode, inconsistent theta */
+#define TREX_EUNKNOWN_SUBPROC -2   /* no kernel compiled in for this key / id */
+#define TREX_ECUDA            -3   /* a CUDA runtime call or a kernel launch failed */
+#define TREX_ENOMEM           -4   /* scratch allocation failed */
+
+#define REX_MAX_BUCKETS 256                     /* the paper's largest sample has 65 classes */
+#define REX_NPOS 0xFFFFFFFFFFFFFFFFull          /* "no class": always the last bucket */
+
+/* theta[]: flat parameter vector replacing the SLHA `BLOCK ID VALUE` cards of PAPER.md:996-1002 */
+#define TREX_NTHETA 16
+enum { TREX_TH_ALPHA_S = 0, TREX_TH_ALPHA_EM = 1, TREX_TH_SIN2W = 2, TREX_TH_MZ = 3, TREX_TH_GAMMAZ = 4,
+       TREX_TH_MT = 5, TREX_TH_GAMMAT = 6, TREX_TH_CTG = 7, TREX_TH_LAMBDA = 8, TREX_TH_VEV = 9 };
+
+/* compiled-in subprocesses (particle order inside a block = order of the process string) */
+enum { TREX_SP_EEMUMU = 0,   /* e- e+ > mu- mu+   (photon + Z)          */
+       TREX_SP_GG_TT = 1,    /* g g > t t~                              */
+       TREX_SP_GG_TTG = 2,   /* g g > t t~ g                            */
+       TREX_SP_GG_TTGG = 3,  /* g g > t t~ g g                          */
+       TREX_SP_GG_TTGGG = 4, /* g g > t t~ g g g                        */
+       TREX_SP_UUX_TTG = 5,  /* u u~ > t t~ g                           */
+       TREX_SP_DDX_TTG = 6,  /* d d~ > t t~ g                           */
+       TREX_SP_UG_TTU = 7,   /* u g > t t~ u                            */
+       TREX_SP_GUX_TTUX = 8, /* g u~ > t t~ u~                          */
+       TREX_NSUBPROC = 9 };
+
+/* ---- flavour keys (PAPER.md:334 default comparator: unordered PDG codes of external legs, initial and final state
+ * kept apart; Alg.1).
+ * HOST helper. pdg[nlegs], status[nlegs] (-1 incoming, +1 outgoing; other statuses are ignored). Legs of each group
+ * sorted ascending by PDG code; byte i = (|pdg| & 0x7F) | (pdg < 0 ? 0x80 : 0); byte 7 = (n_in << 4) | n_out.
+ * At most 7 external legs; returns REX_NPOS if there are more or if |pdg| > 127. */
+uint64_t rex_pack_key(const int32_t* pdg, const int8_t* status, int nlegs);
+
+/* ---- rex_bucket: stable categorisation.
+ * pdg_keys [n] device, in : packed flavour signatures.
+ * perm     [n] device, out: perm[j] = original index of the j-th event in bucketed order. Buckets appear in order of
+ *                           FIRST APPEARANCE of their key in the input; key REX_NPOS is forced last; inside a bucket
+ *                           the input order is kept (stable). The result is unique, hence bit-exact.
+ * offsets  HOST [REX_MAX_BUCKETS+1], out: bucket b occupies perm[offsets[b] .. offsets[b+1]).
+ * Returns the number of buckets (0 for n == 0), TREX_EINVAL if more than REX_MAX_BUCKETS distinct keys occur.
+ * Synchronises the stream. */
+int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int64_t* offsets);
+
+/* HOST [REX_MAX_BUCKETS] out: key of bucket b of the last rex_bucket call. Returns the bucket count. */
+int rex_bucket_keys(uint64_t* bucket_keys);
+
+/* dst[r*n_dst + j] = src[r*n_src + perm[j]], r < nrows, j < n_dst  (SoA rows: momentum components, weights).
+ * perm points at the first entry of the bucket (perm + offsets[b]); n_dst = bucket size; n_src = total events. */
+int rex_gather(const double* src, int64_t n_src, double* dst, int64_t n_dst, int nrows, const int32_t* perm);
+
+/* dst[r*n_dst + perm[j]] = src[r*n_src + j], j < n_src: the inverse move. */
+int rex_scatter(const double* src, int64_t n_src, double* dst, int64_t n_dst, int nrows, const int32_t* perm);
+
+/* ---- subprocess registry (HOST) */
+int trex_subproc_id(uint64_t key);     /* key -> id, TREX_EUNKNOWN_SUBPROC if none (such events get zero weights,
+                                          PAPER.md:868, 1057: the caller zero-fills) */
+int trex_npar(int subproc_id);         /* external legs, or TREX_EUNKNOWN_SUBPROC */
+int trex_ncolor(int subproc_id);       /* colour flows summed in J^dagger C J */
+int trex_nhel(int subproc_id);         /* helicity combinations summed */
+/* HOST out[ncolor*ncolor], row-major: the colour matrix C used for this subprocess. Returns ncolor. */
+int trex_colour_matrix(int subproc_id, double* out);
+
+/* ---- trex_reweight (eqs.(2)-(5); :785-808)
+ * momenta_soa [npar][4][n] device: index (ipar*4 + mu)*n + ievt, mu = (E,px,py,pz), GeV.
+ * theta_old, theta_new HOST [TREX_NTHETA].
+ * w_in [n] device; w_out [n] device = w_in * me2_new / me2_old, exactly 0 where me2_old == 0.
+ * me2_old, me2_new [n] device or NULL.
+ * One launch evaluates both parameter points and shares all kinematics between them. n == 0 is a no-op. */
+int trex_reweight(int subproc_id, const double* momenta_soa, int64_t n, const double* theta_old,
+                  const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
+
+/* Diagnostic: per-helicity colour-flow amplitudes J_c of ONE event (momenta_one: HOST [npar][4]), for parity at the
+ * level of SURVEY.md I-4. out HOST [nhel][ncolor][2 orders in kappa][re,im], couplings included, order 1 per unit
+ * kappa. Only for TREX_SP_GG_TT .. TREX_SP_GG_TTGGG. Synchronous. */
+int trex_debug_flow_amps(int subproc_id, const double* momenta_one, const double* theta, double* out);
+
+int trex_set_stream(void* cuda_stream);
+int trex_set_precision(int mode);      /* 0 = fp64 (default), 1 = mixed (amplitudes fp64, colour sum fp32,
+                                          PAPER.md:1209 fptype m), 2 = fp32 */
+int trex_get_precision(void);
+/* kernels launched by this library since load (for bench.py's gpu_launches) */
+int64_t trex_launch_count(void);
+const char* trex_last_error(void);
+void trex_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* REX_TREX_H */

@@ -1,0 +1,116 @@
+// trex_ttng.cuh -- colour-flow amplitudes of a heavy quark line with N ordered gluon "sources".
+//
+// One thread evaluates ONE helicity configuration of ONE event. For every ordering sigma of the N sources it forms
+//   A_sigma = sum over all colour-ordered Feynman diagrams of that ordering,
+// by walking the tree of ordering prefixes depth first. At prefix (s_1..s_M) the thread holds
+//   J[a][M]  = off-shell gluon current of the contiguous tuple (s_{a+1}..s_M)     (VVV + VVVV vertices, propagator)
+//   U[p][M]  = top-line spinor after absorbing (s_1..s_M), with propagator, as a dual number in kappa (FFV vertices,
+//              chromomagnetic FFV dipole and FFVV contact at order 1; at most one insertion, R-4)
+// Only the current prefix path is alive (N(N+1)/2 currents, N line states): a few hundred doubles per thread instead
+// of the O(N!) table a memoised recursion needs. p = 0..NPASS-1 indexes parameter points whose top mass / width
+// differ (theta_old, theta_new): the gluon currents are shared between them.
+// g_s is factored out: A = g_s^N (A0 + (kappa/g_s) A1); this file computes A0 and A1 at g_s = 1.
+#pragma once
+#include "trex_math.cuh"
+
+namespace trex {
+
+template <class R> struct TopLine {      // per parameter point
+  R mt, mGt;                             // m_t and m_t * Gamma_t
+};
+
+// Sink: called once per ordering, in lexicographic order of sigma, with the leaf index.
+template <class R, int N, int NPASS, class Sink> struct TTNG {
+  // inputs (thread-private copies; dynamically indexed by the source number, so they live in local memory)
+  rvec4<R> K[N];            // incoming-convention momentum of each source
+  vec4<R> eps[N];           // its polarisation / effective current
+  rvec4<R> pt;              // top momentum (outgoing)
+  spinor<R> ubar_t, v_tb;   // ubar(p_t), v(p_tbar)
+  TopLine<R> line[NPASS];
+  // path state
+  vec4<R> J[N][N + 1];      // J[a][m], a < m
+  rvec4<R> P[N][N + 1];     // momentum of tuple (a+1..m)
+  dspinor<R> U[NPASS][N];   // U[p][m], m = 0..N-1 (U[.][0] = ubar_t, order 1 = 0)
+  int leaf;
+  Sink* sink;
+
+  template <int M> TREX_HD void level(unsigned used) {
+    for (int g = 0; g < N; ++g) {
+      if ((used >> g) & 1u) continue;
+      // --- gluon currents of all tuples ending at position M
+      J[M - 1][M] = eps[g];
+      P[M - 1][M] = K[g];
+#pragma unroll
+      for (int a = M - 2; a >= 0; --a) {
+        P[a][M] = radd(P[a][M - 1], K[g]);
+        vec4<R> acc = vzero<R>();
+#pragma unroll
+        for (int c = a + 1; c < M; ++c) v3_acc(acc, P[a][c], J[a][c], P[c][M], J[c][M]);
+#pragma unroll
+        for (int c1 = a + 1; c1 < M; ++c1)
+#pragma unroll
+          for (int c2 = c1 + 1; c2 < M; ++c2) v4_acc(acc, J[a][c1], J[c1][c2], J[c2][M]);
+        R s = R(-1) / rdot(P[a][M], P[a][M]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) J[a][M].c[i] = acc.c[i] * s;
+      }
+      // --- top line: bracket(M) = sum_a U(a) Gamma(J[a][M]) + order-1 field-strength insertions
+      spinor<R> b0[NPASS], b1[NPASS];
+#pragma unroll
+      for (int p = 0; p < NPASS; ++p) { b0[p] = szero<R>(); b1[p] = szero<R>(); }
+#pragma unroll
+      for (int a = 0; a < M; ++a) {
+        // F = P ^ J (dipole, gluon momentum into the vertex) + sum_c J[a][c] ^ J[c][M] (contact)
+        ften<R> F = fzero<R>();
+        wedge_acc(F, P[a][M], J[a][M]);
+#pragma unroll
+        for (int c = a + 1; c < M; ++c) wedge_acc(F, J[a][c], J[c][M]);
+#pragma unroll
+        for (int p = 0; p < NPASS; ++p) {
+          spinor<R> t0 = row_slash(U[p][a].o0, J[a][M]);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) b0[p].c[i] += mul_i(t0.c[i]);
+          if (a > 0) {                                   // U[.][0] has no order-1 part
+            spinor<R> t1 = row_slash(U[p][a].o1, J[a][M]);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) b1[p].c[i] += mul_i(t1.c[i]);
+          }
+          row_sigma_acc(b1[p], U[p][a].o0, F);
+        }
+      }
+      if constexpr (M < N) {
+        rvec4<R> q = rsub(pt, P[0][M]);
+        R q2 = rdot(q, q);
+#pragma unroll
+        for (int p = 0; p < NPASS; ++p) {
+          // S(q) = i (qslash + m) / (q^2 - m^2 + i m Gamma)
+          cx<R> den(q2 - line[p].mt * line[p].mt, line[p].mGt);
+          cx<R> pr = cdiv(cx<R>(0, 1), den);
+          spinor<R> s0 = row_slash(b0[p], q), s1 = row_slash(b1[p], q);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            cx<R> n0 = s0.c[i]; cfma(n0, b0[p].c[i], line[p].mt);
+            cx<R> n1 = s1.c[i]; cfma(n1, b1[p].c[i], line[p].mt);
+            U[p][M].o0.c[i] = n0 * pr; U[p][M].o1.c[i] = n1 * pr;
+          }
+        }
+        level<(M < N ? M + 1 : N)>(used | (1u << g));
+      } else {
+        cx<R> A0[NPASS], A1[NPASS];
+#pragma unroll
+        for (int p = 0; p < NPASS; ++p) { A0[p] = row_col(b0[p], v_tb); A1[p] = row_col(b1[p], v_tb); }
+        (*sink)(leaf, A0, A1);
+        ++leaf;
+      }
+    }
+  }
+
+  TREX_HD void run(Sink* s) {
+    sink = s; leaf = 0;
+#pragma unroll
+    for (int p = 0; p < NPASS; ++p) { U[p][0].o0 = ubar_t; U[p][0].o1 = szero<R>(); }
+    level<1>(0u);
+  }
+};
+
+}  // namespace trex
