@@ -101,10 +101,32 @@ int trex_colour_matrix(int subproc_id, double* out);
 int trex_reweight(int subproc_id, const double* momenta_soa, int64_t n, const double* theta_old,
                   const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
 
+/* ---- trex_run: the whole path of reweightor::run() steps 2-7 on DEVICE buffers:
+ * categorise (rex_bucket), transpose momenta and weights into per-subprocess SoA blocks (rex_gather), one trex_reweight
+ * launch per block, transpose the results back to the input order (rex_scatter).
+ * pdg_keys [n] device; momenta_soa [npar][4][n] device in INPUT order (all events have npar legs; particle order of
+ * every class = its process string); w_in, w_out [n] device; me2_old, me2_new [n] device or NULL.
+ * Events whose key has no compiled-in subprocess (or REX_NPOS) get w_out = me2 = 0.
+ * A sample with a single known class skips the transposition. Returns the number of buckets. Synchronises the stream
+ * once (inside rex_bucket); the reweighting launches themselves are asynchronous. */
+int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
+             const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
+
+/* The same with HOST buffers (pinned or pageable): copies keys, momenta and weights to internal device scratch on the
+ * stream, runs trex_run, copies the results back and synchronises the stream before returning. */
+int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
+                  const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
+
 /* Diagnostic: per-helicity colour-flow amplitudes J_c of ONE event (momenta_one: HOST [npar][4]), for parity at the
  * level of SURVEY.md I-4. out HOST [nhel][ncolor][2 orders in kappa][re,im], couplings included, order 1 per unit
  * kappa. Only for TREX_SP_GG_TT .. TREX_SP_GG_TTGGG. Synchronous. */
 int trex_debug_flow_amps(int subproc_id, const double* momenta_one, const double* theta, double* out);
+
+/* Roofline denominator: enqueues ONE launch of a register-resident FMA chain kernel (blocks x 256 threads, 64 FMAs per
+ * thread and iteration) on the library stream and returns the floating-point operations it executes (2 per FMA), or a
+ * negative error code. fp32 != 0 exercises the FP32 pipe instead of the FP64 pipe. The caller times it with events
+ * on that stream (no FP64 peak is provided, it has to be measured in the same run). */
+double trex_probe_fma(int fp32, int blocks, int iters);
 
 int trex_set_stream(void* cuda_stream);
 int trex_set_precision(int mode);      /* 0 = fp64 (default), 1 = mixed (amplitudes fp64, colour sum fp32,

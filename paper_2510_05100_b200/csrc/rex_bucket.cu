@@ -1,0 +1,328 @@
+// rex_bucket.cu -- device-side stable categorisation of events by flavour signature and the SoA "transposition"
+// (SURVEY.md 8(a) a2-a4, a10; PAPER.md:354 bucket order, :362 npos rule, :675-694 sort + transpose, :877 scatter back).
+//
+// rex_bucket in five small launches, all bound by HBM traffic (keys are read three times, perm written once):
+//   discover : distinct keys + index of first appearance, per-block shared-memory hash table merged into a global one
+//   rank     : bucket id = rank of the key's first appearance; REX_NPOS forced last
+//   hist     : per (bucket, warp-chunk) counts; a warp owns a contiguous chunk of events
+//   scan     : exclusive scan of the counts in (bucket-major, chunk-minor) order -> write positions, bucket offsets
+//   scatter  : every warp walks its chunk in input order, 32 events at a time, ranks equal buckets inside the warp
+//              with __match_any_sync and writes perm; running positions live in shared memory  => stable, bit-exact
+#include "trex_ctx.h"
+
+namespace trex {
+
+namespace {
+
+constexpr int TS = 1024;                       // hash slots (>= 4 x REX_MAX_BUCKETS)
+constexpr uint64_t EMPTY = REX_NPOS;           // REX_NPOS never enters the table: it has its own bucket
+constexpr int NBMAX = REX_MAX_BUCKETS;
+constexpr int WARPS = 8;
+
+struct BucketResult {                          // copied to pinned host memory at the end of the scan
+  int64_t offsets[NBMAX + 1];
+  uint64_t keys[NBMAX];
+  int nb;
+  int err;                                     // 1: more than REX_MAX_BUCKETS distinct keys
+};
+
+struct Table {
+  unsigned long long* keys;   // [TS]
+  unsigned* first;            // [TS] index of first appearance
+  int* bid;                   // [TS] bucket id
+  int* meta;                  // [0] ndistinct, [1] has_npos, [2] overflow, [3] nb
+  unsigned* npos_first;       // [1]
+};
+
+__device__ __forceinline__ unsigned hash_key(unsigned long long k) { return (unsigned)((k * 0x9E3779B97F4A7C15ull) >> 54); }
+
+__global__ void k_init(Table t) {
+  int i = threadIdx.x;
+  t.keys[i] = EMPTY; t.first[i] = 0xFFFFFFFFu; t.bid[i] = -1;
+  if (i < 4) t.meta[i] = 0;
+  if (i == 0) *t.npos_first = 0xFFFFFFFFu;
+}
+
+__global__ void __launch_bounds__(256) k_discover(const unsigned long long* __restrict__ keys, long n, long per_block, Table t) {
+  __shared__ unsigned long long sk[TS];
+  __shared__ unsigned sf[TS];
+  __shared__ unsigned s_npos;
+  __shared__ int s_over;
+  for (int i = threadIdx.x; i < TS; i += blockDim.x) { sk[i] = EMPTY; sf[i] = 0xFFFFFFFFu; }
+  if (threadIdx.x == 0) { s_npos = 0xFFFFFFFFu; s_over = 0; }
+  __syncthreads();
+  const long lo = (long)blockIdx.x * per_block, hi = min(n, lo + per_block);
+  for (long i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+    const unsigned long long k = keys[i];
+    if (k == EMPTY) { if ((unsigned)i < s_npos) atomicMin(&s_npos, (unsigned)i); continue; }
+    unsigned h = hash_key(k);
+    int slot = -1;
+    for (int probe = 0; probe < TS; ++probe) {
+      const unsigned s = (h + probe) & (TS - 1);
+      unsigned long long cur = sk[s];
+      if (cur == EMPTY) cur = atomicCAS(&sk[s], EMPTY, k);
+      if (cur == EMPTY || cur == k) { slot = (int)s; break; }
+    }
+    if (slot < 0) { s_over = 1; continue; }
+    // indices seen by one thread only grow and sf only shrinks: a stale read can only cause a redundant atomic
+    if ((unsigned)i < sf[slot]) atomicMin(&sf[slot], (unsigned)i);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (s_npos != 0xFFFFFFFFu) { atomicMin(t.npos_first, s_npos); t.meta[1] = 1; }
+    if (s_over) t.meta[2] = 1;
+  }
+  for (int i = threadIdx.x; i < TS; i += blockDim.x) {
+    const unsigned long long k = sk[i];
+    if (k == EMPTY) continue;
+    unsigned h = hash_key(k);
+    int slot = -1;
+    for (int probe = 0; probe < TS; ++probe) {
+      const unsigned s = (h + probe) & (TS - 1);
+      unsigned long long cur = t.keys[s];
+      if (cur == EMPTY) { cur = atomicCAS(&t.keys[s], EMPTY, k); if (cur == EMPTY) atomicAdd(&t.meta[0], 1); }
+      if (cur == EMPTY || cur == k) { slot = (int)s; break; }
+    }
+    if (slot < 0) { t.meta[2] = 1; continue; }
+    atomicMin(&t.first[slot], sf[i]);
+  }
+}
+
+__global__ void __launch_bounds__(TS) k_rank(Table t, BucketResult* res) {
+  __shared__ unsigned sf[TS];
+  const int s = threadIdx.x;
+  const unsigned long long k = t.keys[s];
+  const unsigned f = t.first[s];
+  sf[s] = (k == EMPTY) ? 0xFFFFFFFFu : f;
+  __syncthreads();
+  const int nd = t.meta[0], has_npos = t.meta[1];
+  const int nb = nd + has_npos;
+  const bool bad = (nb > NBMAX) || t.meta[2];
+  if (k != EMPTY) {
+    int rank = 0;
+    for (int j = 0; j < TS; ++j) rank += (sf[j] < f) ? 1 : 0;
+    t.bid[s] = rank;
+    if (!bad) res->keys[rank] = k;
+  }
+  if (s == 0) {
+    t.meta[3] = bad ? 0 : nb;
+    res->nb = bad ? 0 : nb;
+    res->err = bad ? 1 : 0;
+    if (!bad && has_npos) res->keys[nd] = EMPTY;
+  }
+}
+
+// shared-memory copy of the key -> bucket table for the lookups of hist / scatter
+struct SmemTable {
+  unsigned long long k[TS];
+  int b[TS];
+  __device__ void load(const Table& t) {
+    for (int i = threadIdx.x; i < TS; i += blockDim.x) { k[i] = t.keys[i]; b[i] = t.bid[i]; }
+  }
+  __device__ __forceinline__ int lookup(unsigned long long key, int npos_bid) const {
+    if (key == EMPTY) return npos_bid;
+    unsigned h = hash_key(key);
+    for (int probe = 0; probe < TS; ++probe) {
+      const unsigned s = (h + probe) & (TS - 1);
+      if (k[s] == key) return b[s];
+    }
+    return npos_bid;   // unreachable: every key was inserted by k_discover
+  }
+};
+
+__global__ void __launch_bounds__(WARPS * 32) k_hist(const unsigned long long* __restrict__ keys, long n, long wch, long nchunks,
+                                                   Table t, unsigned* __restrict__ counts) {
+  __shared__ SmemTable tab;
+  __shared__ unsigned hist[WARPS][NBMAX];
+  const int nb = t.meta[3];
+  if (nb == 0) return;
+  tab.load(t);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  for (int i = lane; i < nb; i += 32) hist[warp][i] = 0;
+  __syncthreads();
+  const long chunk = (long)blockIdx.x * WARPS + warp;
+  if (chunk >= nchunks) return;
+  const long lo = chunk * wch, hi = min(n, lo + wch);
+  for (long i = lo + lane; i < hi; i += 32) atomicAdd(&hist[warp][tab.lookup(keys[i], nb - 1)], 1u);
+  __syncwarp();
+  for (int b = lane; b < nb; b += 32) counts[(long)b * nchunks + chunk] = hist[warp][b];
+}
+
+__global__ void __launch_bounds__(1024) k_scan(unsigned* __restrict__ counts, long nchunks, long n, Table t, BucketResult* res) {
+  __shared__ unsigned long long part[1024];
+  const int nb = t.meta[3];
+  const long total = (long)nb * nchunks;
+  const long seg = (total + 1023) / 1024;
+  const long lo = min(total, (long)threadIdx.x * seg), hi = min(total, lo + seg);
+  unsigned long long s = 0;
+  for (long i = lo; i < hi; ++i) s += counts[i];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  // inclusive Hillis-Steele scan over the 1024 partial sums
+  for (int off = 1; off < 1024; off <<= 1) {
+    unsigned long long v = threadIdx.x >= off ? part[threadIdx.x - off] : 0ull;
+    __syncthreads();
+    part[threadIdx.x] += v;
+    __syncthreads();
+  }
+  unsigned long long run = part[threadIdx.x] - s;
+  for (long i = lo; i < hi; ++i) {
+    const unsigned c = counts[i];
+    counts[i] = (unsigned)run;
+    if (i % nchunks == 0) res->offsets[i / nchunks] = (int64_t)run;
+    run += c;
+  }
+  if (threadIdx.x == 0) res->offsets[nb] = nb ? n : 0;
+}
+
+__global__ void __launch_bounds__(WARPS * 32) k_scatter(const unsigned long long* __restrict__ keys, long n, long wch, long nchunks,
+                                                      Table t, const unsigned* __restrict__ base, int* __restrict__ perm) {
+  __shared__ SmemTable tab;
+  __shared__ unsigned pos[WARPS][NBMAX];
+  const int nb = t.meta[3];
+  if (nb == 0) return;
+  tab.load(t);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long chunk = (long)blockIdx.x * WARPS + warp;
+  if (chunk < nchunks)
+    for (int b = lane; b < nb; b += 32) pos[warp][b] = base[(long)b * nchunks + chunk];
+  __syncthreads();
+  if (chunk >= nchunks) return;
+  const long lo = chunk * wch, hi = min(n, lo + wch);
+  for (long i0 = lo; i0 < hi; i0 += 32) {
+    const long i = i0 + lane;
+    const bool live = i < hi;
+    const unsigned active = __ballot_sync(0xFFFFFFFFu, live);
+    if (live) {
+      const int b = tab.lookup(keys[i], nb - 1);
+      const unsigned peers = __match_any_sync(active, b);
+      const unsigned rank = __popc(peers & ((1u << lane) - 1u));
+      perm[pos[warp][b] + rank] = (int)i;
+      __syncwarp(active);
+      if (rank == 0) pos[warp][b] += __popc(peers);
+    }
+    __syncwarp();
+  }
+}
+
+__global__ void k_gather(const double* __restrict__ src, long n_src, double* __restrict__ dst, long n_dst, int nrows,
+                         const int* __restrict__ perm) {
+  const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n_dst) return;
+  const long p = perm[j];
+  for (int r = 0; r < nrows; ++r) dst[(long)r * n_dst + j] = src[(long)r * n_src + p];
+}
+
+__global__ void k_scatter_rows(const double* __restrict__ src, long n_src, double* __restrict__ dst, long n_dst, int nrows,
+                               const int* __restrict__ perm) {
+  const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n_src) return;
+  const long p = perm[j];
+  for (int r = 0; r < nrows; ++r) dst[(long)r * n_dst + p] = src[(long)r * n_src + j];
+}
+
+size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
+
+}  // namespace
+
+}  // namespace trex
+
+using namespace trex;
+
+extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int64_t* offsets) {
+  Context& c = ctx();
+  if (n < 0 || !offsets || (n > 0 && (!pdg_keys || !perm))) return fail(TREX_EINVAL, "rex_bucket: null pointer or negative n");
+  if (n >= (int64_t(1) << 31)) return fail(TREX_EINVAL, "rex_bucket: n must be < 2^31 (perm is int32)");
+  c.last_nbuckets = 0;
+  if (n == 0) { offsets[0] = 0; return 0; }
+  // a warp owns `wch` consecutive events; at most 4096 chunks so that the single-block scan stays short
+  long wch = 1024;
+  while ((n + wch - 1) / wch > 4096) wch *= 2;
+  const long nchunks = (n + wch - 1) / wch;
+  const size_t off_keys = 0, off_first = align_up(off_keys + TS * 8), off_bid = align_up(off_first + TS * 4),
+               off_meta = align_up(off_bid + TS * 4), off_npos = align_up(off_meta + 16), off_res = align_up(off_npos + 4),
+               off_counts = align_up(off_res + sizeof(BucketResult)),
+               total = align_up(off_counts + (size_t)NBMAX * nchunks * 4);
+  if (c.bucket_scratch_bytes < total) {
+    if (c.bucket_scratch) cudaFree(c.bucket_scratch);
+    c.bucket_scratch = nullptr; c.bucket_scratch_bytes = 0;
+    TREX_CUDA_CHECK(cudaMalloc(&c.bucket_scratch, total));
+    c.bucket_scratch_bytes = total;
+  }
+  if (!c.bucket_host) TREX_CUDA_CHECK(cudaMallocHost(&c.bucket_host, sizeof(BucketResult)));
+  char* base = (char*)c.bucket_scratch;
+  Table t{(unsigned long long*)(base + off_keys), (unsigned*)(base + off_first), (int*)(base + off_bid),
+          (int*)(base + off_meta), (unsigned*)(base + off_npos)};
+  BucketResult* res = (BucketResult*)(base + off_res);
+  unsigned* counts = (unsigned*)(base + off_counts);
+  const unsigned long long* keys = (const unsigned long long*)pdg_keys;
+
+  k_init<<<1, TS, 0, c.stream>>>(t);
+  const long per_block = 8192;
+  const unsigned nblk = (unsigned)((n + per_block - 1) / per_block);
+  k_discover<<<nblk, 256, 0, c.stream>>>(keys, n, per_block, t);
+  k_rank<<<1, TS, 0, c.stream>>>(t, res);
+  const unsigned cblk = (unsigned)((nchunks + WARPS - 1) / WARPS);
+  k_hist<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts);
+  k_scan<<<1, 1024, 0, c.stream>>>(counts, nchunks, n, t, res);
+  k_scatter<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts, perm);
+  c.launches += 6;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  TREX_CUDA_CHECK(cudaMemcpyAsync(c.bucket_host, res, sizeof(BucketResult), cudaMemcpyDeviceToHost, c.stream));
+  TREX_CUDA_CHECK(cudaStreamSynchronize(c.stream));
+  const BucketResult* h = (const BucketResult*)c.bucket_host;
+  if (h->err) return fail(TREX_EINVAL, "rex_bucket: more than %d distinct flavour keys", REX_MAX_BUCKETS);
+  for (int b = 0; b <= h->nb; ++b) offsets[b] = h->offsets[b];
+  for (int b = 0; b < h->nb; ++b) c.last_keys[b] = h->keys[b];
+  c.last_nbuckets = h->nb;
+  return h->nb;
+}
+
+extern "C" int rex_bucket_keys(uint64_t* bucket_keys) {
+  Context& c = ctx();
+  if (!bucket_keys) return fail(TREX_EINVAL, "rex_bucket_keys: null pointer");
+  for (int b = 0; b < c.last_nbuckets; ++b) bucket_keys[b] = c.last_keys[b];
+  return c.last_nbuckets;
+}
+
+extern "C" int rex_gather(const double* src, int64_t n_src, double* dst, int64_t n_dst, int nrows, const int32_t* perm) {
+  Context& c = ctx();
+  if (n_src < 0 || n_dst < 0 || nrows < 0) return fail(TREX_EINVAL, "rex_gather: negative size");
+  if (n_dst == 0 || nrows == 0) return 0;
+  if (!src || !dst || !perm) return fail(TREX_EINVAL, "rex_gather: null pointer");
+  k_gather<<<(unsigned)((n_dst + 255) / 256), 256, 0, c.stream>>>(src, n_src, dst, n_dst, nrows, perm);
+  c.launches += 1;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return 0;
+}
+
+extern "C" int rex_scatter(const double* src, int64_t n_src, double* dst, int64_t n_dst, int nrows, const int32_t* perm) {
+  Context& c = ctx();
+  if (n_src < 0 || n_dst < 0 || nrows < 0) return fail(TREX_EINVAL, "rex_scatter: negative size");
+  if (n_src == 0 || nrows == 0) return 0;
+  if (!src || !dst || !perm) return fail(TREX_EINVAL, "rex_scatter: null pointer");
+  k_scatter_rows<<<(unsigned)((n_src + 255) / 256), 256, 0, c.stream>>>(src, n_src, dst, n_dst, nrows, perm);
+  c.launches += 1;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return 0;
+}
+
+extern "C" uint64_t rex_pack_key(const int32_t* pdg, const int8_t* status, int nlegs) {
+  if (!pdg || !status || nlegs < 0) return REX_NPOS;
+  int ini[8], fin[8], ni = 0, nf = 0;
+  for (int i = 0; i < nlegs; ++i) {
+    if (status[i] != -1 && status[i] != 1) continue;
+    const int a = pdg[i] < 0 ? -pdg[i] : pdg[i];
+    if (a > 127 || ni + nf >= 7) return REX_NPOS;
+    (status[i] == -1 ? ini[ni++] : fin[nf++]) = pdg[i];
+  }
+  auto sort_small = [](int* v, int m) { for (int i = 1; i < m; ++i) { int x = v[i], j = i - 1; while (j >= 0 && v[j] > x) { v[j + 1] = v[j]; --j; } v[j + 1] = x; } };
+  sort_small(ini, ni); sort_small(fin, nf);
+  uint64_t key = 0;
+  int pos = 0;
+  auto put = [&](int p) { const uint64_t b = (uint64_t)((p < 0 ? -p : p) & 0x7F) | (p < 0 ? 0x80u : 0u); key |= b << (8 * pos++); };
+  for (int i = 0; i < ni; ++i) put(ini[i]);
+  for (int i = 0; i < nf; ++i) put(fin[i]);
+  key |= (uint64_t)((ni << 4) | nf) << 56;
+  return key;
+}

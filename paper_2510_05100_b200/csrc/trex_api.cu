@@ -1,0 +1,314 @@
+// trex_api.cu -- reweighting kernels and the C ABI of include/rex_trex.h.
+#include <cstring>
+#include <vector>
+
+#include "trex_colour.h"
+#include "trex_ctx.h"
+#include "trex_host.h"
+#include "trex_kernels.cuh"
+
+namespace trex {
+
+Context& ctx() { static Context c; return c; }
+
+namespace {
+
+template <class R, class RC>
+__global__ void __launch_bounds__(WARPS * 32) k_qq(const ReweightArgs a) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long e = (long)blockIdx.x * 32 + lane;
+  const long ev = e < a.n ? e : a.n - 1;
+  RC acc[2] = {RC(0), RC(0)};
+  for (int u = warp; u < 16; u += WARPS) {
+    RC out[2];
+    qq_unit<R, RC>(a.mom, a.ld, ev, a.q, u, a.T, out);
+    acc[0] += out[0]; acc[1] += out[1];
+  }
+  reduce_and_finish<RC>(a, acc[0], acc[1], e);
+}
+
+template <class R>
+__global__ void __launch_bounds__(128) k_eemumu(const ReweightArgs a) {
+  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= a.n) return;
+  R out[2];
+  eemumu_event<R>(a.mom, a.ld, e, a.T, out);
+  const double mo = (double)out[0] * a.T.pref[0], mn = (double)out[1] * a.T.pref[1];
+  const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;
+  a.w_out[e] = a.w_in[e] * norm * mn;
+  if (a.me2_old) a.me2_old[e] = mo;
+  if (a.me2_new) a.me2_new[e] = mn;
+}
+
+// diagnostic: colour-flow amplitudes of one event, one thread per full helicity index h (bit `leg` of h = helicity
+// of that leg in process order)
+template <int N> struct DebugSink {
+  double* out; spinor<double> v; double gsN, gsN1;
+  __device__ void operator()(int leaf, const spinor<double>* b0, const spinor<double>* b1) {
+    cx<double> a0 = row_col(b0[0], v), a1 = row_col(b1[0], v);
+    out[4 * leaf + 0] = a0.re * gsN; out[4 * leaf + 1] = a0.im * gsN;
+    out[4 * leaf + 2] = a1.re * gsN1; out[4 * leaf + 3] = a1.im * gsN1;
+  }
+};
+template <int N> __global__ void k_debug_flows(const double* mom, double mt, double mGt, double gs, double* out) {
+  const int h = blockIdx.x * blockDim.x + threadIdx.x;
+  if (h >= (1 << (N + 2))) return;
+  DebugSink<N> sink;
+  constexpr int NC = factorial(N);
+  sink.out = out + (long)h * NC * 4;
+  sink.gsN = pow(gs, (double)N); sink.gsN1 = pow(gs, (double)(N - 1));
+  TTNG<double, N, 1, DebugSink<N>> t;
+  for (int g = 0; g < N; ++g) {
+    const int leg = g < 2 ? g : g + 2;
+    double p[4]; load_leg<double>(mom, 1, 0, leg, p);
+    const bool incoming = g < 2;
+    t.eps[g] = polvec<double>(p, ((h >> leg) & 1) ? 1 : -1, !incoming);
+    for (int mu = 0; mu < 4; ++mu) t.K[g].c[mu] = incoming ? p[mu] : -p[mu];
+  }
+  double p[4]; load_leg<double>(mom, 1, 0, 2, p);
+  for (int mu = 0; mu < 4; ++mu) t.pt.c[mu] = p[mu];
+  t.ubar_t = bar(spinor_u<double>(p, ((h >> 2) & 1) ? 1 : -1, false));
+  double q[4]; load_leg<double>(mom, 1, 0, 3, q);
+  sink.v = spinor_v<double>(q, ((h >> 3) & 1) ? 1 : -1, false);
+  t.line[0].mt = mt; t.line[0].mGt = mGt;
+  t.run(&sink);
+}
+
+const TtngLaunchFn kLaunch[4][3] = {
+    {trex_tu_launch_n2_m0, trex_tu_launch_n2_m1, trex_tu_launch_n2_m2}, {trex_tu_launch_n3_m0, trex_tu_launch_n3_m1, trex_tu_launch_n3_m2},
+    {trex_tu_launch_n4_m0, trex_tu_launch_n4_m1, trex_tu_launch_n4_m2}, {trex_tu_launch_n5_m0, trex_tu_launch_n5_m1, trex_tu_launch_n5_m2}};
+const TtngUploadFn kUpload[4][3] = {
+    {trex_tu_upload_n2_m0, trex_tu_upload_n2_m1, trex_tu_upload_n2_m2}, {trex_tu_upload_n3_m0, trex_tu_upload_n3_m1, trex_tu_upload_n3_m2},
+    {trex_tu_upload_n4_m0, trex_tu_upload_n4_m1, trex_tu_upload_n4_m2}, {trex_tu_upload_n5_m0, trex_tu_upload_n5_m1, trex_tu_upload_n5_m2}};
+
+int ensure_colour() {
+  Context& c = ctx();
+  if (c.colour_ready) return 0;
+  for (int N = 2; N <= 5; ++N) {
+    std::vector<double> C = trex_colour::ttng_colour_matrix(N);
+    for (int m = 0; m < 3; ++m)
+      if (kUpload[N - 2][m](C.data(), (int)C.size()) != 0) return fail(TREX_ECUDA, "colour matrix upload failed (N=%d)", N);
+    if (N == 5) {
+      TREX_CUDA_CHECK(cudaMalloc((void**)&c.C120, sizeof(double) * C.size()));
+      TREX_CUDA_CHECK(cudaMemcpy(c.C120, C.data(), sizeof(double) * C.size(), cudaMemcpyHostToDevice));
+    }
+  }
+  c.colour_ready = true;
+  return 0;
+}
+
+}  // namespace
+}  // namespace trex
+
+using namespace trex;
+
+extern "C" int trex_subproc_id(uint64_t key) {
+  for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
+    const SubprocInfo* sp = subproc_info(sid);
+    int8_t status[7];
+    for (int i = 0; i < sp->npar; ++i) status[i] = i < 2 ? -1 : 1;
+    if (rex_pack_key(sp->pdg, status, sp->npar) == key) return sid;
+  }
+  return TREX_EUNKNOWN_SUBPROC;
+}
+extern "C" int trex_npar(int sid) { const SubprocInfo* sp = subproc_info(sid); return sp ? sp->npar : TREX_EUNKNOWN_SUBPROC; }
+extern "C" int trex_ncolor(int sid) { const SubprocInfo* sp = subproc_info(sid); return sp ? sp->ncolor : TREX_EUNKNOWN_SUBPROC; }
+extern "C" int trex_nhel(int sid) { const SubprocInfo* sp = subproc_info(sid); return sp ? sp->nhel : TREX_EUNKNOWN_SUBPROC; }
+
+extern "C" int trex_colour_matrix(int sid, double* out) {
+  const SubprocInfo* sp = subproc_info(sid);
+  if (!sp) return fail(TREX_EUNKNOWN_SUBPROC, "trex_colour_matrix: unknown subprocess %d", sid);
+  if (!out) return fail(TREX_EINVAL, "trex_colour_matrix: null pointer");
+  if (sid == TREX_SP_EEMUMU) { out[0] = 1.0; return 1; }
+  if (sid >= TREX_SP_GG_TT && sid <= TREX_SP_GG_TTGGG) {
+    std::vector<double> C = trex_colour::ttng_colour_matrix(sp->npar - 2);
+    std::memcpy(out, C.data(), C.size() * sizeof(double));
+    return sp->ncolor;
+  }
+  static const double CQ[16] = {12, 0, 4, 4, 0, 12, 4, 4, 4, 4, 12, 0, 4, 4, 0, 12};
+  std::memcpy(out, CQ, sizeof CQ);
+  return 4;
+}
+
+// one launch: |M|^2 at theta_old and theta_new + epilogue for the n events of an SoA block with row stride ld
+static int launch_reweight(int sid, const double* mom, long n, long ld, const ThetaPair& T, const double* w_in, double* w_out,
+                           double* me2_old, double* me2_new) {
+  Context& c = ctx();
+  const SubprocInfo* sp = subproc_info(sid);
+  ReweightArgs a;
+  a.T = T; a.mom = mom; a.n = n; a.ld = ld; a.w_in = w_in; a.w_out = w_out; a.me2_old = me2_old; a.me2_new = me2_new;
+  a.q = sp->qlegs;
+  if (int rc = ensure_colour()) return rc;
+  a.C120 = c.C120;
+  const unsigned grid32 = (unsigned)((n + 31) / 32);
+  const int mode = c.precision;
+  if (sid == TREX_SP_EEMUMU) {
+    const unsigned grid = (unsigned)((n + 127) / 128);
+    if (mode == 2) k_eemumu<float><<<grid, 128, 0, c.stream>>>(a);
+    else k_eemumu<double><<<grid, 128, 0, c.stream>>>(a);
+  } else if (sid <= TREX_SP_GG_TTGGG) {
+    const int N = sp->npar - 2;
+    const int npass = (T.mt[0] != T.mt[1] || T.mGt[0] != T.mGt[1]) ? 2 : 1;
+    if (kLaunch[N - 2][mode](a, npass, grid32, c.stream) != 0) return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+  } else {
+    if (mode == 0) k_qq<double, double><<<grid32, WARPS * 32, 0, c.stream>>>(a);
+    else if (mode == 1) k_qq<double, float><<<grid32, WARPS * 32, 0, c.stream>>>(a);
+    else k_qq<float, float><<<grid32, WARPS * 32, 0, c.stream>>>(a);
+  }
+  c.launches += 1;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return 0;
+}
+
+extern "C" int trex_reweight(int sid, const double* momenta_soa, int64_t n, const double* theta_old, const double* theta_new,
+                             const double* w_in, double* w_out, double* me2_old, double* me2_new) {
+  const SubprocInfo* sp = subproc_info(sid);
+  if (!sp) return fail(TREX_EUNKNOWN_SUBPROC, "trex_reweight: unknown subprocess %d", sid);
+  if (n < 0 || !theta_old || !theta_new) return fail(TREX_EINVAL, "trex_reweight: negative n or null theta");
+  if (n == 0) return 0;
+  if (!momenta_soa || !w_in || !w_out) return fail(TREX_EINVAL, "trex_reweight: null device pointer");
+  ThetaPair T;
+  if (!make_theta_pair(sid, theta_old, theta_new, T)) return fail(TREX_EINVAL, "trex_reweight: theta outside its domain");
+  return launch_reweight(sid, momenta_soa, n, n, T, w_in, w_out, me2_old, me2_new);
+}
+
+static int ensure_scratch(void** p, size_t* have, size_t need) {
+  if (*have >= need) return 0;
+  if (*p) cudaFree(*p);
+  *p = nullptr; *have = 0;
+  TREX_CUDA_CHECK(cudaMalloc(p, need));
+  *have = need;
+  return 0;
+}
+
+__global__ void k_zero_rows(double* __restrict__ dst, long ld, long off, long cnt, int nrows) {
+  const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= cnt) return;
+  for (int r = 0; r < nrows; ++r) dst[(long)r * ld + off + j] = 0.0;
+}
+
+// the whole path on device buffers: categorise, transpose into per-subprocess blocks, reweight every block, transpose back
+extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
+                        const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new) {
+  Context& c = ctx();
+  if (n < 0 || npar < 1 || npar > 7 || !theta_old || !theta_new) return fail(TREX_EINVAL, "trex_run: bad size or null theta");
+  if (n == 0) return 0;
+  if (!pdg_keys || !momenta_soa || !w_in || !w_out) return fail(TREX_EINVAL, "trex_run: null device pointer");
+  const int nrows_in = 4 * npar + 1;
+  if (int rc = ensure_scratch(&c.run_perm, &c.run_perm_bytes, sizeof(int32_t) * (size_t)n)) return rc;
+  int64_t offsets[REX_MAX_BUCKETS + 1];
+  const int nb = rex_bucket(pdg_keys, n, (int32_t*)c.run_perm, offsets);
+  if (nb < 0) return nb;
+  // a single known class needs no transposition at all
+  if (nb == 1) {
+    const int sid = trex_subproc_id(c.last_keys[0]);
+    if (sid >= 0 && subproc_info(sid)->npar == npar) {
+      ThetaPair T;
+      if (!make_theta_pair(sid, theta_old, theta_new, T)) return fail(TREX_EINVAL, "trex_run: theta outside its domain");
+      const int rc = launch_reweight(sid, momenta_soa, n, n, T, w_in, w_out, me2_old, me2_new);
+      return rc < 0 ? rc : 1;
+    }
+  }
+  if (int rc = ensure_scratch(&c.run_blocks, &c.run_blocks_bytes, sizeof(double) * (size_t)n * (nrows_in + 3))) return rc;
+  double* blk = (double*)c.run_blocks;          // [4 npar][n] momenta, [1][n] w_in  -- in bucketed order
+  double* res = blk + (size_t)nrows_in * n;     // [3][n]: w_out, me2_old, me2_new  -- in bucketed order
+  if (int rc = rex_gather(momenta_soa, n, blk, n, 4 * npar, (const int32_t*)c.run_perm)) return rc;
+  if (int rc = rex_gather(w_in, n, blk + (size_t)4 * npar * n, n, 1, (const int32_t*)c.run_perm)) return rc;
+  for (int b = 0; b < nb; ++b) {
+    const long off = offsets[b], cnt = offsets[b + 1] - offsets[b];
+    if (cnt == 0) continue;
+    const int sid = trex_subproc_id(c.last_keys[b]);
+    ThetaPair T;
+    if (sid < 0 || subproc_info(sid)->npar != npar) {
+      // no amplitude routine for this class: zero weights
+      k_zero_rows<<<(unsigned)((cnt + 255) / 256), 256, 0, c.stream>>>(res, n, off, cnt, 3);
+      c.launches += 1;
+      continue;
+    }
+    if (!make_theta_pair(sid, theta_old, theta_new, T)) return fail(TREX_EINVAL, "trex_run: theta outside its domain");
+    if (int rc = launch_reweight(sid, blk + off, cnt, n, T, blk + (size_t)4 * npar * n + off, res + off, res + n + off, res + 2 * (size_t)n + off))
+      return rc;
+  }
+  if (int rc = rex_scatter(res, n, w_out, n, 1, (const int32_t*)c.run_perm)) return rc;
+  if (me2_old) if (int rc = rex_scatter(res + n, n, me2_old, n, 1, (const int32_t*)c.run_perm)) return rc;
+  if (me2_new) if (int rc = rex_scatter(res + 2 * (size_t)n, n, me2_new, n, 1, (const int32_t*)c.run_perm)) return rc;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return nb;
+}
+
+// the same with HOST buffers: copies in, runs, copies out, synchronises (bench.py's end-to-end figure)
+extern "C" int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
+                             const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new) {
+  Context& c = ctx();
+  if (n < 0 || npar < 1 || npar > 7) return fail(TREX_EINVAL, "trex_run_host: bad size");
+  if (n == 0) return 0;
+  if (!pdg_keys || !momenta_soa || !w_in || !w_out) return fail(TREX_EINVAL, "trex_run_host: null pointer");
+  const size_t nn = (size_t)n, rows = (size_t)4 * npar;
+  if (int rc = ensure_scratch(&c.host_io, &c.host_io_bytes, 8 * nn * (1 + rows + 1 + 3))) return rc;
+  uint64_t* d_keys = (uint64_t*)c.host_io;
+  double* d_mom = (double*)c.host_io + nn;
+  double* d_win = d_mom + rows * nn;
+  double* d_out = d_win + nn;
+  TREX_CUDA_CHECK(cudaMemcpyAsync(d_keys, pdg_keys, 8 * nn, cudaMemcpyHostToDevice, c.stream));
+  TREX_CUDA_CHECK(cudaMemcpyAsync(d_mom, momenta_soa, 8 * nn * rows, cudaMemcpyHostToDevice, c.stream));
+  TREX_CUDA_CHECK(cudaMemcpyAsync(d_win, w_in, 8 * nn, cudaMemcpyHostToDevice, c.stream));
+  const int rc = trex_run(d_keys, d_mom, n, npar, theta_old, theta_new, d_win, d_out, me2_old ? d_out + nn : nullptr,
+                          me2_new ? d_out + 2 * nn : nullptr);
+  if (rc < 0) return rc;
+  TREX_CUDA_CHECK(cudaMemcpyAsync(w_out, d_out, 8 * nn, cudaMemcpyDeviceToHost, c.stream));
+  if (me2_old) TREX_CUDA_CHECK(cudaMemcpyAsync(me2_old, d_out + nn, 8 * nn, cudaMemcpyDeviceToHost, c.stream));
+  if (me2_new) TREX_CUDA_CHECK(cudaMemcpyAsync(me2_new, d_out + 2 * nn, 8 * nn, cudaMemcpyDeviceToHost, c.stream));
+  TREX_CUDA_CHECK(cudaStreamSynchronize(c.stream));
+  return rc;
+}
+
+extern "C" int trex_debug_flow_amps(int sid, const double* momenta_one, const double* theta, double* out) {
+  Context& c = ctx();
+  const SubprocInfo* sp = subproc_info(sid);
+  if (!sp || sid < TREX_SP_GG_TT || sid > TREX_SP_GG_TTGGG) return fail(TREX_EUNKNOWN_SUBPROC, "trex_debug_flow_amps: only g g > t t~ (+g..)");
+  if (!momenta_one || !theta || !out) return fail(TREX_EINVAL, "trex_debug_flow_amps: null pointer");
+  const int N = sp->npar - 2, nhel = sp->nhel;
+  const size_t nout = (size_t)nhel * sp->ncolor * 4;
+  double *d_mom = nullptr, *d_out = nullptr;
+  TREX_CUDA_CHECK(cudaMalloc((void**)&d_mom, sizeof(double) * 4 * sp->npar));
+  TREX_CUDA_CHECK(cudaMalloc((void**)&d_out, sizeof(double) * nout));
+  TREX_CUDA_CHECK(cudaMemcpyAsync(d_mom, momenta_one, sizeof(double) * 4 * sp->npar, cudaMemcpyHostToDevice, c.stream));
+  const double gs = std::sqrt(4.0 * 3.14159265358979323846 * theta[TREX_TH_ALPHA_S]);
+  const double mt = theta[TREX_TH_MT], mGt = mt * theta[TREX_TH_GAMMAT];
+  const unsigned grid = (unsigned)((nhel + 63) / 64);
+  switch (N) {
+    case 2: k_debug_flows<2><<<grid, 64, 0, c.stream>>>(d_mom, mt, mGt, gs, d_out); break;
+    case 3: k_debug_flows<3><<<grid, 64, 0, c.stream>>>(d_mom, mt, mGt, gs, d_out); break;
+    case 4: k_debug_flows<4><<<grid, 64, 0, c.stream>>>(d_mom, mt, mGt, gs, d_out); break;
+    default: k_debug_flows<5><<<grid, 64, 0, c.stream>>>(d_mom, mt, mGt, gs, d_out); break;
+  }
+  c.launches += 1;
+  cudaError_t e1 = cudaGetLastError();
+  cudaError_t e2 = cudaMemcpyAsync(out, d_out, sizeof(double) * nout, cudaMemcpyDeviceToHost, c.stream);
+  cudaError_t e3 = cudaStreamSynchronize(c.stream);
+  cudaFree(d_mom); cudaFree(d_out);
+  TREX_CUDA_CHECK(e1); TREX_CUDA_CHECK(e2); TREX_CUDA_CHECK(e3);
+  return 0;
+}
+
+extern "C" int trex_set_stream(void* cuda_stream) { ctx().stream = (cudaStream_t)cuda_stream; return 0; }
+extern "C" int trex_set_precision(int mode) {
+  if (mode < 0 || mode > 2) return fail(TREX_EINVAL, "trex_set_precision: mode must be 0, 1 or 2");
+  ctx().precision = mode; return 0;
+}
+extern "C" int trex_get_precision(void) { return ctx().precision; }
+extern "C" int64_t trex_launch_count(void) { return ctx().launches; }
+extern "C" const char* trex_last_error(void) { return ctx().err; }
+extern "C" void trex_shutdown(void) {
+  Context& c = ctx();
+  if (c.bucket_scratch) cudaFree(c.bucket_scratch);
+  if (c.bucket_host) cudaFreeHost(c.bucket_host);
+  if (c.C120) cudaFree(c.C120);
+  if (c.run_perm) cudaFree(c.run_perm);
+  if (c.run_blocks) cudaFree(c.run_blocks);
+  if (c.host_io) cudaFree(c.host_io);
+  if (c.probe_out) cudaFree(c.probe_out);
+  c.probe_out = nullptr;
+  c.run_perm = c.run_blocks = c.host_io = nullptr; c.run_perm_bytes = c.run_blocks_bytes = c.host_io_bytes = 0;
+  c.bucket_scratch = nullptr; c.bucket_scratch_bytes = 0; c.bucket_host = nullptr; c.C120 = nullptr; c.colour_ready = false;
+}

@@ -1,0 +1,66 @@
+// trex_host.h -- host-side registry of compiled-in subprocesses and translation of theta[] into kernel parameters.
+#pragma once
+#include <cmath>
+#include <cstdint>
+
+#include "../../include/rex_trex.h"
+#include "trex_proc.cuh"
+
+namespace trex {
+
+struct SubprocInfo {
+  int npar;        // external legs
+  int ncolor;      // colour flows in J^dagger C J
+  int nhel;        // helicity combinations summed
+  int nunits;      // helicity units a thread block distributes over its warps (antitop helicity closed inside a unit)
+  int nvert;       // power of g_s in the amplitude
+  double navg;     // spin x colour average x identical-particle factor (R-7)
+  int pdg[7];      // process-string order
+  QLineLegs qlegs; // light-quark line (quark channels only)
+};
+
+inline const SubprocInfo* subproc_info(int sid) {
+  static const SubprocInfo tab[TREX_NSUBPROC] = {
+      /* e- e+ > mu- mu+ */ {4, 1, 16, 1, 0, 4.0, {11, -11, 13, -13}, {0, 0, 0}},
+      /* g g > t t~      */ {4, 2, 16, 8, 2, 4.0 * 64.0, {21, 21, 6, -6}, {0, 0, 0}},
+      /* g g > t t~ g    */ {5, 6, 32, 16, 3, 4.0 * 64.0, {21, 21, 6, -6, 21}, {0, 0, 0}},
+      /* g g > t t~ g g  */ {6, 24, 64, 32, 4, 4.0 * 64.0 * 2.0, {21, 21, 6, -6, 21, 21}, {0, 0, 0}},
+      /* g g > t t~ g g g*/ {7, 120, 128, 64, 5, 4.0 * 64.0 * 6.0, {21, 21, 6, -6, 21, 21, 21}, {0, 0, 0}},
+      /* u u~ > t t~ g   */ {5, 4, 32, 16, 3, 4.0 * 9.0, {2, -2, 6, -6, 21}, {1, 0, 4}},
+      /* d d~ > t t~ g   */ {5, 4, 32, 16, 3, 4.0 * 9.0, {1, -1, 6, -6, 21}, {1, 0, 4}},
+      /* u g > t t~ u    */ {5, 4, 32, 16, 3, 4.0 * 24.0, {2, 21, 6, -6, 2}, {4, 0, 1}},
+      /* g u~ > t t~ u~  */ {5, 4, 32, 16, 3, 4.0 * 24.0, {21, -2, 6, -6, -2}, {1, 4, 0}},
+  };
+  return (sid >= 0 && sid < TREX_NSUBPROC) ? &tab[sid] : nullptr;
+}
+
+// returns false if theta is unusable (negative couplings, non-positive scale)
+inline bool make_theta_pair(int sid, const double* th_old, const double* th_new, ThetaPair& T) {
+  const SubprocInfo* sp = subproc_info(sid);
+  if (!sp) return false;
+  const double pi = 3.14159265358979323846;
+  for (int k = 0; k < 2; ++k) {
+    const double* th = k == 0 ? th_old : th_new;
+    const double as = th[TREX_TH_ALPHA_S], aem = th[TREX_TH_ALPHA_EM];
+    if (sid == TREX_SP_EEMUMU) {
+      const double sw2 = th[TREX_TH_SIN2W];
+      if (!(aem >= 0.0) || !(sw2 > 0.0) || !(sw2 < 1.0)) return false;
+      const double e2 = 4.0 * pi * aem, e = std::sqrt(e2), sc = std::sqrt(sw2 * (1.0 - sw2));
+      T.e2[k] = e2; T.gL[k] = e / sc * (-0.5 + sw2); T.gR[k] = e / sc * sw2;
+      T.mZ2[k] = th[TREX_TH_MZ] * th[TREX_TH_MZ]; T.mZGZ[k] = th[TREX_TH_MZ] * th[TREX_TH_GAMMAZ];
+      T.mt[k] = T.mGt[k] = T.kq[k] = 0.0;
+      T.pref[k] = 1.0 / sp->navg;
+    } else {
+      if (!(as >= 0.0) || !(th[TREX_TH_LAMBDA] > 0.0)) return false;
+      const double gs = std::sqrt(4.0 * pi * as);
+      const double kappa = th[TREX_TH_CTG] * th[TREX_TH_VEV] / (std::sqrt(2.0) * th[TREX_TH_LAMBDA] * th[TREX_TH_LAMBDA]);
+      T.mt[k] = th[TREX_TH_MT]; T.mGt[k] = th[TREX_TH_MT] * th[TREX_TH_GAMMAT];
+      T.kq[k] = gs > 0.0 ? kappa / gs : 0.0;      // alpha_s = 0: pref = 0, so |M|^2 = 0 exactly (zero guard applies)
+      T.pref[k] = std::pow(gs, 2 * sp->nvert) / sp->navg;
+      T.e2[k] = T.gL[k] = T.gR[k] = T.mZ2[k] = T.mZGZ[k] = 0.0;
+    }
+  }
+  return true;
+}
+
+}  // namespace trex

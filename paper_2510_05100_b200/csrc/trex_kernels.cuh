@@ -1,0 +1,70 @@
+// trex_kernels.cuh -- launch geometry shared by every |M|^2 kernel.
+//
+// A block is 32 consecutive events (one per lane, so every momentum component is one coalesced 256-byte row read per
+// warp) times WARPS warps; the warps split the helicity units of those events between them, each thread accumulating
+// its units' J^dagger C J for theta_old and theta_new. A fixed-order shared-memory reduction over the warps and the
+// epilogue (normalisation, zero guard, ratio) finish inside the same launch: one launch per
+// trex_reweight call, deterministic results.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "trex_proc.cuh"
+
+namespace trex {
+
+constexpr int WARPS = 8;
+
+struct ReweightArgs {
+  const double* mom; long n; long ld;   // ld = row stride of the SoA block (== n for a caller-provided block)
+  const double* w_in; double* w_out; double* me2_old; double* me2_new;
+  const double* C120;
+  ThetaPair T;
+  QLineLegs q;
+};
+
+// fixed-order reduction over the warps of a block + epilogue by warp 0
+template <class RC> __device__ __forceinline__ void reduce_and_finish(const ReweightArgs& a, RC acc0, RC acc1, long e) {
+  __shared__ double red[2][WARPS][32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  red[0][warp][lane] = (double)acc0; red[1][warp][lane] = (double)acc1;
+  __syncthreads();
+  if (warp == 0 && e < a.n) {
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
+    const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
+    const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
+    a.w_out[e] = a.w_in[e] * norm * mn;                        // evaluate + append_wgts
+    if (a.me2_old) a.me2_old[e] = mo;
+    if (a.me2_new) a.me2_new[e] = mn;
+  }
+}
+
+template <class R, class RC, int N, int NPASS>
+__global__ void __launch_bounds__(WARPS * 32) k_ttng(const ReweightArgs a) {
+  constexpr int NU = 1 << (N + 1);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long e = (long)blockIdx.x * 32 + lane;
+  const long ev = e < a.n ? e : a.n - 1;
+  RC acc[2] = {RC(0), RC(0)};
+  for (int u = warp; u < NU; u += WARPS) {
+    RC out[2];
+    ttng_unit<R, RC, N, NPASS>(a.mom, a.ld, ev, u >> 1, (u & 1) ? 1 : -1, a.T, a.C120, out);
+    acc[0] += out[0]; acc[1] += out[1];
+  }
+  reduce_and_finish<RC>(a, acc[0], acc[1], e);
+}
+
+// one translation unit per (N, precision mode): trex_ttng_tu.cu compiled with -DTREX_TU_N=.. -DTREX_TU_MODE=..
+using TtngLaunchFn = int (*)(const ReweightArgs&, int npass, unsigned grid, cudaStream_t stream);
+using TtngUploadFn = int (*)(const double* C, int count);
+#define TREX_TU_DECL(N, M)                                                                   \
+  int trex_tu_launch_n##N##_m##M(const ReweightArgs&, int npass, unsigned grid, cudaStream_t); \
+  int trex_tu_upload_n##N##_m##M(const double* C, int count);
+TREX_TU_DECL(2, 0) TREX_TU_DECL(2, 1) TREX_TU_DECL(2, 2)
+TREX_TU_DECL(3, 0) TREX_TU_DECL(3, 1) TREX_TU_DECL(3, 2)
+TREX_TU_DECL(4, 0) TREX_TU_DECL(4, 1) TREX_TU_DECL(4, 2)
+TREX_TU_DECL(5, 0) TREX_TU_DECL(5, 1) TREX_TU_DECL(5, 2)
+#undef TREX_TU_DECL
+
+}  // namespace trex

@@ -1,0 +1,38 @@
+// trex_probe.cu -- FP64 / FP32 FMA-pipe microbenchmark used as the roofline denominator of the |M|^2 kernels
+// (MEASURED_PEAKS.json has no FP64 entry, so the peak is measured on the box in the same run).
+// Every thread runs 8 independent register chains of fused multiply-adds; 2 flop per FMA.
+#include "trex_ctx.h"
+
+namespace trex {
+namespace {
+
+template <class R> __global__ void __launch_bounds__(256) k_fma_probe(R* out, int iters, R a, R b) {
+  R x0 = R(threadIdx.x), x1 = x0 + R(1), x2 = x0 + R(2), x3 = x0 + R(3), x4 = x0 + R(4), x5 = x0 + R(5), x6 = x0 + R(6), x7 = x0 + R(7);
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  R s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (s == R(-12345.678)) out[0] = s;     // never true: keeps the chains alive
+}
+
+}  // namespace
+}  // namespace trex
+
+using namespace trex;
+
+// Enqueues one probe launch on the library stream and returns the number of floating-point operations it executes
+// (time it with events on that stream). fp32 != 0 selects the FP32 pipe. Returns < 0 on error.
+extern "C" double trex_probe_fma(int fp32, int blocks, int iters) {
+  Context& c = ctx();
+  if (blocks <= 0 || iters <= 0) return (double)fail(TREX_EINVAL, "trex_probe_fma: blocks and iters must be positive");
+  if (!c.probe_out && cudaMalloc(&c.probe_out, 64) != cudaSuccess) return (double)fail(TREX_ENOMEM, "trex_probe_fma: cudaMalloc failed");
+  if (fp32) k_fma_probe<float><<<blocks, 256, 0, c.stream>>>((float*)c.probe_out, iters, 0.999f, 0.001f);
+  else k_fma_probe<double><<<blocks, 256, 0, c.stream>>>((double*)c.probe_out, iters, 0.999, 0.001);
+  c.launches += 1;
+  if (cudaGetLastError() != cudaSuccess) return (double)fail(TREX_ECUDA, "trex_probe_fma: launch failed");
+  return 2.0 * 64.0 * (double)iters * 256.0 * (double)blocks;
+}

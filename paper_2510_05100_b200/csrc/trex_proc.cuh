@@ -1,0 +1,306 @@
+// trex_proc.cuh -- per-thread evaluation of one helicity "unit" of one event for every compiled-in subprocess
+// (SURVEY.md 8(a) a6-a8): external wavefunctions, colour-flow amplitudes, colour sum J^dagger C J.
+//
+// A unit fixes the helicities of every leg except the antitop (gluons / light quarks and the top); both antitop
+// helicities are closed inside the unit because they only differ in the final contraction with v(p_tbar, lambda).
+// All functions return sum over the unit's helicities of  x^dagger C x  for theta_old and theta_new at g_s = 1;
+// the caller multiplies by g_s^(2 n_vertices) / N_avg.
+#pragma once
+#include "trex_ttng.cuh"
+
+namespace trex {
+
+// ---------------------------------------------------------------- per-call parameters (uniform over the grid)
+struct ThetaPair {           // index 0 = theta_old, 1 = theta_new
+  double mt[2], mGt[2];      // top mass, m_t * Gamma_t
+  double kq[2];              // kappa / g_s
+  double pref[2];            // g_s^(2 nv) / N_avg
+  // electroweak (e- e+ -> mu- mu+)
+  double e2[2], gL[2], gR[2], mZ2[2], mZGZ[2];
+};
+
+// ---------------------------------------------------------------- colour matrices
+// t t~ + n gluons: C_{sigma sigma'} = sum_a tr(T^{a_s1}..T^{a_sn} T^{a_s'n}..T^{a_s'1}), built by the host at first use
+// (trex_colour.h: Fierz reduction in exact rational arithmetic). Every translation unit that instantiates the
+// g g -> t t~ + gluons kernel for one N owns one constant-memory table holding that N's matrix (ncol = 2, 6, 24), so
+// that the fully unrolled colour sums read the entries as instruction operands; ncol = 120 lives in global memory.
+#if defined(__CUDACC__)
+static __constant__ double c_Ctab[576];
+#else
+static double c_Ctab[576];
+#endif
+
+template <int NC> TREX_HD double colour_entry(const double* __restrict__ Cg, int i, int j) {
+  if constexpr (NC <= 24) return c_Ctab[i * NC + j];
+  else {
+#if defined(__CUDA_ARCH__)
+    return __ldg(Cg + i * NC + j);
+#else
+    return Cg[i * NC + j];
+#endif
+  }
+}
+
+// x^dagger C x for real symmetric C: sum_j [ C_jj |x_j|^2 + 2 Re(conj(x_j) sum_{i<j} C_ji x_i) ]
+template <class RC, int NC, int STRIDE> TREX_HD RC colour_quadform(const cx<RC>* x, const double* __restrict__ Cg) {
+  RC tot = RC(0);
+  if constexpr (NC <= 24) {
+#pragma unroll
+    for (int j = 0; j < NC; ++j) {
+      cx<RC> t(RC(0), RC(0));
+#pragma unroll
+      for (int i = 0; i < j; ++i) cfma(t, x[i * STRIDE], RC(colour_entry<NC>(Cg, j, i)));
+      cx<RC> xj = x[j * STRIDE];
+      cfma(t, xj, RC(0.5 * colour_entry<NC>(Cg, j, j)));
+      tot += RC(2) * (xj.re * t.re + xj.im * t.im);
+    }
+  } else {
+    // rolled, 4 rows of C at a time so that every x_i loaded from local memory feeds 8 FMAs
+    static_assert(NC % 4 == 0, "ncolor must be a multiple of 4");
+    for (int j0 = 0; j0 < NC; j0 += 4) {
+      cx<RC> t[4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) t[r] = cx<RC>(RC(0), RC(0));
+      for (int i = 0; i < j0; ++i) {
+        cx<RC> xi = x[i * STRIDE];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) cfma(t[r], xi, RC(colour_entry<NC>(Cg, j0 + r, i)));
+      }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+#pragma unroll
+        for (int i = 0; i < r; ++i) cfma(t[r], x[(j0 + i) * STRIDE], RC(colour_entry<NC>(Cg, j0 + r, j0 + i)));
+        cx<RC> xj = x[(j0 + r) * STRIDE];
+        cfma(t[r], xj, RC(0.5 * colour_entry<NC>(Cg, j0 + r, j0 + r)));
+        tot += RC(2) * (xj.re * t[r].re + xj.im * t[r].im);
+      }
+    }
+  }
+  return tot;
+}
+
+// ---------------------------------------------------------------- momenta
+// SoA block [npar][4][n]: component (ipar*4+mu) of event e at (ipar*4+mu)*n + e  (coalesced across a warp)
+template <class R> TREX_HD void load_leg(const double* __restrict__ mom, long n, long e, int leg, R p[4]) {
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) p[mu] = R(mom[(long)(leg * 4 + mu) * n + e]);
+}
+
+#if defined(__CUDACC__)
+__host__ __device__
+#endif
+constexpr int factorial(int n) { return n <= 1 ? 1 : n * factorial(n - 1); }
+
+// ---------------------------------------------------------------- g g -> t t~ + (N-2) g
+// legs: 0,1 incoming gluons; 2 top; 3 antitop; 4.. outgoing gluons. unit = gluon helicity bits (bit g of `gh` for
+// gluon g in the order g1 g2 g3.. ) and the top helicity. x[leaf][v][theta] is stored in precision RC.
+template <class R, class RC, int N, int NPASS> struct TtngLeafStore {
+  static constexpr int NC = factorial(N);
+  cx<RC> x[NC][2][2];
+  spinor<R> v[2];          // v(p_tbar, -), v(p_tbar, +)
+  R kq[2];
+  TREX_HD void operator()(int leaf, const spinor<R>* b0, const spinor<R>* b1) {
+#pragma unroll
+    for (int th = 0; th < 2; ++th) {
+      const int p = NPASS == 2 ? th : 0;
+#pragma unroll
+      for (int iv = 0; iv < 2; ++iv) {
+        cx<R> a0 = row_col(b0[p], v[iv]), a1 = row_col(b1[p], v[iv]);
+        cfma(a0, a1, kq[th]);
+        x[leaf][iv][th] = cx<RC>(RC(a0.re), RC(a0.im));
+      }
+    }
+  }
+};
+
+template <class R, class RC, int N, int NPASS>
+TREX_HD void ttng_unit(const double* __restrict__ mom, long n, long e, int gh, int lam_t, const ThetaPair& T,
+                       const double* __restrict__ Cg, RC out[2]) {
+  constexpr int NC = factorial(N);
+  using Store = TtngLeafStore<R, RC, N, NPASS>;
+  Store st;
+  TTNG<R, N, NPASS, Store> t;
+#pragma unroll
+  for (int g = 0; g < N; ++g) {
+    const int leg = g < 2 ? g : g + 2;
+    R p[4]; load_leg<R>(mom, n, e, leg, p);
+    const int lam = ((gh >> g) & 1) ? +1 : -1;
+    const bool incoming = g < 2;
+    t.eps[g] = polvec<R>(p, lam, !incoming);
+    const R sg = incoming ? R(1) : R(-1);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) t.K[g].c[mu] = sg * p[mu];
+  }
+  {
+    R p[4]; load_leg<R>(mom, n, e, 2, p);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) t.pt.c[mu] = p[mu];
+    t.ubar_t = bar(spinor_u<R>(p, lam_t, false));
+    R q[4]; load_leg<R>(mom, n, e, 3, q);
+    st.v[0] = spinor_v<R>(q, -1, false);
+    st.v[1] = spinor_v<R>(q, +1, false);
+  }
+#pragma unroll
+  for (int p = 0; p < NPASS; ++p) { t.line[p].mt = R(T.mt[p]); t.line[p].mGt = R(T.mGt[p]); }
+  st.kq[0] = R(T.kq[0]); st.kq[1] = R(T.kq[1]);
+  t.run(&st);
+#pragma unroll
+  for (int th = 0; th < 2; ++th) {
+    RC s = RC(0);
+#pragma unroll
+    for (int iv = 0; iv < 2; ++iv) s += colour_quadform<RC, NC, 4>(&st.x[0][iv][th], Cg);
+    out[th] = s;
+  }
+}
+
+// ---------------------------------------------------------------- one light-quark line + t t~ + one gluon
+// (q q~ -> t t~ g, q g -> t t~ q, g q~ -> t t~ q~; R-8). The light line (row spinor w at leg lrow, column
+// spinor x at leg lcol) acts on the top line as a second gluon source; with the Fierz identity the five SM diagrams
+// (+ dipole / contact insertions) reduce to four colour flows
+//   c1 = T^a_{i1 j3} d_{i4 j2}, c2 = d_{i1 j3} T^a_{i4 j2}, c3 = T^a_{i1 j2} d_{i4 j3}, c4 = d_{i1 j2} T^a_{i4 j3}
+//   J1 = (A(g,Q) + K4)/2, J2 = (A(Q,g) + K3)/2, J3 = -(A(g,Q) + A(Q,g))/6, J4 = -(K3 + K4)/6
+// where A(.,.) are the two orderings of (gluon, quark-pair current) on the top line and K3 / K4 attach the current
+// of the light line that has radiated the gluon at its row / column end. C = [[12,0,4,4],[0,12,4,4],[4,4,12,0],[4,4,0,12]].
+struct QLineLegs { int lrow, lcol, lg; };   // leg numbers; legs 0,1 are incoming
+
+template <class R> struct QqLeafStore {
+  cx<R> a0[2][2], a1[2][2];   // [leaf][v]
+  spinor<R> v[2];
+  TREX_HD void operator()(int leaf, const spinor<R>* b0, const spinor<R>* b1) {
+#pragma unroll
+    for (int iv = 0; iv < 2; ++iv) { a0[leaf][iv] = row_col(b0[0], v[iv]); a1[leaf][iv] = row_col(b1[0], v[iv]); }
+  }
+};
+
+// unit = (lam_row, lam_col, lam_g, lam_t) packed in 4 bits of `u` (bit0 row, bit1 col, bit2 gluon, bit3 top)
+template <class R, class RC>
+TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L, int u, const ThetaPair& T, RC out[2]) {
+  const int lam_row = (u & 1) ? 1 : -1, lam_col = (u & 2) ? 1 : -1, lam_g = (u & 4) ? 1 : -1, lam_t = (u & 8) ? 1 : -1;
+  R pr[4], pc[4], pg[4], pt[4], ptb[4];
+  load_leg<R>(mom, n, e, L.lrow, pr); load_leg<R>(mom, n, e, L.lcol, pc); load_leg<R>(mom, n, e, L.lg, pg);
+  load_leg<R>(mom, n, e, 2, pt); load_leg<R>(mom, n, e, 3, ptb);
+  const bool row_in = L.lrow < 2, col_in = L.lcol < 2, g_in = L.lg < 2;
+  // light line ends: row = vbar (incoming antiquark) or ubar (outgoing quark); column = u (incoming) or v (outgoing)
+  spinor<R> w = row_in ? bar(spinor_v<R>(pr, lam_row, true)) : bar(spinor_u<R>(pr, lam_row, true));
+  spinor<R> x = col_in ? spinor_u<R>(pc, lam_col, true) : spinor_v<R>(pc, lam_col, true);
+  rvec4<R> Kr, Kc, Kg, Kq;
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) {
+    Kr.c[mu] = row_in ? pr[mu] : -pr[mu]; Kc.c[mu] = col_in ? pc[mu] : -pc[mu]; Kg.c[mu] = g_in ? pg[mu] : -pg[mu];
+    Kq.c[mu] = Kr.c[mu] + Kc.c[mu];
+  }
+  vec4<R> eg = polvec<R>(pg, lam_g, !g_in);
+  // quark-pair current  Jq = (w gamma^mu x) / Kq^2        [ (i g_s) * (-i / Kq^2) at g_s = 1 ]
+  vec4<R> Jq = bilinear(w, x);
+  { R s = R(1) / rdot(Kq, Kq);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) Jq.c[i] = Jq.c[i] * s; }
+  // light line after radiating the gluon: W = w (i eslash)(i qslash)/q^2, q = -(Kr + Kg);  X = (i qslash)(i eslash) x / q^2, q = Kc + Kg
+  rvec4<R> Ptot = radd(Kq, Kg);
+  R iP2 = R(1) / rdot(Ptot, Ptot);
+  vec4<R> Jq3, Jq4;
+  { rvec4<R> q; for (int mu = 0; mu < 4; ++mu) q.c[mu] = -(Kr.c[mu] + Kg.c[mu]);
+    spinor<R> W = row_slash(row_slash(w, eg), q);
+    R s = -iP2 / rdot(q, q);
+    Jq3 = bilinear(W, x);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) Jq3.c[i] = Jq3.c[i] * s; }
+  { rvec4<R> q = radd(Kc, Kg);
+    spinor<R> X = slash_col(q, slash_col(eg, x));
+    R s = -iP2 / rdot(q, q);
+    Jq4 = bilinear(w, X);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) Jq4.c[i] = Jq4.c[i] * s; }
+
+  QqLeafStore<R> st;
+  st.v[0] = spinor_v<R>(ptb, -1, false); st.v[1] = spinor_v<R>(ptb, +1, false);
+  spinor<R> ubar_t = bar(spinor_u<R>(pt, lam_t, false));
+  // two-source ordered amplitudes: source 0 = gluon, source 1 = quark-pair current
+  TTNG<R, 2, 1, QqLeafStore<R>> t;
+  t.K[0] = Kg; t.eps[0] = eg; t.K[1] = Kq; t.eps[1] = Jq;
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) t.pt.c[mu] = pt[mu];
+  t.ubar_t = ubar_t;
+  // top mass/width may differ between theta_old and theta_new: evaluate per theta when they do
+  RC res[2];
+  const bool same_line = (T.mt[0] == T.mt[1]) && (T.mGt[0] == T.mGt[1]);
+  cx<R> A12[2][2], A21[2][2];   // [order][v]
+  for (int th = 0; th < 2; ++th) {
+    if (th == 0 || !same_line) {
+      t.line[0].mt = R(T.mt[th]); t.line[0].mGt = R(T.mGt[th]);
+      t.run(&st);
+#pragma unroll
+      for (int iv = 0; iv < 2; ++iv) { A12[0][iv] = st.a0[0][iv]; A12[1][iv] = st.a1[0][iv]; A21[0][iv] = st.a0[1][iv]; A21[1][iv] = st.a1[1][iv]; }
+    }
+    // single-source amplitudes K3, K4: ubar_t [ i Jslash + (kappa/g_s) 2 sigma(P ^ J) ] v
+    RC s = RC(0);
+#pragma unroll
+    for (int iv = 0; iv < 2; ++iv) {
+      cx<R> k3, k4;
+      {
+        spinor<R> b0 = row_slash(ubar_t, Jq3), b1 = szero<R>();
+        ften<R> F = fzero<R>(); wedge_acc(F, Ptot, Jq3); row_sigma_acc(b1, ubar_t, F);
+        cx<R> a0 = mul_i(row_col(b0, st.v[iv])); cfma(a0, row_col(b1, st.v[iv]), R(T.kq[th])); k3 = a0;
+      }
+      {
+        spinor<R> b0 = row_slash(ubar_t, Jq4), b1 = szero<R>();
+        ften<R> F = fzero<R>(); wedge_acc(F, Ptot, Jq4); row_sigma_acc(b1, ubar_t, F);
+        cx<R> a0 = mul_i(row_col(b0, st.v[iv])); cfma(a0, row_col(b1, st.v[iv]), R(T.kq[th])); k4 = a0;
+      }
+      cx<R> a12 = A12[0][iv]; cfma(a12, A12[1][iv], R(T.kq[th]));
+      cx<R> a21 = A21[0][iv]; cfma(a21, A21[1][iv], R(T.kq[th]));
+      cx<R> j1 = R(0.5) * (a12 + k4), j2 = R(0.5) * (a21 + k3);
+      cx<R> j3 = R(-1.0 / 6.0) * (a12 + a21), j4 = R(-1.0 / 6.0) * (k3 + k4);
+      cx<RC> J[4] = {cx<RC>(RC(j1.re), RC(j1.im)), cx<RC>(RC(j2.re), RC(j2.im)), cx<RC>(RC(j3.re), RC(j3.im)), cx<RC>(RC(j4.re), RC(j4.im))};
+      // J^dagger C J with C = 12 on the diagonal, 4 between {1,2} and {3,4}, 0 inside the pairs
+      RC d = RC(12) * (norm2(J[0]) + norm2(J[1]) + norm2(J[2]) + norm2(J[3]));
+      cx<RC> a = J[0] + J[1], b = J[2] + J[3];
+      d += RC(8) * (a.re * b.re + a.im * b.im);
+      s += d;
+    }
+    res[th] = s;
+  }
+  out[0] = res[0]; out[1] = res[1];
+}
+
+// ---------------------------------------------------------------- e- e+ -> mu- mu+ (photon + Z), all 16 helicities
+// M = i [ e^2 (Je.Jm)/s + (gL JeL + gR JeR).(gL JmL + gR JmR)/(s - mZ^2 + i mZ GZ) ], J^mu_{L,R} = wbar gamma^mu P_{L,R} x.
+// The four chiral current products d_ab = Je_a . Jm_b do not depend on theta: evaluated once, closed with both
+// coupling sets.
+template <class R>
+TREX_HD void eemumu_event(const double* __restrict__ mom, long n, long e, const ThetaPair& T, R out[2]) {
+  R p0[4], p1[4], p2[4], p3[4];
+  load_leg<R>(mom, n, e, 0, p0); load_leg<R>(mom, n, e, 1, p1); load_leg<R>(mom, n, e, 2, p2); load_leg<R>(mom, n, e, 3, p3);
+  R q[4]; for (int mu = 0; mu < 4; ++mu) q[mu] = p0[mu] + p1[mu];
+  const R s = q[0] * q[0] - q[1] * q[1] - q[2] * q[2] - q[3] * q[3];
+  cx<R> propZ[2]; R propA[2];
+  for (int th = 0; th < 2; ++th) {
+    propA[th] = R(T.e2[th]) / s;
+    propZ[th] = cdiv(cx<R>(1, 0), cx<R>(s - R(T.mZ2[th]), R(T.mZGZ[th])));
+  }
+  R sum[2] = {R(0), R(0)};
+  for (int h = 0; h < 16; ++h) {
+    spinor<R> u1 = spinor_u<R>(p0, (h & 1) ? 1 : -1, true);
+    spinor<R> vb2 = bar(spinor_v<R>(p1, (h & 2) ? 1 : -1, true));
+    spinor<R> ub3 = bar(spinor_u<R>(p2, (h & 4) ? 1 : -1, true));
+    spinor<R> v4 = spinor_v<R>(p3, (h & 8) ? 1 : -1, true);
+    // P_L keeps the upper two components in the chiral basis, P_R the lower two
+    spinor<R> uL = u1, uR = u1, vL = v4, vR = v4;
+    uL.c[2] = uL.c[3] = cx<R>(0, 0); uR.c[0] = uR.c[1] = cx<R>(0, 0);
+    vL.c[2] = vL.c[3] = cx<R>(0, 0); vR.c[0] = vR.c[1] = cx<R>(0, 0);
+    vec4<R> Je[2] = {bilinear(vb2, uL), bilinear(vb2, uR)};
+    vec4<R> Jm[2] = {bilinear(ub3, vL), bilinear(ub3, vR)};
+    cx<R> d[2][2];
+    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) d[a][b] = dot(Je[a], Jm[b]);
+    for (int th = 0; th < 2; ++th) {
+      const R g[2] = {R(T.gL[th]), R(T.gR[th])};
+      cx<R> za(0, 0), ga(0, 0);
+      for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) { ga += d[a][b]; cfma(za, d[a][b], g[a] * g[b]); }
+      cx<R> M = ga * propA[th] + za * propZ[th];
+      sum[th] += norm2(M);
+    }
+  }
+  out[0] = sum[0]; out[1] = sum[1];
+}
+
+}  // namespace trex

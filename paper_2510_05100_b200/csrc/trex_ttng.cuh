@@ -1,6 +1,7 @@
 // trex_ttng.cuh -- colour-flow amplitudes of a heavy quark line with N ordered gluon "sources".
 //
-// One thread evaluates ONE helicity configuration of ONE event. For every ordering sigma of the N sources it forms
+// One thread evaluates ONE gluon-helicity / top-helicity configuration of ONE event. For every ordering sigma of the
+// N sources it forms
 //   A_sigma = sum over all colour-ordered Feynman diagrams of that ordering,
 // by walking the tree of ordering prefixes depth first. At prefix (s_1..s_M) the thread holds
 //   J[a][M]  = off-shell gluon current of the contiguous tuple (s_{a+1}..s_M)     (VVV + VVVV vertices, propagator)
@@ -9,7 +10,8 @@
 // Only the current prefix path is alive (N(N+1)/2 currents, N line states): a few hundred doubles per thread instead
 // of the O(N!) table a memoised recursion needs. p = 0..NPASS-1 indexes parameter points whose top mass / width
 // differ (theta_old, theta_new): the gluon currents are shared between them.
-// g_s is factored out: A = g_s^N (A0 + (kappa/g_s) A1); this file computes A0 and A1 at g_s = 1.
+// g_s is factored out: A = g_s^N (A0 + (kappa/g_s) A1); this file computes the open brackets b0, b1 (row spinors, to
+// be contracted with v(p_tbar, lambda)) at g_s = 1 and hands them to a sink, leaves in lexicographic order of sigma.
 #pragma once
 #include "trex_math.cuh"
 
@@ -19,13 +21,12 @@ template <class R> struct TopLine {      // per parameter point
   R mt, mGt;                             // m_t and m_t * Gamma_t
 };
 
-// Sink: called once per ordering, in lexicographic order of sigma, with the leaf index.
 template <class R, int N, int NPASS, class Sink> struct TTNG {
   // inputs (thread-private copies; dynamically indexed by the source number, so they live in local memory)
   rvec4<R> K[N];            // incoming-convention momentum of each source
   vec4<R> eps[N];           // its polarisation / effective current
   rvec4<R> pt;              // top momentum (outgoing)
-  spinor<R> ubar_t, v_tb;   // ubar(p_t), v(p_tbar)
+  spinor<R> ubar_t;         // ubar(p_t, lambda_t)
   TopLine<R> line[NPASS];
   // path state
   vec4<R> J[N][N + 1];      // J[a][m], a < m
@@ -50,6 +51,7 @@ template <class R, int N, int NPASS, class Sink> struct TTNG {
         for (int c1 = a + 1; c1 < M; ++c1)
 #pragma unroll
           for (int c2 = c1 + 1; c2 < M; ++c2) v4_acc(acc, J[a][c1], J[c1][c2], J[c2][M]);
+        // (-i/P^2) * [(-i)V3 + (-i)V4] = -(V3 + V4)/P^2 at g_s = 1
         R s = R(-1) / rdot(P[a][M], P[a][M]);
 #pragma unroll
         for (int i = 0; i < 4; ++i) J[a][M].c[i] = acc.c[i] * s;
@@ -96,10 +98,7 @@ template <class R, int N, int NPASS, class Sink> struct TTNG {
         }
         level<(M < N ? M + 1 : N)>(used | (1u << g));
       } else {
-        cx<R> A0[NPASS], A1[NPASS];
-#pragma unroll
-        for (int p = 0; p < NPASS; ++p) { A0[p] = row_col(b0[p], v_tb); A1[p] = row_col(b1[p], v_tb); }
-        (*sink)(leaf, A0, A1);
+        (*sink)(leaf, b0, b1);
         ++leaf;
       }
     }

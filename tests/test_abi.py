@@ -1,0 +1,107 @@
+"""The C-ABI library builds, loads, and exports every symbol include/rex_trex.h declares (no compute calls: no GPU here).
+Host-only entry points (keys, registry, colour matrices) are exercised against independent expectations."""
+import ctypes
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2510_05100_b200 as T
+from paper_2510_05100_b200 import build as B
+from trex_inputs import SUBPROCESSES, pack_key
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    B.build()
+    return T.lib()
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "rex_trex.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b((?:rex|trex)_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported_and_bound(lib):
+    names = declared_functions()
+    assert len(names) >= 20
+    for name in names:
+        assert hasattr(lib, name), name
+    assert set(names) == set(T.exported_symbols())
+
+
+def test_no_torch_types_in_signatures():
+    text = open(os.path.join(ROOT, "include", "rex_trex.h")).read()
+    assert "torch" not in text and "at::" not in text and 'extern "C"' in text
+
+
+def test_pack_key_matches_input_generator_and_alg1_semantics(lib):
+    for sp in SUBPROCESSES:
+        assert T.rex_pack_key(sp.pdg, sp.status) == int(pack_key(sp.pdg, sp.status))
+        assert T.trex_subproc_id(int(sp.key)) == sp.sid
+        assert T.trex_npar(sp.sid) == sp.npar
+    # unordered legs, initial and final state kept apart (Alg.1 :419-444)
+    a = T.rex_pack_key([21, 2, 6, -6, 2], [-1, -1, 1, 1, 1])
+    b = T.rex_pack_key([2, 21, 2, -6, 6], [-1, -1, 1, 1, 1])
+    assert a == b
+    assert T.rex_pack_key([21, 21, 6, -6], [-1, -1, 1, 1]) != T.rex_pack_key([2, -2, 6, -6], [-1, -1, 1, 1])
+    assert T.rex_pack_key([21, 6, 21, -6], [-1, -1, 1, 1]) != T.rex_pack_key([21, 21, 6, -6], [-1, -1, 1, 1])
+    # intermediate (status 2) legs are ignored; too many legs / unknown codes give REX_NPOS
+    assert T.rex_pack_key([21, 21, 23, 6, -6], [-1, -1, 2, 1, 1]) == T.rex_pack_key([21, 21, 6, -6], [-1, -1, 1, 1])
+    assert T.rex_pack_key([1] * 8, [-1, -1, 1, 1, 1, 1, 1, 1]) == T.REX_NPOS
+    assert T.rex_pack_key([1000022, 21, 6, -6], [-1, -1, 1, 1]) == T.REX_NPOS
+    assert T.trex_subproc_id(T.REX_NPOS) == -2 and T.trex_npar(99) == -2
+
+
+def test_registry_counts_match_baseline_configs(lib):
+    # BASELINE.json configs: ncolor 2 / 6 / 24 / 120 and 16 / 32 / 64 / 128 helicities for g g > t t~ + 0..3 g
+    for sid, nc, nh in [(0, 1, 16), (1, 2, 16), (2, 6, 32), (3, 24, 64), (4, 120, 128), (5, 4, 32), (7, 4, 32), (8, 4, 32)]:
+        assert T.trex_ncolor(sid) == nc and T.trex_nhel(sid) == nh
+
+
+def test_colour_matrices_against_group_theory(lib):
+    """Independent of the oracle: values quoted in tests/golden/colour_matrices.txt and SU(3) sum rules."""
+    c2 = T.trex_colour_matrix(1)
+    assert np.allclose(c2 * 3, [[16, -2], [-2, 16]], atol=1e-12)
+    c6 = T.trex_colour_matrix(2)
+    assert np.allclose(c6[0] * 9, [64, -8, -8, 1, 1, 10], atol=1e-12)
+    c24 = T.trex_colour_matrix(3)
+    k = np.round(c24 * 54).astype(int)
+    assert np.allclose(c24 * 54, k, atol=1e-9) and set(np.unique(k)) == {512, 80, 71, 62, 8, -1, -10, -28, -64}
+    c120 = T.trex_colour_matrix(4)
+    k = np.round(c120 * 324).astype(int)
+    assert np.allclose(c120 * 324, k, atol=1e-8) and k[0, 0] == 4096 and len(np.unique(k)) == 24
+    for n, c in ((2, c2), (3, c6), (4, c24), (5, c120)):
+        assert np.allclose(c, c.T) and np.all(np.linalg.eigvalsh(c) > 0)
+        # diagonal = C_F^n N ; each row sums to the same value (the matrix is a group convolution)
+        assert np.allclose(np.diag(c), (4.0 / 3.0) ** n * 3)
+        assert np.allclose(c.sum(axis=1), c.sum(axis=1)[0])
+        assert c.shape == (math.factorial(n),) * 2
+    cq = T.trex_colour_matrix(5)
+    assert np.array_equal(cq, [[12, 0, 4, 4], [0, 12, 4, 4], [4, 4, 12, 0], [4, 4, 0, 12]])
+
+
+def test_compute_calls_fail_loudly_without_gpu(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(T.TrexError):
+        T.trex_reweight(1, None, np.zeros(16), np.zeros(16), None)
+
+
+def test_argument_errors_do_not_crash(lib):
+    th = (ctypes.c_double * 16)()
+    assert lib.trex_reweight(99, None, 4, th, th, None, None, None, None) == -2
+    assert lib.trex_reweight(1, None, -1, th, th, None, None, None, None) == -1
+    assert lib.trex_reweight(1, None, 4, th, th, None, None, None, None) == -1
+    assert b"null" in lib.trex_last_error()
+    assert lib.trex_reweight(1, None, 0, th, th, None, None, None, None) == 0      # n == 0 is a no-op
+    assert lib.trex_set_precision(7) == -1 and lib.trex_set_precision(0) == 0
+    off = (ctypes.c_int64 * 257)()
+    assert lib.rex_bucket(None, 0, None, off) == 0 and off[0] == 0
+    assert lib.rex_bucket(None, 5, None, off) == -1

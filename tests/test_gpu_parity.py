@@ -1,0 +1,264 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs (-m gpu).
+
+Tolerances (BASELINE.json north_star): bucketing / permutations bit-exact; per-event |M|^2 and weight ratios within a
+relative 1e-11 in fp64; fp32 / mixed modes median 5e-5, maximum 1e-3."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from trex_inputs import make_config, default_theta, SUBPROCESSES, REX_NPOS, TH_CTG, TH_GAMMAT, TH_ALPHA_S
+
+pytestmark = pytest.mark.gpu
+
+RTOL64 = 1e-11
+
+
+@pytest.fixture(scope="module")
+def T():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2510_05100_b200 as T
+    T.lib()                                   # raises if the CUDA library is not built: no fallback
+    T.trex_set_stream(None)
+    T.trex_set_precision(0)
+    return T
+
+
+def dev(a):
+    import torch
+    a = np.ascontiguousarray(a)
+    if a.dtype == np.uint64:
+        a = a.view(np.int64)
+    return torch.from_numpy(a).cuda()
+
+
+def rel(a, b):
+    return np.abs(a - b) / np.abs(b)
+
+
+def gpu_reweight(T, sid, mom, tho, thn, w):
+    wo, mo, mn = T.trex_reweight(sid, dev(mom), tho, thn, dev(w))
+    import torch
+    torch.cuda.synchronize()
+    return wo.cpu().numpy(), mo.cpu().numpy(), mn.cpu().numpy()
+
+
+# ---------------------------------------------------------------- bucketing (bit-exact)
+def _check_bucket(T, keys):
+    perm, offsets, bkeys = T.rex_bucket(dev(keys))
+    rperm, roff, rkeys = O.bucket(keys)
+    assert np.array_equal(offsets, roff)
+    assert np.array_equal(bkeys, rkeys)
+    assert np.array_equal(perm.cpu().numpy(), rperm)
+
+
+@pytest.mark.parametrize("n", [1, 2, 31, 32, 33, 1000, 1024, 1025, 40000, 300001])
+def test_bucket_random_keys_bit_exact(T, n):
+    rng = np.random.default_rng(n)
+    pool = np.array([int(sp.key) for sp in SUBPROCESSES] + [int(REX_NPOS), 12345, 2**63 + 17], dtype=np.uint64)
+    p = rng.random(len(pool)) ** 3
+    keys = pool[rng.choice(len(pool), size=n, p=p / p.sum())]
+    _check_bucket(T, keys)
+
+
+def test_bucket_edge_cases(T):
+    _check_bucket(T, np.full(5000, REX_NPOS, dtype=np.uint64))                 # only the "no class" bucket
+    _check_bucket(T, np.full(70000, 7, dtype=np.uint64))                       # one class
+    rng = np.random.default_rng(3)
+    keys = rng.integers(1, 2**62, size=256, dtype=np.uint64)                   # REX_MAX_BUCKETS distinct keys
+    _check_bucket(T, keys[rng.integers(0, 256, size=100000)])
+    keys65 = rng.integers(1, 2**62, size=65, dtype=np.uint64)                  # the paper's QCD sample: 65 classes,
+    p = 1.0 / np.arange(1, 66) ** 2                                            # very uneven
+    _check_bucket(T, keys65[rng.choice(65, size=200000, p=p / p.sum())])
+    perm, offsets, bkeys = T.rex_bucket(dev(np.zeros(0, dtype=np.uint64)))     # empty input
+    assert perm.numel() == 0 and list(offsets) == [0] and len(bkeys) == 0
+    with pytest.raises(T.TrexError):                                           # 257 distinct keys
+        T.rex_bucket(dev(np.arange(1, 258, dtype=np.uint64)))
+
+
+def test_bucket_cfg3_full_size_and_transposition(T):
+    import torch
+    w = make_config(3)
+    perm, offsets, bkeys = T.rex_bucket(dev(w.keys))
+    rperm, roff, rkeys = O.bucket(w.keys)
+    assert np.array_equal(offsets, roff) and np.array_equal(bkeys, rkeys)
+    assert np.array_equal(perm.cpu().numpy(), rperm)
+    mom = dev(w.momenta)
+    g = T.rex_gather(mom, perm)
+    assert np.array_equal(g.cpu().numpy(), O.gather(w.momenta, rperm))
+    back = torch.zeros_like(mom)
+    T.rex_scatter(g, perm, back)
+    assert torch.equal(back, mom)
+    # a bucket-local gather (perm + offsets[b]) gives that bucket's SoA block
+    b = 2
+    sub = perm[int(offsets[b]):int(offsets[b + 1])].contiguous()
+    blk = T.rex_gather(mom, sub)
+    assert np.array_equal(blk.cpu().numpy(), w.momenta[:, :, rperm[roff[b]:roff[b + 1]]])
+
+
+# ---------------------------------------------------------------- |M|^2 and weights, element by element
+# (sid, config, events): several 32-event tiles and a ragged tail, sized so the oracle finishes in seconds
+CASES = [(0, 1, 4096), (1, 2, 4133), (2, 3, 677), (3, 4, 101), (4, 5, 37)]
+
+
+@pytest.mark.parametrize("sid,cfg,nev", CASES)
+def test_reweight_matches_oracle(T, sid, cfg, nev):
+    w = make_config(cfg, n=max(nev, 64))
+    mom = np.ascontiguousarray(w.momenta[:, :, :nev])
+    win = w.w_in[:nev]
+    wo, mo, mn = gpu_reweight(T, sid, mom, w.theta_old, w.theta_new, win)
+    rw, ro, rn = O.reweight(sid, mom, w.theta_old, w.theta_new, win)
+    assert rel(mo, ro).max() < RTOL64 and rel(mn, rn).max() < RTOL64, (rel(mo, ro).max(), rel(mn, rn).max())
+    assert rel(wo, rw).max() < RTOL64
+    assert np.all(wo != win)                       # the reweighting really changed something
+
+
+@pytest.mark.parametrize("sid", [5, 6, 7, 8])
+def test_quark_channels_match_explicit_colour_oracle(T, sid):
+    w = make_config(3, n=2048)
+    sel = np.where(w.keys == SUBPROCESSES[sid].key)[0][:37]
+    mom = np.ascontiguousarray(w.momenta[:, :, sel])
+    wo, mo, mn = gpu_reweight(T, sid, mom, w.theta_old, w.theta_new, w.w_in[sel])
+    rw, ro, rn = O.reweight(sid, mom, w.theta_old, w.theta_new, w.w_in[sel])
+    assert rel(mo, ro).max() < RTOL64 and rel(mn, rn).max() < RTOL64 and rel(wo, rw).max() < RTOL64
+
+
+@pytest.mark.parametrize("sid,cfg", [(1, 2), (2, 3), (3, 4)])
+def test_colour_flow_amplitudes_match_oracle(T, sid, cfg):
+    """every J_c of every helicity, both orders in kappa (finer than |M|^2)."""
+    w = make_config(cfg, n=64)
+    th = w.theta_old
+    for e in (0, 5):
+        mom1 = np.ascontiguousarray(w.momenta[:, :, e:e + 1])
+        got = T.trex_debug_flow_amps(sid, mom1[:, :, 0], th)
+        scale = np.abs(got).max(axis=(0, 1))
+        for h in range(T.trex_nhel(sid)):
+            ref = O.ttng_amps(sid, mom1, th, h)
+            assert np.all(np.abs(got[h] - ref) <= 1e-12 * scale), h
+
+
+def test_debug_flow_amps_five_gluons_one_helicity(T):
+    w = make_config(5, n=64)
+    mom1 = np.ascontiguousarray(w.momenta[:, :, 3:4])
+    got = T.trex_debug_flow_amps(4, mom1[:, :, 0], w.theta_old)
+    scale = np.abs(got).max(axis=(0, 1))
+    for h in (0, 77, 127):
+        ref = O.ttng_amps(4, mom1, w.theta_old, h)
+        assert np.all(np.abs(got[h] - ref) <= 1e-12 * scale)
+
+
+# ---------------------------------------------------------------- properties that hold at any size / edge cases
+def test_unit_ratio_zero_guard_and_empty(T):
+    import torch
+    w = make_config(2, n=1000)
+    wo, mo, mn = gpu_reweight(T, 1, w.momenta, w.theta_old, w.theta_old, w.w_in)
+    assert np.array_equal(mo, mn) and np.allclose(wo, w.w_in, rtol=4e-16, atol=0)
+    th0 = w.theta_old.copy()
+    th0[TH_ALPHA_S] = 0.0                                  # me2_old == 0 exactly -> weight 0
+    wo, mo, mn = gpu_reweight(T, 1, w.momenta, th0, w.theta_new, w.w_in)
+    assert np.all(mo == 0) and np.all(wo == 0) and np.all(mn > 0)
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    out = T.trex_reweight(1, torch.empty((4, 4, 0), dtype=torch.float64, device="cuda"), w.theta_old, w.theta_new, e)
+    assert out[0].numel() == 0
+    with pytest.raises(T.TrexError):
+        T.trex_reweight(42, dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    bad = w.theta_old.copy()
+    bad[TH_ALPHA_S] = -1.0
+    with pytest.raises(T.TrexError):
+        T.trex_reweight(1, dev(w.momenta), bad, w.theta_new, dev(w.w_in))
+
+
+def test_me2_exactly_quadratic_in_ctg_on_gpu(T):
+    w = make_config(4, n=96)
+    cs = np.array([0.0, 0.7, 1.9, -2.6, 4.0])
+    vals = []
+    for c in cs:
+        th = default_theta()
+        th[TH_CTG] = c
+        vals.append(gpu_reweight(T, 3, w.momenta, default_theta(), th, w.w_in)[2])
+    vals = np.array(vals)
+    for e in range(vals.shape[1]):
+        coef = np.polyfit(cs, vals[:, e], 4)
+        assert abs(coef[0]) < 1e-10 * abs(vals[0, e]) and abs(coef[1]) < 1e-10 * abs(vals[0, e])
+
+
+FULL = [(1, 0, 64), (2, 1, 64), (4, 3, 24), (5, 4, 6)]
+
+
+@pytest.mark.parametrize("cfg,sid,nsample", FULL)
+def test_full_size_configs_sampled_against_oracle(T, cfg, sid, nsample):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (trex_run on the whole sample)."""
+    import torch
+    w = make_config(cfg)
+    wo, mo, mn, nb = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    torch.cuda.synchronize()
+    wo, mo, mn = wo.cpu().numpy(), mo.cpu().numpy(), mn.cpu().numpy()
+    assert nb == 1 and np.all(np.isfinite(wo)) and np.all(mo > 0) and np.all(mn > 0)
+    rng = np.random.default_rng(100 + cfg)
+    idx = np.sort(rng.choice(w.n, size=nsample, replace=False))
+    idx[-1] = w.n - 1                                                        # the ragged end of the last tile
+    mom = np.ascontiguousarray(w.momenta[:, :, idx])
+    rw, ro, rn = O.reweight(sid, mom, w.theta_old, w.theta_new, w.w_in[idx])
+    assert rel(mo[idx], ro).max() < RTOL64 and rel(mn[idx], rn).max() < RTOL64 and rel(wo[idx], rw).max() < RTOL64
+
+
+def test_cfg3_full_path_bucket_gather_reweight_scatter(T):
+    import torch
+    w = make_config(3)
+    wo, mo, mn, nb = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    torch.cuda.synchronize()
+    wo, mo, mn = wo.cpu().numpy(), mo.cpu().numpy(), mn.cpu().numpy()
+    assert nb == 5 and np.all(np.isfinite(wo)) and np.all(mo > 0)
+    rng = np.random.default_rng(33)
+    for sp in w.classes:
+        cand = np.where(w.keys == sp.key)[0]
+        idx = np.sort(rng.choice(cand, size=24 if sp.sid == 2 else 6, replace=False))
+        mom = np.ascontiguousarray(w.momenta[:, :, idx])
+        rw, ro, rn = O.reweight(sp.sid, mom, w.theta_old, w.theta_new, w.w_in[idx])
+        assert rel(mo[idx], ro).max() < RTOL64 and rel(mn[idx], rn).max() < RTOL64 and rel(wo[idx], rw).max() < RTOL64, sp.name
+
+
+def test_unknown_classes_get_zero_weights(T):
+    """events no procReweightor claims are given zero weights."""
+    import torch
+    w = make_config(3, n=5000)
+    keys = w.keys.copy()
+    keys[::7] = np.uint64(REX_NPOS)
+    keys[3::11] = np.uint64(424242)
+    wo, mo, mn, nb = T.trex_run(dev(keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    torch.cuda.synchronize()
+    wo = wo.cpu().numpy()
+    unknown = (keys == np.uint64(REX_NPOS)) | (keys == np.uint64(424242))
+    assert nb == 7 and np.all(wo[unknown] == 0) and np.all(mo.cpu().numpy()[unknown] == 0) and np.all(wo[~unknown] > 0)
+    ref, _, _, _ = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    assert np.array_equal(ref.cpu().numpy()[~unknown], wo[~unknown])
+
+
+def test_host_buffer_entry_point_matches_device_path(T):
+    import torch
+    w = make_config(3, n=20000)
+    ref, _, _, _ = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    out = np.empty(w.n)
+    mo = np.empty(w.n)
+    nb = T.trex_run_host(w.keys, w.momenta, w.theta_old, w.theta_new, w.w_in, out, mo, None)
+    assert nb == 5 and np.array_equal(out, ref.cpu().numpy()) and np.all(mo > 0)
+
+
+# ---------------------------------------------------------------- reduced-precision modes (PAPER.md:1209 fptype m / f)
+@pytest.mark.parametrize("mode", [1, 2])
+def test_reduced_precision_modes_cfg4(T, mode):
+    w = make_config(4, n=4096)
+    ref_w, ref_o, ref_n = gpu_reweight(T, 3, w.momenta, w.theta_old, w.theta_new, w.w_in)
+    T.trex_set_precision(mode)
+    try:
+        assert T.trex_get_precision() == mode
+        wo, mo, mn = gpu_reweight(T, 3, w.momenta, w.theta_old, w.theta_new, w.w_in)
+    finally:
+        T.trex_set_precision(0)
+    for got, ref in ((wo, ref_w), (mo, ref_o), (mn, ref_n)):
+        r = rel(got, ref)
+        assert np.median(r) < 5e-5 and r.max() < 1e-3, (mode, np.median(r), r.max())
+    # and the fp64 reference itself is oracle-checked on a sample
+    idx = np.arange(0, 4096, 512)
+    rw, ro, rn = O.reweight(3, np.ascontiguousarray(w.momenta[:, :, idx]), w.theta_old, w.theta_new, w.w_in[idx])
+    assert rel(ref_o[idx], ro).max() < RTOL64 and rel(ref_w[idx], rw).max() < RTOL64

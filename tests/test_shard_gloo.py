@@ -1,0 +1,61 @@
+"""N > 1 host logic on CPU: world_size-2 gloo run of the sharding used by bench.py. The data path has
+no collective; the ranks only agree on disjoint covering ranges and on the max-over-ranks timing reduction."""
+import os
+import socket
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2510_05100_b200.shard import shard_range
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, n, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    lo, hi = shard_range(n, rank, world)
+    mine = torch.zeros(n, dtype=torch.int64)
+    mine[lo:hi] = 1
+    dist.all_reduce(mine)                                   # coverage count per event
+    t = torch.tensor([float(rank + 1)], dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)                # bench.py: time = max over ranks
+    cnt = torch.tensor([hi - lo], dtype=torch.int64)
+    dist.all_reduce(cnt)
+    if rank == 0:
+        out.put((mine.numpy().copy(), float(t.item()), int(cnt.item())))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_sharding_covers_every_event_once():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    n, world, port = 1001, 2, _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, n, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    cover, tmax, total = q.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert np.all(cover == 1) and tmax == 2.0 and total == n
+
+
+def test_shard_range_properties():
+    for n in (0, 1, 7, 64, 1001):
+        for world in (1, 2, 3, 8):
+            r = [shard_range(n, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == n
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))
+            sizes = [b - a for a, b in r]
+            assert max(sizes) - min(sizes) <= 1
