@@ -145,6 +145,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--configs", default="all", choices=["all", "headline"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile", default="", help="comma-separated configs: run each once (after one warm-up) on --events "
+                    "events through trex_run and exit; the command ncu wraps for profiles/")
+    ap.add_argument("--events", type=int, default=0)
+    ap.add_argument("--precision", type=int, default=0)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -236,6 +240,16 @@ def main():
         T.trex_set_precision(0)
         del keys, mom, win, wout
         return res
+
+    if args.profile:
+        T.trex_set_precision(args.precision)
+        for cfg in [int(c) for c in args.profile.split(",")]:
+            w = make_config(cfg, n=args.events or None)
+            keys, mom, win = dev(w.keys), dev(w.momenta), dev(w.w_in)
+            for _ in range(2):
+                T.trex_run(keys, mom, w.theta_old, w.theta_new, win)
+            torch.cuda.synchronize()
+        return
 
     # ---- FP64 pipe peak, measured in this run
     def probe(fp32):

@@ -48,6 +48,13 @@ template <class R> struct spinor { cx<R> c[4]; };    // row or column 4-spinor, 
 template <class R> struct dspinor { spinor<R> o0, o1; };  // dual number in kappa on the top line (R-4)
 template <class R> struct ften { cx<R> b[3], e[3]; };     // antisymmetric tensor a^mu b^nu - a^nu b^mu: (a x b, a0 b - b0 a)
 
+// precision casts: momenta and kinematic invariants are always carried in double (an fp32 amplitude must not lose
+// s_ij = 2 k_i.k_j of nearly collinear legs, or q^2 - m^2 of a nearly on-shell propagator, to cancellation)
+template <class R> TREX_HD rvec4<R> cast(const rvec4<double>& a) { rvec4<R> o; for (int i = 0; i < 4; ++i) o.c[i] = R(a.c[i]); return o; }
+template <class R> TREX_HD cx<R> cast(const cx<double>& a) { return cx<R>(R(a.re), R(a.im)); }
+template <class R> TREX_HD vec4<R> cast(const vec4<double>& a) { vec4<R> o; for (int i = 0; i < 4; ++i) o.c[i] = cast<R>(a.c[i]); return o; }
+template <class R> TREX_HD spinor<R> cast(const spinor<double>& a) { spinor<R> o; for (int i = 0; i < 4; ++i) o.c[i] = cast<R>(a.c[i]); return o; }
+
 template <class R> TREX_HD R rdot(const rvec4<R>& a, const rvec4<R>& b) {
   return a.c[0] * b.c[0] - a.c[1] * b.c[1] - a.c[2] * b.c[2] - a.c[3] * b.c[3]; }
 // Minkowski products without complex conjugation
@@ -202,9 +209,9 @@ template <class R> TREX_HD void row_sigma_acc(spinor<R>& o, const spinor<R>& r, 
 
 // ---------------------------------------------------------------- ordered gluon vertices (R-6), g_s = 1
 // acc += J1 ((-P-k1).J2) + (k1-k2)(J1.J2) + J2 ((k2+P).J1), P = k1 + k2
-template <class R> TREX_HD void v3_acc(vec4<R>& acc, const rvec4<R>& k1, const vec4<R>& J1, const rvec4<R>& k2, const vec4<R>& J2) {
+template <class R> TREX_HD void v3_acc(vec4<R>& acc, const rvec4<double>& k1, const vec4<R>& J1, const rvec4<double>& k2, const vec4<R>& J2) {
   rvec4<R> a, b, d;
-  for (int i = 0; i < 4; ++i) { a.c[i] = -(R(2) * k1.c[i] + k2.c[i]); b.c[i] = R(2) * k2.c[i] + k1.c[i]; d.c[i] = k1.c[i] - k2.c[i]; }
+  for (int i = 0; i < 4; ++i) { a.c[i] = R(-(2.0 * k1.c[i] + k2.c[i])); b.c[i] = R(2.0 * k2.c[i] + k1.c[i]); d.c[i] = R(k1.c[i] - k2.c[i]); }
   cx<R> aJ2 = dot(a, J2), bJ1 = dot(b, J1), J1J2 = dot(J1, J2);
   for (int i = 0; i < 4; ++i) { cfma(acc.c[i], J1.c[i], aJ2); cfma(acc.c[i], J1J2, d.c[i]); cfma(acc.c[i], J2.c[i], bJ1); }
 }

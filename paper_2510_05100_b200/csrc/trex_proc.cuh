@@ -123,25 +123,25 @@ TREX_HD void ttng_unit(const double* __restrict__ mom, long n, long e, int gh, i
 #pragma unroll
   for (int g = 0; g < N; ++g) {
     const int leg = g < 2 ? g : g + 2;
-    R p[4]; load_leg<R>(mom, n, e, leg, p);
+    double p[4]; load_leg<double>(mom, n, e, leg, p);
     const int lam = ((gh >> g) & 1) ? +1 : -1;
     const bool incoming = g < 2;
-    t.eps[g] = polvec<R>(p, lam, !incoming);
-    const R sg = incoming ? R(1) : R(-1);
+    t.eps[g] = cast<R>(polvec<double>(p, lam, !incoming));
+    const double sg = incoming ? 1.0 : -1.0;
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) t.K[g].c[mu] = sg * p[mu];
   }
   {
-    R p[4]; load_leg<R>(mom, n, e, 2, p);
+    double p[4]; load_leg<double>(mom, n, e, 2, p);
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) t.pt.c[mu] = p[mu];
-    t.ubar_t = bar(spinor_u<R>(p, lam_t, false));
-    R q[4]; load_leg<R>(mom, n, e, 3, q);
-    st.v[0] = spinor_v<R>(q, -1, false);
-    st.v[1] = spinor_v<R>(q, +1, false);
+    t.ubar_t = cast<R>(bar(spinor_u<double>(p, lam_t, false)));
+    double q[4]; load_leg<double>(mom, n, e, 3, q);
+    st.v[0] = cast<R>(spinor_v<double>(q, -1, false));
+    st.v[1] = cast<R>(spinor_v<double>(q, +1, false));
   }
 #pragma unroll
-  for (int p = 0; p < NPASS; ++p) { t.line[p].mt = R(T.mt[p]); t.line[p].mGt = R(T.mGt[p]); }
+  for (int p = 0; p < NPASS; ++p) { t.line[p].mt = T.mt[p]; t.line[p].mGt = T.mGt[p]; }
   st.kq[0] = R(T.kq[0]); st.kq[1] = R(T.kq[1]);
   t.run(&st);
 #pragma unroll
@@ -176,45 +176,45 @@ template <class R> struct QqLeafStore {
 template <class R, class RC>
 TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L, int u, const ThetaPair& T, RC out[2]) {
   const int lam_row = (u & 1) ? 1 : -1, lam_col = (u & 2) ? 1 : -1, lam_g = (u & 4) ? 1 : -1, lam_t = (u & 8) ? 1 : -1;
-  R pr[4], pc[4], pg[4], pt[4], ptb[4];
-  load_leg<R>(mom, n, e, L.lrow, pr); load_leg<R>(mom, n, e, L.lcol, pc); load_leg<R>(mom, n, e, L.lg, pg);
-  load_leg<R>(mom, n, e, 2, pt); load_leg<R>(mom, n, e, 3, ptb);
+  double pr[4], pc[4], pg[4], pt[4], ptb[4];
+  load_leg<double>(mom, n, e, L.lrow, pr); load_leg<double>(mom, n, e, L.lcol, pc); load_leg<double>(mom, n, e, L.lg, pg);
+  load_leg<double>(mom, n, e, 2, pt); load_leg<double>(mom, n, e, 3, ptb);
   const bool row_in = L.lrow < 2, col_in = L.lcol < 2, g_in = L.lg < 2;
   // light line ends: row = vbar (incoming antiquark) or ubar (outgoing quark); column = u (incoming) or v (outgoing)
-  spinor<R> w = row_in ? bar(spinor_v<R>(pr, lam_row, true)) : bar(spinor_u<R>(pr, lam_row, true));
-  spinor<R> x = col_in ? spinor_u<R>(pc, lam_col, true) : spinor_v<R>(pc, lam_col, true);
-  rvec4<R> Kr, Kc, Kg, Kq;
+  spinor<R> w = cast<R>(row_in ? bar(spinor_v<double>(pr, lam_row, true)) : bar(spinor_u<double>(pr, lam_row, true)));
+  spinor<R> x = cast<R>(col_in ? spinor_u<double>(pc, lam_col, true) : spinor_v<double>(pc, lam_col, true));
+  rvec4<double> Kr, Kc, Kg, Kq;
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) {
     Kr.c[mu] = row_in ? pr[mu] : -pr[mu]; Kc.c[mu] = col_in ? pc[mu] : -pc[mu]; Kg.c[mu] = g_in ? pg[mu] : -pg[mu];
     Kq.c[mu] = Kr.c[mu] + Kc.c[mu];
   }
-  vec4<R> eg = polvec<R>(pg, lam_g, !g_in);
+  vec4<R> eg = cast<R>(polvec<double>(pg, lam_g, !g_in));
   // quark-pair current  Jq = (w gamma^mu x) / Kq^2        [ (i g_s) * (-i / Kq^2) at g_s = 1 ]
   vec4<R> Jq = bilinear(w, x);
-  { R s = R(1) / rdot(Kq, Kq);
+  { R s = R(1.0 / rdot(Kq, Kq));
 #pragma unroll
     for (int i = 0; i < 4; ++i) Jq.c[i] = Jq.c[i] * s; }
   // light line after radiating the gluon: W = w (i eslash)(i qslash)/q^2, q = -(Kr + Kg);  X = (i qslash)(i eslash) x / q^2, q = Kc + Kg
-  rvec4<R> Ptot = radd(Kq, Kg);
-  R iP2 = R(1) / rdot(Ptot, Ptot);
+  rvec4<double> Ptot = radd(Kq, Kg);
+  const double iP2 = 1.0 / rdot(Ptot, Ptot);
   vec4<R> Jq3, Jq4;
-  { rvec4<R> q; for (int mu = 0; mu < 4; ++mu) q.c[mu] = -(Kr.c[mu] + Kg.c[mu]);
-    spinor<R> W = row_slash(row_slash(w, eg), q);
-    R s = -iP2 / rdot(q, q);
+  { rvec4<double> q; for (int mu = 0; mu < 4; ++mu) q.c[mu] = -(Kr.c[mu] + Kg.c[mu]);
+    spinor<R> W = row_slash(row_slash(w, eg), cast<R>(q));
+    R s = R(-iP2 / rdot(q, q));
     Jq3 = bilinear(W, x);
 #pragma unroll
     for (int i = 0; i < 4; ++i) Jq3.c[i] = Jq3.c[i] * s; }
-  { rvec4<R> q = radd(Kc, Kg);
-    spinor<R> X = slash_col(q, slash_col(eg, x));
-    R s = -iP2 / rdot(q, q);
+  { rvec4<double> q = radd(Kc, Kg);
+    spinor<R> X = slash_col(cast<R>(q), slash_col(eg, x));
+    R s = R(-iP2 / rdot(q, q));
     Jq4 = bilinear(w, X);
 #pragma unroll
     for (int i = 0; i < 4; ++i) Jq4.c[i] = Jq4.c[i] * s; }
 
   QqLeafStore<R> st;
-  st.v[0] = spinor_v<R>(ptb, -1, false); st.v[1] = spinor_v<R>(ptb, +1, false);
-  spinor<R> ubar_t = bar(spinor_u<R>(pt, lam_t, false));
+  st.v[0] = cast<R>(spinor_v<double>(ptb, -1, false)); st.v[1] = cast<R>(spinor_v<double>(ptb, +1, false));
+  spinor<R> ubar_t = cast<R>(bar(spinor_u<double>(pt, lam_t, false)));
   // two-source ordered amplitudes: source 0 = gluon, source 1 = quark-pair current
   TTNG<R, 2, 1, QqLeafStore<R>> t;
   t.K[0] = Kg; t.eps[0] = eg; t.K[1] = Kq; t.eps[1] = Jq;
@@ -227,7 +227,7 @@ TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L
   cx<R> A12[2][2], A21[2][2];   // [order][v]
   for (int th = 0; th < 2; ++th) {
     if (th == 0 || !same_line) {
-      t.line[0].mt = R(T.mt[th]); t.line[0].mGt = R(T.mGt[th]);
+      t.line[0].mt = T.mt[th]; t.line[0].mGt = T.mGt[th];
       t.run(&st);
 #pragma unroll
       for (int iv = 0; iv < 2; ++iv) { A12[0][iv] = st.a0[0][iv]; A12[1][iv] = st.a1[0][iv]; A21[0][iv] = st.a0[1][iv]; A21[1][iv] = st.a1[1][iv]; }
@@ -239,12 +239,12 @@ TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L
       cx<R> k3, k4;
       {
         spinor<R> b0 = row_slash(ubar_t, Jq3), b1 = szero<R>();
-        ften<R> F = fzero<R>(); wedge_acc(F, Ptot, Jq3); row_sigma_acc(b1, ubar_t, F);
+        ften<R> F = fzero<R>(); wedge_acc(F, cast<R>(Ptot), Jq3); row_sigma_acc(b1, ubar_t, F);
         cx<R> a0 = mul_i(row_col(b0, st.v[iv])); cfma(a0, row_col(b1, st.v[iv]), R(T.kq[th])); k3 = a0;
       }
       {
         spinor<R> b0 = row_slash(ubar_t, Jq4), b1 = szero<R>();
-        ften<R> F = fzero<R>(); wedge_acc(F, Ptot, Jq4); row_sigma_acc(b1, ubar_t, F);
+        ften<R> F = fzero<R>(); wedge_acc(F, cast<R>(Ptot), Jq4); row_sigma_acc(b1, ubar_t, F);
         cx<R> a0 = mul_i(row_col(b0, st.v[iv])); cfma(a0, row_col(b1, st.v[iv]), R(T.kq[th])); k4 = a0;
       }
       cx<R> a12 = A12[0][iv]; cfma(a12, A12[1][iv], R(T.kq[th]));
@@ -269,21 +269,21 @@ TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L
 // coupling sets.
 template <class R>
 TREX_HD void eemumu_event(const double* __restrict__ mom, long n, long e, const ThetaPair& T, R out[2]) {
-  R p0[4], p1[4], p2[4], p3[4];
-  load_leg<R>(mom, n, e, 0, p0); load_leg<R>(mom, n, e, 1, p1); load_leg<R>(mom, n, e, 2, p2); load_leg<R>(mom, n, e, 3, p3);
-  R q[4]; for (int mu = 0; mu < 4; ++mu) q[mu] = p0[mu] + p1[mu];
-  const R s = q[0] * q[0] - q[1] * q[1] - q[2] * q[2] - q[3] * q[3];
+  double p0[4], p1[4], p2[4], p3[4];
+  load_leg<double>(mom, n, e, 0, p0); load_leg<double>(mom, n, e, 1, p1); load_leg<double>(mom, n, e, 2, p2); load_leg<double>(mom, n, e, 3, p3);
+  double q[4]; for (int mu = 0; mu < 4; ++mu) q[mu] = p0[mu] + p1[mu];
+  const double s = q[0] * q[0] - q[1] * q[1] - q[2] * q[2] - q[3] * q[3];
   cx<R> propZ[2]; R propA[2];
   for (int th = 0; th < 2; ++th) {
-    propA[th] = R(T.e2[th]) / s;
-    propZ[th] = cdiv(cx<R>(1, 0), cx<R>(s - R(T.mZ2[th]), R(T.mZGZ[th])));
+    propA[th] = R(T.e2[th] / s);
+    propZ[th] = cast<R>(cdiv(cx<double>(1, 0), cx<double>(s - T.mZ2[th], T.mZGZ[th])));
   }
   R sum[2] = {R(0), R(0)};
   for (int h = 0; h < 16; ++h) {
-    spinor<R> u1 = spinor_u<R>(p0, (h & 1) ? 1 : -1, true);
-    spinor<R> vb2 = bar(spinor_v<R>(p1, (h & 2) ? 1 : -1, true));
-    spinor<R> ub3 = bar(spinor_u<R>(p2, (h & 4) ? 1 : -1, true));
-    spinor<R> v4 = spinor_v<R>(p3, (h & 8) ? 1 : -1, true);
+    spinor<R> u1 = cast<R>(spinor_u<double>(p0, (h & 1) ? 1 : -1, true));
+    spinor<R> vb2 = cast<R>(bar(spinor_v<double>(p1, (h & 2) ? 1 : -1, true)));
+    spinor<R> ub3 = cast<R>(bar(spinor_u<double>(p2, (h & 4) ? 1 : -1, true)));
+    spinor<R> v4 = cast<R>(spinor_v<double>(p3, (h & 8) ? 1 : -1, true));
     // P_L keeps the upper two components in the chiral basis, P_R the lower two
     spinor<R> uL = u1, uR = u1, vL = v4, vR = v4;
     uL.c[2] = uL.c[3] = cx<R>(0, 0); uR.c[0] = uR.c[1] = cx<R>(0, 0);

@@ -17,20 +17,20 @@
 
 namespace trex {
 
-template <class R> struct TopLine {      // per parameter point
-  R mt, mGt;                             // m_t and m_t * Gamma_t
+struct TopLine {                         // per parameter point
+  double mt, mGt;                        // m_t and m_t * Gamma_t
 };
 
 template <class R, int N, int NPASS, class Sink> struct TTNG {
   // inputs (thread-private copies; dynamically indexed by the source number, so they live in local memory)
-  rvec4<R> K[N];            // incoming-convention momentum of each source
+  rvec4<double> K[N];       // incoming-convention momentum of each source (always double)
   vec4<R> eps[N];           // its polarisation / effective current
-  rvec4<R> pt;              // top momentum (outgoing)
+  rvec4<double> pt;         // top momentum (outgoing)
   spinor<R> ubar_t;         // ubar(p_t, lambda_t)
-  TopLine<R> line[NPASS];
+  TopLine line[NPASS];
   // path state
   vec4<R> J[N][N + 1];      // J[a][m], a < m
-  rvec4<R> P[N][N + 1];     // momentum of tuple (a+1..m)
+  rvec4<double> P[N][N + 1];// momentum of tuple (a+1..m)
   dspinor<R> U[NPASS][N];   // U[p][m], m = 0..N-1 (U[.][0] = ubar_t, order 1 = 0)
   int leaf;
   Sink* sink;
@@ -52,7 +52,7 @@ template <class R, int N, int NPASS, class Sink> struct TTNG {
 #pragma unroll
           for (int c2 = c1 + 1; c2 < M; ++c2) v4_acc(acc, J[a][c1], J[c1][c2], J[c2][M]);
         // (-i/P^2) * [(-i)V3 + (-i)V4] = -(V3 + V4)/P^2 at g_s = 1
-        R s = R(-1) / rdot(P[a][M], P[a][M]);
+        R s = R(-1.0 / rdot(P[a][M], P[a][M]));
 #pragma unroll
         for (int i = 0; i < 4; ++i) J[a][M].c[i] = acc.c[i] * s;
       }
@@ -64,7 +64,7 @@ template <class R, int N, int NPASS, class Sink> struct TTNG {
       for (int a = 0; a < M; ++a) {
         // F = P ^ J (dipole, gluon momentum into the vertex) + sum_c J[a][c] ^ J[c][M] (contact)
         ften<R> F = fzero<R>();
-        wedge_acc(F, P[a][M], J[a][M]);
+        wedge_acc(F, cast<R>(P[a][M]), J[a][M]);
 #pragma unroll
         for (int c = a + 1; c < M; ++c) wedge_acc(F, J[a][c], J[c][M]);
 #pragma unroll
@@ -81,18 +81,19 @@ template <class R, int N, int NPASS, class Sink> struct TTNG {
         }
       }
       if constexpr (M < N) {
-        rvec4<R> q = rsub(pt, P[0][M]);
-        R q2 = rdot(q, q);
+        rvec4<double> qd = rsub(pt, P[0][M]);
+        const double q2 = rdot(qd, qd);
+        rvec4<R> q = cast<R>(qd);
 #pragma unroll
         for (int p = 0; p < NPASS; ++p) {
           // S(q) = i (qslash + m) / (q^2 - m^2 + i m Gamma)
-          cx<R> den(q2 - line[p].mt * line[p].mt, line[p].mGt);
-          cx<R> pr = cdiv(cx<R>(0, 1), den);
+          cx<double> den(q2 - line[p].mt * line[p].mt, line[p].mGt);
+          cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), den));
           spinor<R> s0 = row_slash(b0[p], q), s1 = row_slash(b1[p], q);
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            cx<R> n0 = s0.c[i]; cfma(n0, b0[p].c[i], line[p].mt);
-            cx<R> n1 = s1.c[i]; cfma(n1, b1[p].c[i], line[p].mt);
+            cx<R> n0 = s0.c[i]; cfma(n0, b0[p].c[i], R(line[p].mt));
+            cx<R> n1 = s1.c[i]; cfma(n1, b1[p].c[i], R(line[p].mt));
             U[p][M].o0.c[i] = n0 * pr; U[p][M].o1.c[i] = n1 * pr;
           }
         }
