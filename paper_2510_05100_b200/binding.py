@@ -42,6 +42,7 @@ _SIGNATURES = {
     "trex_set_stream": (_int, [_vp]),
     "trex_set_precision": (_int, [_int]),
     "trex_get_precision": (_int, []),
+    "trex_set_algorithm": (_int, [_int]),
     "trex_launch_count": (ctypes.c_int64, []),
     "trex_last_error": (ctypes.c_char_p, []),
     "trex_shutdown": (None, []),
@@ -142,6 +143,10 @@ def trex_set_stream(stream=None):
 
 def trex_set_precision(mode):
     return _check(lib().trex_set_precision(int(mode)), "trex_set_precision")
+
+
+def trex_set_algorithm(algo):
+    return _check(lib().trex_set_algorithm(int(algo)), "trex_set_algorithm")
 
 
 def trex_get_precision():

@@ -1,4 +1,5 @@
 // trex_api.cu -- reweighting kernels and the C ABI of include/rex_trex.h.
+#include <algorithm>
 #include <cstring>
 #include <vector>
 
@@ -81,11 +82,29 @@ const TtngUploadFn kUpload[4][3] = {
     {trex_tu_upload_n2_m0, trex_tu_upload_n2_m1, trex_tu_upload_n2_m2}, {trex_tu_upload_n3_m0, trex_tu_upload_n3_m1, trex_tu_upload_n3_m2},
     {trex_tu_upload_n4_m0, trex_tu_upload_n4_m1, trex_tu_upload_n4_m2}, {trex_tu_upload_n5_m0, trex_tu_upload_n5_m1, trex_tu_upload_n5_m2}};
 
+const MemoLaunchFn kMemoLaunch[2][3] = {{trex_tu_memo_launch_n4_m0, trex_tu_memo_launch_n4_m1, trex_tu_memo_launch_n4_m2},
+                                        {trex_tu_memo_launch_n5_m0, trex_tu_memo_launch_n5_m1, trex_tu_memo_launch_n5_m2}};
+const MemoBytesFn kMemoBytes[2][3] = {{trex_tu_memo_xbytes_n4_m0, trex_tu_memo_xbytes_n4_m1, trex_tu_memo_xbytes_n4_m2},
+                                      {trex_tu_memo_xbytes_n5_m0, trex_tu_memo_xbytes_n5_m1, trex_tu_memo_xbytes_n5_m2}};
+
+// C'(i,j) = 0 (j < i), C_ii (j == i), 2 C_ij (j > i); row i keeps the columns j >= 8 floor(i/8) (k_memo_colour)
+std::vector<double> fold_colour(const std::vector<double>& C, int NC) {
+  std::vector<double> f;
+  for (int i = 0; i < NC; ++i)
+    for (int j = 8 * (i / 8); j < NC; ++j) f.push_back(j < i ? 0.0 : (j == i ? C[i * NC + i] : 2.0 * C[i * NC + j]));
+  return f;
+}
+
 int ensure_colour() {
   Context& c = ctx();
   if (c.colour_ready) return 0;
   for (int N = 2; N <= 5; ++N) {
     std::vector<double> C = trex_colour::ttng_colour_matrix(N);
+    if (N >= 4) {
+      std::vector<double> f = fold_colour(C, N == 4 ? 24 : 120);
+      TREX_CUDA_CHECK(cudaMalloc((void**)&c.Cfold[N - 4], sizeof(double) * f.size()));
+      TREX_CUDA_CHECK(cudaMemcpy(c.Cfold[N - 4], f.data(), sizeof(double) * f.size(), cudaMemcpyHostToDevice));
+    }
     for (int m = 0; m < 3; ++m)
       if (kUpload[N - 2][m](C.data(), (int)C.size()) != 0) return fail(TREX_ECUDA, "colour matrix upload failed (N=%d)", N);
     if (N == 5) {
@@ -130,6 +149,15 @@ extern "C" int trex_colour_matrix(int sid, double* out) {
   return 4;
 }
 
+static int ensure_scratch(void** p, size_t* have, size_t need) {
+  if (*have >= need) return 0;
+  if (*p) cudaFree(*p);
+  *p = nullptr; *have = 0;
+  TREX_CUDA_CHECK(cudaMalloc(p, need));
+  *have = need;
+  return 0;
+}
+
 // one launch: |M|^2 at theta_old and theta_new + epilogue for the n events of an SoA block with row stride ld
 static int launch_reweight(int sid, const double* mom, long n, long ld, const ThetaPair& T, const double* w_in, double* w_out,
                            double* me2_old, double* me2_new) {
@@ -149,6 +177,19 @@ static int launch_reweight(int sid, const double* mom, long n, long ld, const Th
   } else if (sid <= TREX_SP_GG_TTGGG) {
     const int N = sp->npar - 2;
     const int npass = (T.mt[0] != T.mt[1] || T.mGt[0] != T.mGt[1]) ? 2 : 1;
+    if (N >= 4 && c.use_memo) {
+      // current-table kernels: amplitudes of a chunk of events -> scratch X -> colour sum + epilogue
+      const size_t xb = kMemoBytes[N - 4][mode]();
+      const long chunk = (long)std::min<size_t>((size_t)n, std::max<size_t>(1, ((size_t)1 << 30) / xb));
+      if (int rc = ensure_scratch(&c.memo_x, &c.memo_x_bytes, xb * (size_t)chunk)) return rc;
+      for (long ev0 = 0; ev0 < n; ev0 += chunk) {
+        const long nev = std::min<long>(chunk, n - ev0);
+        if (kMemoLaunch[N - 4][mode](a, npass, (double*)c.memo_x, c.Cfold[N - 4], ev0, nev, c.stream) != 0)
+          return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        c.launches += 2;
+      }
+      return 0;
+    }
     if (kLaunch[N - 2][mode](a, npass, grid32, c.stream) != 0) return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
   } else {
     if (mode == 0) k_qq<double, double><<<grid32, WARPS * 32, 0, c.stream>>>(a);
@@ -170,15 +211,6 @@ extern "C" int trex_reweight(int sid, const double* momenta_soa, int64_t n, cons
   ThetaPair T;
   if (!make_theta_pair(sid, theta_old, theta_new, T)) return fail(TREX_EINVAL, "trex_reweight: theta outside its domain");
   return launch_reweight(sid, momenta_soa, n, n, T, w_in, w_out, me2_old, me2_new);
-}
-
-static int ensure_scratch(void** p, size_t* have, size_t need) {
-  if (*have >= need) return 0;
-  if (*p) cudaFree(*p);
-  *p = nullptr; *have = 0;
-  TREX_CUDA_CHECK(cudaMalloc(p, need));
-  *have = need;
-  return 0;
 }
 
 __global__ void k_zero_rows(double* __restrict__ dst, long ld, long off, long cnt, int nrows) {
@@ -297,6 +329,10 @@ extern "C" int trex_set_precision(int mode) {
   ctx().precision = mode; return 0;
 }
 extern "C" int trex_get_precision(void) { return ctx().precision; }
+extern "C" int trex_set_algorithm(int algo) {
+  if (algo < 0 || algo > 1) return fail(TREX_EINVAL, "trex_set_algorithm: algo must be 0 or 1");
+  ctx().use_memo = algo == 1; return 0;
+}
 extern "C" int64_t trex_launch_count(void) { return ctx().launches; }
 extern "C" const char* trex_last_error(void) { return ctx().err; }
 extern "C" void trex_shutdown(void) {
@@ -304,6 +340,9 @@ extern "C" void trex_shutdown(void) {
   if (c.bucket_scratch) cudaFree(c.bucket_scratch);
   if (c.bucket_host) cudaFreeHost(c.bucket_host);
   if (c.C120) cudaFree(c.C120);
+  for (int i = 0; i < 2; ++i) { if (c.Cfold[i]) cudaFree(c.Cfold[i]); c.Cfold[i] = nullptr; }
+  if (c.memo_x) cudaFree(c.memo_x);
+  c.memo_x = nullptr; c.memo_x_bytes = 0;
   if (c.run_perm) cudaFree(c.run_perm);
   if (c.run_blocks) cudaFree(c.run_blocks);
   if (c.host_io) cudaFree(c.host_io);

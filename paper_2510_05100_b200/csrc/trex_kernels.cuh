@@ -67,4 +67,14 @@ TREX_TU_DECL(4, 0) TREX_TU_DECL(4, 1) TREX_TU_DECL(4, 2)
 TREX_TU_DECL(5, 0) TREX_TU_DECL(5, 1) TREX_TU_DECL(5, 2)
 #undef TREX_TU_DECL
 
+// current-table kernels (trex_memo_tu.cu), one translation unit per (N = 4, 5; precision mode)
+using MemoLaunchFn = int (*)(const ReweightArgs&, int npass, double* X, const double* Cfold, long ev0, long nev, cudaStream_t);
+using MemoBytesFn = size_t (*)();
+#define TREX_MEMO_DECL(N, M)                                                                                          \
+  int trex_tu_memo_launch_n##N##_m##M(const ReweightArgs&, int npass, double* X, const double* Cfold, long ev0, long nev, cudaStream_t); \
+  size_t trex_tu_memo_xbytes_n##N##_m##M();
+TREX_MEMO_DECL(4, 0) TREX_MEMO_DECL(4, 1) TREX_MEMO_DECL(4, 2)
+TREX_MEMO_DECL(5, 0) TREX_MEMO_DECL(5, 1) TREX_MEMO_DECL(5, 2)
+#undef TREX_MEMO_DECL
+
 }  // namespace trex
