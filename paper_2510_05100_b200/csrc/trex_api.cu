@@ -82,28 +82,29 @@ const TtngUploadFn kUpload[4][3] = {
     {trex_tu_upload_n2_m0, trex_tu_upload_n2_m1, trex_tu_upload_n2_m2}, {trex_tu_upload_n3_m0, trex_tu_upload_n3_m1, trex_tu_upload_n3_m2},
     {trex_tu_upload_n4_m0, trex_tu_upload_n4_m1, trex_tu_upload_n4_m2}, {trex_tu_upload_n5_m0, trex_tu_upload_n5_m1, trex_tu_upload_n5_m2}};
 
-const MemoLaunchFn kMemoLaunch[2][3] = {{trex_tu_memo_launch_n4_m0, trex_tu_memo_launch_n4_m1, trex_tu_memo_launch_n4_m2},
-                                        {trex_tu_memo_launch_n5_m0, trex_tu_memo_launch_n5_m1, trex_tu_memo_launch_n5_m2}};
-const MemoBytesFn kMemoBytes[2][3] = {{trex_tu_memo_xbytes_n4_m0, trex_tu_memo_xbytes_n4_m1, trex_tu_memo_xbytes_n4_m2},
-                                      {trex_tu_memo_xbytes_n5_m0, trex_tu_memo_xbytes_n5_m1, trex_tu_memo_xbytes_n5_m2}};
-
-// C'(i,j) = 0 (j < i), C_ii (j == i), 2 C_ij (j > i); row i keeps the columns j >= 8 floor(i/8) (k_memo_colour)
-std::vector<double> fold_colour(const std::vector<double>& C, int NC) {
-  std::vector<double> f;
-  for (int i = 0; i < NC; ++i)
-    for (int j = 8 * (i / 8); j < NC; ++j) f.push_back(j < i ? 0.0 : (j == i ? C[i * NC + i] : 2.0 * C[i * NC + j]));
-  return f;
-}
+#define TREX_TAB_ROW(stem) {{stem##3_m0, stem##3_m1, stem##3_m2}, {stem##4_m0, stem##4_m1, stem##4_m2}, {stem##5_m0, stem##5_m1, stem##5_m2}}
+const TableLaunchFn kTableLaunch[3][3] = TREX_TAB_ROW(trex_tu_table_launch_n);
+const TableMetaFn kTableMeta[3][3] = TREX_TAB_ROW(trex_tu_table_meta_n);
+const TableFoldFn kTableFold[3][3] = TREX_TAB_ROW(trex_tu_table_fold_n);
+#undef TREX_TAB_ROW
 
 int ensure_colour() {
   Context& c = ctx();
   if (c.colour_ready) return 0;
+  int dev = 0;
+  TREX_CUDA_CHECK(cudaGetDevice(&dev));
+  TREX_CUDA_CHECK(cudaDeviceGetAttribute(&c.nsm, cudaDevAttrMultiProcessorCount, dev));
   for (int N = 2; N <= 5; ++N) {
     std::vector<double> C = trex_colour::ttng_colour_matrix(N);
-    if (N >= 4) {
-      std::vector<double> f = fold_colour(C, N == 4 ? 24 : 120);
-      TREX_CUDA_CHECK(cudaMalloc((void**)&c.Cfold[N - 4], sizeof(double) * f.size()));
-      TREX_CUDA_CHECK(cudaMemcpy(c.Cfold[N - 4], f.data(), sizeof(double) * f.size(), cudaMemcpyHostToDevice));
+    if (N >= 3) {
+      std::vector<double> f((size_t)kTableFold[N - 3][0](C.data(), nullptr));
+      kTableFold[N - 3][0](C.data(), f.data());
+      TREX_CUDA_CHECK(cudaMalloc((void**)&c.Cfold[N - 3], sizeof(double) * f.size()));
+      TREX_CUDA_CHECK(cudaMemcpy(c.Cfold[N - 3], f.data(), sizeof(double) * f.size(), cudaMemcpyHostToDevice));
+      std::vector<int> meta((size_t)kTableMeta[N - 3][0](nullptr));
+      kTableMeta[N - 3][0](meta.data());
+      TREX_CUDA_CHECK(cudaMalloc((void**)&c.table_meta[N - 3], sizeof(int) * meta.size()));
+      TREX_CUDA_CHECK(cudaMemcpy(c.table_meta[N - 3], meta.data(), sizeof(int) * meta.size(), cudaMemcpyHostToDevice));
     }
     for (int m = 0; m < 3; ++m)
       if (kUpload[N - 2][m](C.data(), (int)C.size()) != 0) return fail(TREX_ECUDA, "colour matrix upload failed (N=%d)", N);
@@ -177,17 +178,10 @@ static int launch_reweight(int sid, const double* mom, long n, long ld, const Th
   } else if (sid <= TREX_SP_GG_TTGGG) {
     const int N = sp->npar - 2;
     const int npass = (T.mt[0] != T.mt[1] || T.mGt[0] != T.mGt[1]) ? 2 : 1;
-    if (N >= 4 && c.use_memo) {
-      // current-table kernels: amplitudes of a chunk of events -> scratch X -> colour sum + epilogue
-      const size_t xb = kMemoBytes[N - 4][mode]();
-      const long chunk = (long)std::min<size_t>((size_t)n, std::max<size_t>(1, ((size_t)1 << 30) / xb));
-      if (int rc = ensure_scratch(&c.memo_x, &c.memo_x_bytes, xb * (size_t)chunk)) return rc;
-      for (long ev0 = 0; ev0 < n; ev0 += chunk) {
-        const long nev = std::min<long>(chunk, n - ev0);
-        if (kMemoLaunch[N - 4][mode](a, npass, (double*)c.memo_x, c.Cfold[N - 4], ev0, nev, c.stream) != 0)
-          return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-        c.launches += 2;
-      }
+    if (N >= 3 && N >= c.table_min_n) {
+      if (kTableLaunch[N - 3][mode](a, npass, c.table_meta[N - 3], c.Cfold[N - 3], c.nsm, c.stream) != 0)
+        return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+      c.launches += 1;
       return 0;
     }
     if (kLaunch[N - 2][mode](a, npass, grid32, c.stream) != 0) return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -330,8 +324,8 @@ extern "C" int trex_set_precision(int mode) {
 }
 extern "C" int trex_get_precision(void) { return ctx().precision; }
 extern "C" int trex_set_algorithm(int algo) {
-  if (algo < 0 || algo > 1) return fail(TREX_EINVAL, "trex_set_algorithm: algo must be 0 or 1");
-  ctx().use_memo = algo == 1; return 0;
+  if (algo != 0 && (algo < 3 || algo > 5)) return fail(TREX_EINVAL, "trex_set_algorithm: algo must be 0, 3, 4 or 5");
+  ctx().table_min_n = algo == 0 ? 99 : algo; return 0;
 }
 extern "C" int64_t trex_launch_count(void) { return ctx().launches; }
 extern "C" const char* trex_last_error(void) { return ctx().err; }
@@ -340,9 +334,11 @@ extern "C" void trex_shutdown(void) {
   if (c.bucket_scratch) cudaFree(c.bucket_scratch);
   if (c.bucket_host) cudaFreeHost(c.bucket_host);
   if (c.C120) cudaFree(c.C120);
-  for (int i = 0; i < 2; ++i) { if (c.Cfold[i]) cudaFree(c.Cfold[i]); c.Cfold[i] = nullptr; }
-  if (c.memo_x) cudaFree(c.memo_x);
-  c.memo_x = nullptr; c.memo_x_bytes = 0;
+  for (int i = 0; i < 3; ++i) {
+    if (c.Cfold[i]) cudaFree(c.Cfold[i]);
+    if (c.table_meta[i]) cudaFree(c.table_meta[i]);
+    c.Cfold[i] = nullptr; c.table_meta[i] = nullptr;
+  }
   if (c.run_perm) cudaFree(c.run_perm);
   if (c.run_blocks) cudaFree(c.run_blocks);
   if (c.host_io) cudaFree(c.host_io);

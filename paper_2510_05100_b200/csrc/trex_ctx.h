@@ -13,7 +13,8 @@ namespace trex {
 struct Context {
   cudaStream_t stream = nullptr;
   int precision = 0;
-  bool use_memo = true;              // N >= 4: current-table kernels (false: prefix-walk kernels, kept for comparison)
+  int table_min_n = 4;               // gluon multiplicities >= this use the fused current-table kernel (trex_set_algorithm)
+  int nsm = 0;                       // multiprocessors of the device
   int64_t launches = 0;
   char err[512] = {0};
   // rex_bucket scratch (device) and results of the last call (host)
@@ -30,8 +31,8 @@ struct Context {
   // colour matrices on the device
   bool colour_ready = false;
   double* C120 = nullptr;            // 120 x 120, global memory
-  double* Cfold[2] = {nullptr, nullptr};   // folded upper-triangular colour matrices of N = 4, 5 (trex_memo_tu.cu)
-  void* memo_x = nullptr; size_t memo_x_bytes = 0;   // colour-flow amplitude scratch of the current-table kernels
+  double* Cfold[3] = {nullptr, nullptr, nullptr};   // folded upper-triangular colour matrices of N = 3, 4, 5 (trex_table_tu.cu)
+  int* table_meta[3] = {nullptr, nullptr, nullptr}; // tuple / entry index tables of the current-table kernels
 };
 
 Context& ctx();

@@ -67,14 +67,17 @@ TREX_TU_DECL(4, 0) TREX_TU_DECL(4, 1) TREX_TU_DECL(4, 2)
 TREX_TU_DECL(5, 0) TREX_TU_DECL(5, 1) TREX_TU_DECL(5, 2)
 #undef TREX_TU_DECL
 
-// current-table kernels (trex_memo_tu.cu), one translation unit per (N = 4, 5; precision mode)
-using MemoLaunchFn = int (*)(const ReweightArgs&, int npass, double* X, const double* Cfold, long ev0, long nev, cudaStream_t);
-using MemoBytesFn = size_t (*)();
-#define TREX_MEMO_DECL(N, M)                                                                                          \
-  int trex_tu_memo_launch_n##N##_m##M(const ReweightArgs&, int npass, double* X, const double* Cfold, long ev0, long nev, cudaStream_t); \
-  size_t trex_tu_memo_xbytes_n##N##_m##M();
-TREX_MEMO_DECL(4, 0) TREX_MEMO_DECL(4, 1) TREX_MEMO_DECL(4, 2)
-TREX_MEMO_DECL(5, 0) TREX_MEMO_DECL(5, 1) TREX_MEMO_DECL(5, 2)
-#undef TREX_MEMO_DECL
+// fused current-table kernels (trex_table_tu.cu), one translation unit per (N = 3, 4, 5; precision mode)
+using TableLaunchFn = int (*)(const ReweightArgs&, int npass, const int* meta, const double* Cfold, int nsm, cudaStream_t);
+using TableMetaFn = int (*)(int* meta);                       // fills the meta block (if non-null), returns its size in ints
+using TableFoldFn = int (*)(const double* C, double* f);      // fills the folded colour matrix (if non-null), returns its size
+#define TREX_TABLE_DECL(N, M)                                                                                       \
+  int trex_tu_table_launch_n##N##_m##M(const ReweightArgs&, int npass, const int* meta, const double* Cfold, int nsm, cudaStream_t); \
+  int trex_tu_table_meta_n##N##_m##M(int* meta);                                                                    \
+  int trex_tu_table_fold_n##N##_m##M(const double* C, double* f);
+TREX_TABLE_DECL(3, 0) TREX_TABLE_DECL(3, 1) TREX_TABLE_DECL(3, 2)
+TREX_TABLE_DECL(4, 0) TREX_TABLE_DECL(4, 1) TREX_TABLE_DECL(4, 2)
+TREX_TABLE_DECL(5, 0) TREX_TABLE_DECL(5, 1) TREX_TABLE_DECL(5, 2)
+#undef TREX_TABLE_DECL
 
 }  // namespace trex

@@ -1,0 +1,364 @@
+// trex_table.cuh -- g g -> t t~ + (N-2) g from a per-event table of off-shell gluon currents.
+//
+// A thread block owns one event. The colour-ordered recursion of SURVEY.md C-4 needs, for every ordering sigma and every
+// helicity configuration, the current J(t_1 .. t_k) of every contiguous gluon tuple and, at order kappa, the
+// field-strength bracket   F(t_1 .. t_k) = P ^ J(t_1 .. t_k) + sum_c J(t_1 .. t_c) ^ J(t_c+1 .. t_k)
+// (dipole + contact insertions on the top line, R-4). Both depend only on the tuple and on the helicities of
+// ITS OWN gluons ("helicity recycling"), and J(t_k .. t_1) = (-1)^(k+1) J(t_1 .. t_k), same for F. So the block builds,
+// level by level in shared memory, one table entry (J: 4 complex, 2 sigma.F as two 2x2 blocks: 6 complex) per
+// canonical tuple (t_1 < t_k) and helicity assignment, and the top-quark line is then walked depth first by one thread
+// per (ordering prefix, free helicities, top helicity [, parameter point]): every vertex on the line is two row-spinor x
+// slash products and one row-spinor x sigma.F product with operands fetched from the table.
+//
+// To make the table, the colour-flow amplitudes X and the colour matrix fit the 227 KB of one SM for N = 5, the
+// helicities of the first NFIX gluons are fixed by an outer loop of 2^NFIX iterations: the table of one iteration only
+// holds the helicity assignments of the remaining ("free") gluons; X holds the columns (free helicities, lambda_t,
+// lambda_tbar, theta) of that iteration and is closed with J^dagger C J before the next iteration starts.
+#pragma once
+#include "trex_math.cuh"
+#include "trex_ttng.cuh"
+
+namespace trex {
+
+// ---------------------------------------------------------------- indexing of canonical tuples and table entries
+template <int N, int NFIX> struct TabIdx {
+  TREX_HD static constexpr int falling(int n, int k) { int r = 1; for (int i = 0; i < k; ++i) r *= (n - i); return r; }
+  TREX_HD static constexpr int binom(int n, int k) { if (k < 0 || k > n) return 0; int r = 1; for (int i = 0; i < k; ++i) r = r * (n - i) / (i + 1); return r; }
+  TREX_HD static constexpr int ncanon(int k) { return k == 1 ? N : falling(N, k) / 2; }       // canonical k-tuples
+  TREX_HD static constexpr int cid_base(int k) { int b = 0; for (int j = 1; j < k; ++j) b += ncanon(j); return b; }
+  static constexpr int NCID = cid_base(N + 1);
+  static constexpr int NFREE = N - NFIX;
+  // entries of level k: sum over canonical k-tuples of 2^(free gluons in the tuple)
+  TREX_HD static constexpr int level_entries(int k) {
+    int s = 0;
+    for (int f = 0; f <= k; ++f) s += binom(NFIX, f) * binom(NFREE, k - f) * falling(k, k) * (1 << (k - f));
+    return k == 1 ? s : s / 2;
+  }
+  TREX_HD static constexpr int entries_below(int k) { int s = 0; for (int j = 1; j < k; ++j) s += level_entries(j); return s; }
+  static constexpr int NE = entries_below(N + 1);
+
+  // canonical id of an ordered k-tuple with t[0] < t[k-1] (k >= 2): (pair {first,last}) x (rank of the middle)
+  template <int K> TREX_HD static int canon_id(const int* t) {
+    const int a = t[0], b = t[K - 1];
+    int id = a * (2 * N - a - 1) / 2 + (b - a - 1);
+    unsigned used = (1u << a) | (1u << b);
+    int mid = 0;
+#pragma unroll
+    for (int i = 1; i < K - 1; ++i) {
+      const int m = t[i];
+      const int c = m - __builtin_popcount(used & ((1u << m) - 1u));
+      mid = mid * (N - 1 - i) + c;              // mixed radix: N-2, N-3, ...
+      used |= 1u << m;
+    }
+    return id * falling(N - 2, K - 2) + mid;
+  }
+  // inverse of canon_id (host side: the tuples are shipped to the kernel in the meta block)
+  static void canon_tuple(int K, int id, int* t) {
+    const int nmid = falling(N - 2, K - 2);
+    int pair = id / nmid, mid = id - pair * nmid;
+    int a = 0;
+    while (pair >= N - 1 - a) { pair -= N - 1 - a; ++a; }
+    const int b = a + 1 + pair;
+    t[0] = a; t[K - 1] = b;
+    unsigned used = (1u << a) | (1u << b);
+    int digit[8];
+    for (int i = K - 2; i >= 1; --i) { const int radix = N - 1 - i; digit[i - 1] = mid % radix; mid /= radix; }
+    for (int i = 1; i < K - 1; ++i) {
+      int c = digit[i - 1], m = 0;
+      for (;; ++m) { if (!((used >> m) & 1u)) { if (c == 0) break; --c; } }
+      t[i] = m; used |= 1u << m;
+    }
+  }
+  TREX_HD static unsigned bitrev(unsigned bits, int k) {           // reverse the low k bits (bits above k are zero)
+#if defined(__CUDA_ARCH__)
+    return (__brev(bits) >> 1) >> (31 - k);
+#else
+    unsigned r = 0;
+    for (int i = 0; i < k; ++i) r |= ((bits >> i) & 1u) << (k - 1 - i);
+    return r;
+#endif
+  }
+  // the r-th (r = 0, 1, ..) gluon not in `used`
+  TREX_HD static int nth_unused(unsigned used, int r) {
+    int g = 0, c = r;
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+      const bool freeslot = !((used >> m) & 1u);
+      if (freeslot && c == 0) g = m;
+      if (freeslot) --c;
+    }
+    return g;
+  }
+  // meta block (ints), built once on the host: entry offset of every canonical tuple, first entry of every level,
+  // the tuples themselves (4 bits per position) and the canonical tuple of every entry
+  static constexpr int M_OFF = 0;                  // [NCID + 1]
+  static constexpr int M_LVL = M_OFF + NCID + 1;   // [N + 2]: index K = first entry of level K, K = 1 .. N+1
+  static constexpr int M_TUP = M_LVL + N + 2;      // [NCID]
+  static constexpr int M_CID = M_TUP + NCID;       // [NE]
+  static constexpr int M_SIZE = M_CID + NE;
+  static void build_meta(int* meta) {
+    int e = 0, cid = 0;
+    for (int K = 1; K <= N; ++K) {
+      meta[M_LVL + K] = e;
+      for (int id = 0; id < ncanon(K); ++id, ++cid) {
+        int t[8];
+        if (K == 1) t[0] = id; else canon_tuple(K, id, t);
+        int nf = 0, packed = 0;
+        for (int i = 0; i < K; ++i) { nf += t[i] >= NFIX; packed |= t[i] << (4 * i); }
+        meta[M_OFF + cid] = e;
+        meta[M_TUP + cid] = packed;
+        for (int b = 0; b < (1 << nf); ++b) meta[M_CID + e++] = cid;
+      }
+    }
+    meta[M_OFF + cid] = e;
+    meta[M_LVL + N + 1] = e;
+    meta[M_LVL] = 0;
+  }
+};
+
+// ---------------------------------------------------------------- table access
+// 20 real components per entry, component-major: tab[comp * NE + entry]; comp 0..7 = J (re, im per mu),
+// 8..13 = xp = 2 (B + iE) (re, im per axis), 14..19 = xm = 2 (B - iE)
+constexpr int TAB_NCOMP = 20;
+
+template <class R> struct sigF { cx<R> xp[3], xm[3]; };
+
+// entry index and sign of the ordered tuple t[0..L) whose free gluons carry the (position-ordered) bits `cbits`
+template <int N, int NFIX, int L> TREX_HD int tab_entry(const int* __restrict__ off, const int* t, unsigned cbits, int nf, int& sign) {
+  using I = TabIdx<N, NFIX>;
+  if constexpr (L == 1) { sign = 1; return off[t[0]] + (int)cbits; }
+  else {
+    const bool fwd = t[0] < t[L - 1];
+    int tt[L];
+#pragma unroll
+    for (int i = 0; i < L; ++i) tt[i] = fwd ? t[i] : t[L - 1 - i];
+    const unsigned bb = fwd ? cbits : I::bitrev(cbits, nf);
+    sign = (fwd || (L & 1)) ? 1 : -1;            // reversed: (-1)^(L+1)
+    return off[I::cid_base(L) + I::template canon_id<L>(tt)] + (int)bb;
+  }
+}
+// x or -x without touching the floating-point pipes (sign-bit flip on the integer pipe)
+TREX_HD double with_sign(double x, int sign) {
+#if defined(__CUDA_ARCH__)
+  return __hiloint2double(__double2hiint(x) ^ (sign < 0 ? (int)0x80000000 : 0), __double2loint(x));
+#else
+  return sign < 0 ? -x : x;
+#endif
+}
+TREX_HD float with_sign(float x, int sign) {
+#if defined(__CUDA_ARCH__)
+  return __int_as_float(__float_as_int(x) ^ (sign < 0 ? (int)0x80000000 : 0));
+#else
+  return sign < 0 ? -x : x;
+#endif
+}
+template <class R, int NE> TREX_HD vec4<R> tab_J(const R* __restrict__ tab, int e, int sign) {
+  vec4<R> J;
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) J.c[mu] = cx<R>(with_sign(tab[(2 * mu) * NE + e], sign), with_sign(tab[(2 * mu + 1) * NE + e], sign));
+  return J;
+}
+template <class R, int NE> TREX_HD sigF<R> tab_F(const R* __restrict__ tab, int e, int sign) {
+  sigF<R> F;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    F.xp[i] = cx<R>(with_sign(tab[(8 + 2 * i) * NE + e], sign), with_sign(tab[(9 + 2 * i) * NE + e], sign));
+    F.xm[i] = cx<R>(with_sign(tab[(14 + 2 * i) * NE + e], sign), with_sign(tab[(15 + 2 * i) * NE + e], sign));
+  }
+  return F;
+}
+template <class R, int NE> TREX_HD void tab_store(R* __restrict__ tab, int e, const vec4<R>& J, const ften<R>& f) {
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) { tab[(2 * mu) * NE + e] = J.c[mu].re; tab[(2 * mu + 1) * NE + e] = J.c[mu].im; }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    const cx<R> ie = mul_i(f.e[i]);
+    const cx<R> xp = R(2) * (f.b[i] + ie), xm = R(2) * (f.b[i] - ie);
+    tab[(8 + 2 * i) * NE + e] = xp.re; tab[(9 + 2 * i) * NE + e] = xp.im;
+    tab[(14 + 2 * i) * NE + e] = xm.re; tab[(15 + 2 * i) * NE + e] = xm.im;
+  }
+}
+// o += r * (2 sigma^{mu nu} F_{mu nu} / 2) with the two 2x2 blocks xp.s, xm.s given (cf. row_sigma_acc)
+template <class R> TREX_HD void row_sigma_acc_x(spinor<R>& o, const spinor<R>& r, const sigF<R>& F) {
+  const cx<R> pt = F.xp[0] + mul_i(F.xp[1]), pb = F.xp[0] - mul_i(F.xp[1]);
+  const cx<R> mt = F.xm[0] + mul_i(F.xm[1]), mb = F.xm[0] - mul_i(F.xm[1]);
+  cfma(o.c[0], r.c[0], F.xp[2]); cfma(o.c[0], r.c[1], pt);
+  cfma(o.c[1], r.c[0], pb);      cfma(o.c[1], -r.c[1], F.xp[2]);
+  cfma(o.c[2], r.c[2], F.xm[2]); cfma(o.c[2], r.c[3], mt);
+  cfma(o.c[3], r.c[2], mb);      cfma(o.c[3], -r.c[3], F.xm[2]);
+}
+
+// ---------------------------------------------------------------- phase 1: one table entry of level K >= 2
+// t[0..K) canonical tuple, fpos[i] = free gluons among t[0..i), fb = helicity bits of the free gluons in position order
+template <class R, int N, int NFIX, int K> struct TabBuild {
+  using I = TabIdx<N, NFIX>;
+  static constexpr int NE = I::NE;
+  const R* tab; const int* off; const rvec4<double>* pset;
+  int t[K], fpos[K + 1]; unsigned fb;
+
+  template <int L> TREX_HD vec4<R> sub(int a) const {
+    int sign;
+    const int nf = fpos[a + L] - fpos[a];
+    const int e = tab_entry<N, NFIX, L>(off, t + a, (fb >> fpos[a]) & ((1u << nf) - 1u), nf, sign);
+    return tab_J<R, NE>(tab, e, sign);
+  }
+  template <int L> TREX_HD unsigned mask(int a) const {
+    unsigned m = 0;
+#pragma unroll
+    for (int i = 0; i < L; ++i) m |= 1u << t[a + i];
+    return m;
+  }
+  // splits (left | right) of the tuple: three-gluon vertex and the contact part of F
+  template <int J1> TREX_HD void v3_splits(vec4<R>& acc, ften<R>& F) const {
+    if constexpr (J1 < K) {
+      const vec4<R> JL = sub<J1>(0), JR = sub<K - J1>(J1);
+      v3_acc(acc, pset[mask<J1>(0)], JL, pset[mask<K - J1>(J1)], JR);
+      wedge_acc(F, JL, JR);
+      v3_splits<J1 + 1>(acc, F);
+    }
+  }
+  template <int J1, int J2> TREX_HD void v4_splits(vec4<R>& acc) const {
+    if constexpr (J2 < K) {
+      const vec4<R> A = sub<J1>(0), B = sub<J2 - J1>(J1), C = sub<K - J2>(J2);
+      v4_acc(acc, A, B, C);
+      if constexpr (J2 + 1 < K) v4_splits<J1, J2 + 1>(acc);
+      else if constexpr (J1 + 2 < K) v4_splits<J1 + 1, J1 + 2>(acc);
+    }
+  }
+  TREX_HD void run(R* tabw, int e) const {
+    vec4<R> acc = vzero<R>();
+    ften<R> F = fzero<R>();
+    v3_splits<1>(acc, F);
+    v4_splits<1, 2>(acc);
+    const rvec4<double>& P = pset[mask<K>(0)];
+    // (-i/P^2) [(-i) V3 + (-i) V4] at g_s = 1; for K == N the propagator is that of the gluon feeding the t t~ line
+    const R s = R(-1.0 / rdot(P, P));
+    vec4<R> J;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) J.c[i] = acc.c[i] * s;
+    wedge_acc(F, cast<R>(P), J);
+    tab_store<R, NE>(tabw, e, J, F);
+  }
+};
+
+template <class R, int N, int NFIX, int K>
+TREX_HD void tab_build_entry(R* __restrict__ tab, const int* __restrict__ meta, const rvec4<double>* __restrict__ pset, int e) {
+  using I = TabIdx<N, NFIX>;
+  TabBuild<R, N, NFIX, K> b;
+  b.tab = tab; b.off = meta + I::M_OFF; b.pset = pset;
+  const int cid = meta[I::M_CID + e];
+  const int packed = meta[I::M_TUP + cid];
+  b.fb = (unsigned)(e - meta[I::M_OFF + cid]);
+  b.fpos[0] = 0;
+#pragma unroll
+  for (int i = 0; i < K; ++i) { b.t[i] = (packed >> (4 * i)) & 15; b.fpos[i + 1] = b.fpos[i] + (b.t[i] >= NFIX ? 1 : 0); }
+  b.run(tab, e);
+}
+// level 1: J = polarisation vector, F = K ^ eps.  eps_all[(g * 2 + lambda) * 8 + (re, im per mu)]
+template <class R, int N, int NFIX>
+TREX_HD void tab_build_level1(R* __restrict__ tab, const int* __restrict__ meta, const rvec4<double>* __restrict__ pset,
+                              const double* __restrict__ eps_all, unsigned itbits, int e) {
+  using I = TabIdx<N, NFIX>;
+  const int g = meta[I::M_CID + e];
+  const int lam = g < NFIX ? (int)((itbits >> g) & 1u) : e - meta[I::M_OFF + g];
+  vec4<R> J;
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) J.c[mu] = cx<R>(R(eps_all[(g * 2 + lam) * 8 + 2 * mu]), R(eps_all[(g * 2 + lam) * 8 + 2 * mu + 1]));
+  ften<R> F = fzero<R>();
+  wedge_acc(F, cast<R>(pset[1u << g]), J);
+  tab_store<R, I::NE>(tab, e, J, F);
+}
+
+// ---------------------------------------------------------------- phase 2: depth-first walk of the top line
+// The first D gluons of the ordering are given (the task); below them every remaining ordering is visited. Private
+// state: the line spinors U[1..N-1] (dual numbers in kappa). Every vertex operand comes from the table.
+template <class R, int N, int NFIX, int D, class Sink> struct TabWalk {
+  using I = TabIdx<N, NFIX>;
+  static constexpr int NE = I::NE;
+  const R* tab; const int* off; const rvec4<double>* pset;
+  rvec4<double> pt;
+  spinor<R> ubar_t;
+  TopLine line;
+  unsigned hfree;                     // helicity bit of free gluon g at bit (g - NFIX)
+  int pref[D];
+  int s[N];                           // ordering prefix
+  unsigned cb;                        // helicity bits of the free gluons of the prefix, in path order
+  int fpos[N + 1];                    // free gluons among s[0..m)
+  unsigned prefmask[N + 1];
+  dspinor<R> U[N];                    // U[m], m = 1..N-1 (U[0] = ubar_t, order 1 = 0)
+  int leaf;
+  Sink* sink;
+
+  template <int M, int A> TREX_HD void bracket_terms(spinor<R>& b0, spinor<R>& b1) {
+    if constexpr (A < M) {
+      int sign;
+      const int e = tab_entry<N, NFIX, M - A>(off, s + A, cb >> fpos[A], fpos[M] - fpos[A], sign);
+      const vec4<R> J = tab_J<R, NE>(tab, e, sign);
+      const spinor<R>& u0 = A == 0 ? ubar_t : U[A].o0;
+      const spinor<R> t0 = row_slash(u0, J);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) b0.c[i] += mul_i(t0.c[i]);
+      if constexpr (A > 0) {
+        const spinor<R> t1 = row_slash(U[A].o1, J);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) b1.c[i] += mul_i(t1.c[i]);
+      }
+      row_sigma_acc_x(b1, u0, tab_F<R, NE>(tab, e, sign));
+      bracket_terms<M, A + 1>(b0, b1);
+    }
+  }
+
+  template <int M> TREX_HD void node(int g) {
+    s[M - 1] = g;
+    const bool isfree = g >= NFIX;
+    const unsigned bit = isfree ? (hfree >> (g - NFIX)) & 1u : 0u;
+    cb = (cb & ((1u << fpos[M - 1]) - 1u)) | (bit << fpos[M - 1]);
+    fpos[M] = fpos[M - 1] + (isfree ? 1 : 0);
+    prefmask[M] = prefmask[M - 1] | (1u << g);
+    spinor<R> b0 = szero<R>(), b1 = szero<R>();
+    bracket_terms<M, 0>(b0, b1);
+    if constexpr (M < N) {
+      const rvec4<double> qd = rsub(pt, pset[prefmask[M]]);
+      const double q2 = rdot(qd, qd);
+      const rvec4<R> q = cast<R>(qd);
+      const cx<double> den(q2 - line.mt * line.mt, line.mGt);
+      const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), den));
+      const spinor<R> s0 = row_slash(b0, q), s1 = row_slash(b1, q);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        cx<R> n0 = s0.c[i]; cfma(n0, b0.c[i], R(line.mt));
+        cx<R> n1 = s1.c[i]; cfma(n1, b1.c[i], R(line.mt));
+        U[M].o0.c[i] = n0 * pr; U[M].o1.c[i] = n1 * pr;
+      }
+      if constexpr (M < D) node<M + 1>(pref[M]);
+      else {
+        // every thread visits the r-th unused gluon at the same trip: uniform control flow across ordering prefixes
+        for (int r = 0; r < N - M; ++r) node<(M < N ? M + 1 : N)>(I::nth_unused(prefmask[M], r));
+      }
+    } else {
+      (*sink)(leaf, b0, b1);
+      ++leaf;
+    }
+  }
+
+  TREX_HD void run(Sink* sk) {
+    sink = sk; leaf = 0; cb = 0; prefmask[0] = 0; fpos[0] = 0;
+    node<1>(pref[0]);
+  }
+};
+
+// the d-th ordered D-tuple of distinct gluons in lexicographic order
+template <int N, int D> TREX_HD void prefix_of_rank(int rank, int* pref) {
+  unsigned used = 0;
+  int radix = TabIdx<N, 0>::falling(N, D);
+#pragma unroll
+  for (int i = 0; i < D; ++i) {
+    radix /= (N - i);
+    int c = rank / radix; rank -= c * radix;
+    int m = 0;
+    for (;; ++m) { if (!((used >> m) & 1u)) { if (c == 0) break; --c; } }
+    pref[i] = m; used |= 1u << m;
+  }
+}
+
+}  // namespace trex

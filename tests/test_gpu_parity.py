@@ -113,6 +113,21 @@ def test_reweight_matches_oracle(T, sid, cfg, nev):
     assert np.all(wo != win)                       # the reweighting really changed something
 
 
+@pytest.mark.parametrize("sid,cfg,nev,algo", [(2, 3, 333, 3), (2, 3, 333, 0), (3, 4, 67, 0), (4, 5, 9, 0), (3, 4, 67, 3)])
+def test_both_evaluation_strategies_match_oracle(T, sid, cfg, nev, algo):
+    """trex_set_algorithm: the fused current-table kernel and the one-thread-per-helicity-unit walk are both oracle-exact."""
+    w = make_config(cfg, n=max(nev, 64))
+    mom = np.ascontiguousarray(w.momenta[:, :, :nev])
+    win = w.w_in[:nev]
+    T.trex_set_algorithm(algo)
+    try:
+        wo, mo, mn = gpu_reweight(T, sid, mom, w.theta_old, w.theta_new, win)
+    finally:
+        T.trex_set_algorithm(4)
+    rw, ro, rn = O.reweight(sid, mom, w.theta_old, w.theta_new, win)
+    assert rel(mo, ro).max() < RTOL64 and rel(mn, rn).max() < RTOL64 and rel(wo, rw).max() < RTOL64
+
+
 @pytest.mark.parametrize("sid", [5, 6, 7, 8])
 def test_quark_channels_match_explicit_colour_oracle(T, sid):
     w = make_config(3, n=2048)
