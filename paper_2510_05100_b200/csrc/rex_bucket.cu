@@ -236,7 +236,9 @@ extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, in
   c.last_nbuckets = 0;
   if (n == 0) { offsets[0] = 0; return 0; }
   // a warp owns `wch` consecutive events; at most 4096 chunks so that the single-block scan stays short
-  long wch = 1024;
+  // (small samples: short chunks, so that the launches still cover the machine)
+  long wch = 64;
+  while (wch < 1024 && (n + wch - 1) / wch > 2368) wch *= 2;
   while ((n + wch - 1) / wch > 4096) wch *= 2;
   const long nchunks = (n + wch - 1) / wch;
   const size_t off_keys = 0, off_first = align_up(off_keys + TS * 8), off_bid = align_up(off_first + TS * 4),
@@ -258,7 +260,8 @@ extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, in
   const unsigned long long* keys = (const unsigned long long*)pdg_keys;
 
   k_init<<<1, TS, 0, c.stream>>>(t);
-  const long per_block = 8192;
+  long per_block = 512;
+  while (per_block < 8192 && (n + per_block - 1) / per_block > 592) per_block *= 2;
   const unsigned nblk = (unsigned)((n + per_block - 1) / per_block);
   k_discover<<<nblk, 256, 0, c.stream>>>(keys, n, per_block, t);
   k_rank<<<1, TS, 0, c.stream>>>(t, res);

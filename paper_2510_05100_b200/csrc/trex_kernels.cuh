@@ -23,15 +23,15 @@ struct ReweightArgs {
 };
 
 // fixed-order reduction over the warps of a block + epilogue by warp 0
-template <class RC> __device__ __forceinline__ void reduce_and_finish(const ReweightArgs& a, RC acc0, RC acc1, long e) {
-  __shared__ double red[2][WARPS][32];
+template <class RC, int NW = WARPS> __device__ __forceinline__ void reduce_and_finish(const ReweightArgs& a, RC acc0, RC acc1, long e) {
+  __shared__ double red[2][NW][32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   red[0][warp][lane] = (double)acc0; red[1][warp][lane] = (double)acc1;
   __syncthreads();
   if (warp == 0 && e < a.n) {
     double s0 = 0.0, s1 = 0.0;
 #pragma unroll
-    for (int w = 0; w < WARPS; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
+    for (int w = 0; w < NW; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
     const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
     const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
     a.w_out[e] = a.w_in[e] * norm * mn;                        // evaluate + append_wgts
@@ -40,9 +40,18 @@ template <class RC> __device__ __forceinline__ void reduce_and_finish(const Rewe
   }
 }
 
+// warps per block and resident blocks per SM the register allocation is sized for
+#ifndef TREX_N2_WARPS
+#define TREX_N2_WARPS 2
+#endif
+#ifndef TREX_N2_MINB
+#define TREX_N2_MINB 4
+#endif
+template <int N> struct TtngGeom { static constexpr int NW = N == 2 ? TREX_N2_WARPS : WARPS, MINB = N == 2 ? TREX_N2_MINB : 1; };
+
 template <class R, class RC, int N, int NPASS>
-__global__ void __launch_bounds__(WARPS * 32) k_ttng(const ReweightArgs a) {
-  constexpr int NU = 1 << (N + 1);
+__global__ void __launch_bounds__(TtngGeom<N>::NW * 32, TtngGeom<N>::MINB) k_ttng(const ReweightArgs a) {
+  constexpr int NU = 1 << (N + 1), WARPS = TtngGeom<N>::NW;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long e = (long)blockIdx.x * 32 + lane;
   const long ev = e < a.n ? e : a.n - 1;
@@ -52,7 +61,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_ttng(const ReweightArgs a) {
     ttng_unit<R, RC, N, NPASS>(a.mom, a.ld, ev, u >> 1, (u & 1) ? 1 : -1, a.T, a.C120, out);
     acc[0] += out[0]; acc[1] += out[1];
   }
-  reduce_and_finish<RC>(a, acc[0], acc[1], e);
+  reduce_and_finish<RC, WARPS>(a, acc[0], acc[1], e);
 }
 
 // one translation unit per (N, precision mode): trex_ttng_tu.cu compiled with -DTREX_TU_N=.. -DTREX_TU_MODE=..

@@ -6,6 +6,8 @@
 // All functions return sum over the unit's helicities of  x^dagger C x  for theta_old and theta_new at g_s = 1;
 // the caller multiplies by g_s^(2 n_vertices) / N_avg.
 #pragma once
+#include <type_traits>
+
 #include "trex_ttng.cuh"
 
 namespace trex {
@@ -99,6 +101,7 @@ template <class R, class RC, int N, int NPASS> struct TtngLeafStore {
   cx<RC> x[NC][2][2];
   spinor<R> v[2];          // v(p_tbar, -), v(p_tbar, +)
   R kq[2];
+  template <int LEAF> TREX_HD void put(const spinor<R>* b0, const spinor<R>* b1) { (*this)(LEAF, b0, b1); }
   TREX_HD void operator()(int leaf, const spinor<R>* b0, const spinor<R>* b1) {
 #pragma unroll
     for (int th = 0; th < 2; ++th) {
@@ -119,7 +122,7 @@ TREX_HD void ttng_unit(const double* __restrict__ mom, long n, long e, int gh, i
   constexpr int NC = factorial(N);
   using Store = TtngLeafStore<R, RC, N, NPASS>;
   Store st;
-  TTNG<R, N, NPASS, Store> t;
+  typename std::conditional<(N <= 2), TTNGS<R, N, NPASS, Store>, TTNG<R, N, NPASS, Store>>::type t;
 #pragma unroll
   for (int g = 0; g < N; ++g) {
     const int leg = g < 2 ? g : g + 2;
@@ -166,6 +169,7 @@ struct QLineLegs { int lrow, lcol, lg; };   // leg numbers; legs 0,1 are incomin
 template <class R> struct QqLeafStore {
   cx<R> a0[2][2], a1[2][2];   // [leaf][v]
   spinor<R> v[2];
+  template <int LEAF> TREX_HD void put(const spinor<R>* b0, const spinor<R>* b1) { (*this)(LEAF, b0, b1); }
   TREX_HD void operator()(int leaf, const spinor<R>* b0, const spinor<R>* b1) {
 #pragma unroll
     for (int iv = 0; iv < 2; ++iv) { a0[leaf][iv] = row_col(b0[0], v[iv]); a1[leaf][iv] = row_col(b1[0], v[iv]); }
@@ -216,7 +220,7 @@ TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L
   st.v[0] = cast<R>(spinor_v<double>(ptb, -1, false)); st.v[1] = cast<R>(spinor_v<double>(ptb, +1, false));
   spinor<R> ubar_t = cast<R>(bar(spinor_u<double>(pt, lam_t, false)));
   // two-source ordered amplitudes: source 0 = gluon, source 1 = quark-pair current
-  TTNG<R, 2, 1, QqLeafStore<R>> t;
+  TTNGS<R, 2, 1, QqLeafStore<R>> t;
   t.K[0] = Kg; t.eps[0] = eg; t.K[1] = Kq; t.eps[1] = Jq;
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) t.pt.c[mu] = pt[mu];
