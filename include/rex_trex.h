@@ -132,7 +132,7 @@ int trex_set_stream(void* cuda_stream);
 int trex_set_precision(int mode);      /* 0 = fp64 (default), 1 = mixed (amplitudes fp64, colour sum fp32,
                                           PAPER.md:1209 fptype m), 2 = fp32 */
 int trex_get_precision(void);
-/* Evaluation strategy of g g -> t t~ + (N-2) g: processes with N >= algo gluons (algo = 3, 4, 5; default 4) use the
+/* Evaluation strategy of g g -> t t~ + (N-2) g: processes with N >= algo gluons (algo = 3, 4, 5; default 3) use the
  * fused current-table kernel (per-event shared-memory table of off-shell gluon currents shared by all helicities,
  * "helicity recycling"); the others, and all of them for algo = 0, use one thread per helicity unit walking every
  * ordering with private currents. Both evaluate the same colour-ordered recursion. */

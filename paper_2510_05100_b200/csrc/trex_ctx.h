@@ -13,7 +13,7 @@ namespace trex {
 struct Context {
   cudaStream_t stream = nullptr;
   int precision = 0;
-  int table_min_n = 4;               // gluon multiplicities >= this use the fused current-table kernel (trex_set_algorithm)
+  int table_min_n = 3;               // gluon multiplicities >= this use the fused current-table kernel (trex_set_algorithm)
   int nsm = 0;                       // multiprocessors of the device
   int64_t launches = 0;
   char err[512] = {0};

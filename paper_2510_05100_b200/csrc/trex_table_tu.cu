@@ -25,15 +25,34 @@ using TuR = float; using TuRC = float;
 namespace trex {
 namespace {
 
+#ifndef TREX_T3_TB
+#define TREX_T3_TB 128
+#endif
+#ifndef TREX_T3_EPB
+#define TREX_T3_EPB 4
+#endif
+#ifndef TREX_T3_MINB
+#define TREX_T3_MINB 3
+#endif
+#ifndef TREX_T4_TB
+#define TREX_T4_TB 128
+#endif
+#ifndef TREX_T4_MINB
+#define TREX_T4_MINB 2
+#endif
+// NFIX: gluons whose helicity the outer loop fixes; D: depth of the ordering prefix that defines a walk task;
+// TB: threads per block; EPB: events a block works on at the same time, each by its own group of TB / EPB threads
+// (a group of 32 = one warp synchronises with __syncwarp and runs free of the other warps); MINB: blocks per SM
 template <int N> struct TabCfg;
-template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = 2, TB = 96; };
-template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = 2, TB = 256; };
-template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256; };
+template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB; };
+template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = 2, TB = TREX_T4_TB, EPB = 1, MINB = TREX_T4_MINB; };
+template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1; };
 
 template <int NC> struct FoldedC {
   // C'(i,j) = 0 (j < i), C_ii (j == i), 2 C_ij (j > i), stored by rows i for j >= RB floor(i/RB)
   static constexpr int RB = NC % 8 == 0 ? 8 : NC;            // rows per register block (NC = 6: one block)
   static constexpr int NB = NC / RB;
+  static constexpr int NPAIR = (NB + 1) / 2;                 // row blocks are paired (p, NB-1-p) for balance
   __host__ __device__ static constexpr int row_len(int i) { return NC - RB * (i / RB); }
   __host__ __device__ static constexpr int size() { int s = 0; for (int i = 0; i < NC; ++i) s += row_len(i); return s; }
 };
@@ -41,7 +60,8 @@ template <int NC> struct FoldedC {
 template <class R, class RC, int N> struct TabGeom {
   using Cfg = TabCfg<N>;
   using I = TabIdx<N, Cfg::NFIX>;
-  static constexpr int NFIX = Cfg::NFIX, D = Cfg::D, TB = Cfg::TB;
+  static constexpr int NFIX = Cfg::NFIX, D = Cfg::D, TB = Cfg::TB, EPB = Cfg::EPB, GS = TB / EPB;
+  static_assert(GS * EPB == TB && (GS == TB || GS == 32), "an event group is one warp or the whole block");
   static constexpr int NE = I::NE;
   static constexpr int NC = I::falling(N, N);
   static constexpr int NIT = 1 << NFIX;
@@ -51,17 +71,19 @@ template <class R, class RC, int N> struct TabGeom {
   static constexpr int NCOLT = NHL * 4;                      // X tile columns: (hfree, lt, ltb, theta)
   static constexpr int XS = NCOLT + 1;
   static constexpr int NSUB = 1 << N;
-  // shared-memory carve-up (bytes, every region 16-byte aligned)
+  static constexpr int NCI = NCOLT * FoldedC<NC>::NPAIR;     // colour-sum work items (and partial sums) per event
+  // shared-memory carve-up (bytes, every region 16-byte aligned): EPB event slots, then the block-wide constants
   static constexpr size_t al(size_t x) { return (x + 15) / 16 * 16; }
   static constexpr size_t o_tab = 0;
   static constexpr size_t o_x = o_tab + al(sizeof(R) * TAB_NCOMP * NE);
-  static constexpr size_t o_c = o_x + al(sizeof(cx<RC>) * NC * XS);
-  static constexpr size_t o_pset = o_c + al(sizeof(RC) * FoldedC<NC>::size());
+  static constexpr size_t o_pset = o_x + al(sizeof(cx<RC>) * NC * XS);
   static constexpr size_t o_eps = o_pset + al(sizeof(rvec4<double>) * NSUB);
   static constexpr size_t o_spin = o_eps + al(sizeof(double) * 16 * N);
-  static constexpr size_t o_meta = o_spin + al(sizeof(double) * 8 * 4);
-  static constexpr size_t o_red = o_meta + al(sizeof(int) * I::M_SIZE);
-  static constexpr size_t bytes = o_red + al(sizeof(double) * 2 * (TB / 32));
+  static constexpr size_t o_part = o_spin + al(sizeof(double) * 8 * 4);
+  static constexpr size_t slot = o_part + al(sizeof(double) * NCI);
+  static constexpr size_t o_c = slot * EPB;
+  static constexpr size_t o_meta = o_c + al(sizeof(RC) * FoldedC<NC>::size());
+  static constexpr size_t bytes = o_meta + al(sizeof(int) * I::M_SIZE);
 };
 
 // leaf sink of the walk: x_sigma = A0 + (kappa/g_s) A1 for both antitop helicities -> X tile
@@ -87,40 +109,48 @@ template <class R, class RC, int XS> struct TabLeafStore {
   }
 };
 
-template <class R, int N, int NFIX, int K> __device__ __forceinline__ void build_levels(R* tab, const int* meta, const rvec4<double>* pset) {
-  using I = TabIdx<N, NFIX>;
+template <int GS> __device__ __forceinline__ void group_sync() {
+  if constexpr (GS == 32) __syncwarp(); else __syncthreads();
+}
+
+template <class R, class RC, int N, int K> __device__ __forceinline__ void build_levels(unsigned char* sb, const int* meta, int gtid) {
+  using G = TabGeom<R, RC, N>;
+  using I = typename G::I;
   if constexpr (K <= N) {
     const int e1 = meta[I::M_LVL + K + 1];
-    for (int e = meta[I::M_LVL + K] + threadIdx.x; e < e1; e += blockDim.x) tab_build_entry<R, N, NFIX, K>(tab, meta, pset, e);
-    __syncthreads();
-    build_levels<R, N, NFIX, K + 1>(tab, meta, pset);
+    for (int e = meta[I::M_LVL + K] + gtid; e < e1; e += G::GS)
+      tab_build_entry<R, N, G::NFIX, K>(reinterpret_cast<R*>(sb + G::o_tab), meta, reinterpret_cast<const rvec4<double>*>(sb + G::o_pset), e);
+    group_sync<G::GS>();
+    build_levels<R, RC, N, K + 1>(sb, meta, gtid);
   }
 }
 
 template <class R, class RC, int N, int NPASS>
-__global__ void __launch_bounds__(TabCfg<N>::TB, 1) k_table(const ReweightArgs a, const int* __restrict__ gmeta, const double* __restrict__ Cfold) {
+__global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const ReweightArgs a, const int* __restrict__ gmeta, const double* __restrict__ Cfold) {
   using G = TabGeom<R, RC, N>;
   using I = typename G::I;
   using F = FoldedC<G::NC>;
-  constexpr int NFIX = G::NFIX, D = G::D, TB = G::TB, XS = G::XS;
+  constexpr int NFIX = G::NFIX, D = G::D, TB = G::TB, XS = G::XS, EPB = G::EPB, GS = G::GS;
   extern __shared__ __align__(16) unsigned char smem[];
-  R* tab = reinterpret_cast<R*>(smem + G::o_tab);
-  cx<RC>* xs = reinterpret_cast<cx<RC>*>(smem + G::o_x);
   RC* Cs = reinterpret_cast<RC*>(smem + G::o_c);
-  rvec4<double>* pset = reinterpret_cast<rvec4<double>*>(smem + G::o_pset);
-  double* eps_all = reinterpret_cast<double*>(smem + G::o_eps);
-  double* spin = reinterpret_cast<double*>(smem + G::o_spin);
   int* meta = reinterpret_cast<int*>(smem + G::o_meta);
-  double* red = reinterpret_cast<double*>(smem + G::o_red);
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, sl = tid / GS, gtid = tid - sl * GS;
+  unsigned char* sb = smem + sl * G::slot;                    // this group's event slot
+  R* tab = reinterpret_cast<R*>(sb + G::o_tab);
+  cx<RC>* xs = reinterpret_cast<cx<RC>*>(sb + G::o_x);
+  rvec4<double>* pset = reinterpret_cast<rvec4<double>*>(sb + G::o_pset);
+  double* eps_all = reinterpret_cast<double*>(sb + G::o_eps);
+  double* spin = reinterpret_cast<double*>(sb + G::o_spin);
+  double* part = reinterpret_cast<double*>(sb + G::o_part);
 
   for (int i = tid; i < I::M_SIZE; i += TB) meta[i] = gmeta[i];
   for (int i = tid; i < F::size(); i += TB) Cs[i] = RC(Cfold[i]);
+  for (int i = gtid; i < G::NCI; i += GS) part[i] = 0.0;
   __syncthreads();
 
-  for (long e = blockIdx.x; e < a.n; e += gridDim.x) {
+  for (long e = (long)blockIdx.x * EPB + sl; e < a.n; e += (long)gridDim.x * EPB) {
     // ---- per-event set-up: momentum of every gluon subset (incoming convention), polarisation vectors, t / t~ spinors
-    for (int sset = tid; sset < G::NSUB; sset += TB) {
+    for (int sset = gtid; sset < G::NSUB; sset += GS) {
       rvec4<double> P;
 #pragma unroll
       for (int mu = 0; mu < 4; ++mu) P.c[mu] = 0.0;
@@ -133,7 +163,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, 1) k_table(const ReweightArgs a
       }
       pset[sset] = P;
     }
-    for (int it = tid; it < 2 * N + 4; it += TB) {
+    for (int it = gtid; it < 2 * N + 4; it += GS) {
       double p[4];
       if (it < 2 * N) {
         const int g = it >> 1, leg = g < 2 ? g : g + 2;
@@ -149,17 +179,16 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, 1) k_table(const ReweightArgs a
         for (int i = 0; i < 4; ++i) { spin[k * 8 + 2 * i] = sp.c[i].re; spin[k * 8 + 2 * i + 1] = sp.c[i].im; }
       }
     }
-    __syncthreads();
+    group_sync<GS>();
 
-    RC acc0 = RC(0), acc1 = RC(0);
     for (unsigned itb = 0; itb < (unsigned)G::NIT; ++itb) {
       // ---- phase 1: current table of this helicity iteration
-      for (int e1 = tid; e1 < meta[I::M_LVL + 2]; e1 += TB) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
-      __syncthreads();
-      build_levels<R, N, NFIX, 2>(tab, meta, pset);
+      for (int e1 = gtid; e1 < meta[I::M_LVL + 2]; e1 += GS) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
+      group_sync<GS>();
+      build_levels<R, RC, N, 2>(sb, meta, gtid);
 
       // ---- phase 2: top-line walk
-      for (int task = tid; task < G::NTASK * NPASS; task += TB) {
+      for (int task = gtid; task < G::NTASK * NPASS; task += GS) {
         const int pass = task / G::NTASK, r = task - pass * G::NTASK;
         const int hl = r % G::NHL, prank = r / G::NHL;
         using Store = TabLeafStore<R, RC, XS>;
@@ -181,11 +210,12 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, 1) k_table(const ReweightArgs a
         st.kq[0] = R(a.T.kq[0]); st.kq[1] = R(a.T.kq[1]);
         w.run(&st);
       }
-      __syncthreads();
+      group_sync<GS>();
 
-      // ---- phase 3: x^dagger C x of every X column; row blocks paired (p, NB-1-p) for balance
-      constexpr int RB = F::RB, NB = F::NB, NPAIR = (NB + 1) / 2;
-      for (int item = tid; item < G::NCOLT * NPAIR; item += TB) {
+      // ---- phase 3: x^dagger C x of every X column, 8-row register blocks, row blocks paired (p, NB-1-p) for balance.
+      // A work item is always handled by the same thread, so its partial sum accumulates race-free in shared memory.
+      constexpr int RB = F::RB, NB = F::NB;
+      for (int item = gtid; item < G::NCI; item += GS) {
         const int c = item % G::NCOLT, p = item / G::NCOLT;
         RC accl = RC(0);
         for (int side = 0; side < 2; ++side) {
@@ -207,25 +237,27 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, 1) k_table(const ReweightArgs a
 #pragma unroll
           for (int r = 0; r < RB; ++r) { const cx<RC> xj = xs[(RB * b + r) * XS + c]; accl += xj.re * t[r].re + xj.im * t[r].im; }
         }
-        if (c & 1) acc1 += accl; else acc0 += accl;
+        part[item] += (double)accl;
       }
       // no barrier needed here: the next writes to X happen after the barriers of the next iteration's phase 1
     }
+    group_sync<GS>();
 
-    // ---- fixed-order block reduction + epilogue
-    double v0 = (double)acc0, v1 = (double)acc1;
+    // ---- fixed-order reduction of the partial sums (column parity = theta) + epilogue by the group's first warp, which
+    // clears what it has read; the other warps of the group may already set up the next event
+    if (gtid < 32) {
+      double v = 0.0;
+      for (int i = gtid; i < G::NCI; i += 32) { v += part[i]; part[i] = 0.0; }
 #pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) { v0 += __shfl_xor_sync(0xFFFFFFFFu, v0, o); v1 += __shfl_xor_sync(0xFFFFFFFFu, v1, o); }
-    if ((tid & 31) == 0) { red[(tid >> 5) * 2] = v0; red[(tid >> 5) * 2 + 1] = v1; }
-    __syncthreads();
-    if (tid == 0) {
-      double s0 = 0.0, s1 = 0.0;
-      for (int w = 0; w < TB / 32; ++w) { s0 += red[2 * w]; s1 += red[2 * w + 1]; }
-      const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
-      const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
-      a.w_out[e] = a.w_in[e] * norm * mn;                        // evaluate + append_wgts
-      if (a.me2_old) a.me2_old[e] = mo;
-      if (a.me2_new) a.me2_new[e] = mn;
+      for (int o = 16; o >= 2; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+      const double s1 = __shfl_sync(0xFFFFFFFFu, v, 1);
+      if (gtid == 0) {
+        const double mo = v * a.T.pref[0], mn = s1 * a.T.pref[1];
+        const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
+        a.w_out[e] = a.w_in[e] * norm * mn;                        // evaluate + append_wgts
+        if (a.me2_old) a.me2_old[e] = mo;
+        if (a.me2_new) a.me2_new[e] = mn;
+      }
     }
   }
 }
@@ -263,8 +295,8 @@ int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const Reweight
     blocks_per_sm = b1 < b2 ? b1 : b2;
     if (blocks_per_sm < 1) return (int)cudaErrorLaunchOutOfResources;
   }
-  const long want = (long)nsm * blocks_per_sm;
-  const unsigned grid = (unsigned)(a.n < want ? a.n : want);
+  const long want = (long)nsm * blocks_per_sm, have = (a.n + G::EPB - 1) / G::EPB;
+  const unsigned grid = (unsigned)(have < want ? have : want);
   if (npass == 1) k_table<TuR, TuRC, N, 1><<<grid, G::TB, G::bytes, s>>>(a, meta, Cfold);
   else k_table<TuR, TuRC, N, 2><<<grid, G::TB, G::bytes, s>>>(a, meta, Cfold);
   return (int)cudaGetLastError();

@@ -113,7 +113,7 @@ def test_reweight_matches_oracle(T, sid, cfg, nev):
     assert np.all(wo != win)                       # the reweighting really changed something
 
 
-@pytest.mark.parametrize("sid,cfg,nev,algo", [(2, 3, 333, 3), (2, 3, 333, 0), (3, 4, 67, 0), (4, 5, 9, 0), (3, 4, 67, 3)])
+@pytest.mark.parametrize("sid,cfg,nev,algo", [(2, 3, 333, 3), (2, 3, 333, 0), (2, 3, 333, 4), (3, 4, 67, 0), (4, 5, 9, 0), (3, 4, 67, 4), (1, 2, 555, 0)])
 def test_both_evaluation_strategies_match_oracle(T, sid, cfg, nev, algo):
     """trex_set_algorithm: the fused current-table kernel and the one-thread-per-helicity-unit walk are both oracle-exact."""
     w = make_config(cfg, n=max(nev, 64))
@@ -123,8 +123,23 @@ def test_both_evaluation_strategies_match_oracle(T, sid, cfg, nev, algo):
     try:
         wo, mo, mn = gpu_reweight(T, sid, mom, w.theta_old, w.theta_new, win)
     finally:
-        T.trex_set_algorithm(4)
+        T.trex_set_algorithm(3)
     rw, ro, rn = O.reweight(sid, mom, w.theta_old, w.theta_new, win)
+    assert rel(mo, ro).max() < RTOL64 and rel(mn, rn).max() < RTOL64 and rel(wo, rw).max() < RTOL64
+
+
+@pytest.mark.parametrize("sid,cfg,nev", [(1, 2, 300), (2, 3, 70), (4, 5, 5), (5, 3, 20)])
+def test_top_width_and_mass_change_two_pass_kernels(T, sid, cfg, nev):
+    """theta_new with another top width / mass: the top line is carried once per parameter point (NPASS = 2 kernels)."""
+    w = make_config(cfg, n=4096)
+    sel = np.where(w.keys == SUBPROCESSES[sid].key)[0][:nev]
+    mom = np.ascontiguousarray(w.momenta[:, :, sel])
+    tho, thn = w.theta_old.copy(), w.theta_new.copy()
+    tho[6], thn[6] = 1.5, 1.2                      # Gamma_t
+    if sid == 1:
+        thn[5] = 171.5                             # m_t enters the propagators only through theta: externals keep their momenta
+    wo, mo, mn = gpu_reweight(T, sid, mom, tho, thn, w.w_in[sel])
+    rw, ro, rn = O.reweight(sid, mom, tho, thn, w.w_in[sel])
     assert rel(mo, ro).max() < RTOL64 and rel(mn, rn).max() < RTOL64 and rel(wo, rw).max() < RTOL64
 
 
