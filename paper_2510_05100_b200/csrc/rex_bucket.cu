@@ -89,20 +89,24 @@ __global__ void __launch_bounds__(256) k_discover(const unsigned long long* __re
 }
 
 __global__ void __launch_bounds__(TS) k_rank(Table t, BucketResult* res) {
-  __shared__ unsigned sf[TS];
+  __shared__ unsigned sf[NBMAX + 1];
+  __shared__ int s_cnt;
   const int s = threadIdx.x;
+  if (s == 0) s_cnt = 0;
+  __syncthreads();
   const unsigned long long k = t.keys[s];
   const unsigned f = t.first[s];
-  sf[s] = (k == EMPTY) ? 0xFFFFFFFFu : f;
+  // the occupied slots are few (one per class): compact their first-appearance indices, then rank among those
+  if (k != EMPTY) { const int j = atomicAdd(&s_cnt, 1); if (j <= NBMAX) sf[j] = f; }
   __syncthreads();
   const int nd = t.meta[0], has_npos = t.meta[1];
   const int nb = nd + has_npos;
   const bool bad = (nb > NBMAX) || t.meta[2];
-  if (k != EMPTY) {
+  if (k != EMPTY && !bad) {
     int rank = 0;
-    for (int j = 0; j < TS; ++j) rank += (sf[j] < f) ? 1 : 0;
+    for (int j = 0; j < nd; ++j) rank += (sf[j] < f) ? 1 : 0;
     t.bid[s] = rank;
-    if (!bad) res->keys[rank] = k;
+    res->keys[rank] = k;
   }
   if (s == 0) {
     t.meta[3] = bad ? 0 : nb;
@@ -148,7 +152,8 @@ __global__ void __launch_bounds__(WARPS * 32) k_hist(const unsigned long long* _
   for (int b = lane; b < nb; b += 32) counts[(long)b * nchunks + chunk] = hist[warp][b];
 }
 
-__global__ void __launch_bounds__(1024) k_scan(unsigned* __restrict__ counts, long nchunks, long n, Table t, BucketResult* res) {
+__global__ void __launch_bounds__(1024) k_scan(unsigned* __restrict__ counts, long nchunks, long n, Table t, BucketResult* res,
+                                               const unsigned long long* __restrict__ sub, int npar, DevPlan* __restrict__ plan) {
   __shared__ unsigned long long part[1024];
   const int nb = t.meta[3];
   const long total = (long)nb * nchunks;
@@ -173,6 +178,21 @@ __global__ void __launch_bounds__(1024) k_scan(unsigned* __restrict__ counts, lo
     run += c;
   }
   if (threadIdx.x == 0) res->offsets[nb] = nb ? n : 0;
+  if (npar <= 0) return;
+  // device plan of trex_run: bucket of every compiled-in subprocess (key in sub[2 sid], leg count in sub[2 sid + 1])
+  __threadfence_block();
+  __syncthreads();
+  const int sid = threadIdx.x;
+  bool found = false;
+  if (sid < TREX_NSUBPROC) {
+    long long off = 0, cnt = 0;
+    if ((int)sub[2 * sid + 1] == npar)
+      for (int b = 0; b < nb; ++b)
+        if (res->keys[b] == sub[2 * sid]) { off = res->offsets[b]; cnt = res->offsets[b + 1] - off; found = true; }
+    plan->off[sid] = off; plan->cnt[sid] = cnt;
+  }
+  const int any = __syncthreads_or(found ? 1 : 0);
+  if (sid == 0) { plan->single = (nb == 1 && any) ? 1 : 0; plan->nb = nb; }
 }
 
 __global__ void __launch_bounds__(WARPS * 32) k_scatter(const unsigned long long* __restrict__ keys, long n, long wch, long nchunks,
@@ -221,6 +241,155 @@ __global__ void k_scatter_rows(const double* __restrict__ src, long n_src, doubl
   for (int r = 0; r < nrows; ++r) dst[(long)r * n_dst + p] = src[(long)r * n_src + j];
 }
 
+// ---------------------------------------------------------------- small samples: the whole chain in ONE block
+// For n <= SMALL_N the six launches above are latency, not bandwidth: one block of 1024 threads does discover -> rank ->
+// per-warp histogram -> scan -> stable scatter (+ the device plan of trex_run) with block barriers in between. Same
+// definitions, same result bit for bit: bucket id = rank of the key's first appearance, REX_NPOS last, a warp owns a
+// contiguous chunk and ranks equal buckets with __match_any_sync.
+constexpr long SMALL_N = 8192;      // beyond this one SM's load latency loses against six launches (16-bit counts: n <= 65536)
+constexpr int SB_WARPS = 32;
+
+__global__ void __launch_bounds__(1024) k_bucket_small(const unsigned long long* __restrict__ keys, long n, int* __restrict__ perm,
+                                                       BucketResult* __restrict__ res, const unsigned long long* __restrict__ sub,
+                                                       int npar, DevPlan* __restrict__ plan) {
+  __shared__ unsigned long long sk[TS];
+  __shared__ unsigned sf[TS];
+  __shared__ int sb[TS];
+  __shared__ unsigned short cnt[SB_WARPS][NBMAX + 1];     // per (warp, bucket) counts, then write cursors relative to the bucket
+  __shared__ unsigned s_npos;
+  __shared__ int s_over, s_nd;
+  __shared__ int slots[NBMAX + 1];
+  __shared__ long long boff[NBMAX + 2];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  sk[tid] = EMPTY; sf[tid] = 0xFFFFFFFFu; sb[tid] = -1;
+  if (tid == 0) { s_npos = 0xFFFFFFFFu; s_over = 0; s_nd = 0; }
+  __syncthreads();
+  // discover
+  for (long i = tid; i < n; i += 1024) {
+    const unsigned long long k = keys[i];
+    if (k == EMPTY) { if ((unsigned)i < s_npos) atomicMin(&s_npos, (unsigned)i); continue; }
+    const unsigned h = hash_key(k);
+    int slot = -1;
+    for (int probe = 0; probe < TS; ++probe) {
+      const unsigned s = (h + probe) & (TS - 1);
+      unsigned long long cur = sk[s];
+      if (cur == EMPTY) cur = atomicCAS(&sk[s], EMPTY, k);
+      if (cur == EMPTY || cur == k) { slot = (int)s; break; }
+    }
+    if (slot < 0) { s_over = 1; continue; }
+    if ((unsigned)i < sf[slot]) atomicMin(&sf[slot], (unsigned)i);
+  }
+  __syncthreads();
+  // rank: compact the occupied slots, rank them by first appearance
+  if (sk[tid] != EMPTY) { const int j = atomicAdd(&s_nd, 1); if (j <= NBMAX) slots[j] = tid; }
+  __syncthreads();
+  const int nd = s_nd, has_npos = s_npos != 0xFFFFFFFFu ? 1 : 0;
+  const int nbr = nd + has_npos;
+  const bool bad = nbr > NBMAX || s_over;
+  const int nb = bad ? 0 : nbr;
+  if (!bad && tid < nd) {
+    const int s = slots[tid];
+    int rank = 0;
+    for (int j = 0; j < nd; ++j) rank += sf[slots[j]] < sf[s] ? 1 : 0;
+    sb[s] = rank;
+    res->keys[rank] = sk[s];
+  }
+  if (tid == 0) { res->nb = nb; res->err = bad ? 1 : 0; if (!bad && has_npos) res->keys[nd] = EMPTY; }
+  for (int i = lane; i <= NBMAX; i += 32) cnt[warp][i] = 0;
+  __syncthreads();
+  auto lookup = [&](unsigned long long key) -> int {
+    if (key == EMPTY) return nb - 1;
+    const unsigned h = hash_key(key);
+    for (int probe = 0; probe < TS; ++probe) { const unsigned s = (h + probe) & (TS - 1); if (sk[s] == key) return sb[s]; }
+    return nb - 1;
+  };
+  // histogram: warp w owns events [w * wch, (w + 1) * wch)
+  const long wch = (n + SB_WARPS - 1) / SB_WARPS;
+  const long lo = min(n, warp * wch), hi = min(n, lo + wch);
+  if (nb) {
+    for (long i0 = lo; i0 < hi; i0 += 32) {
+      const long i = i0 + lane;
+      const bool live = i < hi;
+      const unsigned active = __ballot_sync(0xFFFFFFFFu, live);
+      if (live) {
+        const int b = lookup(keys[i]);
+        const unsigned peers = __match_any_sync(active, b);
+        if (lane == __ffs(peers) - 1) cnt[warp][b] += (unsigned short)__popc(peers);
+      }
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+  // scan: bucket totals (thread b), bucket offsets (thread 0), per-warp write cursors (thread b)
+  if (tid < nb) {
+    unsigned run = 0;
+    for (int w = 0; w < SB_WARPS; ++w) { const unsigned c = cnt[w][tid]; cnt[w][tid] = (unsigned short)run; run += c; }
+    boff[tid + 1] = run;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    long long run = 0;
+    boff[0] = 0;
+    for (int b = 0; b < nb; ++b) { const long long c = boff[b + 1]; boff[b] = run; run += c; }
+    boff[nb] = nb ? n : 0;
+  }
+  __syncthreads();
+  if (tid <= nb) res->offsets[tid] = boff[tid];
+  // stable scatter
+  if (nb) {
+    for (long i0 = lo; i0 < hi; i0 += 32) {
+      const long i = i0 + lane;
+      const bool live = i < hi;
+      const unsigned active = __ballot_sync(0xFFFFFFFFu, live);
+      if (live) {
+        const int b = lookup(keys[i]);
+        const unsigned peers = __match_any_sync(active, b);
+        const unsigned rank = __popc(peers & ((1u << lane) - 1u));
+        perm[boff[b] + cnt[warp][b] + rank] = (int)i;
+        __syncwarp(active);
+        if (rank == 0) cnt[warp][b] += (unsigned short)__popc(peers);
+      }
+      __syncwarp();
+    }
+  }
+  // device plan of trex_run
+  if (npar > 0) {
+    bool found = false;
+    if (tid < TREX_NSUBPROC) {
+      long long off = 0, c = 0;
+      if ((int)sub[2 * tid + 1] == npar)
+        for (int b = 0; b < nd && !bad; ++b)
+          if (sk[slots[b]] == sub[2 * tid]) { const int r = sb[slots[b]]; off = boff[r]; c = boff[r + 1] - off; found = true; }
+      plan->off[tid] = off; plan->cnt[tid] = c;
+    }
+    const int any = __syncthreads_or(found ? 1 : 0);
+    if (tid == 0) { plan->single = (nb == 1 && any) ? 1 : 0; plan->nb = nb; }
+  }
+}
+
+// momenta rows + weights into bucketed order; result rows cleared (classes nobody claims keep zero weights)
+__global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __restrict__ mom, const double* __restrict__ w_in, long n,
+                             int nrows, const int* __restrict__ perm, double* __restrict__ blk, double* __restrict__ res) {
+  if (plan->single) return;
+  const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const long p = perm[j];
+  for (int r = 0; r < nrows; ++r) blk[(long)r * n + j] = mom[(long)r * n + p];
+  blk[(long)nrows * n + j] = w_in[p];
+  res[j] = 0.0; res[n + j] = 0.0; res[2 * n + j] = 0.0;
+}
+
+__global__ void k_run_scatter(const DevPlan* __restrict__ plan, const double* __restrict__ res, long n, const int* __restrict__ perm,
+                              double* __restrict__ w_out, double* __restrict__ me2_old, double* __restrict__ me2_new) {
+  if (plan->single) return;
+  const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const long p = perm[j];
+  w_out[p] = res[j];
+  if (me2_old) me2_old[p] = res[n + j];
+  if (me2_new) me2_new[p] = res[2 * n + j];
+}
+
 size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
 
 }  // namespace
@@ -229,36 +398,59 @@ size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
 
 using namespace trex;
 
-extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int64_t* offsets) {
-  Context& c = ctx();
-  if (n < 0 || !offsets || (n > 0 && (!pdg_keys || !perm))) return fail(TREX_EINVAL, "rex_bucket: null pointer or negative n");
-  if (n >= (int64_t(1) << 31)) return fail(TREX_EINVAL, "rex_bucket: n must be < 2^31 (perm is int32)");
-  c.last_nbuckets = 0;
-  if (n == 0) { offsets[0] = 0; return 0; }
+namespace {
+struct BucketLayout {
+  long wch, nchunks;
+  size_t off_keys, off_first, off_bid, off_meta, off_npos, off_res, off_counts, total;
+};
+BucketLayout bucket_layout(int64_t n) {
+  BucketLayout L;
   // a warp owns `wch` consecutive events; at most 4096 chunks so that the single-block scan stays short
   // (small samples: short chunks, so that the launches still cover the machine)
-  long wch = 64;
-  while (wch < 1024 && (n + wch - 1) / wch > 2368) wch *= 2;
-  while ((n + wch - 1) / wch > 4096) wch *= 2;
-  const long nchunks = (n + wch - 1) / wch;
-  const size_t off_keys = 0, off_first = align_up(off_keys + TS * 8), off_bid = align_up(off_first + TS * 4),
-               off_meta = align_up(off_bid + TS * 4), off_npos = align_up(off_meta + 16), off_res = align_up(off_npos + 4),
-               off_counts = align_up(off_res + sizeof(BucketResult)),
-               total = align_up(off_counts + (size_t)NBMAX * nchunks * 4);
-  if (c.bucket_scratch_bytes < total) {
+  L.wch = 64;
+  while (L.wch < 1024 && (n + L.wch - 1) / L.wch > 2368) L.wch *= 2;
+  while ((n + L.wch - 1) / L.wch > 4096) L.wch *= 2;
+  L.nchunks = (n + L.wch - 1) / L.wch;
+  L.off_keys = 0; L.off_first = align_up(L.off_keys + TS * 8); L.off_bid = align_up(L.off_first + TS * 4);
+  L.off_meta = align_up(L.off_bid + TS * 4); L.off_npos = align_up(L.off_meta + 16); L.off_res = align_up(L.off_npos + 4);
+  L.off_counts = align_up(L.off_res + sizeof(BucketResult));
+  L.total = align_up(L.off_counts + (size_t)NBMAX * L.nchunks * 4);
+  return L;
+}
+}  // namespace
+
+int trex::bucket_reserve(int64_t n) {
+  Context& c = ctx();
+  const BucketLayout L = bucket_layout(n);
+  if (c.bucket_scratch_bytes < L.total) {
+    c.exec_valid = false;                             // a captured trex_run graph holds the old address
     if (c.bucket_scratch) cudaFree(c.bucket_scratch);
     c.bucket_scratch = nullptr; c.bucket_scratch_bytes = 0;
-    TREX_CUDA_CHECK(cudaMalloc(&c.bucket_scratch, total));
-    c.bucket_scratch_bytes = total;
+    TREX_CUDA_CHECK(cudaMalloc(&c.bucket_scratch, L.total));
+    c.bucket_scratch_bytes = L.total;
   }
   if (!c.bucket_host) TREX_CUDA_CHECK(cudaMallocHost(&c.bucket_host, sizeof(BucketResult)));
+  return 0;
+}
+
+int trex::bucket_enqueue(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int npar) {
+  Context& c = ctx();
+  const BucketLayout L = bucket_layout(n);
+  const long wch = L.wch, nchunks = L.nchunks;
   char* base = (char*)c.bucket_scratch;
-  Table t{(unsigned long long*)(base + off_keys), (unsigned*)(base + off_first), (int*)(base + off_bid),
-          (int*)(base + off_meta), (unsigned*)(base + off_npos)};
-  BucketResult* res = (BucketResult*)(base + off_res);
-  unsigned* counts = (unsigned*)(base + off_counts);
+  Table t{(unsigned long long*)(base + L.off_keys), (unsigned*)(base + L.off_first), (int*)(base + L.off_bid),
+          (int*)(base + L.off_meta), (unsigned*)(base + L.off_npos)};
+  BucketResult* res = (BucketResult*)(base + L.off_res);
+  unsigned* counts = (unsigned*)(base + L.off_counts);
   const unsigned long long* keys = (const unsigned long long*)pdg_keys;
 
+  if (n <= SMALL_N) {
+    k_bucket_small<<<1, 1024, 0, c.stream>>>(keys, n, perm, res, (const unsigned long long*)c.plan_keys, npar, c.plan);
+    c.launches += 1;
+    TREX_CUDA_CHECK(cudaGetLastError());
+    TREX_CUDA_CHECK(cudaMemcpyAsync(c.bucket_host, res, sizeof(BucketResult), cudaMemcpyDeviceToHost, c.stream));
+    return 0;
+  }
   k_init<<<1, TS, 0, c.stream>>>(t);
   long per_block = 512;
   while (per_block < 8192 && (n + per_block - 1) / per_block > 592) per_block *= 2;
@@ -267,11 +459,16 @@ extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, in
   k_rank<<<1, TS, 0, c.stream>>>(t, res);
   const unsigned cblk = (unsigned)((nchunks + WARPS - 1) / WARPS);
   k_hist<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts);
-  k_scan<<<1, 1024, 0, c.stream>>>(counts, nchunks, n, t, res);
+  k_scan<<<1, 1024, 0, c.stream>>>(counts, nchunks, n, t, res, (const unsigned long long*)c.plan_keys, npar, c.plan);
   k_scatter<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts, perm);
   c.launches += 6;
   TREX_CUDA_CHECK(cudaGetLastError());
   TREX_CUDA_CHECK(cudaMemcpyAsync(c.bucket_host, res, sizeof(BucketResult), cudaMemcpyDeviceToHost, c.stream));
+  return 0;
+}
+
+int trex::bucket_finish(int64_t* offsets) {
+  Context& c = ctx();
   TREX_CUDA_CHECK(cudaStreamSynchronize(c.stream));
   const BucketResult* h = (const BucketResult*)c.bucket_host;
   if (h->err) return fail(TREX_EINVAL, "rex_bucket: more than %d distinct flavour keys", REX_MAX_BUCKETS);
@@ -279,6 +476,33 @@ extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, in
   for (int b = 0; b < h->nb; ++b) c.last_keys[b] = h->keys[b];
   c.last_nbuckets = h->nb;
   return h->nb;
+}
+
+extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int64_t* offsets) {
+  Context& c = ctx();
+  if (n < 0 || !offsets || (n > 0 && (!pdg_keys || !perm))) return fail(TREX_EINVAL, "rex_bucket: null pointer or negative n");
+  if (n >= (int64_t(1) << 31)) return fail(TREX_EINVAL, "rex_bucket: n must be < 2^31 (perm is int32)");
+  c.last_nbuckets = 0;
+  if (n == 0) { offsets[0] = 0; return 0; }
+  if (int rc = bucket_reserve(n)) return rc;
+  if (int rc = bucket_enqueue(pdg_keys, n, perm, 0)) return rc;
+  return bucket_finish(offsets);
+}
+
+int trex::run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* perm, double* blk, double* res) {
+  Context& c = ctx();
+  k_run_gather<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, mom, w_in, n, nrows, perm, blk, res);
+  c.launches += 1;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return 0;
+}
+
+int trex::run_scatter(const double* res, int64_t n, const int32_t* perm, double* w_out, double* me2_old, double* me2_new) {
+  Context& c = ctx();
+  k_run_scatter<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, res, n, perm, w_out, me2_old, me2_new);
+  c.launches += 1;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return 0;
 }
 
 extern "C" int rex_bucket_keys(uint64_t* bucket_keys) {

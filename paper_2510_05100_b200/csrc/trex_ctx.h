@@ -10,6 +10,15 @@
 
 namespace trex {
 
+// Device-resident plan of one trex_run: where every compiled-in subprocess finds its events in bucketed order. Written
+// by the last kernel of rex_bucket's chain, read by every later kernel of the run -- the host never waits for it.
+struct DevPlan {
+  long long off[TREX_NSUBPROC];   // first event of the subprocess's bucket in bucketed order
+  long long cnt[TREX_NSUBPROC];   // events of that bucket (0: subprocess absent from the sample, or leg count mismatch)
+  int single;                     // 1: the sample is ONE known class -> kernels work on the caller's arrays, no transposition
+  int nb;
+};
+
 struct Context {
   cudaStream_t stream = nullptr;
   int precision = 0;
@@ -28,6 +37,17 @@ struct Context {
   void* run_blocks = nullptr; size_t run_blocks_bytes = 0;
   void* host_io = nullptr; size_t host_io_bytes = 0;
   void* probe_out = nullptr;
+  // trex_run replayed as a CUDA graph when it is called again with the same buffers, sizes and parameter points
+  struct RunKey {
+    const void* ptr[6]; int64_t n; int npar, precision, table_min_n; double th[2 * TREX_NTHETA];
+  };
+  bool in_host_run = false;
+  RunKey last_key{}; bool last_key_valid = false;
+  RunKey exec_key{}; bool exec_valid = false; bool graphs_ok = true;
+  cudaGraphExec_t run_exec = nullptr; int64_t exec_launches = 0;
+  cudaStream_t cap_stream = nullptr;
+  DevPlan* plan = nullptr;           // device
+  void* plan_keys = nullptr;         // device: key and leg count of every compiled-in subprocess
   // colour matrices on the device
   bool colour_ready = false;
   double* C120 = nullptr;            // 120 x 120, global memory
@@ -36,6 +56,15 @@ struct Context {
 };
 
 Context& ctx();
+
+// rex_bucket in two halves (rex_bucket.cu): enqueue the kernel chain (+ the device plan for a run over `npar`-leg events,
+// if sub_keys != nullptr), then fetch sizes and keys -- the only point where the host waits for the device
+int bucket_reserve(int64_t n);          // (re)allocates the scratch of bucket_enqueue; never called while capturing
+int bucket_enqueue(const uint64_t* keys, int64_t n, int32_t* perm, int npar);
+int bucket_finish(int64_t* offsets);
+// transposition kernels of trex_run driven by the device plan (both are no-ops for a single-class sample)
+int run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* perm, double* blk, double* res);
+int run_scatter(const double* res, int64_t n, const int32_t* perm, double* w_out, double* me2_old, double* me2_new);
 
 inline int fail(int code, const char* fmt, ...) {
   va_list ap;

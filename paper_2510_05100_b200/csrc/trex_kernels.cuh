@@ -8,35 +8,56 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "trex_ctx.h"
 #include "trex_proc.cuh"
 
 namespace trex {
 
 constexpr int WARPS = 8;
 
-struct ReweightArgs {
+struct EvIO {
   const double* mom; long n; long ld;   // ld = row stride of the SoA block (== n for a caller-provided block)
   const double* w_in; double* w_out; double* me2_old; double* me2_new;
+};
+struct ReweightArgs {
+  EvIO io;                 // the caller's arrays (trex_reweight; single-class samples in trex_run)
+  EvIO alt;                // trex_run's scratch in bucketed order (mom, w_in, results), ld = sample size
+  const DevPlan* plan;     // trex_run: device-resident bucket ranges; nullptr for trex_reweight
+  int sid;
   const double* C120;
   ThetaPair T;
   QLineLegs q;
 };
 
+// which events this launch works on: decided on the device for trex_run (the host has not seen the bucket sizes)
+__device__ __forceinline__ EvIO resolve_io(const ReweightArgs& a) {
+  EvIO io = a.io;
+  if (a.plan) {
+    const long off = a.plan->off[a.sid], cnt = a.plan->cnt[a.sid];
+    if (!a.plan->single) {
+      io = a.alt;
+      io.mom += off; io.w_in += off; io.w_out += off; io.me2_old += off; io.me2_new += off;
+    }
+    io.n = cnt;
+  }
+  return io;
+}
+
 // fixed-order reduction over the warps of a block + epilogue by warp 0
-template <class RC, int NW = WARPS> __device__ __forceinline__ void reduce_and_finish(const ReweightArgs& a, RC acc0, RC acc1, long e) {
+template <class RC, int NW = WARPS> __device__ __forceinline__ void reduce_and_finish(const ReweightArgs& a, const EvIO& io, RC acc0, RC acc1, long e) {
   __shared__ double red[2][NW][32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   red[0][warp][lane] = (double)acc0; red[1][warp][lane] = (double)acc1;
   __syncthreads();
-  if (warp == 0 && e < a.n) {
+  if (warp == 0 && e < io.n) {
     double s0 = 0.0, s1 = 0.0;
 #pragma unroll
     for (int w = 0; w < NW; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
     const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
     const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
-    a.w_out[e] = a.w_in[e] * norm * mn;                        // evaluate + append_wgts
-    if (a.me2_old) a.me2_old[e] = mo;
-    if (a.me2_new) a.me2_new[e] = mn;
+    io.w_out[e] = io.w_in[e] * norm * mn;                        // evaluate + append_wgts
+    if (io.me2_old) io.me2_old[e] = mo;
+    if (io.me2_new) io.me2_new[e] = mn;
   }
 }
 
@@ -52,16 +73,18 @@ template <int N> struct TtngGeom { static constexpr int NW = N == 2 ? TREX_N2_WA
 template <class R, class RC, int N, int NPASS>
 __global__ void __launch_bounds__(TtngGeom<N>::NW * 32, TtngGeom<N>::MINB) k_ttng(const ReweightArgs a) {
   constexpr int NU = 1 << (N + 1), WARPS = TtngGeom<N>::NW;
+  const EvIO io = resolve_io(a);
+  if ((long)blockIdx.x * 32 >= io.n) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long e = (long)blockIdx.x * 32 + lane;
-  const long ev = e < a.n ? e : a.n - 1;
+  const long ev = e < io.n ? e : io.n - 1;
   RC acc[2] = {RC(0), RC(0)};
   for (int u = warp; u < NU; u += WARPS) {
     RC out[2];
-    ttng_unit<R, RC, N, NPASS>(a.mom, a.ld, ev, u >> 1, (u & 1) ? 1 : -1, a.T, a.C120, out);
+    ttng_unit<R, RC, N, NPASS>(io.mom, io.ld, ev, u >> 1, (u & 1) ? 1 : -1, a.T, a.C120, out);
     acc[0] += out[0]; acc[1] += out[1];
   }
-  reduce_and_finish<RC, WARPS>(a, acc[0], acc[1], e);
+  reduce_and_finish<RC, WARPS>(a, io, acc[0], acc[1], e);
 }
 
 // one translation unit per (N, precision mode): trex_ttng_tu.cu compiled with -DTREX_TU_N=.. -DTREX_TU_MODE=..
@@ -77,11 +100,11 @@ TREX_TU_DECL(5, 0) TREX_TU_DECL(5, 1) TREX_TU_DECL(5, 2)
 #undef TREX_TU_DECL
 
 // fused current-table kernels (trex_table_tu.cu), one translation unit per (N = 3, 4, 5; precision mode)
-using TableLaunchFn = int (*)(const ReweightArgs&, int npass, const int* meta, const double* Cfold, int nsm, cudaStream_t);
+using TableLaunchFn = int (*)(const ReweightArgs&, int npass, long nmax, const int* meta, const double* Cfold, int nsm, cudaStream_t);
 using TableMetaFn = int (*)(int* meta);                       // fills the meta block (if non-null), returns its size in ints
 using TableFoldFn = int (*)(const double* C, double* f);      // fills the folded colour matrix (if non-null), returns its size
 #define TREX_TABLE_DECL(N, M)                                                                                       \
-  int trex_tu_table_launch_n##N##_m##M(const ReweightArgs&, int npass, const int* meta, const double* Cfold, int nsm, cudaStream_t); \
+  int trex_tu_table_launch_n##N##_m##M(const ReweightArgs&, int npass, long nmax, const int* meta, const double* Cfold, int nsm, cudaStream_t); \
   int trex_tu_table_meta_n##N##_m##M(int* meta);                                                                    \
   int trex_tu_table_fold_n##N##_m##M(const double* C, double* f);
 TREX_TABLE_DECL(3, 0) TREX_TABLE_DECL(3, 1) TREX_TABLE_DECL(3, 2)

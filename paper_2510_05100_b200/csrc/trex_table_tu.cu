@@ -143,12 +143,13 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
   double* spin = reinterpret_cast<double*>(sb + G::o_spin);
   double* part = reinterpret_cast<double*>(sb + G::o_part);
 
+  const EvIO io = resolve_io(a);
   for (int i = tid; i < I::M_SIZE; i += TB) meta[i] = gmeta[i];
   for (int i = tid; i < F::size(); i += TB) Cs[i] = RC(Cfold[i]);
   for (int i = gtid; i < G::NCI; i += GS) part[i] = 0.0;
   __syncthreads();
 
-  for (long e = (long)blockIdx.x * EPB + sl; e < a.n; e += (long)gridDim.x * EPB) {
+  for (long e = (long)blockIdx.x * EPB + sl; e < io.n; e += (long)gridDim.x * EPB) {
     // ---- per-event set-up: momentum of every gluon subset (incoming convention), polarisation vectors, t / t~ spinors
     for (int sset = gtid; sset < G::NSUB; sset += GS) {
       rvec4<double> P;
@@ -159,7 +160,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
         const int leg = g < 2 ? g : g + 2;
         const double sg = g < 2 ? 1.0 : -1.0;
 #pragma unroll
-        for (int mu = 0; mu < 4; ++mu) P.c[mu] += sg * a.mom[(long)(leg * 4 + mu) * a.ld + e];
+        for (int mu = 0; mu < 4; ++mu) P.c[mu] += sg * io.mom[(long)(leg * 4 + mu) * io.ld + e];
       }
       pset[sset] = P;
     }
@@ -167,13 +168,13 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
       double p[4];
       if (it < 2 * N) {
         const int g = it >> 1, leg = g < 2 ? g : g + 2;
-        load_leg<double>(a.mom, a.ld, e, leg, p);
+        load_leg<double>(io.mom, io.ld, e, leg, p);
         const vec4<double> ev = polvec<double>(p, (it & 1) ? 1 : -1, g >= 2);
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) { eps_all[it * 8 + 2 * mu] = ev.c[mu].re; eps_all[it * 8 + 2 * mu + 1] = ev.c[mu].im; }
       } else {
         const int k = it - 2 * N;                          // 0, 1: ubar(p_t, -/+); 2, 3: v(p_tbar, -/+)
-        load_leg<double>(a.mom, a.ld, e, k < 2 ? 2 : 3, p);
+        load_leg<double>(io.mom, io.ld, e, k < 2 ? 2 : 3, p);
         const spinor<double> sp = k < 2 ? bar(spinor_u<double>(p, (k & 1) ? 1 : -1, false)) : spinor_v<double>(p, (k & 1) ? 1 : -1, false);
 #pragma unroll
         for (int i = 0; i < 4; ++i) { spin[k * 8 + 2 * i] = sp.c[i].re; spin[k * 8 + 2 * i + 1] = sp.c[i].im; }
@@ -197,7 +198,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
         prefix_of_rank<N, D>(prank, w.pref);
         const int lt = hl & 1;
 #pragma unroll
-        for (int mu = 0; mu < 4; ++mu) w.pt.c[mu] = a.mom[(long)(2 * 4 + mu) * a.ld + e];
+        for (int mu = 0; mu < 4; ++mu) w.pt.c[mu] = io.mom[(long)(2 * 4 + mu) * io.ld + e];
 #pragma unroll
         for (int i = 0; i < 4; ++i) w.ubar_t.c[i] = cx<R>(R(spin[lt * 8 + 2 * i]), R(spin[lt * 8 + 2 * i + 1]));
         w.tab = tab; w.off = meta + I::M_OFF; w.pset = pset;
@@ -254,9 +255,9 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
       if (gtid == 0) {
         const double mo = v * a.T.pref[0], mn = s1 * a.T.pref[1];
         const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
-        a.w_out[e] = a.w_in[e] * norm * mn;                        // evaluate + append_wgts
-        if (a.me2_old) a.me2_old[e] = mo;
-        if (a.me2_new) a.me2_new[e] = mn;
+        io.w_out[e] = io.w_in[e] * norm * mn;                        // evaluate + append_wgts
+        if (io.me2_old) io.me2_old[e] = mo;
+        if (io.me2_new) io.me2_new[e] = mn;
       }
     }
   }
@@ -281,7 +282,7 @@ int TREX_TU_NAME(trex_tu_table_fold_n, TREX_TU_N, TREX_TU_MODE)(const double* C,
   return F::size();
 }
 
-int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const ReweightArgs& a, int npass, const int* meta, const double* Cfold,
+int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const ReweightArgs& a, int npass, long nmax, const int* meta, const double* Cfold,
                                                                   int nsm, cudaStream_t s) {
   constexpr int N = TREX_TU_N;
   using G = TabGeom<TuR, TuRC, N>;
@@ -295,7 +296,7 @@ int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const Reweight
     blocks_per_sm = b1 < b2 ? b1 : b2;
     if (blocks_per_sm < 1) return (int)cudaErrorLaunchOutOfResources;
   }
-  const long want = (long)nsm * blocks_per_sm, have = (a.n + G::EPB - 1) / G::EPB;
+  const long want = (long)nsm * blocks_per_sm, have = (nmax + G::EPB - 1) / G::EPB;
   const unsigned grid = (unsigned)(have < want ? have : want);
   if (npass == 1) k_table<TuR, TuRC, N, 1><<<grid, G::TB, G::bytes, s>>>(a, meta, Cfold);
   else k_table<TuR, TuRC, N, 2><<<grid, G::TB, G::bytes, s>>>(a, meta, Cfold);

@@ -35,13 +35,15 @@ template <class R, class RC>
 __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArgs a) {
   __shared__ double wf[8][8][32];
   __shared__ double red[2][8][32];
+  const EvIO io = resolve_io(a);
+  if ((long)blockIdx.x * 32 >= io.n) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long e = (long)blockIdx.x * 32 + lane;
-  const long ev = e < a.n ? e : a.n - 1;
+  const long ev = e < io.n ? e : io.n - 1;
   {
     double p[4];
     const int leg = warp >> 1, lam = (warp & 1) ? 1 : -1;      // legs in process order: g g t t~
-    load_leg<double>(a.mom, a.ld, ev, leg, p);
+    load_leg<double>(io.mom, io.ld, ev, leg, p);
     if (leg < 2) {
       const vec4<double> w = polvec<double>(p, lam, false);
 #pragma unroll
@@ -60,7 +62,7 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
 #pragma unroll
   for (int i = 0; i < 4; ++i) ubar.c[i] = cx<R>(R(wf[4 + lt][2 * i][lane]), R(wf[4 + lt][2 * i + 1][lane]));
 #pragma unroll
-  for (int mu = 0; mu < 4; ++mu) pt.c[mu] = a.mom[(long)(8 + mu) * a.ld + ev];
+  for (int mu = 0; mu < 4; ++mu) pt.c[mu] = io.mom[(long)(8 + mu) * io.ld + ev];
   // ---- tuple (1,2) attached to the line at once: i ubar Jslash_12 and ubar sigma.F_12; ordering (2,1) takes the opposite sign
   spinor<R> d0, d1 = szero<R>();
   {
@@ -70,7 +72,7 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
     for (int i = 0; i < 4; ++i) {
       e1.c[i] = cx<R>(R(wf[wsel[0]][2 * i][lane]), R(wf[wsel[0]][2 * i + 1][lane]));
       e2.c[i] = cx<R>(R(wf[wsel[1]][2 * i][lane]), R(wf[wsel[1]][2 * i + 1][lane]));
-      K1.c[i] = a.mom[(long)i * a.ld + ev]; K2.c[i] = a.mom[(long)(4 + i) * a.ld + ev];
+      K1.c[i] = io.mom[(long)i * io.ld + ev]; K2.c[i] = io.mom[(long)(4 + i) * io.ld + ev];
     }
     const rvec4<double> P12 = radd(K1, K2);
     vec4<R> acc = vzero<R>();
@@ -105,7 +107,7 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
     for (int i = 0; i < 4; ++i) {
       ea.c[i] = cx<R>(R(wf[wsel[ga]][2 * i][lane]), R(wf[wsel[ga]][2 * i + 1][lane]));
       eb.c[i] = cx<R>(R(wf[wsel[gb]][2 * i][lane]), R(wf[wsel[gb]][2 * i + 1][lane]));
-      Ka.c[i] = a.mom[(long)(ga * 4 + i) * a.ld + ev]; Kb.c[i] = a.mom[(long)(gb * 4 + i) * a.ld + ev];
+      Ka.c[i] = io.mom[(long)(ga * 4 + i) * io.ld + ev]; Kb.c[i] = io.mom[(long)(gb * 4 + i) * io.ld + ev];
     }
     // U(a) = ubar Gamma(eps_a) S(p_t - K_a)
     dspinor<R> U1;
@@ -163,15 +165,15 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
   }
   red[0][warp][lane] = (double)acc[0]; red[1][warp][lane] = (double)acc[1];
   __syncthreads();
-  if (warp == 0 && e < a.n) {
+  if (warp == 0 && e < io.n) {
     double s0 = 0.0, s1 = 0.0;
 #pragma unroll
     for (int w = 0; w < 8; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
     const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
     const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
-    a.w_out[e] = a.w_in[e] * norm * mn;                        // evaluate + append_wgts
-    if (a.me2_old) a.me2_old[e] = mo;
-    if (a.me2_new) a.me2_new[e] = mn;
+    io.w_out[e] = io.w_in[e] * norm * mn;                        // evaluate + append_wgts
+    if (io.me2_old) io.me2_old[e] = mo;
+    if (io.me2_new) io.me2_new[e] = mn;
   }
 }
 #endif
