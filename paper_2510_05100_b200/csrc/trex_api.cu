@@ -22,12 +22,18 @@ __global__ void __launch_bounds__(WARPS * 32) k_qq(const ReweightArgs a) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long e = (long)blockIdx.x * 32 + lane;
   const long ev = e < io.n ? e : io.n - 1;
-  RC acc[2] = {RC(0), RC(0)};
-  for (int u = warp; u < 16; u += WARPS) {
-    RC out[2];
-    qq_unit<R, RC>(io.mom, io.ld, ev, a.q, u, a.T, out);
-    acc[0] += out[0]; acc[1] += out[1];
-  }
+  // Helicity selection on the massless light line: in the chiral basis a massless spinor has one non-zero 2-block
+  // (u(+), v(-): lower; u(-), v(+): upper; the bar swaps them) and gamma^mu couples upper to lower, so the light-line
+  // currents vanish EXACTLY unless row and column sit in different blocks. Only those 8 of the 16 units are evaluated,
+  // one per warp: warp = (gluon helicity, top helicity, which of the two allowed light-line combinations).
+  static_assert(WARPS == 8, "one allowed helicity unit per warp");
+  const bool row_in = a.q.lrow < 2, col_in = a.q.lcol < 2;
+  const bool row_upper = (warp >> 2) & 1, col_upper = !row_upper;
+  const int lam_row = (row_in ? !row_upper : row_upper) ? 1 : -1;     // vbar(+): lower, ubar(+): upper
+  const int lam_col = (col_in ? !col_upper : col_upper) ? 1 : -1;     // u(+): lower, v(+): upper
+  const int u = (lam_row > 0 ? 1 : 0) | (lam_col > 0 ? 2 : 0) | ((warp & 1) << 2) | (((warp >> 1) & 1) << 3);
+  RC acc[2];
+  qq_unit<R, RC>(io.mom, io.ld, ev, a.q, u, a.T, acc);
   reduce_and_finish<RC>(a, io, acc[0], acc[1], e);
 }
 

@@ -118,10 +118,12 @@ template <int N, int NFIX> struct TabIdx {
 
 // ---------------------------------------------------------------- table access
 // 20 real components per entry, component-major: tab[comp * NE + entry]; comp 0..7 = J (re, im per mu),
-// 8..13 = xp = 2 (B + iE) (re, im per axis), 14..19 = xm = 2 (B - iE)
+// 8..19 = -i * 2 sigma.F in the form the row-spinor product consumes: with X+- = 2 (B +- iE) (the two chiral 2x2 blocks
+// are X+.s and X-.s) the entries are -i (X+_3, X+_1 + i X+_2, X+_1 - i X+_2, X-_3, X-_1 + i X-_2, X-_1 - i X-_2).
+// The factor -i lets the walk accumulate  sum_a [U_a Jslash_a - i U_a sigma.F_a]  and multiply by i once per node.
 constexpr int TAB_NCOMP = 20;
 
-template <class R> struct sigF { cx<R> xp[3], xm[3]; };
+template <class R> struct sigF { cx<R> p3, pt, pb, m3, mt, mb; };
 
 // entry index and sign of the ordered tuple t[0..L) whose free gluons carry the (position-ordered) bits `cbits`
 template <int N, int NFIX, int L> TREX_HD int tab_entry(const int* __restrict__ off, const int* t, unsigned cbits, int nf, int& sign) {
@@ -160,32 +162,39 @@ template <class R, int NE> TREX_HD vec4<R> tab_J(const R* __restrict__ tab, int 
 }
 template <class R, int NE> TREX_HD sigF<R> tab_F(const R* __restrict__ tab, int e, int sign) {
   sigF<R> F;
+  cx<R>* f = &F.p3;
 #pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    F.xp[i] = cx<R>(with_sign(tab[(8 + 2 * i) * NE + e], sign), with_sign(tab[(9 + 2 * i) * NE + e], sign));
-    F.xm[i] = cx<R>(with_sign(tab[(14 + 2 * i) * NE + e], sign), with_sign(tab[(15 + 2 * i) * NE + e], sign));
-  }
+  for (int i = 0; i < 6; ++i) f[i] = cx<R>(with_sign(tab[(8 + 2 * i) * NE + e], sign), with_sign(tab[(9 + 2 * i) * NE + e], sign));
   return F;
 }
 template <class R, int NE> TREX_HD void tab_store(R* __restrict__ tab, int e, const vec4<R>& J, const ften<R>& f) {
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) { tab[(2 * mu) * NE + e] = J.c[mu].re; tab[(2 * mu + 1) * NE + e] = J.c[mu].im; }
+  cx<R> xp[3], xm[3];
 #pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    const cx<R> ie = mul_i(f.e[i]);
-    const cx<R> xp = R(2) * (f.b[i] + ie), xm = R(2) * (f.b[i] - ie);
-    tab[(8 + 2 * i) * NE + e] = xp.re; tab[(9 + 2 * i) * NE + e] = xp.im;
-    tab[(14 + 2 * i) * NE + e] = xm.re; tab[(15 + 2 * i) * NE + e] = xm.im;
-  }
+  for (int i = 0; i < 3; ++i) { const cx<R> ie = mul_i(f.e[i]); xp[i] = R(2) * (f.b[i] + ie); xm[i] = R(2) * (f.b[i] - ie); }
+  const cx<R> out[6] = {xp[2], xp[0] + mul_i(xp[1]), xp[0] - mul_i(xp[1]), xm[2], xm[0] + mul_i(xm[1]), xm[0] - mul_i(xm[1])};
+#pragma unroll
+  for (int i = 0; i < 6; ++i) { const cx<R> v = mul_mi(out[i]); tab[(8 + 2 * i) * NE + e] = v.re; tab[(9 + 2 * i) * NE + e] = v.im; }
 }
-// o += r * (2 sigma^{mu nu} F_{mu nu} / 2) with the two 2x2 blocks xp.s, xm.s given (cf. row_sigma_acc)
-template <class R> TREX_HD void row_sigma_acc_x(spinor<R>& o, const spinor<R>& r, const sigF<R>& F) {
-  const cx<R> pt = F.xp[0] + mul_i(F.xp[1]), pb = F.xp[0] - mul_i(F.xp[1]);
-  const cx<R> mt = F.xm[0] + mul_i(F.xm[1]), mb = F.xm[0] - mul_i(F.xm[1]);
-  cfma(o.c[0], r.c[0], F.xp[2]); cfma(o.c[0], r.c[1], pt);
-  cfma(o.c[1], r.c[0], pb);      cfma(o.c[1], -r.c[1], F.xp[2]);
-  cfma(o.c[2], r.c[2], F.xm[2]); cfma(o.c[2], r.c[3], mt);
-  cfma(o.c[3], r.c[2], mb);      cfma(o.c[3], -r.c[3], F.xm[2]);
+// a -= b * c
+template <class R> TREX_HD void cfnma(cx<R>& a, cx<R> b, cx<R> c) {
+  a.re -= b.re * c.re; a.re += b.im * c.im; a.im -= b.re * c.im; a.im -= b.im * c.re; }
+// acc += r * aslash   (pure FMA form of row_slash; the caller multiplies the sum by i once)
+template <class R> TREX_HD void row_slash_acc(spinor<R>& acc, const spinor<R>& r, const vec4<R>& a) {
+  const cx<R> ap = a.c[0] + a.c[3], am = a.c[0] - a.c[3];
+  const cx<R> at = a.c[1] + mul_i(a.c[2]), ab = a.c[1] - mul_i(a.c[2]);
+  cfma(acc.c[0], r.c[2], ap); cfma(acc.c[0], r.c[3], at);
+  cfma(acc.c[1], r.c[2], ab); cfma(acc.c[1], r.c[3], am);
+  cfma(acc.c[2], r.c[0], am); cfnma(acc.c[2], r.c[1], at);
+  cfma(acc.c[3], r.c[1], ap); cfnma(acc.c[3], r.c[0], ab);
+}
+// acc += r * (-i 2 sigma.F) with the pre-combined blocks of the table
+template <class R> TREX_HD void row_sigma_acc_x(spinor<R>& acc, const spinor<R>& r, const sigF<R>& F) {
+  cfma(acc.c[0], r.c[0], F.p3); cfma(acc.c[0], r.c[1], F.pt);
+  cfma(acc.c[1], r.c[0], F.pb); cfnma(acc.c[1], r.c[1], F.p3);
+  cfma(acc.c[2], r.c[2], F.m3); cfma(acc.c[2], r.c[3], F.mt);
+  cfma(acc.c[3], r.c[2], F.mb); cfnma(acc.c[3], r.c[3], F.m3);
 }
 
 // ---------------------------------------------------------------- phase 1: one table entry of level K >= 2
@@ -271,11 +280,26 @@ TREX_HD void tab_build_level1(R* __restrict__ tab, const int* __restrict__ meta,
 
 // ---------------------------------------------------------------- phase 2: depth-first walk of the top line
 // The first D gluons of the ordering are given (the task); below them every remaining ordering is visited. Private
-// state: the line spinors U[1..N-1] (dual numbers in kappa). Every vertex operand comes from the table.
-template <class R, int N, int NFIX, int D, class Sink> struct TabWalk {
+// state: the line spinors U[UT+1..N-1] (dual numbers in kappa). Every vertex operand comes from the table.
+// UT > 0 (all helicities free, NFIX = 0): the line states of the prefixes of length <= UT do not depend on the rest of
+// the ordering nor on the other helicities; they are tabulated once per event and parameter point (utab, built by
+// walks with STOP = 1 .. UT that store U[STOP] instead of descending) and the walk starts at level UT + 1.
+//   utab[comp * nut + ubase + index], comp = (order 0 / 1, spinor component, re / im) = 0..15
+//   index level 1: (g1 * 2 + hel) * 2 + lt;   level 2: 4 N + ((rank of (g1,g2) among ordered pairs) * 4 + hels) * 2 + lt
+template <int N> struct UTabIdx {
+  static constexpr int N1 = 4 * N, N2 = 8 * N * (N - 1), NU = N1 + N2;
+  TREX_HD static int level1(int g1, unsigned bits, int lt) { return (g1 * 2 + (int)(bits & 1u)) * 2 + lt; }
+  TREX_HD static int level2(int g1, int g2, unsigned bits, int lt) {
+    return N1 + ((g1 * (N - 1) + g2 - (g2 > g1 ? 1 : 0)) * 4 + (int)(bits & 3u)) * 2 + lt;
+  }
+};
+
+template <class R, int N, int NFIX, int D, class Sink, int UT = 0, int STOP = 0> struct TabWalk {
   using I = TabIdx<N, NFIX>;
   static constexpr int NE = I::NE;
+  static_assert(UT == 0 || (NFIX == 0 && UT <= 2), "line-state tables: all helicities free, prefixes of length <= 2");
   const R* tab; const int* off; const rvec4<double>* pset;
+  R* utab; int nut, ubase, lt;        // line-state table (UT > 0 or STOP > 0)
   rvec4<double> pt;
   spinor<R> ubar_t;
   TopLine line;
@@ -289,55 +313,100 @@ template <class R, int N, int NFIX, int D, class Sink> struct TabWalk {
   int leaf;
   Sink* sink;
 
-  template <int M, int A> TREX_HD void bracket_terms(spinor<R>& b0, spinor<R>& b1) {
+  template <int A> TREX_HD int uindex() const {
+    if constexpr (A == 1) return ubase + UTabIdx<N>::level1(s[0], cb, lt);
+    else return ubase + UTabIdx<N>::level2(s[0], s[1], cb, lt);
+  }
+  // line state after the first A gluons: private, or from the per-event table
+  template <int A> TREX_HD dspinor<R> state() const {
+    if constexpr (A <= UT) {
+      dspinor<R> u;
+      const int e = uindex<A>();
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        u.o0.c[i] = cx<R>(utab[(2 * i) * nut + e], utab[(2 * i + 1) * nut + e]);
+        u.o1.c[i] = cx<R>(utab[(8 + 2 * i) * nut + e], utab[(9 + 2 * i) * nut + e]);
+      }
+      return u;
+    } else return U[A];
+  }
+
+  // s0 += U_a^(0) Jslash_a;  s1 += U_a^(1) Jslash_a - i U_a^(0) 2 sigma.F_a;  the bracket is (i s0, i s1)
+  template <int M, int A> TREX_HD void bracket_terms(spinor<R>& s0, spinor<R>& s1) {
     if constexpr (A < M) {
       int sign;
       const int e = tab_entry<N, NFIX, M - A>(off, s + A, cb >> fpos[A], fpos[M] - fpos[A], sign);
       const vec4<R> J = tab_J<R, NE>(tab, e, sign);
-      const spinor<R>& u0 = A == 0 ? ubar_t : U[A].o0;
-      const spinor<R> t0 = row_slash(u0, J);
-#pragma unroll
-      for (int i = 0; i < 4; ++i) b0.c[i] += mul_i(t0.c[i]);
-      if constexpr (A > 0) {
-        const spinor<R> t1 = row_slash(U[A].o1, J);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) b1.c[i] += mul_i(t1.c[i]);
+      if constexpr (A == 0) {
+        row_slash_acc(s0, ubar_t, J);
+        row_sigma_acc_x(s1, ubar_t, tab_F<R, NE>(tab, e, sign));
+      } else {
+        const dspinor<R> u = state<A>();
+        row_slash_acc(s0, u.o0, J);
+        row_slash_acc(s1, u.o1, J);
+        row_sigma_acc_x(s1, u.o0, tab_F<R, NE>(tab, e, sign));
       }
-      row_sigma_acc_x(b1, u0, tab_F<R, NE>(tab, e, sign));
-      bracket_terms<M, A + 1>(b0, b1);
+      bracket_terms<M, A + 1>(s0, s1);
     }
   }
 
-  template <int M> TREX_HD void node(int g) {
+  // bookkeeping of position M (no arithmetic)
+  template <int M> TREX_HD void place(int g) {
     s[M - 1] = g;
     const bool isfree = g >= NFIX;
     const unsigned bit = isfree ? (hfree >> (g - NFIX)) & 1u : 0u;
     cb = (cb & ((1u << fpos[M - 1]) - 1u)) | (bit << fpos[M - 1]);
     fpos[M] = fpos[M - 1] + (isfree ? 1 : 0);
     prefmask[M] = prefmask[M - 1] | (1u << g);
-    spinor<R> b0 = szero<R>(), b1 = szero<R>();
-    bracket_terms<M, 0>(b0, b1);
-    if constexpr (M < N) {
-      const rvec4<double> qd = rsub(pt, pset[prefmask[M]]);
-      const double q2 = rdot(qd, qd);
-      const rvec4<R> q = cast<R>(qd);
-      const cx<double> den(q2 - line.mt * line.mt, line.mGt);
-      const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), den));
-      const spinor<R> s0 = row_slash(b0, q), s1 = row_slash(b1, q);
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        cx<R> n0 = s0.c[i]; cfma(n0, b0.c[i], R(line.mt));
-        cx<R> n1 = s1.c[i]; cfma(n1, b1.c[i], R(line.mt));
-        U[M].o0.c[i] = n0 * pr; U[M].o1.c[i] = n1 * pr;
-      }
+  }
+
+  template <int M> TREX_HD void node(int g) {
+    place<M>(g);
+    if constexpr (M <= UT) {
+      // tabulated level: nothing to compute
       if constexpr (M < D) node<M + 1>(pref[M]);
-      else {
-        // every thread visits the r-th unused gluon at the same trip: uniform control flow across ordering prefixes
-        for (int r = 0; r < N - M; ++r) node<(M < N ? M + 1 : N)>(I::nth_unused(prefmask[M], r));
-      }
+      else descend<M>();
     } else {
-      (*sink)(leaf, b0, b1);
-      ++leaf;
+      spinor<R> b0 = szero<R>(), b1 = szero<R>();
+      bracket_terms<M, 0>(b0, b1);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { b0.c[i] = mul_i(b0.c[i]); b1.c[i] = mul_i(b1.c[i]); }
+      if constexpr (M < N) {
+        const rvec4<double> qd = rsub(pt, pset[prefmask[M]]);
+        const double q2 = rdot(qd, qd);
+        const rvec4<R> q = cast<R>(qd);
+        const cx<double> den(q2 - line.mt * line.mt, line.mGt);
+        const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), den));
+        const spinor<R> s0 = row_slash(b0, q), s1 = row_slash(b1, q);
+        dspinor<R> u;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          cx<R> n0 = s0.c[i]; cfma(n0, b0.c[i], R(line.mt));
+          cx<R> n1 = s1.c[i]; cfma(n1, b1.c[i], R(line.mt));
+          u.o0.c[i] = n0 * pr; u.o1.c[i] = n1 * pr;
+        }
+        if constexpr (M == STOP) {
+          const int e = uindex<M>();
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            utab[(2 * i) * nut + e] = u.o0.c[i].re; utab[(2 * i + 1) * nut + e] = u.o0.c[i].im;
+            utab[(8 + 2 * i) * nut + e] = u.o1.c[i].re; utab[(9 + 2 * i) * nut + e] = u.o1.c[i].im;
+          }
+        } else {
+          U[M] = u;
+          if constexpr (M < D) node<M + 1>(pref[M]);
+          else descend<M>();
+        }
+      } else {
+        (*sink)(leaf, b0, b1);
+        ++leaf;
+      }
+    }
+  }
+  template <int M> TREX_HD void descend() {
+    if constexpr (M < N) {
+      // every thread visits the r-th unused gluon at the same trip: uniform control flow across ordering prefixes
+      for (int r = 0; r < N - M; ++r) node<(M < N ? M + 1 : N)>(I::nth_unused(prefmask[M], r));
     }
   }
 

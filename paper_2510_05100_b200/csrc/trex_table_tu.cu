@@ -35,18 +35,23 @@ namespace {
 #define TREX_T3_MINB 3
 #endif
 #ifndef TREX_T4_TB
-#define TREX_T4_TB 128
+#define TREX_T4_TB 384
 #endif
 #ifndef TREX_T4_MINB
-#define TREX_T4_MINB 2
+#define TREX_T4_MINB 1
+#endif
+#ifndef TREX_T4_UT
+#define TREX_T4_UT 2
 #endif
 // NFIX: gluons whose helicity the outer loop fixes; D: depth of the ordering prefix that defines a walk task;
 // TB: threads per block; EPB: events a block works on at the same time, each by its own group of TB / EPB threads
-// (a group of 32 = one warp synchronises with __syncwarp and runs free of the other warps); MINB: blocks per SM
+// (a group of 32 = one warp synchronises with __syncwarp and runs free of the other warps); MINB: blocks per SM;
+// UT: the top-line states of ordering prefixes up to this length are tabulated per event instead of being carried by
+// every walk thread (fewer registers per thread -> more warps, and no recomputation across tasks)
 template <int N> struct TabCfg;
-template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB; };
-template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = 2, TB = TREX_T4_TB, EPB = 1, MINB = TREX_T4_MINB; };
-template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1; };
+template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB, UT = 0; };
+template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = TREX_T4_UT ? 4 : 2, TB = TREX_T4_TB, EPB = 1, MINB = TREX_T4_MINB, UT = TREX_T4_UT; };
+template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1, UT = 0; };
 
 template <int NC> struct FoldedC {
   // C'(i,j) = 0 (j < i), C_ii (j == i), 2 C_ij (j > i), stored by rows i for j >= RB floor(i/RB)
@@ -60,7 +65,8 @@ template <int NC> struct FoldedC {
 template <class R, class RC, int N> struct TabGeom {
   using Cfg = TabCfg<N>;
   using I = TabIdx<N, Cfg::NFIX>;
-  static constexpr int NFIX = Cfg::NFIX, D = Cfg::D, TB = Cfg::TB, EPB = Cfg::EPB, GS = TB / EPB;
+  static constexpr int NFIX = Cfg::NFIX, D = Cfg::D, TB = Cfg::TB, EPB = Cfg::EPB, GS = TB / EPB, UT = Cfg::UT;
+  static constexpr int NU = UTabIdx<N>::NU, NUT = 2 * NU;    // line-state table entries per parameter point / in all
   static_assert(GS * EPB == TB && (GS == TB || GS == 32), "an event group is one warp or the whole block");
   static constexpr int NE = I::NE;
   static constexpr int NC = I::falling(N, N);
@@ -80,7 +86,8 @@ template <class R, class RC, int N> struct TabGeom {
   static constexpr size_t o_eps = o_pset + al(sizeof(rvec4<double>) * NSUB);
   static constexpr size_t o_spin = o_eps + al(sizeof(double) * 16 * N);
   static constexpr size_t o_part = o_spin + al(sizeof(double) * 8 * 4);
-  static constexpr size_t slot = o_part + al(sizeof(double) * NCI);
+  static constexpr size_t o_utab = o_part + al(sizeof(double) * NCI);
+  static constexpr size_t slot = o_utab + (UT ? al(sizeof(R) * 16 * NUT) : 0);
   static constexpr size_t o_c = slot * EPB;
   static constexpr size_t o_meta = o_c + al(sizeof(RC) * FoldedC<NC>::size());
   static constexpr size_t bytes = o_meta + al(sizeof(int) * I::M_SIZE);
@@ -113,15 +120,56 @@ template <int GS> __device__ __forceinline__ void group_sync() {
   if constexpr (GS == 32) __syncwarp(); else __syncthreads();
 }
 
-template <class R, class RC, int N, int K> __device__ __forceinline__ void build_levels(unsigned char* sb, const int* meta, int gtid) {
+struct NoSink {
+  template <class S> __device__ __forceinline__ void operator()(int, const S&, const S&) {}
+};
+
+// line state of one ordering prefix of length L (item = UTabIdx level-L index, pass) -> utab
+template <class R, class RC, int N, int L>
+__device__ __forceinline__ void build_ustate(unsigned char* sb, const int* meta, const ReweightArgs& a, const rvec4<double>& pt, int item, int pass) {
+  using G = TabGeom<R, RC, N>;
+  using I = typename G::I;
+  TabWalk<R, N, G::NFIX, L, NoSink, L - 1, L> w;
+  NoSink none;
+  const int lt = item & 1;
+  unsigned bits;
+  if constexpr (L == 1) { bits = (item >> 1) & 1u; w.pref[0] = item >> 2; w.hfree = bits << w.pref[0]; }
+  else {
+    bits = (item >> 1) & 3u;
+    const int pr = item >> 3, g1 = pr / (N - 1), r = pr - g1 * (N - 1), g2 = r + (r >= g1 ? 1 : 0);
+    w.pref[0] = g1; w.pref[1] = g2;
+    w.hfree = ((bits & 1u) << g1) | (((bits >> 1) & 1u) << g2);
+  }
+  const double* spin = reinterpret_cast<const double*>(sb + G::o_spin);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) w.ubar_t.c[i] = cx<R>(R(spin[lt * 8 + 2 * i]), R(spin[lt * 8 + 2 * i + 1]));
+  w.pt = pt;
+  w.tab = reinterpret_cast<const R*>(sb + G::o_tab); w.off = meta + I::M_OFF;
+  w.pset = reinterpret_cast<const rvec4<double>*>(sb + G::o_pset);
+  w.utab = reinterpret_cast<R*>(sb + G::o_utab); w.nut = G::NUT; w.ubase = pass * G::NU; w.lt = lt;
+  w.line.mt = a.T.mt[pass]; w.line.mGt = a.T.mGt[pass];
+  w.run(&none);
+}
+
+template <class R, class RC, int N, int NPASS, int K>
+__device__ __forceinline__ void build_levels(unsigned char* sb, const int* meta, int gtid, const ReweightArgs& a, const rvec4<double>& pt) {
   using G = TabGeom<R, RC, N>;
   using I = typename G::I;
   if constexpr (K <= N) {
-    const int e1 = meta[I::M_LVL + K + 1];
-    for (int e = meta[I::M_LVL + K] + gtid; e < e1; e += G::GS)
-      tab_build_entry<R, N, G::NFIX, K>(reinterpret_cast<R*>(sb + G::o_tab), meta, reinterpret_cast<const rvec4<double>*>(sb + G::o_pset), e);
+    const int e0 = meta[I::M_LVL + K], ntab = meta[I::M_LVL + K + 1] - e0;
+    // the line states of the prefixes of length K - 1 need the table levels < K and the states of length K - 2: same phase
+    constexpr int L = K - 1;
+    constexpr int nus = L <= G::UT ? (L == 1 ? UTabIdx<N>::N1 : UTabIdx<N>::N2) : 0;
+    for (int it = gtid; it < ntab + nus * NPASS; it += G::GS) {
+      if (it < ntab) {
+        tab_build_entry<R, N, G::NFIX, K>(reinterpret_cast<R*>(sb + G::o_tab), meta, reinterpret_cast<const rvec4<double>*>(sb + G::o_pset), e0 + it);
+      } else if constexpr (nus > 0) {
+        const int u = it - ntab, pass = u / nus;
+        build_ustate<R, RC, N, L>(sb, meta, a, pt, u - pass * nus, pass);
+      }
+    }
     group_sync<G::GS>();
-    build_levels<R, RC, N, K + 1>(sb, meta, gtid);
+    build_levels<R, RC, N, NPASS, K + 1>(sb, meta, gtid, a, pt);
   }
 }
 
@@ -130,7 +178,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
   using G = TabGeom<R, RC, N>;
   using I = typename G::I;
   using F = FoldedC<G::NC>;
-  constexpr int NFIX = G::NFIX, D = G::D, TB = G::TB, XS = G::XS, EPB = G::EPB, GS = G::GS;
+  constexpr int NFIX = G::NFIX, D = G::D, TB = G::TB, XS = G::XS, EPB = G::EPB, GS = G::GS, UT = G::UT;
   extern __shared__ __align__(16) unsigned char smem[];
   RC* Cs = reinterpret_cast<RC*>(smem + G::o_c);
   int* meta = reinterpret_cast<int*>(smem + G::o_meta);
@@ -182,11 +230,14 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
     }
     group_sync<GS>();
 
+    rvec4<double> ptop;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) ptop.c[mu] = io.mom[(long)(2 * 4 + mu) * io.ld + e];
     for (unsigned itb = 0; itb < (unsigned)G::NIT; ++itb) {
-      // ---- phase 1: current table of this helicity iteration
+      // ---- phase 1: current table of this helicity iteration (+ line states of short prefixes, if tabulated)
       for (int e1 = gtid; e1 < meta[I::M_LVL + 2]; e1 += GS) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
       group_sync<GS>();
-      build_levels<R, RC, N, 2>(sb, meta, gtid);
+      build_levels<R, RC, N, NPASS, 2>(sb, meta, gtid, a, ptop);
 
       // ---- phase 2: top-line walk
       for (int task = gtid; task < G::NTASK * NPASS; task += GS) {
@@ -194,11 +245,11 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
         const int hl = r % G::NHL, prank = r / G::NHL;
         using Store = TabLeafStore<R, RC, XS>;
         Store st;
-        TabWalk<R, N, NFIX, D, Store> w;
+        TabWalk<R, N, NFIX, D, Store, UT> w;
         prefix_of_rank<N, D>(prank, w.pref);
         const int lt = hl & 1;
-#pragma unroll
-        for (int mu = 0; mu < 4; ++mu) w.pt.c[mu] = io.mom[(long)(2 * 4 + mu) * io.ld + e];
+        w.pt = ptop;
+        w.utab = reinterpret_cast<R*>(sb + G::o_utab); w.nut = G::NUT; w.ubase = pass * G::NU; w.lt = lt;
 #pragma unroll
         for (int i = 0; i < 4; ++i) w.ubar_t.c[i] = cx<R>(R(spin[lt * 8 + 2 * i]), R(spin[lt * 8 + 2 * i + 1]));
         w.tab = tab; w.off = meta + I::M_OFF; w.pset = pset;
