@@ -29,7 +29,7 @@ HEADLINE_CFG = 2
 
 # Algorithmic FP64 work per reweighted event of the dominant kernel of each config: thread-level DFMA/DMUL/DADD counted
 # by ncu (smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on.sum; DFMA = 2 flop) on the committed kernels,
-# divided by the events of that launch (profiles/r01_flops_per_event.md). None = not yet counted.
+# divided by the events of that launch (profiles/flops_per_event.json, profiles/r01c_kernels.md). None = not yet counted.
 FLOP_PER_EVENT = {1: None, 2: None, 3: None, 4: None, 5: None}
 SID_OF_CFG = {1: 0, 2: 1, 4: 3, 5: 4}
 # nominal FP64 vector peak of B200: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz
@@ -219,6 +219,9 @@ def main():
         res["ms_per_step"] = 1e3 * sec / steps
         res["value"] = world * w.n * steps / sec
         assert bool(torch.isfinite(wout).all())
+        if precision == 0 and FLOP_PER_EVENT.get(cfg):
+            # FP64 work of the |M|^2 kernels over the WHOLE step time (bucketing, transposition, launch gaps included)
+            res["step_tflops"] = FLOP_PER_EVENT[cfg] * w.n * steps / sec / 1e12
         # the dominant kernel alone (single-class configs: the one |M|^2 launch of the step)
         if cfg in SID_OF_CFG:
             sid = SID_OF_CFG[cfg]
@@ -252,19 +255,21 @@ def main():
         return
 
     # ---- FP64 pipe peak, measured in this run
-    def probe(fp32):
+    def probe(mode):
+        """mode 0 / 1: FP64 / FP32 FMA chains with constant-bank operands (pipe peak); 2 / 3: three register operands."""
         holder = {}
 
         def once():
-            holder["flops"] = T.trex_probe_fma(fp32, blocks=148 * 16, iters=2048)
+            holder["flops"] = T.trex_probe_fma(mode, blocks=148 * 16, iters=2048)
         sec = time_steps(once, 2, 5) / 5
         return holder["flops"] / sec / 1e12
 
     with ClockSampler(local) as clk:
         head = measure(HEADLINE_CFG, W, K, with_e2e=True)
-        fp64_peak = probe(False)
+        fp64_peak = probe(0)
     clocks = clk.summary()
-    fp32_peak = probe(True)
+    fp32_peak = probe(1)
+    fp64_peak_3reg = probe(2)
 
     configs = {}
     if args.configs == "all":
@@ -287,9 +292,13 @@ def main():
         ach = head.get("kernel_tflops")
         roof = {"bound": "alu", "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": (ach / fp64_peak) if ach else None, "traffic": None,
-                "kernel": "k_ttng<double,double,2,1>", "kernel_ms": head.get("kernel_ms"),
+                "kernel": "k_gg_tt<double,double>", "kernel_ms": head.get("kernel_ms"),
                 "peak_source": "FP64 FMA register-chain probe (trex_probe_fma) timed in this run; nominal %.1f TFLOP/s" % FP64_NOMINAL_TFLOPS,
-                "fp32_peak_measured": fp32_peak, "flop_per_event": FLOP_PER_EVENT.get(HEADLINE_CFG)}
+                "fp32_peak_measured": fp32_peak, "flop_per_event": FLOP_PER_EVENT.get(HEADLINE_CFG),
+                # the same probe with three REGISTER operands per FMA (what amplitude code issues): the register file
+                # feeds the FP64 pipe at this rate at most
+                "peak_three_register_operands": fp64_peak_3reg,
+                "frac_of_three_register_peak": (ach / fp64_peak_3reg) if ach else None}
         tpath = os.path.join(ROOT, "profiles", "flops_per_event.json")
         if os.path.exists(tpath):
             with open(tpath) as fh:

@@ -280,7 +280,7 @@ def trex_run_host(pdg_keys, momenta_soa, theta_old, theta_new, w_in, w_out, me2_
 def trex_probe_fma(fp32=False, blocks=148 * 8, iters=4096):
     """Enqueue one FMA-chain probe launch on the library stream; returns the flop count it executes."""
     _torch()
-    flops = lib().trex_probe_fma(int(bool(fp32)), int(blocks), int(iters))
+    flops = lib().trex_probe_fma(int(fp32), int(blocks), int(iters))
     if flops < 0:
         raise TrexError("trex_probe_fma failed: %s" % trex_last_error())
     return flops

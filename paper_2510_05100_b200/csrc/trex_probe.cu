@@ -19,18 +19,38 @@ template <class R> __global__ void __launch_bounds__(256) k_fma_probe(R* out, in
   if (s == R(-12345.678)) out[0] = s;     // never true: keeps the chains alive
 }
 
+// the same with three REGISTER operands per FMA (the form real amplitude code has: no constant-bank operand, no operand
+// reuse between consecutive instructions): what the register file can feed to the pipe
+template <class R> __global__ void __launch_bounds__(256) k_fma_probe3(R* out, int iters, R a, R b) {
+  R x[8], y[8], z[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { x[k] = R(threadIdx.x + k); y[k] = a + R(1e-9) * R(threadIdx.x + 3 * k); z[k] = b + R(1e-9) * R(threadIdx.x + 5 * k); }
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = fma(x[k], y[k], z[k]);
+    }
+  }
+  R s = ((x[0] + x[1]) + (x[2] + x[3])) + ((x[4] + x[5]) + (x[6] + x[7]));
+  if (s == R(-12345.678)) out[0] = s;
+}
+
 }  // namespace
 }  // namespace trex
 
 using namespace trex;
 
 // Enqueues one probe launch on the library stream and returns the number of floating-point operations it executes
-// (time it with events on that stream). fp32 != 0 selects the FP32 pipe. Returns < 0 on error.
+// (time it with events on that stream). fp32: 0 = FP64, 1 = FP32 (one register + two constant-bank operands per FMA);
+// 2 = FP64, 3 = FP32 with three register operands per FMA. Returns < 0 on error.
 extern "C" double trex_probe_fma(int fp32, int blocks, int iters) {
   Context& c = ctx();
   if (blocks <= 0 || iters <= 0) return (double)fail(TREX_EINVAL, "trex_probe_fma: blocks and iters must be positive");
   if (!c.probe_out && cudaMalloc(&c.probe_out, 64) != cudaSuccess) return (double)fail(TREX_ENOMEM, "trex_probe_fma: cudaMalloc failed");
-  if (fp32) k_fma_probe<float><<<blocks, 256, 0, c.stream>>>((float*)c.probe_out, iters, 0.999f, 0.001f);
+  if (fp32 == 2) k_fma_probe3<double><<<blocks, 256, 0, c.stream>>>((double*)c.probe_out, iters, 0.999, 0.001);
+  else if (fp32 == 3) k_fma_probe3<float><<<blocks, 256, 0, c.stream>>>((float*)c.probe_out, iters, 0.999f, 0.001f);
+  else if (fp32) k_fma_probe<float><<<blocks, 256, 0, c.stream>>>((float*)c.probe_out, iters, 0.999f, 0.001f);
   else k_fma_probe<double><<<blocks, 256, 0, c.stream>>>((double*)c.probe_out, iters, 0.999, 0.001);
   c.launches += 1;
   if (cudaGetLastError() != cudaSuccess) return (double)fail(TREX_ECUDA, "trex_probe_fma: launch failed");

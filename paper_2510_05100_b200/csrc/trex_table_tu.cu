@@ -197,9 +197,21 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
   for (int i = gtid; i < G::NCI; i += GS) part[i] = 0.0;
   __syncthreads();
 
+#ifdef TREX_PHASE_CLOCKS
+  long long pc[5] = {0, 0, 0, 0, 0}, t0;
+#define PHASE_TICK(k) do { if (tid == 0) { const long long t1 = clock64(); pc[k] += t1 - t0; t0 = t1; } } while (0)
+#else
+#define PHASE_TICK(k) do { } while (0)
+#endif
   for (long e = (long)blockIdx.x * EPB + sl; e < io.n; e += (long)gridDim.x * EPB) {
+#ifdef TREX_PHASE_CLOCKS
+    if (tid == 0) t0 = clock64();
+#endif
     // ---- per-event set-up: momentum of every gluon subset (incoming convention), polarisation vectors, t / t~ spinors
-    for (int sset = gtid; sset < G::NSUB; sset += GS) {
+    // (subset momenta and wavefunctions are independent: different lanes, one pass, one latency)
+    for (int item = gtid; item < G::NSUB + 2 * N + 4; item += GS) {
+     if (item < G::NSUB) {
+      const int sset = item;
       rvec4<double> P;
 #pragma unroll
       for (int mu = 0; mu < 4; ++mu) P.c[mu] = 0.0;
@@ -211,8 +223,8 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
         for (int mu = 0; mu < 4; ++mu) P.c[mu] += sg * io.mom[(long)(leg * 4 + mu) * io.ld + e];
       }
       pset[sset] = P;
-    }
-    for (int it = gtid; it < 2 * N + 4; it += GS) {
+     } else {
+      const int it = item - G::NSUB;
       double p[4];
       if (it < 2 * N) {
         const int g = it >> 1, leg = g < 2 ? g : g + 2;
@@ -227,8 +239,10 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
 #pragma unroll
         for (int i = 0; i < 4; ++i) { spin[k * 8 + 2 * i] = sp.c[i].re; spin[k * 8 + 2 * i + 1] = sp.c[i].im; }
       }
+     }
     }
     group_sync<GS>();
+    PHASE_TICK(0);
 
     rvec4<double> ptop;
 #pragma unroll
@@ -238,6 +252,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
       for (int e1 = gtid; e1 < meta[I::M_LVL + 2]; e1 += GS) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
       group_sync<GS>();
       build_levels<R, RC, N, NPASS, 2>(sb, meta, gtid, a, ptop);
+      PHASE_TICK(1);
 
       // ---- phase 2: top-line walk
       for (int task = gtid; task < G::NTASK * NPASS; task += GS) {
@@ -263,6 +278,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
         w.run(&st);
       }
       group_sync<GS>();
+      PHASE_TICK(2);
 
       // ---- phase 3: x^dagger C x of every X column, 8-row register blocks, row blocks paired (p, NB-1-p) for balance.
       // A work item is always handled by the same thread, so its partial sum accumulates race-free in shared memory.
@@ -291,6 +307,10 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
         }
         part[item] += (double)accl;
       }
+#ifdef TREX_PHASE_CLOCKS
+      group_sync<GS>();
+      PHASE_TICK(3);
+#endif
       // no barrier needed here: the next writes to X happen after the barriers of the next iteration's phase 1
     }
     group_sync<GS>();
@@ -311,7 +331,11 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
         if (io.me2_new) io.me2_new[e] = mn;
       }
     }
+    PHASE_TICK(4);
   }
+#ifdef TREX_PHASE_CLOCKS
+  if (tid == 0 && blockIdx.x == 0) printf("k_table N=%d phases [cycles of block 0]: setup %lld  table %lld  walk %lld  colour %lld  epilogue %lld\n", N, pc[0], pc[1], pc[2], pc[3], pc[4]);
+#endif
 }
 
 }  // namespace
