@@ -150,3 +150,33 @@ def gather(src, perm):
     """dst[r, j] = src[r, perm[j]] (the SoA 'transpose' of PAPER.md:100, 691)."""
     src = np.asarray(src)
     return np.ascontiguousarray(src.reshape(-1, src.shape[-1])[:, perm]).reshape(src.shape[:-1] + (len(perm),))
+
+
+# ---------------------------------------------------------------- reweighted cross section and its error (NEXT-2)
+def xsec(w_in, w_out, C, sigma, dsigma):
+    """Reweighted cross section and propagated error, written out from PAPER.md:942-948:
+
+        sigma'       = C * sum_i w'_i                                                   eq.(6)
+        Delta sigma' = Delta sigma * (1/N) sum_i w'_i / w_i  +  sigma * std(w')         eq.(7)
+
+    std = population standard deviation (divide by N; R-15). Events with w_i = 0 carry w'_i = 0 by the zero
+    guard of PAPER.md:789-799 and add nothing to the ratio sum (R-16). If the propagated error is infinite, NaN or not
+    positive it is replaced by Delta sigma times whichever of sigma'/sigma, sigma/sigma' is greater than one
+    (PAPER.md:948). Returns (sigma', Delta sigma', fallback_used). Plain Python / math.fsum: exact sums.
+    """
+    w_in = np.asarray(w_in, dtype=np.float64)
+    w_out = np.asarray(w_out, dtype=np.float64)
+    n = len(w_out)
+    if n == 0:
+        return 0.0, float(dsigma), True
+    s1 = math.fsum(w_out.tolist())
+    sigma_p = C * s1
+    ratio = math.fsum([wo / wi for wo, wi in zip(w_out.tolist(), w_in.tolist()) if wi != 0.0]) / n
+    mean = s1 / n
+    var = math.fsum([(x - mean) * (x - mean) for x in w_out.tolist()]) / n
+    d = dsigma * ratio + sigma * math.sqrt(var)
+    fallback = not (math.isfinite(d) and d > 0.0)
+    if fallback:
+        r = sigma_p / sigma if sigma != 0.0 else float("nan")
+        d = dsigma * max(r, 1.0 / r) if (math.isfinite(r) and r > 0.0) else float(dsigma)
+    return sigma_p, d, fallback
