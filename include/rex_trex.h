@@ -112,6 +112,14 @@ int trex_reweight(int subproc_id, const double* momenta_soa, int64_t n, const do
 int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
              const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
 
+/* Many parameter points on one categorisation ("sort once", eqs.(9)-(10); the launch loop over
+ * parameter cards): rex_bucket and the transposition run ONCE, then every theta_new[k] is evaluated.
+ * theta_new HOST [ntheta][TREX_NTHETA]; w_out DEVICE [ntheta][n]; me2_old DEVICE [n] or NULL (the same for every k);
+ * me2_new DEVICE [ntheta][n] or NULL. Row k equals what trex_run gives for (theta_old, theta_new[k]), bit for bit.
+ * Returns the number of buckets; synchronises the stream once, at the end. */
+int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
+                   const double* theta_new, int ntheta, const double* w_in, double* w_out, double* me2_old, double* me2_new);
+
 /* The same with HOST buffers (pinned or pageable): copies keys, momenta and weights to internal device scratch on the
  * stream, runs trex_run, copies the results back and synchronises the stream before returning. */
 int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
@@ -121,6 +129,20 @@ int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n
  * level of SURVEY.md I-4. out HOST [nhel][ncolor][2 orders in kappa][re,im], couplings included, order 1 per unit
  * kappa. Only for TREX_SP_GG_TT .. TREX_SP_GG_TTGGG. Synchronous. */
 int trex_debug_flow_amps(int subproc_id, const double* momenta_one, const double* theta, double* out);
+
+/* ---- reweighted cross section and propagated error:
+ *   sigma' = C sum_i w'_i                                                  eq.(6)
+ *   Delta sigma' = Delta sigma (1/N) sum_i w'_i / w_i + sigma std(w')      eq.(7), population standard deviation;
+ *   events with w_i == 0 add nothing to the ratio sum (their w'_i is 0 by the zero guard) but count in N.
+ * trex_xsec_moments reduces one shard: w_in, w_out DEVICE [n]; moments HOST [4] out = (N, sum w', sum w'/w,
+ * M2 = sum (w' - mean)^2 with the shard's own mean). Two passes over the weights, fixed summation order
+ * (bit-reproducible); synchronises the stream. n == 0 gives zeros.
+ * trex_xsec_finish (host only) combines nparts shards (moments HOST [nparts][4], e.g. one per GPU, gathered by the
+ * caller) and applies eqs.(6)-(7): out HOST [3] = (sigma', Delta sigma', fallback flag). If the propagated error is
+ * infinite, NaN or not positive it is replaced by Delta sigma times whichever of sigma'/sigma, sigma/sigma' exceeds
+ * one (Delta sigma itself if that ratio is unusable too) and the flag is 1. */
+int trex_xsec_moments(const double* w_in, const double* w_out, int64_t n, double* moments);
+int trex_xsec_finish(const double* moments, int nparts, double C, double sigma, double dsigma, double* out);
 
 /* Roofline denominator: enqueues ONE launch of a register-resident FMA chain kernel (blocks x 256 threads, 64 FMAs per
  * thread and iteration) on the library stream and returns the floating-point operations it executes (2 per FMA), or a

@@ -36,9 +36,12 @@ _SIGNATURES = {
     "trex_colour_matrix": (_int, [_int, _dp]),
     "trex_reweight": (_int, [_int, _vp, _i64, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_run": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
+    "trex_run_multi": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _int, _vp, _vp, _vp, _vp]),
     "trex_run_host": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_debug_flow_amps": (_int, [_int, _dp, _dp, _dp]),
     "trex_probe_fma": (ctypes.c_double, [_int, _int, _int]),
+    "trex_xsec_moments": (_int, [_vp, _vp, ctypes.c_int64, _vp]),
+    "trex_xsec_finish": (_int, [_vp, _int, ctypes.c_double, ctypes.c_double, ctypes.c_double, _vp]),
     "trex_set_stream": (_int, [_vp]),
     "trex_set_precision": (_int, [_int]),
     "trex_get_precision": (_int, []),
@@ -250,6 +253,30 @@ def trex_run(pdg_keys, momenta_soa, theta_old, theta_new, w_in, w_out=None, me2_
     return w_out, me2_old, me2_new, nb
 
 
+def trex_run_multi(pdg_keys, momenta_soa, theta_old, thetas_new, w_in, w_out=None, me2_old=None, me2_new=None, want_me2=True):
+    """Many parameter points on one categorisation: thetas_new [K][TREX_NTHETA]. Returns (w_out [K, n], me2_old [n],
+    me2_new [K, n], nbuckets); row k is what trex_run gives for (theta_old, thetas_new[k])."""
+    torch = _torch()
+    n = w_in.numel()
+    npar = momenta_soa.shape[0]
+    tn = np.ascontiguousarray(np.asarray(thetas_new, dtype=np.float64).reshape(-1, TREX_NTHETA))
+    K = tn.shape[0]
+    if w_out is None:
+        w_out = torch.empty((K, n), dtype=torch.float64, device=w_in.device)
+    if want_me2 and me2_old is None:
+        me2_old = torch.empty_like(w_in)
+    if want_me2 and me2_new is None:
+        me2_new = torch.empty((K, n), dtype=torch.float64, device=w_in.device)
+    if tuple(w_out.shape) != (K, n) or (me2_new is not None and tuple(me2_new.shape) != (K, n)):
+        raise TrexError("trex_run_multi: w_out / me2_new must have shape [K, n]")
+    to, pto = _theta(theta_old)
+    f64 = torch.float64
+    nb = _check(lib().trex_run_multi(_dev(pdg_keys, torch.int64, "pdg_keys"), _dev(momenta_soa, f64, "momenta_soa"), n, npar,
+                                     pto, tn.ctypes.data_as(_dp), K, _dev(w_in, f64, "w_in"), _dev(w_out, f64, "w_out"),
+                                     _dev(me2_old, f64, "me2_old"), _dev(me2_new, f64, "me2_new")), "trex_run_multi")
+    return w_out, me2_old, me2_new, nb
+
+
 def _host(t, dtype, what):
     """Host pointer of a contiguous CPU torch tensor or numpy array (None -> NULL)."""
     if t is None:
@@ -275,6 +302,25 @@ def trex_run_host(pdg_keys, momenta_soa, theta_old, theta_new, w_in, w_out, me2_
     return _check(lib().trex_run_host(_host(pdg_keys, kdt, "pdg_keys"), _host(momenta_soa, f64, "momenta_soa"), n, npar,
                                       pto, ptn, _host(w_in, f64, "w_in"), _host(w_out, f64, "w_out"),
                                       _host(me2_old, f64, "me2_old"), _host(me2_new, f64, "me2_new")), "trex_run_host")
+
+
+def trex_xsec_moments(w_in, w_out):
+    """(N, sum w', sum w'/w, M2) of one shard of events; device tensors in, numpy [4] out."""
+    torch = _torch()
+    n = int(w_out.numel())
+    mom = np.zeros(4)
+    _check(lib().trex_xsec_moments(_dev(w_in, torch.float64, "w_in"), _dev(w_out, torch.float64, "w_out"), n,
+                                   mom.ctypes.data_as(ctypes.c_void_p)), "trex_xsec_moments")
+    return mom
+
+
+def trex_xsec_finish(moments, C, sigma, dsigma):
+    """Combine shard moments ([4] or [nparts, 4]) -> (sigma', Delta sigma', fallback_used). Host only: no GPU needed."""
+    m = np.ascontiguousarray(np.asarray(moments, dtype=np.float64).reshape(-1, 4))
+    out = np.zeros(3)
+    _check(lib().trex_xsec_finish(m.ctypes.data_as(ctypes.c_void_p), int(m.shape[0]), float(C), float(sigma), float(dsigma),
+                                  out.ctypes.data_as(ctypes.c_void_p)), "trex_xsec_finish")
+    return float(out[0]), float(out[1]), bool(out[2])
 
 
 def trex_probe_fma(fp32=False, blocks=148 * 8, iters=4096):

@@ -323,6 +323,53 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
   return bucket_finish(offsets);
 }
 
+// Many parameter points on ONE categorisation (the paper's actual workload: "sort once", eqs.(9)-(10) PAPER.md:1306-1310;
+// the iterator loop of PAPER.md:994-1002): bucketing and transposition run once, then every theta_new[k] gets its
+// reweighting launches and its transposition back into w_out[k]. Nothing waits for the device until the end.
+extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
+                              const double* theta_new, int ntheta, const double* w_in, double* w_out, double* me2_old,
+                              double* me2_new) {
+  Context& c = ctx();
+  if (n < 0 || npar < 1 || npar > 7 || ntheta < 0 || !theta_old || (ntheta > 0 && !theta_new))
+    return fail(TREX_EINVAL, "trex_run_multi: bad size or null theta");
+  if (n == 0 || ntheta == 0) return 0;
+  if (!pdg_keys || !momenta_soa || !w_in || !w_out) return fail(TREX_EINVAL, "trex_run_multi: null device pointer");
+  if (n >= (int64_t(1) << 31)) return fail(TREX_EINVAL, "trex_run_multi: n must be < 2^31");
+  std::vector<ThetaPair> T((size_t)ntheta * TREX_NSUBPROC);
+  for (int k = 0; k < ntheta; ++k)
+    for (int sid = 0; sid < TREX_NSUBPROC; ++sid)
+      if (subproc_info(sid)->npar == npar &&
+          !make_theta_pair(sid, theta_old, theta_new + (size_t)k * TREX_NTHETA, T[(size_t)k * TREX_NSUBPROC + sid]))
+        return fail(TREX_EINVAL, "trex_run_multi: theta_new[%d] outside its domain", k);
+  if (int rc = ensure_plan()) return rc;
+  if (int rc = ensure_colour()) return rc;
+  const int nrows = 4 * npar;
+  if (int rc = ensure_scratch(&c.run_perm, &c.run_perm_bytes, sizeof(int32_t) * (size_t)n)) return rc;
+  if (int rc = ensure_scratch(&c.run_blocks, &c.run_blocks_bytes, sizeof(double) * (size_t)n * (nrows + 1 + 3))) return rc;
+  if (int rc = bucket_reserve(n)) return rc;
+  c.last_nbuckets = 0;
+  double* blk = (double*)c.run_blocks;
+  double* res = blk + (size_t)(nrows + 1) * n;
+  if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar)) return rc;
+  if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm, blk, res)) return rc;
+  for (int k = 0; k < ntheta; ++k) {
+    double* wk = w_out + (size_t)k * n;
+    double* mok = k == 0 ? me2_old : nullptr;                   // |M(theta_old)|^2 is the same for every k
+    double* mnk = me2_new ? me2_new + (size_t)k * n : nullptr;
+    for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
+      if (subproc_info(sid)->npar != npar) continue;
+      ReweightArgs a;
+      a.io = EvIO{momenta_soa, (long)n, (long)n, w_in, wk, mok, mnk};
+      a.alt = EvIO{blk, (long)n, (long)n, blk + (size_t)nrows * n, res, res + n, res + 2 * (size_t)n};
+      a.plan = c.plan;
+      if (int rc = launch_reweight(sid, a, n, T[(size_t)k * TREX_NSUBPROC + sid])) return rc;
+    }
+    if (int rc = run_scatter(res, n, (const int32_t*)c.run_perm, wk, mok, mnk)) return rc;
+  }
+  int64_t offsets[REX_MAX_BUCKETS + 1];
+  return bucket_finish(offsets);
+}
+
 // the same with HOST buffers: copies in, runs, copies out, synchronises (bench.py's end-to-end figure)
 extern "C" int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
                              const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new) {
@@ -406,6 +453,9 @@ extern "C" void trex_shutdown(void) {
   if (c.run_blocks) cudaFree(c.run_blocks);
   if (c.host_io) cudaFree(c.host_io);
   if (c.probe_out) cudaFree(c.probe_out);
+  if (c.xsec_scratch) cudaFree(c.xsec_scratch);
+  if (c.xsec_host) cudaFreeHost(c.xsec_host);
+  c.xsec_scratch = c.xsec_host = nullptr;
   if (c.run_exec) cudaGraphExecDestroy(c.run_exec);
   if (c.cap_stream) cudaStreamDestroy(c.cap_stream);
   c.run_exec = nullptr; c.cap_stream = nullptr; c.exec_valid = false; c.last_key_valid = false;

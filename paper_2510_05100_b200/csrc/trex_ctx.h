@@ -37,6 +37,7 @@ struct Context {
   void* run_blocks = nullptr; size_t run_blocks_bytes = 0;
   void* host_io = nullptr; size_t host_io_bytes = 0;
   void* probe_out = nullptr;
+  void* xsec_scratch = nullptr; void* xsec_host = nullptr;   // trex_xsec_moments: block partials (device), result (pinned)
   // trex_run replayed as a CUDA graph when it is called again with the same buffers, sizes and parameter points
   struct RunKey {
     const void* ptr[6]; int64_t n; int npar, precision, table_min_n; double th[2 * TREX_NTHETA];

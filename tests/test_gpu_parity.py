@@ -292,3 +292,71 @@ def test_reduced_precision_modes_cfg4(T, mode):
     idx = np.arange(0, 4096, 512)
     rw, ro, rn = O.reweight(3, np.ascontiguousarray(w.momenta[:, :, idx]), w.theta_old, w.theta_new, w.w_in[idx])
     assert rel(ref_o[idx], ro).max() < RTOL64 and rel(ref_w[idx], rw).max() < RTOL64
+
+
+# ---------------------------------------------------------------- reweighted cross section
+@pytest.mark.parametrize("n", [1, 255, 100017])
+def test_xsec_moments_match_oracle(T, n):
+    import torch
+    rng = np.random.default_rng(n)
+    w = rng.lognormal(0, 0.5, n)
+    w[5::17] = 0.0
+    wo = w * rng.uniform(0.5, 2.0, n)
+    dw, dwo = dev(w), dev(wo)
+    m1 = T.trex_xsec_moments(dw, dwo)
+    m2 = T.trex_xsec_moments(dw, dwo)
+    assert np.array_equal(m1, m2)                               # fixed summation order
+    got = T.trex_xsec_finish(m1, 0.01, 3.0, 0.25)
+    ref = O.xsec(w, wo, 0.01, 3.0, 0.25)
+    assert abs(got[0] / ref[0] - 1) < 1e-12 and abs(got[1] / ref[1] - 1) < 1e-11 and got[2] == ref[2]
+    # three shards reduced separately and combined
+    cut = [0, n // 3, n // 3, n]
+    parts = [T.trex_xsec_moments(dev(w[a:b]), dev(wo[a:b])) if b > a else np.zeros(4) for a, b in zip(cut[:-1], cut[1:])]
+    got3 = T.trex_xsec_finish(parts, 0.01, 3.0, 0.25)
+    assert abs(got3[0] / ref[0] - 1) < 1e-12 and abs(got3[1] / ref[1] - 1) < 1e-11
+
+
+def test_xsec_of_a_reweighted_full_sample(T):
+    """cfg3 at full size: weights straight from trex_run (zero weights for unknown classes included)."""
+    import torch
+    w = make_config(3)
+    keys = w.keys.copy()
+    keys[::1001] = np.uint64(424242)
+    win = dev(w.w_in)
+    wo, _, _, nb = T.trex_run(dev(keys), dev(w.momenta), w.theta_old, w.theta_new, win)
+    got = T.trex_xsec_finish(T.trex_xsec_moments(win, wo), 1e-3, 40.0, 0.4)
+    ref = O.xsec(w.w_in, wo.cpu().numpy(), 1e-3, 40.0, 0.4)
+    assert nb == 6 and abs(got[0] / ref[0] - 1) < 1e-12 and abs(got[1] / ref[1] - 1) < 1e-11 and not got[2]
+
+
+# ---------------------------------------------------------------- many parameter points on one categorisation (NEXT-1)
+@pytest.mark.parametrize("cfg,n", [(3, 30011), (2, 5000)])
+def test_run_multi_equals_one_run_per_parameter_point(T, cfg, n):
+    """PAPER.md:1306-1310 "sort once": K parameter points after ONE rex_bucket + transposition; every row must equal
+    the single-point path bit for bit, and the oracle on a sample."""
+    import torch
+    w = make_config(cfg, n=n)
+    keys = w.keys.copy()
+    if cfg == 3:
+        keys[::97] = np.uint64(REX_NPOS)
+    thetas = []
+    for ctg, gt in ((0.25, 0.0), (1.0, 0.0), (-0.7, 1.4)):
+        th = w.theta_new.copy(); th[TH_CTG] = ctg; th[TH_GAMMAT] = gt
+        thetas.append(th)
+    dk, dm, dw = dev(keys), dev(w.momenta), dev(w.w_in)
+    wo, mo, mn, nb = T.trex_run_multi(dk, dm, w.theta_old, thetas, dw)
+    torch.cuda.synchronize()
+    for k, th in enumerate(thetas):
+        w1, mo1, mn1, nb1 = T.trex_run(dk, dm, w.theta_old, th, dw)
+        assert nb1 == nb and torch.equal(w1, wo[k]) and torch.equal(mn1, mn[k])
+        # |M(theta_old)|^2 is written once (k = 0); another k may run a different kernel variant (two top-line passes)
+        a1, a0 = mo1.cpu().numpy(), mo.cpu().numpy()
+        nz = a0 != 0
+        assert np.array_equal(a1 == 0, a0 == 0) and rel(a1[nz], a0[nz]).max() < 1e-13
+    # oracle on a few events of the largest class
+    sp = w.classes[0]
+    idx = np.where(keys == sp.key)[0][:12]
+    mom = np.ascontiguousarray(w.momenta[:, :, idx])
+    for k, th in enumerate(thetas):
+        rw, ro, rn = O.reweight(sp.sid, mom, w.theta_old, th, w.w_in[idx])
+        assert rel(wo[k].cpu().numpy()[idx], rw).max() < RTOL64 and rel(mn[k].cpu().numpy()[idx], rn).max() < RTOL64

@@ -59,3 +59,44 @@ def test_shard_range_properties():
             assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))
             sizes = [b - a for a, b in r]
             assert max(sizes) - min(sizes) <= 1
+
+
+def _xsec_worker(rank, world, port, n, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_2510_05100_b200.shard import xsec_all_ranks
+    rng = np.random.default_rng(21)
+    w = rng.lognormal(0, 0.5, n)
+    wo = w * rng.uniform(0.5, 2.0, n)
+    lo, hi = shard_range(n, rank, world)
+    a, b = w[lo:hi], wo[lo:hi]
+    mom = [float(hi - lo), float(b.sum()), float((b / a).sum()), float(((b - b.mean()) ** 2).sum())]
+    res = xsec_all_ranks(mom, 0.1, 5.0, 0.2)
+    gathered = [None] * world
+    dist.all_gather_object(gathered, res)
+    if rank == 0:
+        out.put(gathered)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_cross_section_equals_the_single_rank_definition():
+    """eqs.(6)-(7) over a sharded sample: the all-gather of four moments per rank is the only exchange."""
+    from oracle import oracle as O
+    n = 1001
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_xsec_worker, args=(r, 2, port, n, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = out.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+    rng = np.random.default_rng(21)
+    w = rng.lognormal(0, 0.5, n)
+    wo = w * rng.uniform(0.5, 2.0, n)
+    ref = O.xsec(w, wo, 0.1, 5.0, 0.2)
+    assert res[0] == res[1]                                    # every rank holds the same numbers
+    assert abs(res[0][0] / ref[0] - 1) < 1e-13 and abs(res[0][1] / ref[1] - 1) < 1e-12 and not res[0][2]
