@@ -244,6 +244,21 @@ def main():
         del keys, mom, win, wout
         return res
 
+    def measure_multi(cfg, K, poly, warm, steps):
+        """NEXT-1: K parameter points (c_tG scan) on one categorisation; value = events x parameter points per second."""
+        w = make_config(cfg)
+        keys, mom, win = dev(w.keys), dev(w.momenta), dev(w.w_in)
+        thetas = np.tile(w.theta_new, (K, 1))
+        thetas[:, 7] = np.linspace(-1.0, 1.0, K)
+        wout = torch.empty((K, w.n), dtype=torch.float64, device="cuda")
+        T.trex_set_poly_multi(poly)
+        sec = time_steps(lambda: T.trex_run_multi(keys, mom, w.theta_old, thetas, win, w_out=wout, want_me2=False), warm, steps)
+        T.trex_set_poly_multi(True)
+        assert bool(torch.isfinite(wout).all())
+        return {"workload": w.name + ", %d parameter points (c_tG scan), %s" % (K, "polynomial path" if poly else "one pass per point"),
+                "events": w.n, "parameter_points": K, "ms_per_step": 1e3 * sec / steps,
+                "value": world * w.n * K * steps / sec, "unit": "event-parameter-points/s"}
+
     if args.profile:
         T.trex_set_precision(args.precision)
         for cfg in [int(c) for c in args.profile.split(",")]:
@@ -277,6 +292,9 @@ def main():
             configs["cfg%d" % cfg] = measure(cfg, warm, steps)
         configs["cfg4_mixed"] = measure(4, 1, 2, precision=1)
         configs["cfg4_fp32"] = measure(4, 1, 2, precision=2)
+        configs["cfg3_multi8_direct"] = measure_multi(3, 8, False, 1, 2)
+        configs["cfg3_multi8_poly"] = measure_multi(3, 8, True, 1, 2)
+        configs["cfg3_multi64_poly"] = measure_multi(3, 64, True, 1, 2)
         for name, r in configs.items():
             if "kernel_tflops" in r:
                 r["roofline_frac_fp64_measured"] = r["kernel_tflops"] / fp64_peak

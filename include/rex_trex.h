@@ -115,8 +115,14 @@ int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int
 /* Many parameter points on one categorisation ("sort once", eqs.(9)-(10); the launch loop over
  * parameter cards): rex_bucket and the transposition run ONCE, then every theta_new[k] is evaluated.
  * theta_new HOST [ntheta][TREX_NTHETA]; w_out DEVICE [ntheta][n]; me2_old DEVICE [n] or NULL (the same for every k);
- * me2_new DEVICE [ntheta][n] or NULL. Row k equals what trex_run gives for (theta_old, theta_new[k]), bit for bit.
- * Returns the number of buckets; synchronises the stream once, at the end. */
+ * me2_new DEVICE [ntheta][n] or NULL. Returns the number of buckets; synchronises the stream once, at the end.
+ * Direct path: one reweighting pass per parameter point; row k equals what trex_run gives for (theta_old,
+ * theta_new[k]) bit for bit. Polynomial path (ntheta >= 4, a QCD sample, and every theta_new[k] differs from theta_old
+ * only in c_tG / Lambda / vev, i.e. in kappa): |M|^2 is exactly quadratic in kappa (one dimension-6 insertion per
+ * amplitude), so |M|^2 is evaluated at kappa_old and kappa_old +- max_k |kappa_k - kappa_old| (two passes) and every
+ * row is the per-event polynomial through those three values -- the cost no longer grows with ntheta beyond one
+ * HBM-bound write per row; rows agree with the direct path to ~1e-13 relative. trex_set_poly_multi(0) forces the
+ * direct path. */
 int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
                    const double* theta_new, int ntheta, const double* w_in, double* w_out, double* me2_old, double* me2_new);
 
@@ -154,6 +160,7 @@ int trex_set_stream(void* cuda_stream);
 int trex_set_precision(int mode);      /* 0 = fp64 (default), 1 = mixed (amplitudes fp64, colour sum fp32,
                                           PAPER.md:1209 fptype m), 2 = fp32 */
 int trex_get_precision(void);
+int trex_set_poly_multi(int on);         /* 1 (default): trex_run_multi may use its polynomial path */
 /* Evaluation strategy of g g -> t t~ + (N-2) g: processes with N >= algo gluons (algo = 3, 4, 5; default 3) use the
  * fused current-table kernel (per-event shared-memory table of off-shell gluon currents shared by all helicities,
  * "helicity recycling"); the others, and all of them for algo = 0, use one thread per helicity unit walking every

@@ -45,6 +45,7 @@ _SIGNATURES = {
     "trex_set_stream": (_int, [_vp]),
     "trex_set_precision": (_int, [_int]),
     "trex_get_precision": (_int, []),
+    "trex_set_poly_multi": (_int, [_int]),
     "trex_set_algorithm": (_int, [_int]),
     "trex_launch_count": (ctypes.c_int64, []),
     "trex_last_error": (ctypes.c_char_p, []),
@@ -150,6 +151,10 @@ def trex_set_precision(mode):
 
 def trex_set_algorithm(algo):
     return _check(lib().trex_set_algorithm(int(algo)), "trex_set_algorithm")
+
+
+def trex_set_poly_multi(on):
+    return _check(lib().trex_set_poly_multi(int(bool(on))), "trex_set_poly_multi")
 
 
 def trex_get_precision():

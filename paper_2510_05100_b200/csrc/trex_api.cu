@@ -51,6 +51,25 @@ __global__ void __launch_bounds__(128) k_eemumu(const ReweightArgs a) {
   if (io.me2_new) io.me2_new[e] = mn;
 }
 
+// Polynomial parameter points (R-4: |M|^2 is EXACTLY quadratic in kappa): from |M|^2 at kappa0 and kappa0 +- delta,
+//   m(kappa0 + u delta) = m0 + u b + u^2 d,   b = (m+ - m-)/2,   d = (m+ + m-)/2 - m0,
+// every further parameter point costs one fused multiply-add pair and 8-16 B of HBM traffic per event.
+__global__ void __launch_bounds__(256) k_poly_weights(const double* __restrict__ w_in, const double* __restrict__ m0, const double* __restrict__ mp,
+                                                      const double* __restrict__ mm, long n, int K, const double* __restrict__ u,
+                                                      double* __restrict__ w_out, double* __restrict__ me2_new) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double a = m0[i], p = mp[i], q = mm[i];
+  const double b = 0.5 * (p - q), d = 0.5 * (p + q) - a;
+  const double wn = (a == 0.0) ? 0.0 : w_in[i] * (1.0 / a);           // zero guard
+  for (int k = 0; k < K; ++k) {
+    const double uk = u[k];
+    const double m = a + uk * (b + uk * d);
+    w_out[(long)k * n + i] = wn * m;
+    if (me2_new) me2_new[(long)k * n + i] = m;
+  }
+}
+
 // diagnostic: colour-flow amplitudes of one event, one thread per full helicity index h (bit `leg` of h = helicity
 // of that leg in process order)
 template <int N> struct DebugSink {
@@ -350,6 +369,56 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
   c.last_nbuckets = 0;
   double* blk = (double*)c.run_blocks;
   double* res = blk + (size_t)(nrows + 1) * n;
+  // Polynomial path: all parameter points differ from theta_old in kappa = c_tG v / (sqrt2 Lambda^2) only (same alpha_s,
+  // top mass and width; a QCD process) -> three evaluations fix the exact quadratic, the rest is a polynomial per event.
+  bool poly = ntheta >= 4 && npar >= 4 && c.poly_multi;
+  const auto kappa_of = [](const double* th) { return th[TREX_TH_CTG] * th[TREX_TH_VEV] / (std::sqrt(2.0) * th[TREX_TH_LAMBDA] * th[TREX_TH_LAMBDA]); };
+  const double k0 = kappa_of(theta_old);
+  double delta = 0.0;
+  for (int k = 0; k < ntheta && poly; ++k) {
+    const double* th = theta_new + (size_t)k * TREX_NTHETA;
+    for (int j = 0; j < TREX_NTHETA && poly; ++j)
+      if (j != TREX_TH_CTG && j != TREX_TH_LAMBDA && j != TREX_TH_VEV && th[j] != theta_old[j]) poly = false;
+    poly = poly && th[TREX_TH_LAMBDA] > 0.0;
+    delta = std::fmax(delta, std::fabs(kappa_of(th) - k0));
+  }
+  if (poly && delta > 0.0) {
+    if (int rc = ensure_scratch(&c.poly_tmp, &c.poly_tmp_bytes, sizeof(double) * (3 * (size_t)n + (size_t)ntheta))) return rc;
+    double* tmp = (double*)c.poly_tmp;              // [3][n]: m(kappa0), m(kappa0 + delta), m(kappa0 - delta); then u[ntheta]
+    double* du = tmp + 3 * (size_t)n;
+    std::vector<double> u((size_t)ntheta);
+    for (int k = 0; k < ntheta; ++k) u[k] = (kappa_of(theta_new + (size_t)k * TREX_NTHETA) - k0) / delta;
+    TREX_CUDA_CHECK(cudaMemcpyAsync(du, u.data(), sizeof(double) * ntheta, cudaMemcpyHostToDevice, c.stream));
+    // cudaMemcpyAsync from pageable memory returns after staging the source: u may go out of scope
+    double thp[2][TREX_NTHETA];
+    for (int s2 = 0; s2 < 2; ++s2) {
+      std::memcpy(thp[s2], theta_old, sizeof(double) * TREX_NTHETA);
+      thp[s2][TREX_TH_CTG] = (k0 + (s2 == 0 ? delta : -delta)) * std::sqrt(2.0) * theta_old[TREX_TH_LAMBDA] * theta_old[TREX_TH_LAMBDA] / theta_old[TREX_TH_VEV];
+    }
+    if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar)) return rc;
+    if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm, blk, res)) return rc;
+    for (int s2 = 0; s2 < 2; ++s2) {
+      double* mo_out = s2 == 0 ? tmp : nullptr;
+      double* mn_out = tmp + (size_t)(1 + s2) * n;
+      for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
+        if (subproc_info(sid)->npar != npar) continue;
+        ThetaPair Tp;
+        if (!make_theta_pair(sid, theta_old, thp[s2], Tp)) return fail(TREX_EINVAL, "trex_run_multi: theta outside its domain");
+        ReweightArgs a;
+        a.io = EvIO{momenta_soa, (long)n, (long)n, w_in, w_out, mo_out, mn_out};      // w_out row 0 doubles as a dummy here
+        a.alt = EvIO{blk, (long)n, (long)n, blk + (size_t)nrows * n, res, res + n, res + 2 * (size_t)n};
+        a.plan = c.plan;
+        if (int rc = launch_reweight(sid, a, n, Tp)) return rc;
+      }
+      if (int rc = run_scatter(res, n, (const int32_t*)c.run_perm, w_out, mo_out, mn_out)) return rc;
+    }
+    k_poly_weights<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(w_in, tmp, tmp + n, tmp + 2 * (size_t)n, n, ntheta, du, w_out, me2_new);
+    c.launches += 1;
+    if (me2_old) TREX_CUDA_CHECK(cudaMemcpyAsync(me2_old, tmp, sizeof(double) * n, cudaMemcpyDeviceToDevice, c.stream));
+    TREX_CUDA_CHECK(cudaGetLastError());
+    int64_t offs[REX_MAX_BUCKETS + 1];
+    return bucket_finish(offs);
+  }
   if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar)) return rc;
   if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm, blk, res)) return rc;
   for (int k = 0; k < ntheta; ++k) {
@@ -433,6 +502,7 @@ extern "C" int trex_set_precision(int mode) {
   ctx().precision = mode; return 0;
 }
 extern "C" int trex_get_precision(void) { return ctx().precision; }
+extern "C" int trex_set_poly_multi(int on) { ctx().poly_multi = on != 0; return 0; }
 extern "C" int trex_set_algorithm(int algo) {
   if (algo != 0 && (algo < 3 || algo > 5)) return fail(TREX_EINVAL, "trex_set_algorithm: algo must be 0, 3, 4 or 5");
   ctx().table_min_n = algo == 0 ? 99 : algo; return 0;
@@ -453,6 +523,8 @@ extern "C" void trex_shutdown(void) {
   if (c.run_blocks) cudaFree(c.run_blocks);
   if (c.host_io) cudaFree(c.host_io);
   if (c.probe_out) cudaFree(c.probe_out);
+  if (c.poly_tmp) cudaFree(c.poly_tmp);
+  c.poly_tmp = nullptr; c.poly_tmp_bytes = 0;
   if (c.xsec_scratch) cudaFree(c.xsec_scratch);
   if (c.xsec_host) cudaFreeHost(c.xsec_host);
   c.xsec_scratch = c.xsec_host = nullptr;

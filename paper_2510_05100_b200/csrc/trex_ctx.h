@@ -37,6 +37,8 @@ struct Context {
   void* run_blocks = nullptr; size_t run_blocks_bytes = 0;
   void* host_io = nullptr; size_t host_io_bytes = 0;
   void* probe_out = nullptr;
+  void* poly_tmp = nullptr; size_t poly_tmp_bytes = 0;   // trex_run_multi: |M|^2 at three kappa values + the u_k
+  bool poly_multi = true;
   void* xsec_scratch = nullptr; void* xsec_host = nullptr;   // trex_xsec_moments: block partials (device), result (pinned)
   // trex_run replayed as a CUDA graph when it is called again with the same buffers, sizes and parameter points
   struct RunKey {

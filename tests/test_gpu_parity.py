@@ -360,3 +360,44 @@ def test_run_multi_equals_one_run_per_parameter_point(T, cfg, n):
     for k, th in enumerate(thetas):
         rw, ro, rn = O.reweight(sp.sid, mom, w.theta_old, th, w.w_in[idx])
         assert rel(wo[k].cpu().numpy()[idx], rw).max() < RTOL64 and rel(mn[k].cpu().numpy()[idx], rn).max() < RTOL64
+
+
+@pytest.mark.parametrize("cfg,n", [(3, 20011), (2, 9001), (4, 300)])
+def test_run_multi_polynomial_path(T, cfg, n):
+    """Parameter points that differ in kappa only: three evaluations + the exact quadratic (R-4) against the
+    direct path and the oracle."""
+    import torch
+    w = make_config(cfg, n=n)
+    keys = w.keys.copy()
+    if cfg == 3:
+        keys[::97] = np.uint64(REX_NPOS)
+    tho = w.theta_old.copy()
+    if cfg == 4:
+        tho[TH_GAMMAT] = 1.5
+    tho[TH_CTG] = 0.2
+    thetas = []
+    for ctg in (-1.0, -0.3, 0.0, 0.2, 0.45, 2.0):
+        th = tho.copy(); th[TH_CTG] = ctg
+        thetas.append(th)
+    thetas[1][8] = 1200.0                                    # another Lambda: still only kappa moves
+    dk, dm, dw = dev(keys), dev(w.momenta), dev(w.w_in)
+    wp, mop, mnp, nb = T.trex_run_multi(dk, dm, tho, thetas, dw)
+    T.trex_set_poly_multi(False)
+    try:
+        wd, mod, mnd, nbd = T.trex_run_multi(dk, dm, tho, thetas, dw)
+    finally:
+        T.trex_set_poly_multi(True)
+    torch.cuda.synchronize()
+    assert nb == nbd
+    a, b = wp.cpu().numpy(), wd.cpu().numpy()
+    nz = b != 0
+    assert np.array_equal(a == 0, b == 0) and rel(a[nz], b[nz]).max() < 1e-12
+    a, b = mnp.cpu().numpy(), mnd.cpu().numpy()
+    assert rel(a[nz], b[nz]).max() < 1e-12 and torch.equal(mop, mod)
+    assert not np.allclose(wp[0].cpu().numpy()[nz[0]], wp[5].cpu().numpy()[nz[0]])     # the rows really differ
+    sp = w.classes[0]
+    idx = np.where(keys == sp.key)[0][:6]
+    mom = np.ascontiguousarray(w.momenta[:, :, idx])
+    for k in (0, 1, 5):
+        rw, ro, rn = O.reweight(sp.sid, mom, tho, thetas[k], w.w_in[idx])
+        assert rel(wp[k].cpu().numpy()[idx], rw).max() < RTOL64 and rel(mnp[k].cpu().numpy()[idx], rn).max() < RTOL64
