@@ -126,10 +126,12 @@ int ensure_colour() {
   for (int N = 2; N <= 5; ++N) {
     std::vector<double> C = trex_colour::ttng_colour_matrix(N);
     if (N >= 3) {
-      std::vector<double> f((size_t)kTableFold[N - 3][0](C.data(), nullptr));
-      kTableFold[N - 3][0](C.data(), f.data());
-      TREX_CUDA_CHECK(cudaMalloc((void**)&c.Cfold[N - 3], sizeof(double) * f.size()));
-      TREX_CUDA_CHECK(cudaMemcpy(c.Cfold[N - 3], f.data(), sizeof(double) * f.size(), cudaMemcpyHostToDevice));
+      for (int m = 0; m < 3; ++m) {                     // the layout depends on the colour-sum variant of the mode
+        std::vector<double> f((size_t)kTableFold[N - 3][m](C.data(), nullptr));
+        kTableFold[N - 3][m](C.data(), f.data());
+        TREX_CUDA_CHECK(cudaMalloc((void**)&c.Cfold[N - 3][m], sizeof(double) * f.size()));
+        TREX_CUDA_CHECK(cudaMemcpy(c.Cfold[N - 3][m], f.data(), sizeof(double) * f.size(), cudaMemcpyHostToDevice));
+      }
       std::vector<int> meta((size_t)kTableMeta[N - 3][0](nullptr));
       kTableMeta[N - 3][0](meta.data());
       TREX_CUDA_CHECK(cudaMalloc((void**)&c.table_meta[N - 3], sizeof(int) * meta.size()));
@@ -206,7 +208,7 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
     const int N = sp->npar - 2;
     const int npass = (T.mt[0] != T.mt[1] || T.mGt[0] != T.mGt[1]) ? 2 : 1;
     if (N >= 3 && N >= c.table_min_n) {
-      if (kTableLaunch[N - 3][mode](a, npass, nmax, c.table_meta[N - 3], c.Cfold[N - 3], c.nsm, c.stream) != 0)
+      if (kTableLaunch[N - 3][mode](a, npass, nmax, c.table_meta[N - 3], c.Cfold[N - 3][mode], c.nsm, c.stream) != 0)
         return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     } else if (kLaunch[N - 2][mode](a, npass, grid32, c.stream) != 0) {
       return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -515,9 +517,9 @@ extern "C" void trex_shutdown(void) {
   if (c.bucket_host) cudaFreeHost(c.bucket_host);
   if (c.C120) cudaFree(c.C120);
   for (int i = 0; i < 3; ++i) {
-    if (c.Cfold[i]) cudaFree(c.Cfold[i]);
+    for (int m = 0; m < 3; ++m) { if (c.Cfold[i][m]) cudaFree(c.Cfold[i][m]); c.Cfold[i][m] = nullptr; }
     if (c.table_meta[i]) cudaFree(c.table_meta[i]);
-    c.Cfold[i] = nullptr; c.table_meta[i] = nullptr;
+    c.table_meta[i] = nullptr;
   }
   if (c.run_perm) cudaFree(c.run_perm);
   if (c.run_blocks) cudaFree(c.run_blocks);

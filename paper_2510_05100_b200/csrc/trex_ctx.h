@@ -54,7 +54,7 @@ struct Context {
   // colour matrices on the device
   bool colour_ready = false;
   double* C120 = nullptr;            // 120 x 120, global memory
-  double* Cfold[3] = {nullptr, nullptr, nullptr};   // folded upper-triangular colour matrices of N = 3, 4, 5 (trex_table_tu.cu)
+  double* Cfold[3][3] = {};          // folded upper-triangular colour matrices of N = 3, 4, 5 per precision mode (trex_table_tu.cu)
   int* table_meta[3] = {nullptr, nullptr, nullptr}; // tuple / entry index tables of the current-table kernels
 };
 

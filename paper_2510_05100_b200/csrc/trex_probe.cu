@@ -36,6 +36,28 @@ template <class R> __global__ void __launch_bounds__(256) k_fma_probe3(R* out, i
   if (s == R(-12345.678)) out[0] = s;
 }
 
+// FP64 tensor-core rate: mma.sync.m8n8k4.f64 (DMMA), 8 independent accumulator tiles per warp; 512 flop per mma.
+// (tcgen05 has no f64 kind; this is the only tensor path an FP64 colour sum could take.)
+__global__ void __launch_bounds__(256) k_dmma_probe(double* out, int iters, double a, double b) {
+  double c[8][2];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { c[k][0] = threadIdx.x + k; c[k][1] = threadIdx.x - k; }
+  const double fa = a + 1e-9 * threadIdx.x, fb = b + 1e-9 * threadIdx.x;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                     : "+d"(c[k][0]), "+d"(c[k][1]) : "d"(fa), "d"(fb));
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += c[k][0] + c[k][1];
+  if (s == -12345.678) out[0] = s;
+}
+
 }  // namespace
 }  // namespace trex
 
@@ -43,11 +65,17 @@ using namespace trex;
 
 // Enqueues one probe launch on the library stream and returns the number of floating-point operations it executes
 // (time it with events on that stream). fp32: 0 = FP64, 1 = FP32 (one register + two constant-bank operands per FMA);
-// 2 = FP64, 3 = FP32 with three register operands per FMA. Returns < 0 on error.
+// 2 = FP64, 3 = FP32 with three register operands per FMA; 4 = FP64 tensor cores (DMMA m8n8k4). Returns < 0 on error.
 extern "C" double trex_probe_fma(int fp32, int blocks, int iters) {
   Context& c = ctx();
   if (blocks <= 0 || iters <= 0) return (double)fail(TREX_EINVAL, "trex_probe_fma: blocks and iters must be positive");
   if (!c.probe_out && cudaMalloc(&c.probe_out, 64) != cudaSuccess) return (double)fail(TREX_ENOMEM, "trex_probe_fma: cudaMalloc failed");
+  if (fp32 == 4) {
+    k_dmma_probe<<<blocks, 256, 0, c.stream>>>((double*)c.probe_out, iters, 0.999, 0.001);
+    c.launches += 1;
+    if (cudaGetLastError() != cudaSuccess) return (double)fail(TREX_ECUDA, "trex_probe_fma: launch failed");
+    return 512.0 * 64.0 * (double)iters * 8.0 * (double)blocks;        // 512 flop x 64 mma per iteration x 8 warps
+  }
   if (fp32 == 2) k_fma_probe3<double><<<blocks, 256, 0, c.stream>>>((double*)c.probe_out, iters, 0.999, 0.001);
   else if (fp32 == 3) k_fma_probe3<float><<<blocks, 256, 0, c.stream>>>((float*)c.probe_out, iters, 0.999f, 0.001f);
   else if (fp32) k_fma_probe<float><<<blocks, 256, 0, c.stream>>>((float*)c.probe_out, iters, 0.999f, 0.001f);

@@ -40,10 +40,16 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long e = (long)blockIdx.x * 32 + lane;
   const long ev = e < io.n ? e : io.n - 1;
+  // all 16 momentum rows of the block's 32 events: one coalesced pass, one DRAM latency; later reads come from here
+  __shared__ double pm[16][32];
+  pm[warp][lane] = io.mom[(long)warp * io.ld + ev];
+  pm[warp + 8][lane] = io.mom[(long)(warp + 8) * io.ld + ev];
+  __syncthreads();
   {
     double p[4];
     const int leg = warp >> 1, lam = (warp & 1) ? 1 : -1;      // legs in process order: g g t t~
-    load_leg<double>(io.mom, io.ld, ev, leg, p);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) p[mu] = pm[leg * 4 + mu][lane];
     if (leg < 2) {
       const vec4<double> w = polvec<double>(p, lam, false);
 #pragma unroll
@@ -62,7 +68,7 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
 #pragma unroll
   for (int i = 0; i < 4; ++i) ubar.c[i] = cx<R>(R(wf[4 + lt][2 * i][lane]), R(wf[4 + lt][2 * i + 1][lane]));
 #pragma unroll
-  for (int mu = 0; mu < 4; ++mu) pt.c[mu] = io.mom[(long)(8 + mu) * io.ld + ev];
+  for (int mu = 0; mu < 4; ++mu) pt.c[mu] = pm[8 + mu][lane];
   // ---- tuple (1,2) attached to the line at once: i ubar Jslash_12 and ubar sigma.F_12; ordering (2,1) takes the opposite sign
   spinor<R> d0, d1 = szero<R>();
   {
@@ -72,7 +78,7 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
     for (int i = 0; i < 4; ++i) {
       e1.c[i] = cx<R>(R(wf[wsel[0]][2 * i][lane]), R(wf[wsel[0]][2 * i + 1][lane]));
       e2.c[i] = cx<R>(R(wf[wsel[1]][2 * i][lane]), R(wf[wsel[1]][2 * i + 1][lane]));
-      K1.c[i] = io.mom[(long)i * io.ld + ev]; K2.c[i] = io.mom[(long)(4 + i) * io.ld + ev];
+      K1.c[i] = pm[i][lane]; K2.c[i] = pm[4 + i][lane];
     }
     const rvec4<double> P12 = radd(K1, K2);
     vec4<R> acc = vzero<R>();
@@ -107,7 +113,7 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
     for (int i = 0; i < 4; ++i) {
       ea.c[i] = cx<R>(R(wf[wsel[ga]][2 * i][lane]), R(wf[wsel[ga]][2 * i + 1][lane]));
       eb.c[i] = cx<R>(R(wf[wsel[gb]][2 * i][lane]), R(wf[wsel[gb]][2 * i + 1][lane]));
-      Ka.c[i] = io.mom[(long)(ga * 4 + i) * io.ld + ev]; Kb.c[i] = io.mom[(long)(gb * 4 + i) * io.ld + ev];
+      Ka.c[i] = pm[ga * 4 + i][lane]; Kb.c[i] = pm[gb * 4 + i][lane];
     }
     // U(a) = ubar Gamma(eps_a) S(p_t - K_a)
     dspinor<R> U1;
