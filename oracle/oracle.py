@@ -180,3 +180,50 @@ def xsec(w_in, w_out, C, sigma, dsigma):
         r = sigma_p / sigma if sigma != 0.0 else float("nan")
         d = dsigma * max(r, 1.0 / r) if (math.isfinite(r) and r > 0.0) else float(dsigma)
     return sigma_p, d, fallback
+
+
+# ---------------------------------------------------------------- flavour keys and parton re-indexing (NEXT-3)
+def flavour_key(pdg, n_in):
+    """Flavour signature of one event from its PDG codes (first n_in legs incoming): initial-state codes sorted
+    ascending, then final-state codes sorted ascending -- two events are the same process iff their unordered initial and
+    final flavour content agree (default comparator). One byte per leg ((|pdg| & 0x7F) | 0x80 if
+    negative), byte 7 = (n_in << 4) | n_out; codes beyond 127 or more than 7 legs give REX_NPOS (all ones)."""
+    legs = sorted(int(p) for p in pdg[:n_in]) + sorted(int(p) for p in pdg[n_in:])
+    if len(legs) > 7 or any(abs(p) > 127 for p in legs):
+        return np.uint64(0xFFFFFFFFFFFFFFFF)
+    key = 0
+    for i, p in enumerate(legs):
+        key |= ((abs(p) & 0x7F) | (0x80 if p < 0 else 0)) << (8 * i)
+    key |= ((n_in << 4) | (len(legs) - n_in)) << 56
+    return np.uint64(key)
+
+
+def keys_and_legmap(pdg, n_in, process_strings):
+    """pdg int [npar, n]; process_strings: the PDG tuples of the compiled-in subprocesses in process-string order.
+    Returns (keys uint64 [n], legmap int8 [npar, n]): legmap[pos, i] = the leg of event i that plays position `pos` of the
+    process string of the subprocess with the same flavour key (partons are re-indexed to the
+    representative's order) -- for every position, in order, the FIRST not yet used leg on the same side (initial /
+    final) with that PDG code, so identical particles keep their event order. Events no subprocess claims map to the
+    identity. Plain loops."""
+    pdg = np.asarray(pdg)
+    npar, n = pdg.shape
+    table = {int(flavour_key(np.array(ps), n_in)): ps for ps in process_strings if len(ps) == npar}
+    keys = np.zeros(n, dtype=np.uint64)
+    legmap = np.zeros((npar, n), dtype=np.int8)
+    for i in range(n):
+        ev = [int(x) for x in pdg[:, i]]
+        k = flavour_key(ev, n_in)
+        keys[i] = k
+        ps = table.get(int(k))
+        if ps is None:
+            legmap[:, i] = np.arange(npar)
+            continue
+        used = [False] * npar
+        for pos in range(npar):
+            side = range(0, n_in) if pos < n_in else range(n_in, npar)
+            for leg in side:
+                if not used[leg] and ev[leg] == ps[pos]:
+                    used[leg] = True
+                    legmap[pos, i] = leg
+                    break
+    return keys, legmap

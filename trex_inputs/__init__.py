@@ -9,6 +9,6 @@ imports the other.
 from .configs import (  # noqa: F401
     NTHETA, TH_ALPHA_S, TH_ALPHA_EM, TH_SIN2W, TH_MZ, TH_GAMMAZ, TH_MT, TH_GAMMAT,
     TH_CTG, TH_LAMBDA, TH_VEV, default_theta, make_config, Workload, SUBPROCESSES,
-    pack_key, REX_NPOS, subprocess_by_name, subprocess_by_key,
+    pack_key, REX_NPOS, subprocess_by_name, subprocess_by_key, shuffled_legs,
 )
 from .rambo import massive_rambo  # noqa: F401

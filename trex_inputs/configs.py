@@ -198,3 +198,31 @@ def make_config(cfg, n=None):
         return Workload(5, "cfg5 gg -> tt~ggg", n, 7, np.full(n, sp.key, dtype=np.uint64),
                         mom, np.ones(n), th_old, th_new, (sp,))
     raise ValueError(f"unknown config {cfg}")
+
+
+def shuffled_legs(w, seed, unknown_every=0):
+    """LHE-like view of a workload: per-event PDG codes [npar, n] (int32) and momenta whose legs were shuffled inside
+    the initial state and inside the final state with a seeded permutation per event (an LHE file does not promise the
+    parton order of the process string: PAPER.md:227-242). Returns (pdg, momenta, n_in). `unknown_every` > 0 turns
+    every k-th event into a class no subprocess claims (s s~ > ...). No method arithmetic here: only labels move."""
+    rng = np.random.default_rng(seed)
+    npar, n = w.npar, w.n
+    n_in = 2
+    pdg = np.zeros((npar, n), dtype=np.int32)
+    for sp in (w.classes if w.classes else ()):
+        sel = w.keys == sp.key
+        for leg in range(npar):
+            pdg[leg, sel] = sp.pdg[leg]
+    mom = w.momenta.copy()
+    order = np.tile(np.arange(npar)[:, None], (1, n))
+    swap = rng.random(n) < 0.5
+    order[0, swap], order[1, swap] = 1, 0
+    fin = np.argsort(rng.random((npar - n_in, n)), axis=0) + n_in
+    order[n_in:, :] = fin
+    cols = np.arange(n)
+    pdg = pdg[order, cols]
+    mom = np.ascontiguousarray(mom[order, :, cols].transpose(0, 2, 1))     # [npar, n, 4] -> [npar, 4, n]
+    if unknown_every:
+        pdg[0, ::unknown_every] = 3
+        pdg[1, ::unknown_every] = -3
+    return pdg, mom, n_in
