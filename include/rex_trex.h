@@ -112,6 +112,20 @@ int trex_reweight(int subproc_id, const double* momenta_soa, int64_t n, const do
 int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
              const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
 
+/* Flavour keys and parton re-indexing on the device: pdg_soa DEVICE int32 [npar][n]
+ * (first n_in legs incoming, in ANY order inside the initial and inside the final state); keys DEVICE [n] out, the layout
+ * of rex_pack_key (REX_NPOS for codes beyond +-127); legmap DEVICE int8 [npar][n] out or NULL: legmap[pos][i] = the leg of
+ * event i that plays position pos of the process string of the compiled-in subprocess with that key -- for every
+ * position, in order, the first not yet used leg on the same side with that PDG code, so identical particles keep
+ * their event order; the identity for events no subprocess claims. Asynchronous on the library stream. */
+int rex_keys(const int32_t* pdg_soa, int npar, int n_in, int64_t n, uint64_t* keys, int8_t* legmap);
+
+/* trex_run for events given by PDG codes in arbitrary parton order: rex_keys, then the path of trex_run with the
+ * transposition re-indexing every event's legs to the process-string order. momenta_soa [npar][4][n] in the events'
+ * own leg order. Same outputs and return value as trex_run. */
+int trex_run_pdg(const int32_t* pdg_soa, const double* momenta_soa, int64_t n, int npar, int n_in, const double* theta_old,
+                 const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
+
 /* Many parameter points on one categorisation ("sort once", eqs.(9)-(10); the launch loop over
  * parameter cards): rex_bucket and the transposition run ONCE, then every theta_new[k] is evaluated.
  * theta_new HOST [ntheta][TREX_NTHETA]; w_out DEVICE [ntheta][n]; me2_old DEVICE [n] or NULL (the same for every k);

@@ -36,6 +36,8 @@ _SIGNATURES = {
     "trex_colour_matrix": (_int, [_int, _dp]),
     "trex_reweight": (_int, [_int, _vp, _i64, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_run": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
+    "rex_keys": (_int, [_vp, _int, _int, _i64, _vp, _vp]),
+    "trex_run_pdg": (_int, [_vp, _vp, _i64, _int, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_run_multi": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _int, _vp, _vp, _vp, _vp]),
     "trex_run_host": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_debug_flow_amps": (_int, [_int, _dp, _dp, _dp]),
@@ -255,6 +257,38 @@ def trex_run(pdg_keys, momenta_soa, theta_old, theta_new, w_in, w_out=None, me2_
     nb = _check(lib().trex_run(_dev(pdg_keys, torch.int64, "pdg_keys"), _dev(momenta_soa, f64, "momenta_soa"), n, npar,
                                pto, ptn, _dev(w_in, f64, "w_in"), _dev(w_out, f64, "w_out"),
                                _dev(me2_old, f64, "me2_old"), _dev(me2_new, f64, "me2_new")), "trex_run")
+    return w_out, me2_old, me2_new, nb
+
+
+def rex_keys(pdg_soa, n_in, want_legmap=True):
+    """Flavour keys (int64 view of the uint64 keys) and leg maps (int8 [npar, n]) of events given by PDG codes
+    (int32 CUDA tensor [npar, n], first n_in legs incoming, any order inside each side)."""
+    torch = _torch()
+    npar, n = int(pdg_soa.shape[0]), int(pdg_soa.shape[1])
+    keys = torch.empty(n, dtype=torch.int64, device=pdg_soa.device)
+    legmap = torch.empty((npar, n), dtype=torch.int8, device=pdg_soa.device) if want_legmap else None
+    _check(lib().rex_keys(_dev(pdg_soa, torch.int32, "pdg_soa"), npar, int(n_in), n, _dev(keys, torch.int64, "keys"),
+                          _dev(legmap, torch.int8, "legmap")), "rex_keys")
+    return keys, legmap
+
+
+def trex_run_pdg(pdg_soa, momenta_soa, n_in, theta_old, theta_new, w_in, w_out=None, me2_old=None, me2_new=None, want_me2=True):
+    """trex_run for events given by PDG codes in arbitrary parton order. Returns (w_out, me2_old, me2_new, nbuckets)."""
+    torch = _torch()
+    n = w_in.numel()
+    npar = momenta_soa.shape[0]
+    if w_out is None:
+        w_out = torch.empty_like(w_in)
+    if want_me2 and me2_old is None:
+        me2_old = torch.empty_like(w_in)
+    if want_me2 and me2_new is None:
+        me2_new = torch.empty_like(w_in)
+    to, pto = _theta(theta_old)
+    tn, ptn = _theta(theta_new)
+    f64 = torch.float64
+    nb = _check(lib().trex_run_pdg(_dev(pdg_soa, torch.int32, "pdg_soa"), _dev(momenta_soa, f64, "momenta_soa"), n, npar, int(n_in),
+                                   pto, ptn, _dev(w_in, f64, "w_in"), _dev(w_out, f64, "w_out"),
+                                   _dev(me2_old, f64, "me2_old"), _dev(me2_new, f64, "me2_new")), "trex_run_pdg")
     return w_out, me2_old, me2_new, nb
 
 

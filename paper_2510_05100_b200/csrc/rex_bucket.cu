@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_hist(const unsigned long long* _
 }
 
 __global__ void __launch_bounds__(1024) k_scan(unsigned* __restrict__ counts, long nchunks, long n, Table t, BucketResult* res,
-                                               const unsigned long long* __restrict__ sub, int npar, DevPlan* __restrict__ plan) {
+                                               const unsigned long long* __restrict__ sub, int npar, DevPlan* __restrict__ plan, int force_gather) {
   __shared__ unsigned long long part[1024];
   const int nb = t.meta[3];
   const long total = (long)nb * nchunks;
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(1024) k_scan(unsigned* __restrict__ counts, lo
     plan->off[sid] = off; plan->cnt[sid] = cnt;
   }
   const int any = __syncthreads_or(found ? 1 : 0);
-  if (sid == 0) { plan->single = (nb == 1 && any) ? 1 : 0; plan->nb = nb; }
+  if (sid == 0) { plan->single = (nb == 1 && any && !force_gather) ? 1 : 0; plan->nb = nb; }
 }
 
 __global__ void __launch_bounds__(WARPS * 32) k_scatter(const unsigned long long* __restrict__ keys, long n, long wch, long nchunks,
@@ -251,7 +251,7 @@ constexpr int SB_WARPS = 32;
 
 __global__ void __launch_bounds__(1024) k_bucket_small(const unsigned long long* __restrict__ keys, long n, int* __restrict__ perm,
                                                        BucketResult* __restrict__ res, const unsigned long long* __restrict__ sub,
-                                                       int npar, DevPlan* __restrict__ plan) {
+                                                       int npar, DevPlan* __restrict__ plan, int force_gather) {
   __shared__ unsigned long long sk[TS];
   __shared__ unsigned sf[TS];
   __shared__ int sb[TS];
@@ -363,17 +363,61 @@ __global__ void __launch_bounds__(1024) k_bucket_small(const unsigned long long*
       plan->off[tid] = off; plan->cnt[tid] = c;
     }
     const int any = __syncthreads_or(found ? 1 : 0);
-    if (tid == 0) { plan->single = (nb == 1 && any) ? 1 : 0; plan->nb = nb; }
+    if (tid == 0) { plan->single = (nb == 1 && any && !force_gather) ? 1 : 0; plan->nb = nb; }
+  }
+}
+
+// flavour key and leg map of every event from its PDG codes (SoA [npar][n], first n_in legs incoming). Key: rex_pack_key's
+// layout. Leg map: for every position of the process string of the subprocess with that key, in order, the first not yet
+// used leg on the same side with that PDG code (identical particles keep their event order); identity if nobody claims
+// the event. sub: registry uploaded by ensure_plan (keys, leg counts, process strings).
+__global__ void __launch_bounds__(256) k_keys(const int* __restrict__ pdg, int npar, int n_in, long n, const unsigned long long* __restrict__ sub,
+                                              unsigned long long* __restrict__ keys, signed char* __restrict__ legmap) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int ev[7], srt[7];
+  bool bad = false;
+  for (int l = 0; l < npar; ++l) { ev[l] = pdg[(long)l * n + i]; srt[l] = ev[l]; bad = bad || ev[l] > 127 || ev[l] < -127; }
+  for (int side = 0; side < 2; ++side) {                     // insertion sort inside the initial and the final state
+    const int lo = side ? n_in : 0, hi = side ? npar : n_in;
+    for (int a = lo + 1; a < hi; ++a) { const int x = srt[a]; int b = a - 1; while (b >= lo && srt[b] > x) { srt[b + 1] = srt[b]; --b; } srt[b + 1] = x; }
+  }
+  unsigned long long key = 0;
+  for (int l = 0; l < npar; ++l) { const int q = srt[l]; key |= (unsigned long long)(((q < 0 ? -q : q) & 0x7F) | (q < 0 ? 0x80 : 0)) << (8 * l); }
+  key |= (unsigned long long)((n_in << 4) | (npar - n_in)) << 56;
+  if (bad) key = EMPTY;
+  keys[i] = key;
+  if (!legmap) return;
+  int sid = -1;
+  for (int s = 0; s < TREX_NSUBPROC; ++s) if (sub[2 * s] == key && (int)sub[2 * s + 1] == npar) sid = s;
+  unsigned used = 0;
+  for (int pos = 0; pos < npar; ++pos) {
+    int pick = pos;
+    if (sid >= 0) {
+      const int want = (int)(long long)sub[2 * TREX_NSUBPROC + 8 * sid + pos];
+      const int lo = pos < n_in ? 0 : n_in, hi = pos < n_in ? n_in : npar;
+      for (int l = hi - 1; l >= lo; --l) if (!((used >> l) & 1u) && ev[l] == want) pick = l;
+      used |= 1u << pick;
+    }
+    legmap[(long)pos * n + i] = (signed char)pick;
   }
 }
 
 // momenta rows + weights into bucketed order; result rows cleared (classes nobody claims keep zero weights)
 __global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __restrict__ mom, const double* __restrict__ w_in, long n,
-                             int nrows, const int* __restrict__ perm, double* __restrict__ blk, double* __restrict__ res) {
+                             int nrows, const int* __restrict__ perm, double* __restrict__ blk, double* __restrict__ res,
+                             const signed char* __restrict__ legmap) {
   if (plan->single) return;
   const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   const long p = perm[j];
+  if (legmap) {
+    // parton re-indexing: position `leg` of the process string is played by leg legmap[leg] of the event
+    for (int leg = 0; leg < nrows / 4; ++leg) {
+      const int src = legmap[(long)leg * n + p];
+      for (int mu = 0; mu < 4; ++mu) blk[(long)(leg * 4 + mu) * n + j] = mom[(long)(src * 4 + mu) * n + p];
+    }
+  } else
   for (int r = 0; r < nrows; ++r) blk[(long)r * n + j] = mom[(long)r * n + p];
   blk[(long)nrows * n + j] = w_in[p];
   res[j] = 0.0; res[n + j] = 0.0; res[2 * n + j] = 0.0;
@@ -445,7 +489,7 @@ int trex::bucket_enqueue(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int
   const unsigned long long* keys = (const unsigned long long*)pdg_keys;
 
   if (n <= SMALL_N) {
-    k_bucket_small<<<1, 1024, 0, c.stream>>>(keys, n, perm, res, (const unsigned long long*)c.plan_keys, npar, c.plan);
+    k_bucket_small<<<1, 1024, 0, c.stream>>>(keys, n, perm, res, (const unsigned long long*)c.plan_keys, npar, c.plan, c.legmap ? 1 : 0);
     c.launches += 1;
     TREX_CUDA_CHECK(cudaGetLastError());
     TREX_CUDA_CHECK(cudaMemcpyAsync(c.bucket_host, res, sizeof(BucketResult), cudaMemcpyDeviceToHost, c.stream));
@@ -459,7 +503,7 @@ int trex::bucket_enqueue(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int
   k_rank<<<1, TS, 0, c.stream>>>(t, res);
   const unsigned cblk = (unsigned)((nchunks + WARPS - 1) / WARPS);
   k_hist<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts);
-  k_scan<<<1, 1024, 0, c.stream>>>(counts, nchunks, n, t, res, (const unsigned long long*)c.plan_keys, npar, c.plan);
+  k_scan<<<1, 1024, 0, c.stream>>>(counts, nchunks, n, t, res, (const unsigned long long*)c.plan_keys, npar, c.plan, c.legmap ? 1 : 0);
   k_scatter<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts, perm);
   c.launches += 6;
   TREX_CUDA_CHECK(cudaGetLastError());
@@ -491,7 +535,7 @@ extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, in
 
 int trex::run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* perm, double* blk, double* res) {
   Context& c = ctx();
-  k_run_gather<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, mom, w_in, n, nrows, perm, blk, res);
+  k_run_gather<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, mom, w_in, n, nrows, perm, blk, res, (const signed char*)c.legmap);
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());
   return 0;
@@ -500,6 +544,19 @@ int trex::run_gather(const double* mom, const double* w_in, int64_t n, int nrows
 int trex::run_scatter(const double* res, int64_t n, const int32_t* perm, double* w_out, double* me2_old, double* me2_new) {
   Context& c = ctx();
   k_run_scatter<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, res, n, perm, w_out, me2_old, me2_new);
+  c.launches += 1;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return 0;
+}
+
+extern "C" int rex_keys(const int32_t* pdg_soa, int npar, int n_in, int64_t n, uint64_t* keys, int8_t* legmap) {
+  Context& c = ctx();
+  if (n < 0 || npar < 1 || npar > 7 || n_in < 0 || n_in > npar) return fail(TREX_EINVAL, "rex_keys: bad size");
+  if (n == 0) return 0;
+  if (!pdg_soa || !keys) return fail(TREX_EINVAL, "rex_keys: null device pointer");
+  if (int rc = ensure_plan()) return rc;
+  k_keys<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(pdg_soa, npar, n_in, n, (const unsigned long long*)c.plan_keys,
+                                                           (unsigned long long*)keys, (signed char*)legmap);
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());
   return 0;

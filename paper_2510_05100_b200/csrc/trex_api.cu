@@ -238,17 +238,18 @@ extern "C" int trex_reweight(int sid, const double* momenta_soa, int64_t n, cons
   return launch_reweight(sid, a, n, T);
 }
 
-// key and leg count of every compiled-in subprocess, for the device-side plan
-static int ensure_plan() {
+// key, leg count and process string of every compiled-in subprocess, for the device-side plan and rex_keys
+int trex::ensure_plan() {
   Context& c = ctx();
   if (c.plan) return 0;
-  unsigned long long sub[2 * TREX_NSUBPROC];
+  unsigned long long sub[2 * TREX_NSUBPROC + 8 * TREX_NSUBPROC] = {0};
   for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
     const SubprocInfo* sp = subproc_info(sid);
     int8_t status[7];
     for (int i = 0; i < sp->npar; ++i) status[i] = i < 2 ? -1 : 1;
     sub[2 * sid] = rex_pack_key(sp->pdg, status, sp->npar);
     sub[2 * sid + 1] = (unsigned long long)sp->npar;
+    for (int i = 0; i < sp->npar; ++i) sub[2 * TREX_NSUBPROC + 8 * sid + i] = (unsigned long long)(long long)sp->pdg[i];
   }
   TREX_CUDA_CHECK(cudaMalloc(&c.plan_keys, sizeof sub));
   TREX_CUDA_CHECK(cudaMemcpy(c.plan_keys, sub, sizeof sub, cudaMemcpyHostToDevice));
@@ -342,6 +343,25 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
   c.last_key = key; c.last_key_valid = true;
   if (int rc = enqueue()) return rc;
   return bucket_finish(offsets);
+}
+
+// The path for events that carry PDG codes in arbitrary parton order (an LHE file does not promise the order of the
+// process string): flavour keys and per-event leg maps are formed on the device (rex_keys), the
+// transposition re-indexes every event's legs to the representative's order on the fly.
+extern "C" int trex_run_pdg(const int32_t* pdg_soa, const double* momenta_soa, int64_t n, int npar, int n_in, const double* theta_old,
+                            const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new) {
+  Context& c = ctx();
+  if (n < 0 || npar < 1 || npar > 7 || n_in < 0 || n_in > npar) return fail(TREX_EINVAL, "trex_run_pdg: bad size");
+  if (n == 0) return 0;
+  if (!pdg_soa) return fail(TREX_EINVAL, "trex_run_pdg: null device pointer");
+  if (int rc = ensure_scratch(&c.pdg_tmp, &c.pdg_tmp_bytes, (size_t)n * (sizeof(uint64_t) + (size_t)npar))) return rc;
+  uint64_t* keys = (uint64_t*)c.pdg_tmp;
+  int8_t* legmap = (int8_t*)(keys + n);
+  if (int rc = rex_keys(pdg_soa, npar, n_in, n, keys, legmap)) return rc;
+  c.legmap = legmap; c.in_host_run = true;               // no graph replay: the chain depends on the leg maps
+  const int rc = trex_run(keys, momenta_soa, n, npar, theta_old, theta_new, w_in, w_out, me2_old, me2_new);
+  c.legmap = nullptr; c.in_host_run = false;
+  return rc;
 }
 
 // Many parameter points on ONE categorisation (the paper's actual workload: "sort once", eqs.(9)-(10) PAPER.md:1306-1310;
@@ -525,6 +545,8 @@ extern "C" void trex_shutdown(void) {
   if (c.run_blocks) cudaFree(c.run_blocks);
   if (c.host_io) cudaFree(c.host_io);
   if (c.probe_out) cudaFree(c.probe_out);
+  if (c.pdg_tmp) cudaFree(c.pdg_tmp);
+  c.pdg_tmp = nullptr; c.pdg_tmp_bytes = 0;
   if (c.poly_tmp) cudaFree(c.poly_tmp);
   c.poly_tmp = nullptr; c.poly_tmp_bytes = 0;
   if (c.xsec_scratch) cudaFree(c.xsec_scratch);

@@ -50,7 +50,9 @@ struct Context {
   cudaGraphExec_t run_exec = nullptr; int64_t exec_launches = 0;
   cudaStream_t cap_stream = nullptr;
   DevPlan* plan = nullptr;           // device
-  void* plan_keys = nullptr;         // device: key and leg count of every compiled-in subprocess
+  void* plan_keys = nullptr;         // device: key, leg count [2 NSUB] and process string [NSUB][8] of every compiled-in subprocess
+  const int8_t* legmap = nullptr;    // trex_run_pdg: per-event leg order (device [npar][n]); forces the transposition
+  void* pdg_tmp = nullptr; size_t pdg_tmp_bytes = 0;   // trex_run_pdg: keys + leg maps
   // colour matrices on the device
   bool colour_ready = false;
   double* C120 = nullptr;            // 120 x 120, global memory
@@ -64,6 +66,7 @@ Context& ctx();
 // if sub_keys != nullptr), then fetch sizes and keys -- the only point where the host waits for the device
 int bucket_reserve(int64_t n);          // (re)allocates the scratch of bucket_enqueue; never called while capturing
 int bucket_enqueue(const uint64_t* keys, int64_t n, int32_t* perm, int npar);
+int ensure_plan();                      // uploads the subprocess registry the device plan and rex_keys need (trex_api.cu)
 int bucket_finish(int64_t* offsets);
 // transposition kernels of trex_run driven by the device plan (both are no-ops for a single-class sample)
 int run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* perm, double* blk, double* res);

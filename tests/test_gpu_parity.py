@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as O
-from trex_inputs import make_config, default_theta, SUBPROCESSES, REX_NPOS, TH_CTG, TH_GAMMAT, TH_ALPHA_S
+from trex_inputs import make_config, default_theta, SUBPROCESSES, REX_NPOS, TH_CTG, TH_GAMMAT, TH_ALPHA_S, shuffled_legs
 
 pytestmark = pytest.mark.gpu
 
@@ -401,3 +401,42 @@ def test_run_multi_polynomial_path(T, cfg, n):
     for k in (0, 1, 5):
         rw, ro, rn = O.reweight(sp.sid, mom, tho, thetas[k], w.w_in[idx])
         assert rel(wp[k].cpu().numpy()[idx], rw).max() < RTOL64 and rel(mnp[k].cpu().numpy()[idx], rn).max() < RTOL64
+
+
+# ---------------------------------------------------------------- PDG codes in arbitrary parton order (NEXT-3)
+def test_rex_keys_and_legmap_bit_exact(T):
+    import torch
+    w = make_config(3, n=30017)
+    pdg, mom, n_in = shuffled_legs(w, 9, unknown_every=41)
+    pdg[2, 5] = 1000022                                                  # a code the key cannot hold -> REX_NPOS
+    keys, lm = T.rex_keys(torch.from_numpy(pdg).cuda(), n_in)
+    rk, rl = O.keys_and_legmap(pdg, n_in, [sp.pdg for sp in SUBPROCESSES])
+    assert np.array_equal(keys.cpu().numpy().view(np.uint64), rk) and np.array_equal(lm.cpu().numpy(), rl)
+    assert rk[5] == np.uint64(REX_NPOS)
+
+
+@pytest.mark.parametrize("cfg,n", [(3, 20011), (4, 700), (2, 3000)])
+def test_run_pdg_reindexes_partons(T, cfg, n):
+    """events whose partons come in another order than the process string are re-indexed inside the
+    transposition; weights equal the oracle's on the re-indexed momenta, unknown classes get zero."""
+    import torch
+    w = make_config(cfg, n=n)
+    pdg, mom, n_in = shuffled_legs(w, 100 + cfg, unknown_every=53)
+    wo, mo, mn, nb = T.trex_run_pdg(torch.from_numpy(pdg).cuda(), dev(mom), n_in, w.theta_old, w.theta_new, dev(w.w_in))
+    torch.cuda.synchronize()
+    wo, mo, mn = wo.cpu().numpy(), mo.cpu().numpy(), mn.cpu().numpy()
+    rk, rl = O.keys_and_legmap(pdg, n_in, [sp.pdg for sp in SUBPROCESSES])
+    unknown = np.ones(w.n, dtype=bool)
+    for sp in w.classes:
+        sel = np.where(rk == sp.key)[0]
+        unknown[sel] = False
+        idx = sel[:: max(1, len(sel) // 8)][:8]
+        canon = np.ascontiguousarray(mom[rl[:, idx], :, idx].transpose(0, 2, 1))
+        rw, ro, rn = O.reweight(sp.sid, canon, w.theta_old, w.theta_new, w.w_in[idx])
+        assert rel(wo[idx], rw).max() < RTOL64 and rel(mo[idx], ro).max() < RTOL64 and rel(mn[idx], rn).max() < RTOL64, sp.name
+    assert unknown.sum() > 0 and np.all(wo[unknown] == 0) and np.all(mo[unknown] == 0) and np.all(wo[~unknown] > 0)
+    assert nb == len(np.unique(rk))
+    # against the canonical sample through trex_run: the same physics, identical up to the order of identical gluons
+    w0, _, _, _ = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    w0 = w0.cpu().numpy()
+    assert rel(wo[~unknown], w0[~unknown]).max() < 1e-12
