@@ -94,7 +94,9 @@ template <class R, class RC, int N> struct TabGeom {
   static constexpr size_t o_spin = o_eps + al(sizeof(double) * 16 * N);
   static constexpr size_t o_part = o_spin + al(sizeof(double) * 8 * 4);
   static constexpr size_t o_utab = o_part + al(sizeof(double) * NCI);
-  static constexpr size_t slot = o_utab + (UT ? al(sizeof(R) * 16 * NUT) : 0);
+  static constexpr size_t o_pm = o_utab + (UT ? al(sizeof(R) * 16 * NUT) : 0);
+  static constexpr int NROW = 4 * (N + 2);                   // momentum rows of one event
+  static constexpr size_t slot = o_pm + al(sizeof(double) * NROW);
   static constexpr size_t o_c = slot * EPB;
   static constexpr size_t o_meta = o_c + al(sizeof(RC) * FoldedC<NC>::size());
   static constexpr size_t bytes = o_meta + al(sizeof(int) * I::M_SIZE);
@@ -197,6 +199,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
   double* eps_all = reinterpret_cast<double*>(sb + G::o_eps);
   double* spin = reinterpret_cast<double*>(sb + G::o_spin);
   double* part = reinterpret_cast<double*>(sb + G::o_part);
+  double* pm = reinterpret_cast<double*>(sb + G::o_pm);
 
   const EvIO io = resolve_io(a);
   for (int i = tid; i < I::M_SIZE; i += TB) meta[i] = gmeta[i];
@@ -210,10 +213,17 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
 #else
 #define PHASE_TICK(k) do { } while (0)
 #endif
-  for (long e = (long)blockIdx.x * EPB + sl; e < io.n; e += (long)gridDim.x * EPB) {
+  // the momenta of the group's NEXT event are loaded (one row per thread) while the current one is worked on: the DRAM
+  // latency of the only global read of the kernel is paid once per block, not once per event
+  const long e_first = (long)blockIdx.x * EPB + sl, e_step = (long)gridDim.x * EPB;
+  double nxt = (gtid < G::NROW && e_first < io.n) ? io.mom[(long)gtid * io.ld + e_first] : 0.0;
+  for (long e = e_first; e < io.n; e += e_step) {
 #ifdef TREX_PHASE_CLOCKS
     if (tid == 0) t0 = clock64();
 #endif
+    if (gtid < G::NROW) pm[gtid] = nxt;
+    group_sync<GS>();
+    if (gtid < G::NROW && e + e_step < io.n) nxt = io.mom[(long)gtid * io.ld + e + e_step];
     // ---- per-event set-up: momentum of every gluon subset (incoming convention), polarisation vectors, t / t~ spinors
     // (subset momenta and wavefunctions are independent: different lanes, one pass, one latency)
     for (int item = gtid; item < G::NSUB + 2 * N + 4; item += GS) {
@@ -227,7 +237,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
         const int leg = g < 2 ? g : g + 2;
         const double sg = g < 2 ? 1.0 : -1.0;
 #pragma unroll
-        for (int mu = 0; mu < 4; ++mu) P.c[mu] += sg * io.mom[(long)(leg * 4 + mu) * io.ld + e];
+        for (int mu = 0; mu < 4; ++mu) P.c[mu] += sg * pm[leg * 4 + mu];
       }
       pset[sset] = P;
      } else {
@@ -235,13 +245,13 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
       double p[4];
       if (it < 2 * N) {
         const int g = it >> 1, leg = g < 2 ? g : g + 2;
-        load_leg<double>(io.mom, io.ld, e, leg, p);
+        for (int mu = 0; mu < 4; ++mu) p[mu] = pm[leg * 4 + mu];
         const vec4<double> ev = polvec<double>(p, (it & 1) ? 1 : -1, g >= 2);
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) { eps_all[it * 8 + 2 * mu] = ev.c[mu].re; eps_all[it * 8 + 2 * mu + 1] = ev.c[mu].im; }
       } else {
         const int k = it - 2 * N;                          // 0, 1: ubar(p_t, -/+); 2, 3: v(p_tbar, -/+)
-        load_leg<double>(io.mom, io.ld, e, k < 2 ? 2 : 3, p);
+        for (int mu = 0; mu < 4; ++mu) p[mu] = pm[(k < 2 ? 2 : 3) * 4 + mu];
         const spinor<double> sp = k < 2 ? bar(spinor_u<double>(p, (k & 1) ? 1 : -1, false)) : spinor_v<double>(p, (k & 1) ? 1 : -1, false);
 #pragma unroll
         for (int i = 0; i < 4; ++i) { spin[k * 8 + 2 * i] = sp.c[i].re; spin[k * 8 + 2 * i + 1] = sp.c[i].im; }
@@ -253,7 +263,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
 
     rvec4<double> ptop;
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) ptop.c[mu] = io.mom[(long)(2 * 4 + mu) * io.ld + e];
+    for (int mu = 0; mu < 4; ++mu) ptop.c[mu] = pm[2 * 4 + mu];
     for (unsigned itb = 0; itb < (unsigned)G::NIT; ++itb) {
       // ---- phase 1: current table of this helicity iteration (+ line states of short prefixes, if tabulated)
       for (int e1 = gtid; e1 < meta[I::M_LVL + 2]; e1 += GS) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
