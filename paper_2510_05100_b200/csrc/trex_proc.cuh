@@ -282,26 +282,36 @@ TREX_HD void eemumu_event(const double* __restrict__ mom, long n, long e, const 
     propA[th] = R(T.e2[th] / s);
     propZ[th] = cast<R>(cdiv(cx<double>(1, 0), cx<double>(s - T.mZ2[th], T.mZGZ[th])));
   }
+  // the eight external wavefunctions once (not once per helicity combination)
+  spinor<R> u1[2], vb2[2], ub3[2], v4[2];
+#pragma unroll
+  for (int l = 0; l < 2; ++l) {
+    const int lam = l ? 1 : -1;
+    u1[l] = cast<R>(spinor_u<double>(p0, lam, true));
+    vb2[l] = cast<R>(bar(spinor_v<double>(p1, lam, true)));
+    ub3[l] = cast<R>(bar(spinor_u<double>(p2, lam, true)));
+    v4[l] = cast<R>(spinor_v<double>(p3, lam, true));
+  }
   R sum[2] = {R(0), R(0)};
-  for (int h = 0; h < 16; ++h) {
-    spinor<R> u1 = cast<R>(spinor_u<double>(p0, (h & 1) ? 1 : -1, true));
-    spinor<R> vb2 = cast<R>(bar(spinor_v<double>(p1, (h & 2) ? 1 : -1, true)));
-    spinor<R> ub3 = cast<R>(bar(spinor_u<double>(p2, (h & 4) ? 1 : -1, true)));
-    spinor<R> v4 = cast<R>(spinor_v<double>(p3, (h & 8) ? 1 : -1, true));
-    // P_L keeps the upper two components in the chiral basis, P_R the lower two
-    spinor<R> uL = u1, uR = u1, vL = v4, vR = v4;
-    uL.c[2] = uL.c[3] = cx<R>(0, 0); uR.c[0] = uR.c[1] = cx<R>(0, 0);
-    vL.c[2] = vL.c[3] = cx<R>(0, 0); vR.c[0] = vR.c[1] = cx<R>(0, 0);
-    vec4<R> Je[2] = {bilinear(vb2, uL), bilinear(vb2, uR)};
-    vec4<R> Jm[2] = {bilinear(ub3, vL), bilinear(ub3, vR)};
-    cx<R> d[2][2];
-    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) d[a][b] = dot(Je[a], Jm[b]);
-    for (int th = 0; th < 2; ++th) {
-      const R g[2] = {R(T.gL[th]), R(T.gR[th])};
-      cx<R> za(0, 0), ga(0, 0);
-      for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) { ga += d[a][b]; cfma(za, d[a][b], g[a] * g[b]); }
-      cx<R> M = ga * propA[th] + za * propZ[th];
-      sum[th] += norm2(M);
+  // Massless lines: a spinor has one non-zero chiral 2-block (u(+), v(-): lower; u(-), v(+): upper; the bar swaps them)
+  // and gamma^mu couples upper to lower, so vbar(l2) gamma^mu u(l1) vanishes EXACTLY unless l1 = -l2 (and likewise the
+  // muon current): 4 of the 16 helicity combinations contribute, each with ONE chirality (a = L or R) per current.
+#pragma unroll
+  for (int he = 0; he < 2; ++he) {
+#pragma unroll
+    for (int hm = 0; hm < 2; ++hm) {
+      // electron line: u(l1) with vbar(-l1); muon line: ubar(l3) with v(-l3); chirality index 0 = L (upper block of the
+      // column spinor), 1 = R
+      const spinor<R>& ue = u1[he]; const spinor<R>& ve = vb2[1 - he];
+      const spinor<R>& um = ub3[hm]; const spinor<R>& vm = v4[1 - hm];
+      const int a = he, b = hm;                            // u(-): upper block = L; the partner of ubar(-) is v(+): upper block = L
+      const cx<R> d = dot(bilinear(ve, ue), bilinear(um, vm));
+#pragma unroll
+      for (int th = 0; th < 2; ++th) {
+        const R g[2] = {R(T.gL[th]), R(T.gR[th])};
+        const cx<R> M = d * propA[th] + (d * (g[a] * g[b])) * propZ[th];
+        sum[th] += norm2(M);
+      }
     }
   }
   out[0] = sum[0]; out[1] = sum[1];
