@@ -75,13 +75,21 @@ template <class R> TREX_HD ften<R> fzero() { ften<R> f; for (int i = 0; i < 3; +
 
 // ---------------------------------------------------------------- external wavefunctions (R-1, R-2)
 // chi_+ = N (|p|+pz, px + i py), chi_- = N (-px + i py, |p|+pz), N = 1/sqrt(2|p|(|p|+pz)); pz -> -|p|: chi_+ = (0,1), chi_- = (-1,0)
+// 1/sqrt(x): one special-function evaluation + Newton steps on the device, instead of a square root followed by a division
+template <class R> TREX_HD R inv_sqrt(R x) {
+#if defined(__CUDA_ARCH__)
+  return rsqrt(x);
+#else
+  return R(1) / sqrt(x);
+#endif
+}
 template <class R> TREX_HD void two_spinors(const R p[4], cx<R> plus[2], cx<R> minus[2], R& pabs) {
-  R pt2 = p[1] * p[1] + p[2] * p[2];
-  pabs = sqrt(pt2 + p[3] * p[3]);
+  const R pt2 = p[1] * p[1] + p[2] * p[2], p2 = pt2 + p[3] * p[3];
+  if (p2 == R(0)) { pabs = R(0); plus[0] = cx<R>(1, 0); plus[1] = cx<R>(0, 0); minus[0] = cx<R>(0, 0); minus[1] = cx<R>(1, 0); return; }
+  pabs = p2 * inv_sqrt(p2);
   R ppz = p[3] >= R(0) ? pabs + p[3] : pt2 / (pabs - p[3]);     // |p|+pz without cancellation
-  if (pabs == R(0)) { plus[0] = cx<R>(1, 0); plus[1] = cx<R>(0, 0); minus[0] = cx<R>(0, 0); minus[1] = cx<R>(1, 0); return; }
   if (ppz == R(0)) { plus[0] = cx<R>(0, 0); plus[1] = cx<R>(1, 0); minus[0] = cx<R>(-1, 0); minus[1] = cx<R>(0, 0); return; }
-  R N = R(1) / sqrt(R(2) * pabs * ppz);
+  R N = inv_sqrt(R(2) * pabs * ppz);
   plus[0] = cx<R>(N * ppz, 0); plus[1] = cx<R>(N * p[1], N * p[2]);
   minus[0] = cx<R>(-N * p[1], N * p[2]); minus[1] = cx<R>(N * ppz, 0);
 }
@@ -108,16 +116,17 @@ template <class R> TREX_HD spinor<R> bar(const spinor<R>& s) {
   spinor<R> o; o.c[0] = conj(s.c[2]); o.c[1] = conj(s.c[3]); o.c[2] = conj(s.c[0]); o.c[3] = conj(s.c[1]); return o; }
 // eps(p,l) = (-l e1 - i e2)/sqrt2, e1 = (0, px pz/(|p| pT), py pz/(|p| pT), -pT/|p|), e2 = (0, -py/pT, px/pT, 0)
 template <class R> TREX_HD vec4<R> polvec(const R p[4], int lam, bool conjugate) {
-  R pt = sqrt(p[1] * p[1] + p[2] * p[2]);
-  R pabs = sqrt(pt * pt + p[3] * p[3]);
+  const R pt2 = p[1] * p[1] + p[2] * p[2], p2 = pt2 + p[3] * p[3];
   R e1[4], e2[4];
-  if (pt < R(1e-14) * pabs || pt == R(0)) {
+  if (pt2 < R(1e-28) * p2 || pt2 == R(0)) {
     R sg = p[3] >= 0 ? R(1) : R(-1);
     e1[0] = 0; e1[1] = 1; e1[2] = 0; e1[3] = 0;
     e2[0] = 0; e2[1] = 0; e2[2] = sg; e2[3] = 0;
   } else {
-    R ipp = R(1) / (pabs * pt), ipt = R(1) / pt;
-    e1[0] = 0; e1[1] = p[1] * p[3] * ipp; e1[2] = p[2] * p[3] * ipp; e1[3] = -pt / pabs;
+    // two independent reciprocal square roots instead of two square roots and three divisions
+    const R ipt = inv_sqrt(pt2), ip = inv_sqrt(p2);
+    const R ipp = ipt * ip, pt = pt2 * ipt;
+    e1[0] = 0; e1[1] = p[1] * p[3] * ipp; e1[2] = p[2] * p[3] * ipp; e1[3] = -pt * ip;
     e2[0] = 0; e2[1] = -p[2] * ipt; e2[2] = p[1] * ipt; e2[3] = 0;
   }
   const R rs2 = R(0.70710678118654752440);
