@@ -440,3 +440,28 @@ def test_run_pdg_reindexes_partons(T, cfg, n):
     w0, _, _, _ = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
     w0 = w0.cpu().numpy()
     assert rel(wo[~unknown], w0[~unknown]).max() < 1e-12
+
+
+@pytest.mark.parametrize("n", [1, 2, 31, 33, 100, 8191, 8192, 8193, 70001])
+def test_run_sizes_around_every_threshold(T, n):
+    """trex_run against one trex_reweight per class on the gathered block: sizes around the warp, the single-block
+    bucketing (8192) and the graph-replay thresholds; the second identical call replays the captured graph."""
+    import torch
+    w = make_config(3, n=max(n, 64))
+    keys, mom, win = w.keys[:n].copy(), np.ascontiguousarray(w.momenta[:, :, :n]), w.w_in[:n]
+    if n > 40:
+        keys[7::29] = np.uint64(REX_NPOS)
+    dk, dm, dw = dev(keys), dev(mom), dev(win)
+    outs = [T.trex_run(dk, dm, w.theta_old, w.theta_new, dw) for _ in range(3)]
+    torch.cuda.synchronize()
+    wo, mo, mn, nb = outs[0]
+    for o in outs[1:]:
+        assert torch.equal(o[0], wo) and torch.equal(o[2], mn) and o[3] == nb
+    wo = wo.cpu().numpy()
+    ref = np.zeros(n)
+    for sp in w.classes:
+        sel = np.where(keys == sp.key)[0]
+        if len(sel):
+            r, _, _ = gpu_reweight(T, sp.sid, np.ascontiguousarray(mom[:, :, sel]), w.theta_old, w.theta_new, win[sel])
+            ref[sel] = r
+    assert np.array_equal(wo, ref)
