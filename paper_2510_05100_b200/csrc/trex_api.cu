@@ -15,26 +15,154 @@ Context& ctx() { static Context c; return c; }
 
 namespace {
 
+#ifndef TREX_QQ_MINB
+#define TREX_QQ_MINB 1
+#endif
+
+// One light-quark line + t t~ + gluon (q q~ -> t t~ g and crossings; trex_proc.cuh). A block is 32 consecutive events x
+// 8 warps. Helicity selection on the massless light line: in the chiral basis a massless spinor has one non-zero
+// 2-block (u(+), v(-): lower; u(-), v(+): upper; the bar swaps them) and gamma^mu couples upper to lower, so the
+// light-line currents vanish EXACTLY unless row and column sit in different blocks: 2 light-line combinations c, hence
+// 8 of the 16 helicity units (c, lambda_g, lambda_t), one per warp.
+//   phase A : the 10 external wavefunctions of the event (row / column spinor of the light line for c = 0, 1; gluon
+//             polarisation -/+; ubar(t) -/+; v(t~) -/+), one per warp (warps 0, 1 take two), parked in shared memory
+//   phase A2: the 10 light-line currents (Jq[c]; Jq3[c][lambda_g], Jq4[c][lambda_g]: the line after radiating the gluon at
+//             its row / column end), one per warp
+//   phase B : warp = unit: top line (qq_close) with operands read back (lane = event: conflict-free)
 template <class R, class RC>
-__global__ void __launch_bounds__(WARPS * 32) k_qq(const ReweightArgs a) {
+__global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightArgs a) {
+  static_assert(WARPS == 8, "one allowed helicity unit per warp");
+  __shared__ double pm[20][32];
+  __shared__ double wf[10][8][32];
+  __shared__ double cur[10][8][32];
   const EvIO io = resolve_io(a);
   if ((long)blockIdx.x * 32 >= io.n) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long e = (long)blockIdx.x * 32 + lane;
   const long ev = e < io.n ? e : io.n - 1;
-  // Helicity selection on the massless light line: in the chiral basis a massless spinor has one non-zero 2-block
-  // (u(+), v(-): lower; u(-), v(+): upper; the bar swaps them) and gamma^mu couples upper to lower, so the light-line
-  // currents vanish EXACTLY unless row and column sit in different blocks. Only those 8 of the 16 units are evaluated,
-  // one per warp: warp = (gluon helicity, top helicity, which of the two allowed light-line combinations).
-  static_assert(WARPS == 8, "one allowed helicity unit per warp");
-  const bool row_in = a.q.lrow < 2, col_in = a.q.lcol < 2;
-  const bool row_upper = (warp >> 2) & 1, col_upper = !row_upper;
-  const int lam_row = (row_in ? !row_upper : row_upper) ? 1 : -1;     // vbar(+): lower, ubar(+): upper
-  const int lam_col = (col_in ? !col_upper : col_upper) ? 1 : -1;     // u(+): lower, v(+): upper
-  const int u = (lam_row > 0 ? 1 : 0) | (lam_col > 0 ? 2 : 0) | ((warp & 1) << 2) | (((warp >> 1) & 1) << 3);
+  for (int r = warp; r < 20; r += WARPS) pm[r][lane] = io.mom[(long)r * io.ld + ev];
+  __syncthreads();
+  const QLineLegs L = a.q;
+  const bool row_in = L.lrow < 2, col_in = L.lcol < 2, g_in = L.lg < 2;
+  auto leg = [&](int l, double p[4]) {
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) p[mu] = pm[l * 4 + mu][lane];
+  };
+  auto put4 = [&](double (*dst)[32], const cx<double>* c4) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { dst[2 * i][lane] = c4[i].re; dst[2 * i + 1][lane] = c4[i].im; }
+  };
+  auto get_spinor = [&](double (*src)[32]) {
+    spinor<R> o;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) o.c[i] = cx<R>(R(src[2 * i][lane]), R(src[2 * i + 1][lane]));
+    return o;
+  };
+  auto get_vec = [&](double (*src)[32]) {
+    vec4<R> o;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) o.c[i] = cx<R>(R(src[2 * i][lane]), R(src[2 * i + 1][lane]));
+    return o;
+  };
+  // ---- phase A
+  for (int item = warp; item < 10; item += WARPS) {
+    double p[4];
+    if (item < 4) {
+      const int c = item & 1;                               // row spinor sits in the upper block for c = 1
+      const bool row_upper = c != 0, col_upper = !row_upper;
+      if (item < 2) {
+        leg(L.lrow, p);
+        const int lam = (row_in ? !row_upper : row_upper) ? 1 : -1;     // vbar(+): lower, ubar(+): upper
+        const spinor<double> w = row_in ? bar(spinor_v<double>(p, lam, true)) : bar(spinor_u<double>(p, lam, true));
+        put4(wf[item], w.c);
+      } else {
+        leg(L.lcol, p);
+        const int lam = (col_in ? !col_upper : col_upper) ? 1 : -1;     // u(+): lower, v(+): upper
+        const spinor<double> x = col_in ? spinor_u<double>(p, lam, true) : spinor_v<double>(p, lam, true);
+        put4(wf[item], x.c);
+      }
+    } else if (item < 6) {
+      leg(L.lg, p);
+      const vec4<double> eg = polvec<double>(p, (item & 1) ? 1 : -1, !g_in);
+      put4(wf[item], eg.c);
+    } else {
+      leg(item < 8 ? 2 : 3, p);
+      const int lam = (item & 1) ? 1 : -1;
+      const spinor<double> sp = item < 8 ? bar(spinor_u<double>(p, lam, false)) : spinor_v<double>(p, lam, false);
+      put4(wf[item], sp.c);
+    }
+  }
+  __syncthreads();
+  rvec4<double> Kr, Kc, Kg, Kq, Ptot, pt;
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) {
+    const double pr = pm[L.lrow * 4 + mu][lane], pc = pm[L.lcol * 4 + mu][lane], pg = pm[L.lg * 4 + mu][lane];
+    Kr.c[mu] = row_in ? pr : -pr; Kc.c[mu] = col_in ? pc : -pc; Kg.c[mu] = g_in ? pg : -pg;
+    Kq.c[mu] = Kr.c[mu] + Kc.c[mu];
+    pt.c[mu] = pm[8 + mu][lane];
+  }
+  Ptot = radd(Kq, Kg);
+  // ---- phase A2
+  for (int item = warp; item < 10; item += WARPS) {
+    vec4<R> J;
+    if (item < 2) {
+      // quark-pair current  Jq = (w gamma^mu x) / Kq^2        [ (i g_s) * (-i / Kq^2) at g_s = 1 ]
+      J = bilinear(get_spinor(wf[item]), get_spinor(wf[2 + item]));
+      const R sc = R(1.0 / rdot(Kq, Kq));
+#pragma unroll
+      for (int i = 0; i < 4; ++i) J.c[i] = J.c[i] * sc;
+    } else {
+      const int k = item - 2, c = (k >> 1) & 1, lg = k & 1, col_end = k >> 2;
+      const spinor<R> w = get_spinor(wf[c]), x = get_spinor(wf[2 + c]);
+      const vec4<R> eg = get_vec(wf[4 + lg]);
+      const double iP2 = 1.0 / rdot(Ptot, Ptot);
+      if (!col_end) {
+        // W = w (i eslash)(i qslash)/q^2, q = -(Kr + Kg)
+        rvec4<double> q;
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) q.c[mu] = -(Kr.c[mu] + Kg.c[mu]);
+        const spinor<R> W = row_slash(row_slash(w, eg), cast<R>(q));
+        const R sc = R(-iP2 / rdot(q, q));
+        J = bilinear(W, x);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) J.c[i] = J.c[i] * sc;
+      } else {
+        // X = (i qslash)(i eslash) x / q^2, q = Kc + Kg
+        const rvec4<double> q = radd(Kc, Kg);
+        const spinor<R> X = slash_col(cast<R>(q), slash_col(eg, x));
+        const R sc = R(-iP2 / rdot(q, q));
+        J = bilinear(w, X);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) J.c[i] = J.c[i] * sc;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { cur[item][2 * i][lane] = (double)J.c[i].re; cur[item][2 * i + 1][lane] = (double)J.c[i].im; }
+  }
+  __syncthreads();
+  // ---- phase B: unit = (lambda_g, lambda_t, light-line combination)
+  const int lg = warp & 1, lt = (warp >> 1) & 1, c = (warp >> 2) & 1;
   RC acc[2];
-  qq_unit<R, RC>(io.mom, io.ld, ev, a.q, u, a.T, acc);
-  reduce_and_finish<RC>(a, io, acc[0], acc[1], e);
+  {
+    const vec4<R> eg = get_vec(wf[4 + lg]), Jq = get_vec(cur[c]), Jq3 = get_vec(cur[2 + c * 2 + lg]), Jq4 = get_vec(cur[6 + c * 2 + lg]);
+    const spinor<R> ubar_t = get_spinor(wf[6 + lt]);
+    const spinor<R> vtb[2] = {get_spinor(wf[8]), get_spinor(wf[9])};
+    qq_close<R, RC>(eg, Kg, Jq, Kq, Jq3, Jq4, Ptot, ubar_t, vtb, pt, a.T, acc);
+  }
+  // fixed-order reduction over the 8 units (the light row spinors of phase A are dead: their slots carry the partial sums)
+  double (*red)[8][32] = reinterpret_cast<double (*)[8][32]>(&wf[0][0][0]);
+  red[0][warp][lane] = (double)acc[0]; red[1][warp][lane] = (double)acc[1];
+  __syncthreads();
+  if (warp == 0 && e < io.n) {
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
+    const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
+    const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
+    io.w_out[e] = io.w_in[e] * norm * mn;                      // evaluate + append_wgts
+    if (io.me2_old) io.me2_old[e] = mo;
+    if (io.me2_new) io.me2_new[e] = mn;
+  }
 }
 
 template <class R>

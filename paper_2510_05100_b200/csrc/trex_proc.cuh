@@ -176,54 +176,19 @@ template <class R> struct QqLeafStore {
   }
 };
 
-// unit = (lam_row, lam_col, lam_g, lam_t) packed in 4 bits of `u` (bit0 row, bit1 col, bit2 gluon, bit3 top)
+// top line of the quark channels, given the gluon polarisation, the quark-pair current Jq and the two currents Jq3 / Jq4
+// of the light line that has radiated the gluon: two-source ordered amplitudes + single-source amplitudes -> four colour
+// flows -> J^dagger C J for theta_old and theta_new, both antitop helicities (see the comment block above)
 template <class R, class RC>
-TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L, int u, const ThetaPair& T, RC out[2]) {
-  const int lam_row = (u & 1) ? 1 : -1, lam_col = (u & 2) ? 1 : -1, lam_g = (u & 4) ? 1 : -1, lam_t = (u & 8) ? 1 : -1;
-  double pr[4], pc[4], pg[4], pt[4], ptb[4];
-  load_leg<double>(mom, n, e, L.lrow, pr); load_leg<double>(mom, n, e, L.lcol, pc); load_leg<double>(mom, n, e, L.lg, pg);
-  load_leg<double>(mom, n, e, 2, pt); load_leg<double>(mom, n, e, 3, ptb);
-  const bool row_in = L.lrow < 2, col_in = L.lcol < 2, g_in = L.lg < 2;
-  // light line ends: row = vbar (incoming antiquark) or ubar (outgoing quark); column = u (incoming) or v (outgoing)
-  spinor<R> w = cast<R>(row_in ? bar(spinor_v<double>(pr, lam_row, true)) : bar(spinor_u<double>(pr, lam_row, true)));
-  spinor<R> x = cast<R>(col_in ? spinor_u<double>(pc, lam_col, true) : spinor_v<double>(pc, lam_col, true));
-  rvec4<double> Kr, Kc, Kg, Kq;
-#pragma unroll
-  for (int mu = 0; mu < 4; ++mu) {
-    Kr.c[mu] = row_in ? pr[mu] : -pr[mu]; Kc.c[mu] = col_in ? pc[mu] : -pc[mu]; Kg.c[mu] = g_in ? pg[mu] : -pg[mu];
-    Kq.c[mu] = Kr.c[mu] + Kc.c[mu];
-  }
-  vec4<R> eg = cast<R>(polvec<double>(pg, lam_g, !g_in));
-  // quark-pair current  Jq = (w gamma^mu x) / Kq^2        [ (i g_s) * (-i / Kq^2) at g_s = 1 ]
-  vec4<R> Jq = bilinear(w, x);
-  { R s = R(1.0 / rdot(Kq, Kq));
-#pragma unroll
-    for (int i = 0; i < 4; ++i) Jq.c[i] = Jq.c[i] * s; }
-  // light line after radiating the gluon: W = w (i eslash)(i qslash)/q^2, q = -(Kr + Kg);  X = (i qslash)(i eslash) x / q^2, q = Kc + Kg
-  rvec4<double> Ptot = radd(Kq, Kg);
-  const double iP2 = 1.0 / rdot(Ptot, Ptot);
-  vec4<R> Jq3, Jq4;
-  { rvec4<double> q; for (int mu = 0; mu < 4; ++mu) q.c[mu] = -(Kr.c[mu] + Kg.c[mu]);
-    spinor<R> W = row_slash(row_slash(w, eg), cast<R>(q));
-    R s = R(-iP2 / rdot(q, q));
-    Jq3 = bilinear(W, x);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) Jq3.c[i] = Jq3.c[i] * s; }
-  { rvec4<double> q = radd(Kc, Kg);
-    spinor<R> X = slash_col(cast<R>(q), slash_col(eg, x));
-    R s = R(-iP2 / rdot(q, q));
-    Jq4 = bilinear(w, X);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) Jq4.c[i] = Jq4.c[i] * s; }
-
+TREX_HD void qq_close(const vec4<R>& eg, const rvec4<double>& Kg, const vec4<R>& Jq, const rvec4<double>& Kq, const vec4<R>& Jq3,
+                      const vec4<R>& Jq4, const rvec4<double>& Ptot, const spinor<R>& ubar_t, const spinor<R> vtb[2],
+                      const rvec4<double>& pt, const ThetaPair& T, RC out[2]) {
   QqLeafStore<R> st;
-  st.v[0] = cast<R>(spinor_v<double>(ptb, -1, false)); st.v[1] = cast<R>(spinor_v<double>(ptb, +1, false));
-  spinor<R> ubar_t = cast<R>(bar(spinor_u<double>(pt, lam_t, false)));
+  st.v[0] = vtb[0]; st.v[1] = vtb[1];
   // two-source ordered amplitudes: source 0 = gluon, source 1 = quark-pair current
   TTNGS<R, 2, 1, QqLeafStore<R>> t;
   t.K[0] = Kg; t.eps[0] = eg; t.K[1] = Kq; t.eps[1] = Jq;
-#pragma unroll
-  for (int mu = 0; mu < 4; ++mu) t.pt.c[mu] = pt[mu];
+  t.pt = pt;
   t.ubar_t = ubar_t;
   // top mass/width may differ between theta_old and theta_new: evaluate per theta when they do
   RC res[2];
@@ -265,6 +230,54 @@ TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L
     res[th] = s;
   }
   out[0] = res[0]; out[1] = res[1];
+}
+
+// unit = (lam_row, lam_col, lam_g, lam_t) packed in 4 bits of `u` (bit0 row, bit1 col, bit2 gluon, bit3 top)
+template <class R, class RC>
+TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L, int u, const ThetaPair& T, RC out[2]) {
+  const int lam_row = (u & 1) ? 1 : -1, lam_col = (u & 2) ? 1 : -1, lam_g = (u & 4) ? 1 : -1, lam_t = (u & 8) ? 1 : -1;
+  double pr[4], pc[4], pg[4], pt[4], ptb[4];
+  load_leg<double>(mom, n, e, L.lrow, pr); load_leg<double>(mom, n, e, L.lcol, pc); load_leg<double>(mom, n, e, L.lg, pg);
+  load_leg<double>(mom, n, e, 2, pt); load_leg<double>(mom, n, e, 3, ptb);
+  const bool row_in = L.lrow < 2, col_in = L.lcol < 2, g_in = L.lg < 2;
+  // light line ends: row = vbar (incoming antiquark) or ubar (outgoing quark); column = u (incoming) or v (outgoing)
+  spinor<R> w = cast<R>(row_in ? bar(spinor_v<double>(pr, lam_row, true)) : bar(spinor_u<double>(pr, lam_row, true)));
+  spinor<R> x = cast<R>(col_in ? spinor_u<double>(pc, lam_col, true) : spinor_v<double>(pc, lam_col, true));
+  rvec4<double> Kr, Kc, Kg, Kq;
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) {
+    Kr.c[mu] = row_in ? pr[mu] : -pr[mu]; Kc.c[mu] = col_in ? pc[mu] : -pc[mu]; Kg.c[mu] = g_in ? pg[mu] : -pg[mu];
+    Kq.c[mu] = Kr.c[mu] + Kc.c[mu];
+  }
+  vec4<R> eg = cast<R>(polvec<double>(pg, lam_g, !g_in));
+  // quark-pair current  Jq = (w gamma^mu x) / Kq^2        [ (i g_s) * (-i / Kq^2) at g_s = 1 ]
+  vec4<R> Jq = bilinear(w, x);
+  { R s = R(1.0 / rdot(Kq, Kq));
+#pragma unroll
+    for (int i = 0; i < 4; ++i) Jq.c[i] = Jq.c[i] * s; }
+  // light line after radiating the gluon: W = w (i eslash)(i qslash)/q^2, q = -(Kr + Kg);  X = (i qslash)(i eslash) x / q^2, q = Kc + Kg
+  rvec4<double> Ptot = radd(Kq, Kg);
+  const double iP2 = 1.0 / rdot(Ptot, Ptot);
+  vec4<R> Jq3, Jq4;
+  { rvec4<double> q; for (int mu = 0; mu < 4; ++mu) q.c[mu] = -(Kr.c[mu] + Kg.c[mu]);
+    spinor<R> W = row_slash(row_slash(w, eg), cast<R>(q));
+    R s = R(-iP2 / rdot(q, q));
+    Jq3 = bilinear(W, x);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) Jq3.c[i] = Jq3.c[i] * s; }
+  { rvec4<double> q = radd(Kc, Kg);
+    spinor<R> X = slash_col(cast<R>(q), slash_col(eg, x));
+    R s = R(-iP2 / rdot(q, q));
+    Jq4 = bilinear(w, X);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) Jq4.c[i] = Jq4.c[i] * s; }
+
+  spinor<R> vtb[2] = {cast<R>(spinor_v<double>(ptb, -1, false)), cast<R>(spinor_v<double>(ptb, +1, false))};
+  spinor<R> ubar_t = cast<R>(bar(spinor_u<double>(pt, lam_t, false)));
+  rvec4<double> ptv;
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) ptv.c[mu] = pt[mu];
+  qq_close<R, RC>(eg, Kg, Jq, Kq, Jq3, Jq4, Ptot, ubar_t, vtb, ptv, T, out);
 }
 
 // ---------------------------------------------------------------- e- e+ -> mu- mu+ (photon + Z), all 16 helicities
