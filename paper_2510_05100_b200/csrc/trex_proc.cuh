@@ -190,7 +190,18 @@ TREX_HD void qq_close(const vec4<R>& eg, const rvec4<double>& Kg, const vec4<R>&
   t.K[0] = Kg; t.eps[0] = eg; t.K[1] = Kq; t.eps[1] = Jq;
   t.pt = pt;
   t.ubar_t = ubar_t;
-  // top mass/width may differ between theta_old and theta_new: evaluate per theta when they do
+  // single-source brackets of K3, K4: ubar_t [ i Jslash + (kappa/g_s) 2 sigma(P ^ J) ]; they depend neither on theta nor on
+  // the antitop helicity, so they are formed once
+  spinor<R> c30 = row_slash(ubar_t, Jq3), c31 = szero<R>(), c40 = row_slash(ubar_t, Jq4), c41 = szero<R>();
+  { ften<R> F = fzero<R>(); wedge_acc(F, cast<R>(Ptot), Jq3); row_sigma_acc(c31, ubar_t, F); }
+  { ften<R> F = fzero<R>(); wedge_acc(F, cast<R>(Ptot), Jq4); row_sigma_acc(c41, ubar_t, F); }
+  cx<R> k30[2], k31[2], k40[2], k41[2];
+#pragma unroll
+  for (int iv = 0; iv < 2; ++iv) {
+    k30[iv] = mul_i(row_col(c30, st.v[iv])); k31[iv] = row_col(c31, st.v[iv]);
+    k40[iv] = mul_i(row_col(c40, st.v[iv])); k41[iv] = row_col(c41, st.v[iv]);
+  }
+  // top mass/width may differ between theta_old and theta_new: the two-source walk is repeated per theta when they do
   RC res[2];
   const bool same_line = (T.mt[0] == T.mt[1]) && (T.mGt[0] == T.mGt[1]);
   cx<R> A12[2][2], A21[2][2];   // [order][v]
@@ -201,23 +212,14 @@ TREX_HD void qq_close(const vec4<R>& eg, const rvec4<double>& Kg, const vec4<R>&
 #pragma unroll
       for (int iv = 0; iv < 2; ++iv) { A12[0][iv] = st.a0[0][iv]; A12[1][iv] = st.a1[0][iv]; A21[0][iv] = st.a0[1][iv]; A21[1][iv] = st.a1[1][iv]; }
     }
-    // single-source amplitudes K3, K4: ubar_t [ i Jslash + (kappa/g_s) 2 sigma(P ^ J) ] v
+    const R kq = R(T.kq[th]);
     RC s = RC(0);
 #pragma unroll
     for (int iv = 0; iv < 2; ++iv) {
-      cx<R> k3, k4;
-      {
-        spinor<R> b0 = row_slash(ubar_t, Jq3), b1 = szero<R>();
-        ften<R> F = fzero<R>(); wedge_acc(F, cast<R>(Ptot), Jq3); row_sigma_acc(b1, ubar_t, F);
-        cx<R> a0 = mul_i(row_col(b0, st.v[iv])); cfma(a0, row_col(b1, st.v[iv]), R(T.kq[th])); k3 = a0;
-      }
-      {
-        spinor<R> b0 = row_slash(ubar_t, Jq4), b1 = szero<R>();
-        ften<R> F = fzero<R>(); wedge_acc(F, cast<R>(Ptot), Jq4); row_sigma_acc(b1, ubar_t, F);
-        cx<R> a0 = mul_i(row_col(b0, st.v[iv])); cfma(a0, row_col(b1, st.v[iv]), R(T.kq[th])); k4 = a0;
-      }
-      cx<R> a12 = A12[0][iv]; cfma(a12, A12[1][iv], R(T.kq[th]));
-      cx<R> a21 = A21[0][iv]; cfma(a21, A21[1][iv], R(T.kq[th]));
+      cx<R> k3 = k30[iv]; cfma(k3, k31[iv], kq);
+      cx<R> k4 = k40[iv]; cfma(k4, k41[iv], kq);
+      cx<R> a12 = A12[0][iv]; cfma(a12, A12[1][iv], kq);
+      cx<R> a21 = A21[0][iv]; cfma(a21, A21[1][iv], kq);
       cx<R> j1 = R(0.5) * (a12 + k4), j2 = R(0.5) * (a21 + k3);
       cx<R> j3 = R(-1.0 / 6.0) * (a12 + a21), j4 = R(-1.0 / 6.0) * (k3 + k4);
       cx<RC> J[4] = {cx<RC>(RC(j1.re), RC(j1.im)), cx<RC>(RC(j2.re), RC(j2.im)), cx<RC>(RC(j3.re), RC(j3.im)), cx<RC>(RC(j4.re), RC(j4.im))};
