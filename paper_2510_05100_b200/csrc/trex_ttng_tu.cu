@@ -5,6 +5,9 @@
 #ifndef TREX_GGTT_UNROLL
 #define TREX_GGTT_UNROLL 2
 #endif
+#ifndef TREX_GGTT_NW
+#define TREX_GGTT_NW 8
+#endif
 #ifndef TREX_GGTT_MINB
 #define TREX_GGTT_MINB 2
 #endif
@@ -32,9 +35,10 @@ namespace trex {
 // closes the 2 x 2 colour sum. Same recursion and the same operation order per amplitude as TTNGS<R, 2, 1, .>
 // (SURVEY.md C-4); parameter points with equal top mass and width only (otherwise the generic kernel runs).
 template <class R, class RC>
-__global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArgs a) {
+__global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(const ReweightArgs a) {
+  constexpr int NW = TREX_GGTT_NW;                            // warps per block: 8 (one unit each) or 4 (two units each)
   __shared__ double wf[8][8][32];
-  __shared__ double red[2][8][32];
+  __shared__ double red[2][NW][32];
   const EvIO io = resolve_io(a);
   if ((long)blockIdx.x * 32 >= io.n) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -42,26 +46,28 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
   const long ev = e < io.n ? e : io.n - 1;
   // all 16 momentum rows of the block's 32 events: one coalesced pass, one DRAM latency; later reads come from here
   __shared__ double pm[16][32];
-  pm[warp][lane] = io.mom[(long)warp * io.ld + ev];
-  pm[warp + 8][lane] = io.mom[(long)(warp + 8) * io.ld + ev];
+  for (int r = warp; r < 16; r += NW) pm[r][lane] = io.mom[(long)r * io.ld + ev];
   __syncthreads();
-  {
+  for (int item = warp; item < 8; item += NW) {
     double p[4];
-    const int leg = warp >> 1, lam = (warp & 1) ? 1 : -1;      // legs in process order: g g t t~
+    const int leg = item >> 1, lam = (item & 1) ? 1 : -1;      // legs in process order: g g t t~
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) p[mu] = pm[leg * 4 + mu][lane];
     if (leg < 2) {
       const vec4<double> w = polvec<double>(p, lam, false);
 #pragma unroll
-      for (int i = 0; i < 4; ++i) { wf[warp][2 * i][lane] = w.c[i].re; wf[warp][2 * i + 1][lane] = w.c[i].im; }
+      for (int i = 0; i < 4; ++i) { wf[item][2 * i][lane] = w.c[i].re; wf[item][2 * i + 1][lane] = w.c[i].im; }
     } else {
       const spinor<double> w = leg == 2 ? bar(spinor_u<double>(p, lam, false)) : spinor_v<double>(p, lam, false);
 #pragma unroll
-      for (int i = 0; i < 4; ++i) { wf[warp][2 * i][lane] = w.c[i].re; wf[warp][2 * i + 1][lane] = w.c[i].im; }
+      for (int i = 0; i < 4; ++i) { wf[item][2 * i][lane] = w.c[i].re; wf[item][2 * i + 1][lane] = w.c[i].im; }
     }
   }
   __syncthreads();
-  const int gh = warp >> 1, lt = warp & 1;
+  RC acc[2] = {RC(0), RC(0)};
+#pragma unroll 1
+ for (int unit = warp; unit < 8; unit += NW) {
+  const int gh = unit >> 1, lt = unit & 1;
   const int wsel[2] = {gh & 1, 2 + ((gh >> 1) & 1)};           // wavefunction slots of eps(g1), eps(g2) for this unit
   spinor<R> ubar;
   rvec4<double> pt;
@@ -98,7 +104,6 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
   const R mt = R(a.T.mt[0]);
   const RC cd = RC(c_Ctab[0]), co = RC(2.0 * c_Ctab[1]);
   const R kq[2] = {R(a.T.kq[0]), R(a.T.kq[1])};
-  RC acc[2] = {RC(0), RC(0)};
   cx<RC> xprev[2][2];                                         // [lambda_tbar][theta] of the previous ordering
 #pragma unroll
   for (int k = 0; k < 4; ++k) xprev[k >> 1][k & 1] = cx<RC>(RC(0), RC(0));
@@ -169,12 +174,13 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
       }
     }
   }
+ }
   red[0][warp][lane] = (double)acc[0]; red[1][warp][lane] = (double)acc[1];
   __syncthreads();
   if (warp == 0 && e < io.n) {
     double s0 = 0.0, s1 = 0.0;
 #pragma unroll
-    for (int w = 0; w < 8; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
+    for (int w = 0; w < NW; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
     const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
     const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
     io.w_out[e] = io.w_in[e] * norm * mn;                        // evaluate + append_wgts
@@ -187,7 +193,7 @@ __global__ void __launch_bounds__(256, TREX_GGTT_MINB) k_gg_tt(const ReweightArg
 int TREX_TU_NAME(trex_tu_launch_n, TREX_TU_N, TREX_TU_MODE)(const ReweightArgs& a, int npass, unsigned grid, cudaStream_t s) {
 #if TREX_TU_N == 2
   if (npass == 1) {                                   // equal top mass and width at both parameter points
-    k_gg_tt<TuR, TuRC><<<grid, 256, 0, s>>>(a);
+    k_gg_tt<TuR, TuRC><<<grid, 32 * TREX_GGTT_NW, 0, s>>>(a);
     return (int)cudaGetLastError();
   }
 #endif
