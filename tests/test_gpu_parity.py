@@ -465,3 +465,19 @@ def test_run_sizes_around_every_threshold(T, n):
             r, _, _ = gpu_reweight(T, sp.sid, np.ascontiguousarray(mom[:, :, sel]), w.theta_old, w.theta_new, win[sel])
             ref[sel] = r
     assert np.array_equal(wo, ref)
+
+
+@pytest.mark.parametrize("n", [3000, 40000])
+def test_run_with_too_many_classes_fails_loudly(T, n):
+    """More than REX_MAX_BUCKETS distinct flavour keys: rex_bucket and trex_run report the error (both bucketing paths:
+    one block for small samples, six launches otherwise); the library stays usable afterwards."""
+    import torch
+    w = make_config(2, n=n)
+    keys = w.keys.copy()
+    keys[: T.REX_MAX_BUCKETS + 5] = np.arange(1, T.REX_MAX_BUCKETS + 6, dtype=np.uint64) * np.uint64(1000003)
+    with pytest.raises(T.TrexError):
+        T.rex_bucket(dev(keys))
+    with pytest.raises(T.TrexError):
+        T.trex_run(dev(keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    wo, mo, mn, nb = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    assert nb == 1 and bool((wo > 0).all())
