@@ -34,6 +34,9 @@ namespace {
 #ifndef TREX_T3_MINB
 #define TREX_T3_MINB 3
 #endif
+#ifndef TREX_T3_UT
+#define TREX_T3_UT 0
+#endif
 #ifndef TREX_T5_DMMA
 #define TREX_T5_DMMA 1
 #endif
@@ -52,7 +55,7 @@ namespace {
 // UT: the top-line states of ordering prefixes up to this length are tabulated per event instead of being carried by
 // every walk thread (fewer registers per thread -> more warps, and no recomputation across tasks)
 template <int N> struct TabCfg;
-template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB, UT = 0; };
+template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = TREX_T3_UT ? 3 : 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB, UT = TREX_T3_UT; };
 template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = TREX_T4_UT ? 4 : 2, TB = TREX_T4_TB, EPB = 1, MINB = TREX_T4_MINB, UT = TREX_T4_UT; };
 template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1, UT = 0; };
 
