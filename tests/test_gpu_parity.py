@@ -481,3 +481,22 @@ def test_run_with_too_many_classes_fails_loudly(T, n):
         T.trex_run(dev(keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
     wo, mo, mn, nb = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
     assert nb == 1 and bool((wo > 0).all())
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 4096), (2, 20000), (3, 20000), (5, 512)])
+@pytest.mark.parametrize("mode", [1, 2])
+def test_reduced_precision_modes_every_config(T, cfg, n, mode):
+    """fptype m / f through the whole path on every configuration: median 5e-5 / maximum 1e-3 against
+    the fp64 path (north star); kinematic invariants stay in fp64 in every mode (R-12)."""
+    import torch
+    w = make_config(cfg, n=n)
+    k, m, wi = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    ref = [x.cpu().numpy() for x in T.trex_run(k, m, w.theta_old, w.theta_new, wi)[:3]]
+    T.trex_set_precision(mode)
+    try:
+        got = [x.cpu().numpy() for x in T.trex_run(k, m, w.theta_old, w.theta_new, wi)[:3]]
+    finally:
+        T.trex_set_precision(0)
+    for g, r0 in zip(got, ref):
+        r = rel(g, r0)
+        assert np.median(r) < 5e-5 and r.max() < 1e-3, (cfg, mode, np.median(r), r.max())
