@@ -36,7 +36,14 @@ SID_OF_CFG = {1: 0, 2: 1, 4: 3, 5: 4}
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 
+ORACLE_FLOPS = {}
+
+
 def load_flops():
+    opath = os.path.join(ROOT, "profiles", "oracle_flops_per_event.json")
+    if os.path.exists(opath):
+        with open(opath) as fh:
+            ORACLE_FLOPS.update(json.load(fh))
     path = os.path.join(ROOT, "profiles", "flops_per_event.json")
     if os.path.exists(path):
         with open(path) as fh:
@@ -316,6 +323,8 @@ def main():
                 # the same probe with three REGISTER operands per FMA (what amplitude code issues): the register file
                 # feeds the FP64 pipe at this rate at most
                 "peak_three_register_operands": fp64_peak_3reg,
+                # what the oracle's plain algorithm spends on the same event (oracle/count_flops.py: counting scalar type)
+                "oracle_flop_per_event": ORACLE_FLOPS.get("cfg%d g g > t t~" % HEADLINE_CFG, {}).get("flop"),
                 "frac_of_three_register_peak": (ach / fp64_peak_3reg) if ach else None}
         tpath = os.path.join(ROOT, "profiles", "flops_per_event.json")
         if os.path.exists(tpath):

@@ -64,6 +64,23 @@ def abd(sid, momenta, theta, engine=1, gauge_gluon=-1, hel_only=-1, long_double=
     return out
 
 
+def count_flops(sid, momenta_one, theta_old, theta_new):
+    """Real additions/subtractions, multiplications, divisions and square roots the plain evaluator performs for ONE
+    reweighted event (old + new |M|^2 and the weight): the evaluator instantiated on a counting scalar type
+    (SURVEY.md 8(d) count (iii); BASELINE.json: "FLOPs per event counted from the oracle"). Returns a dict."""
+    mom = np.ascontiguousarray(np.asarray(momenta_one, dtype=np.float64).reshape(-1, 4, 1))
+    out = (ctypes.c_longlong * 4)()
+    f = lib().oracle_count_flops
+    f.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                  ctypes.POINTER(ctypes.c_longlong)]
+    tho = np.ascontiguousarray(theta_old, dtype=np.float64)
+    thn = np.ascontiguousarray(theta_new, dtype=np.float64)
+    rc = f(int(sid), _dp(mom), _dp(tho), _dp(thn), out)
+    if rc != 0:
+        raise RuntimeError("oracle_count_flops failed (%d)" % rc)
+    return {"add": int(out[0]), "mul": int(out[1]), "div": int(out[2]), "sqrt": int(out[3]), "flop": int(sum(out))}
+
+
 def kappa(theta):
     return theta[7] * theta[9] / (math.sqrt(2.0) * theta[8] ** 2)
 

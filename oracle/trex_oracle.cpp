@@ -28,6 +28,7 @@
 
 #include <array>
 #include <cmath>
+#include <atomic>
 #include <complex>
 #include <cstdint>
 #include <cstring>
@@ -39,6 +40,39 @@
 
 namespace {
 
+// ---------------------------------------------------------------- counting scalar (flop count (iii))
+// Instantiating the evaluator on this type tallies every real addition / subtraction, multiplication, division and
+// square root the plain algorithm performs: "FLOPs per event counted from the oracle" (BASELINE.json north star).
+struct Count {
+  double v;
+  static std::atomic<long long> n_add, n_mul, n_div, n_sqrt;
+  Count() : v(0) {}
+  Count(double x) : v(x) {}
+  Count(long double x) : v((double)x) {}
+  Count(int x) : v(x) {}
+  explicit operator double() const { return v; }
+  Count operator-() const { return Count(-v); }
+  Count& operator+=(Count o) { ++n_add; v += o.v; return *this; }
+  Count& operator-=(Count o) { ++n_add; v -= o.v; return *this; }
+  Count& operator*=(Count o) { ++n_mul; v *= o.v; return *this; }
+  Count& operator/=(Count o) { ++n_div; v /= o.v; return *this; }
+};
+std::atomic<long long> Count::n_add{0}, Count::n_mul{0}, Count::n_div{0}, Count::n_sqrt{0};
+inline Count operator+(Count a, Count b) { return a += b; }
+inline Count operator-(Count a, Count b) { return a -= b; }
+inline Count operator*(Count a, Count b) { return a *= b; }
+inline Count operator/(Count a, Count b) { return a /= b; }
+inline bool operator==(Count a, Count b) { return a.v == b.v; }
+inline bool operator!=(Count a, Count b) { return a.v != b.v; }
+inline bool operator<(Count a, Count b) { return a.v < b.v; }
+inline bool operator>(Count a, Count b) { return a.v > b.v; }
+inline bool operator<=(Count a, Count b) { return a.v <= b.v; }
+inline bool operator>=(Count a, Count b) { return a.v >= b.v; }
+inline Count osqrt(Count x) { ++Count::n_sqrt; return Count(std::sqrt(x.v)); }
+inline Count oacos(Count x) { return Count(std::acos(x.v)); }
+template <class T> T osqrt(T x) { return std::sqrt(x); }
+template <class T> T oacos(T x) { return std::acos(x); }
+
 constexpr int NTHETA = 16;
 enum { TH_ALPHA_S = 0, TH_ALPHA_EM, TH_SIN2W, TH_MZ, TH_GAMMAZ, TH_MT, TH_GAMMAT, TH_CTG, TH_LAMBDA, TH_VEV };
 
@@ -47,7 +81,7 @@ template <class R> using Spinor = std::array<Cx<R>, 4>;   // column or row, by c
 template <class R> using Vec4 = std::array<Cx<R>, 4>;     // upper-index Lorentz vector (E,x,y,z)
 template <class R> using Mat4 = std::array<std::array<Cx<R>, 4>, 4>;
 
-template <class R> R pi_() { return std::acos(R(-1)); }
+template <class R> R pi_() { return oacos(R(-1)); }
 const int METRIC[4] = {1, -1, -1, -1};
 
 // ---------------------------------------------------------------- Dirac algebra (chiral basis, R-1)
@@ -63,7 +97,8 @@ template <class R> struct Dirac {
     // gamma^0 = [[0,1],[1,0]]
     g[0][0][2] = g[0][1][3] = g[0][2][0] = g[0][3][1] = 1;
     // gamma^i = [[0,sigma^i],[-sigma^i,0]]
-    Cx<R> s[3][2][2] = {{{0, 1}, {1, 0}}, {{0, -I}, {I, 0}}, {{1, 0}, {0, -1}}};
+    const Cx<R> Z(R(0)), E(R(1));
+    Cx<R> s[3][2][2] = {{{Z, E}, {E, Z}}, {{Z, -I}, {I, Z}}, {{E, Z}, {Z, -E}}};
     for (int i = 0; i < 3; ++i)
       for (int a = 0; a < 2; ++a)
         for (int b = 0; b < 2; ++b) {
@@ -81,7 +116,7 @@ template <class R> struct Dirac {
       for (int n = 0; n < 4; ++n)
         for (int a = 0; a < 4; ++a)
           for (int b = 0; b < 4; ++b) {
-            Cx<R> c = 0;
+            Cx<R> c(R(0));
             for (int k = 0; k < 4; ++k) c += g[m][a][k] * g[n][k][b] - g[n][a][k] * g[m][k][b];
             sig[m][n][a][b] = I * c / R(2);
           }
@@ -104,7 +139,7 @@ template <class R> Spinor<R> rowmul(const Spinor<R>& r, const Mat4<R>& m) {
 template <class R> Spinor<R> colmul(const Mat4<R>& m, const Spinor<R>& c) {
   Spinor<R> o; o.fill(Cx<R>(0)); for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) o[i] += m[i][j] * c[j]; return o; }
 template <class R> Cx<R> rowcol(const Spinor<R>& r, const Spinor<R>& c) {
-  Cx<R> s = 0; for (int i = 0; i < 4; ++i) s += r[i] * c[i]; return s; }
+  Cx<R> s(R(0)); for (int i = 0; i < 4; ++i) s += r[i] * c[i]; return s; }
 template <class R> Spinor<R> sadd(const Spinor<R>& a, const Spinor<R>& b) {
   Spinor<R> o; for (int i = 0; i < 4; ++i) o[i] = a[i] + b[i]; return o; }
 template <class R> Spinor<R> szero() { Spinor<R> o; o.fill(Cx<R>(0)); return o; }
@@ -142,7 +177,7 @@ template <class R> struct Chi { Cx<R> plus[2], minus[2]; };
 template <class R> Chi<R> two_spinors(const R p[4]) {
   Chi<R> c;
   R pt2 = p[1] * p[1] + p[2] * p[2];
-  R pabs = std::sqrt(pt2 + p[3] * p[3]);
+  R pabs = osqrt(pt2 + p[3] * p[3]);
   // |p| + pz, evaluated without cancellation when pz < 0
   R ppz = p[3] >= R(0) ? pabs + p[3] : pt2 / (pabs - p[3]);
   if (pabs == R(0)) {           // at rest: the pz -> +0 limit
@@ -151,7 +186,7 @@ template <class R> Chi<R> two_spinors(const R p[4]) {
   if (ppz == R(0)) {            // exactly along -z
     c.plus[0] = 0; c.plus[1] = 1; c.minus[0] = -1; c.minus[1] = 0; return c;
   }
-  R N = R(1) / std::sqrt(R(2) * pabs * ppz);
+  R N = R(1) / osqrt(R(2) * pabs * ppz);
   c.plus[0] = N * ppz; c.plus[1] = N * Cx<R>(p[1], p[2]);
   c.minus[0] = N * Cx<R>(-p[1], p[2]); c.minus[1] = N * ppz;
   return c; }
@@ -161,17 +196,17 @@ template <class R> Chi<R> two_spinors(const R p[4]) {
 // otherwise amplify the rounding of the input momenta to a spurious 1e-8 wrong-chirality component)
 template <class R> Spinor<R> spinor_u(const R p[4], int lam, bool massless = false) {
   Chi<R> c = two_spinors<R>(p);
-  R pabs = std::sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
-  R wp = std::sqrt(std::max(R(0), p[0] + pabs)), wm = std::sqrt(std::max(R(0), p[0] - pabs));
-  if (massless) { wp = std::sqrt(R(2) * pabs); wm = 0; }
+  R pabs = osqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+  R wp = osqrt(std::max(R(0), p[0] + pabs)), wm = osqrt(std::max(R(0), p[0] - pabs));
+  if (massless) { wp = osqrt(R(2) * pabs); wm = 0; }
   const Cx<R>* chi = lam > 0 ? c.plus : c.minus;
   R up = lam > 0 ? wm : wp, lo = lam > 0 ? wp : wm;
   return Spinor<R>{up * chi[0], up * chi[1], lo * chi[0], lo * chi[1]}; }
 template <class R> Spinor<R> spinor_v(const R p[4], int lam, bool massless = false) {
   Chi<R> c = two_spinors<R>(p);
-  R pabs = std::sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
-  R wp = std::sqrt(std::max(R(0), p[0] + pabs)), wm = std::sqrt(std::max(R(0), p[0] - pabs));
-  if (massless) { wp = std::sqrt(R(2) * pabs); wm = 0; }
+  R pabs = osqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+  R wp = osqrt(std::max(R(0), p[0] + pabs)), wm = osqrt(std::max(R(0), p[0] - pabs));
+  if (massless) { wp = osqrt(R(2) * pabs); wm = 0; }
   const Cx<R>* chi = lam > 0 ? c.minus : c.plus;   // chi_{-lambda}
   R up = lam > 0 ? -wp : wm, lo = lam > 0 ? wm : -wp;
   return Spinor<R>{up * chi[0], up * chi[1], lo * chi[0], lo * chi[1]}; }
@@ -182,8 +217,8 @@ template <class R> Spinor<R> bar(const Spinor<R>& s) {
   return rowmul(cj, d.g[0]); }
 // eps(p,lambda) = (-lambda e1 - i e2)/sqrt2 for a massless vector
 template <class R> Vec4<R> polvec(const R p[4], int lam) {
-  R pt = std::sqrt(p[1] * p[1] + p[2] * p[2]);
-  R pabs = std::sqrt(pt * pt + p[3] * p[3]);
+  R pt = osqrt(p[1] * p[1] + p[2] * p[2]);
+  R pabs = osqrt(pt * pt + p[3] * p[3]);
   R e1[4], e2[4];
   if (pt < R(1e-14) * pabs || pt == R(0)) {
     R sg = p[3] >= 0 ? R(1) : R(-1);
@@ -193,7 +228,7 @@ template <class R> Vec4<R> polvec(const R p[4], int lam) {
     e1[0] = 0; e1[1] = p[1] * p[3] / (pabs * pt); e1[2] = p[2] * p[3] / (pabs * pt); e1[3] = -pt / pabs;
     e2[0] = 0; e2[1] = -p[2] / pt; e2[2] = p[1] / pt; e2[3] = 0;
   }
-  const R rs2 = R(1) / std::sqrt(R(2));
+  const R rs2 = R(1) / osqrt(R(2));
   Vec4<R> e;
   for (int i = 0; i < 4; ++i) e[i] = Cx<R>(-R(lam) * e1[i], -e2[i]) * rs2;
   return e; }
@@ -215,7 +250,7 @@ struct SU3 {
     T[4][0][2] = -0.5 * I; T[4][2][0] = 0.5 * I;
     T[5][1][2] = T[5][2][1] = 0.5;
     T[6][1][2] = -0.5 * I; T[6][2][1] = 0.5 * I;
-    double s3 = 1.0 / std::sqrt(3.0);
+    double s3 = 1.0 / osqrt(3.0);
     T[7][0][0] = T[7][1][1] = 0.5 * s3; T[7][2][2] = -s3;
     // f^{abc} = -2i tr([T^a,T^b] T^c)
     for (int a = 0; a < 8; ++a) for (int b = 0; b < 8; ++b) for (int c = 0; c < 8; ++c) {
@@ -282,10 +317,10 @@ const std::vector<double>& colour_matrix(int n) {   // n! x n!, row-major, lexic
 template <class R> struct Params {
   R gs, ee, sw2, mZ, GZ, mt, Gt, kappa;
   explicit Params(const double* th) {
-    gs = std::sqrt(R(4) * pi_<R>() * R(th[TH_ALPHA_S]));
-    ee = std::sqrt(R(4) * pi_<R>() * R(th[TH_ALPHA_EM]));
+    gs = osqrt(R(4) * pi_<R>() * R(th[TH_ALPHA_S]));
+    ee = osqrt(R(4) * pi_<R>() * R(th[TH_ALPHA_EM]));
     sw2 = th[TH_SIN2W]; mZ = th[TH_MZ]; GZ = th[TH_GAMMAZ]; mt = th[TH_MT]; Gt = th[TH_GAMMAT];
-    kappa = R(th[TH_CTG]) * R(th[TH_VEV]) / (std::sqrt(R(2)) * R(th[TH_LAMBDA]) * R(th[TH_LAMBDA]));
+    kappa = R(th[TH_CTG]) * R(th[TH_VEV]) / (osqrt(R(2)) * R(th[TH_LAMBDA]) * R(th[TH_LAMBDA]));
   }
 };
 
@@ -336,7 +371,7 @@ template <class R> R eemumu_me2(const Event<R>& ev, const Params<R>& P) {
   const auto& d = dirac<R>();
   R s = 0;
   { R q[4]; for (int m = 0; m < 4; ++m) q[m] = ev.p[0][m] + ev.p[1][m]; s = q[0] * q[0] - q[1] * q[1] - q[2] * q[2] - q[3] * q[3]; }
-  R cw2 = R(1) - P.sw2, sc = std::sqrt(P.sw2 * cw2);
+  R cw2 = R(1) - P.sw2, sc = osqrt(P.sw2 * cw2);
   R gL = P.ee / sc * (R(-0.5) + P.sw2), gR = P.ee / sc * P.sw2;
   Mat4<R> GZ = madd(mscale(d.PL, Cx<R>(gL)), mscale(d.PR, Cx<R>(gR)));
   const Cx<R> I(0, 1);
@@ -347,7 +382,7 @@ template <class R> R eemumu_me2(const Event<R>& ev, const Params<R>& P) {
     Spinor<R> vb2 = bar(spinor_v<R>(ev.p[1], hel_of(h, 1), true)); // incoming e+
     Spinor<R> ub3 = bar(spinor_u<R>(ev.p[2], hel_of(h, 2), true)); // outgoing mu-
     Spinor<R> v4 = spinor_v<R>(ev.p[3], hel_of(h, 3), true);       // outgoing mu+
-    Cx<R> M = 0;
+    Cx<R> M(R(0));
     for (int mu = 0; mu < 4; ++mu) {
       Mat4<R> va = mscale(d.g[mu], I * P.ee);                     // i e gamma^mu
       Mat4<R> vz = mscale(mmul(d.g[mu], GZ), I);                  // i gamma^mu (gL PL + gR PR)
@@ -809,5 +844,17 @@ int oracle_gamma(int mu, double* out) {
   const Mat4<double>& m = mu == 4 ? d.g5 : d.g[mu];
   for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) { out[(i * 4 + j) * 2] = m[i][j].real(); out[(i * 4 + j) * 2 + 1] = m[i][j].imag(); }
   return 0; }
+
+// flop count of the plain algorithm for ONE event (old + new |M|^2 and the weight): out[4] = additions/subtractions,
+// multiplications, divisions, square roots on real numbers
+int oracle_count_flops(int sid, const double* mom_one, const double* th_old, const double* th_new, long long* out) {
+  int npar = npar_of(sid); if (npar < 0) return -2;
+  if (sid >= 1 && sid <= 4) colour_matrix(npar - 2);
+  double w_in = 1.0, w_out, mo, mn;
+  reweight_batch<Count>(sid, mom_one, 1, th_old, th_new, &w_in, &w_out, &mo, &mn);   // builds the static Dirac tables once
+  Count::n_add = 0; Count::n_mul = 0; Count::n_div = 0; Count::n_sqrt = 0;
+  int rc = reweight_batch<Count>(sid, mom_one, 1, th_old, th_new, &w_in, &w_out, &mo, &mn);
+  out[0] = Count::n_add; out[1] = Count::n_mul; out[2] = Count::n_div; out[3] = Count::n_sqrt;
+  return rc; }
 
 }  // extern "C"

@@ -105,3 +105,19 @@ def test_top_width_enters_continuously_and_double_matches_long_double():
     th1 = th.copy(); th1[TH_GAMMAT] = 1e-6
     assert np.allclose(O.me2(3, w.momenta, th0), O.me2(3, w.momenta, th1), rtol=1e-6, atol=0)
     assert not np.allclose(a, O.me2(3, w.momenta, th0), rtol=1e-9, atol=0)     # Gamma_t = 1.5 really changes the value
+
+
+def test_flop_counter_counts_the_same_evaluation():
+    """The counting scalar runs the very same templated evaluator: counts are deterministic, grow with the multiplicity,
+    and the 2 -> 2 count has the size the plain algorithm implies (16 helicities x 2 orderings x 2 parameter points of
+    4 x 4 complex matrix-vector chains: 1e5 - 1e7 operations)."""
+    from trex_inputs import make_config
+    counts = []
+    for cfg, sid in ((2, 1), (3, 2), (4, 3)):
+        w = make_config(cfg, n=64)
+        i = int(np.where(w.keys == w.classes[0].key)[0][0])
+        c1 = O.count_flops(sid, w.momenta[:, :, i], w.theta_old, w.theta_new)
+        c2 = O.count_flops(sid, w.momenta[:, :, i], w.theta_old, w.theta_new)
+        assert c1 == c2 and c1["flop"] == c1["add"] + c1["mul"] + c1["div"] + c1["sqrt"]
+        counts.append(c1["flop"])
+    assert 1e5 < counts[0] < 1e7 and counts[0] * 5 < counts[1] and counts[1] * 5 < counts[2]
