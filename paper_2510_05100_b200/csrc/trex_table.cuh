@@ -117,8 +117,8 @@ template <int N, int NFIX> struct TabIdx {
 };
 
 // ---------------------------------------------------------------- table access
-// 20 real components per entry, component-major: tab[comp * NE + entry]; comp 0..7 = J (re, im per mu),
-// 8..19 = -i * 2 sigma.F in the form the row-spinor product consumes: with X+- = 2 (B +- iE) (the two chiral 2x2 blocks
+// 10 complex components per entry, component-major: tab[comp * NE + entry] (re, im adjacent); comp 0..3 = J^mu,
+// 4..9 = -i * 2 sigma.F in the form the row-spinor product consumes: with X+- = 2 (B +- iE) (the two chiral 2x2 blocks
 // are X+.s and X-.s) the entries are -i (X+_3, X+_1 + i X+_2, X+_1 - i X+_2, X-_3, X-_1 + i X-_2, X-_1 - i X-_2).
 // The factor -i lets the walk accumulate  sum_a [U_a Jslash_a - i U_a sigma.F_a]  and multiply by i once per node.
 constexpr int TAB_NCOMP = 20;
@@ -154,28 +154,42 @@ TREX_HD float with_sign(float x, int sign) {
   return sign < 0 ? -x : x;
 #endif
 }
+// (re, im) of one table component travel together: one 16-byte (fp64) / 8-byte (fp32) shared-memory access
+template <class R> struct pair_of;
+template <> struct pair_of<double> { using type = double2; };
+template <> struct pair_of<float> { using type = float2; };
+template <class R> TREX_HD cx<R> tab_get(const R* __restrict__ tab, int idx, int sign) {
+  using P = typename pair_of<R>::type;
+  const P v = reinterpret_cast<const P*>(tab)[idx];
+  return cx<R>(with_sign(v.x, sign), with_sign(v.y, sign));
+}
+template <class R> TREX_HD void tab_put(R* __restrict__ tab, int idx, cx<R> c) {
+  using P = typename pair_of<R>::type;
+  P v; v.x = c.re; v.y = c.im;
+  reinterpret_cast<P*>(tab)[idx] = v;
+}
 template <class R, int NE> TREX_HD vec4<R> tab_J(const R* __restrict__ tab, int e, int sign) {
   vec4<R> J;
 #pragma unroll
-  for (int mu = 0; mu < 4; ++mu) J.c[mu] = cx<R>(with_sign(tab[(2 * mu) * NE + e], sign), with_sign(tab[(2 * mu + 1) * NE + e], sign));
+  for (int mu = 0; mu < 4; ++mu) J.c[mu] = tab_get<R>(tab, mu * NE + e, sign);
   return J;
 }
 template <class R, int NE> TREX_HD sigF<R> tab_F(const R* __restrict__ tab, int e, int sign) {
   sigF<R> F;
   cx<R>* f = &F.p3;
 #pragma unroll
-  for (int i = 0; i < 6; ++i) f[i] = cx<R>(with_sign(tab[(8 + 2 * i) * NE + e], sign), with_sign(tab[(9 + 2 * i) * NE + e], sign));
+  for (int i = 0; i < 6; ++i) f[i] = tab_get<R>(tab, (4 + i) * NE + e, sign);
   return F;
 }
 template <class R, int NE> TREX_HD void tab_store(R* __restrict__ tab, int e, const vec4<R>& J, const ften<R>& f) {
 #pragma unroll
-  for (int mu = 0; mu < 4; ++mu) { tab[(2 * mu) * NE + e] = J.c[mu].re; tab[(2 * mu + 1) * NE + e] = J.c[mu].im; }
+  for (int mu = 0; mu < 4; ++mu) tab_put<R>(tab, mu * NE + e, J.c[mu]);
   cx<R> xp[3], xm[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) { const cx<R> ie = mul_i(f.e[i]); xp[i] = R(2) * (f.b[i] + ie); xm[i] = R(2) * (f.b[i] - ie); }
   const cx<R> out[6] = {xp[2], xp[0] + mul_i(xp[1]), xp[0] - mul_i(xp[1]), xm[2], xm[0] + mul_i(xm[1]), xm[0] - mul_i(xm[1])};
 #pragma unroll
-  for (int i = 0; i < 6; ++i) { const cx<R> v = mul_mi(out[i]); tab[(8 + 2 * i) * NE + e] = v.re; tab[(9 + 2 * i) * NE + e] = v.im; }
+  for (int i = 0; i < 6; ++i) tab_put<R>(tab, (4 + i) * NE + e, mul_mi(out[i]));
 }
 // a -= b * c
 template <class R> TREX_HD void cfnma(cx<R>& a, cx<R> b, cx<R> c) {
@@ -324,8 +338,8 @@ template <class R, int N, int NFIX, int D, class Sink, int UT = 0, int STOP = 0>
       const int e = uindex<A>();
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
-        u.o0.c[i] = cx<R>(utab[(2 * i) * nut + e], utab[(2 * i + 1) * nut + e]);
-        u.o1.c[i] = cx<R>(utab[(8 + 2 * i) * nut + e], utab[(9 + 2 * i) * nut + e]);
+        u.o0.c[i] = tab_get<R>(utab, i * nut + e, 1);
+        u.o1.c[i] = tab_get<R>(utab, (4 + i) * nut + e, 1);
       }
       return u;
     } else return U[A];
@@ -389,8 +403,8 @@ template <class R, int N, int NFIX, int D, class Sink, int UT = 0, int STOP = 0>
           const int e = uindex<M>();
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            utab[(2 * i) * nut + e] = u.o0.c[i].re; utab[(2 * i + 1) * nut + e] = u.o0.c[i].im;
-            utab[(8 + 2 * i) * nut + e] = u.o1.c[i].re; utab[(9 + 2 * i) * nut + e] = u.o1.c[i].im;
+            tab_put<R>(utab, i * nut + e, u.o0.c[i]);
+            tab_put<R>(utab, (4 + i) * nut + e, u.o1.c[i]);
           }
         } else {
           U[M] = u;
