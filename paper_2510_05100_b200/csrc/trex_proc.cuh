@@ -176,6 +176,78 @@ template <class R> struct QqLeafStore {
   }
 };
 
+// Top line with TWO ordered sources (currents e1, e2 with momenta K1, K2 flowing into the line): the two orderings
+// A(1,2), A(2,1), each as (order 0, order 1 in kappa) for both antitop helicities: A12[order][v], A21[order][v].
+// Same recursion as TTNGS<R, 2, 1, .>, written out with the merged current formed once (J_21 = -J_12)
+// and the orderings in a rolled loop, so that the live state is one line spinor pair (cf. k_gg_tt).
+template <class R>
+TREX_HD void two_source_line(const spinor<R>& ubar, const rvec4<double>& pt, const vec4<R>& e1, const rvec4<double>& K1,
+                             const vec4<R>& e2, const rvec4<double>& K2, double mt_d, double mGt, const spinor<R> v[2],
+                             cx<R> A12[2][2], cx<R> A21[2][2]) {
+  spinor<R> d0, d1 = szero<R>();
+  {
+    const rvec4<double> P12 = radd(K1, K2);
+    vec4<R> acc = vzero<R>();
+    v3_acc(acc, K1, e1, K2, e2);
+    const R sc = R(-1.0 / rdot(P12, P12));
+    vec4<R> J12;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) J12.c[i] = acc.c[i] * sc;
+    ften<R> F = fzero<R>();
+    wedge_acc(F, cast<R>(P12), J12);
+    wedge_acc(F, e1, e2);
+    const spinor<R> t0 = row_slash(ubar, J12);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) d0.c[i] = mul_i(t0.c[i]);
+    row_sigma_acc(d1, ubar, F);
+  }
+  const R mt = R(mt_d);
+#pragma unroll 1
+  for (int ord = 0; ord < 2; ++ord) {
+    const vec4<R>& ea = ord ? e2 : e1; const vec4<R>& eb = ord ? e1 : e2;
+    const rvec4<double>& Ka = ord ? K2 : K1; const rvec4<double>& Kb = ord ? K1 : K2;
+    dspinor<R> U1;
+    {
+      spinor<R> c0, c1 = szero<R>();
+      ften<R> F = fzero<R>();
+      wedge_acc(F, cast<R>(Ka), ea);
+      const spinor<R> t0 = row_slash(ubar, ea);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) c0.c[i] = mul_i(t0.c[i]);
+      row_sigma_acc(c1, ubar, F);
+      const rvec4<double> qd = rsub(pt, Ka);
+      const double q2 = rdot(qd, qd);
+      const rvec4<R> q = cast<R>(qd);
+      const cx<double> den(q2 - mt_d * mt_d, mGt);
+      const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), den));
+      const spinor<R> s0 = row_slash(c0, q), s1 = row_slash(c1, q);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        cx<R> n0 = s0.c[i]; cfma(n0, c0.c[i], mt);
+        cx<R> n1 = s1.c[i]; cfma(n1, c1.c[i], mt);
+        U1.o0.c[i] = n0 * pr; U1.o1.c[i] = n1 * pr;
+      }
+    }
+    spinor<R> b0, b1;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { b0.c[i] = ord ? -d0.c[i] : d0.c[i]; b1.c[i] = ord ? -d1.c[i] : d1.c[i]; }
+    {
+      ften<R> F = fzero<R>();
+      wedge_acc(F, cast<R>(Kb), eb);
+      const spinor<R> t0 = row_slash(U1.o0, eb);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) b0.c[i] += mul_i(t0.c[i]);
+      const spinor<R> t1 = row_slash(U1.o1, eb);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) b1.c[i] += mul_i(t1.c[i]);
+      row_sigma_acc(b1, U1.o0, F);
+    }
+    cx<R> (*A)[2] = ord ? A21 : A12;
+#pragma unroll
+    for (int iv = 0; iv < 2; ++iv) { A[0][iv] = row_col(b0, v[iv]); A[1][iv] = row_col(b1, v[iv]); }
+  }
+}
+
 // top line of the quark channels, given the gluon polarisation, the quark-pair current Jq and the two currents Jq3 / Jq4
 // of the light line that has radiated the gluon: two-source ordered amplitudes + single-source amplitudes -> four colour
 // flows -> J^dagger C J for theta_old and theta_new, both antitop helicities (see the comment block above)
@@ -183,13 +255,7 @@ template <class R, class RC>
 TREX_HD void qq_close(const vec4<R>& eg, const rvec4<double>& Kg, const vec4<R>& Jq, const rvec4<double>& Kq, const vec4<R>& Jq3,
                       const vec4<R>& Jq4, const rvec4<double>& Ptot, const spinor<R>& ubar_t, const spinor<R> vtb[2],
                       const rvec4<double>& pt, const ThetaPair& T, RC out[2]) {
-  QqLeafStore<R> st;
-  st.v[0] = vtb[0]; st.v[1] = vtb[1];
-  // two-source ordered amplitudes: source 0 = gluon, source 1 = quark-pair current
-  TTNGS<R, 2, 1, QqLeafStore<R>> t;
-  t.K[0] = Kg; t.eps[0] = eg; t.K[1] = Kq; t.eps[1] = Jq;
-  t.pt = pt;
-  t.ubar_t = ubar_t;
+  const spinor<R>* stv = vtb;
   // single-source brackets of K3, K4: ubar_t [ i Jslash + (kappa/g_s) 2 sigma(P ^ J) ]; they depend neither on theta nor on
   // the antitop helicity, so they are formed once
   spinor<R> c30 = row_slash(ubar_t, Jq3), c31 = szero<R>(), c40 = row_slash(ubar_t, Jq4), c41 = szero<R>();
@@ -198,20 +264,16 @@ TREX_HD void qq_close(const vec4<R>& eg, const rvec4<double>& Kg, const vec4<R>&
   cx<R> k30[2], k31[2], k40[2], k41[2];
 #pragma unroll
   for (int iv = 0; iv < 2; ++iv) {
-    k30[iv] = mul_i(row_col(c30, st.v[iv])); k31[iv] = row_col(c31, st.v[iv]);
-    k40[iv] = mul_i(row_col(c40, st.v[iv])); k41[iv] = row_col(c41, st.v[iv]);
+    k30[iv] = mul_i(row_col(c30, stv[iv])); k31[iv] = row_col(c31, stv[iv]);
+    k40[iv] = mul_i(row_col(c40, stv[iv])); k41[iv] = row_col(c41, stv[iv]);
   }
   // top mass/width may differ between theta_old and theta_new: the two-source walk is repeated per theta when they do
   RC res[2];
   const bool same_line = (T.mt[0] == T.mt[1]) && (T.mGt[0] == T.mGt[1]);
   cx<R> A12[2][2], A21[2][2];   // [order][v]
   for (int th = 0; th < 2; ++th) {
-    if (th == 0 || !same_line) {
-      t.line[0].mt = T.mt[th]; t.line[0].mGt = T.mGt[th];
-      t.run(&st);
-#pragma unroll
-      for (int iv = 0; iv < 2; ++iv) { A12[0][iv] = st.a0[0][iv]; A12[1][iv] = st.a1[0][iv]; A21[0][iv] = st.a0[1][iv]; A21[1][iv] = st.a1[1][iv]; }
-    }
+    if (th == 0 || !same_line)
+      two_source_line<R>(ubar_t, pt, eg, Kg, Jq, Kq, T.mt[th], T.mGt[th], vtb, A12, A21);
     const R kq = R(T.kq[th]);
     RC s = RC(0);
 #pragma unroll
