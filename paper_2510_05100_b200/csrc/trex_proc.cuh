@@ -166,15 +166,6 @@ TREX_HD void ttng_unit(const double* __restrict__ mom, long n, long e, int gh, i
 // of the light line that has radiated the gluon at its row / column end. C = [[12,0,4,4],[0,12,4,4],[4,4,12,0],[4,4,0,12]].
 struct QLineLegs { int lrow, lcol, lg; };   // leg numbers; legs 0,1 are incoming
 
-template <class R> struct QqLeafStore {
-  cx<R> a0[2][2], a1[2][2];   // [leaf][v]
-  spinor<R> v[2];
-  template <int LEAF> TREX_HD void put(const spinor<R>* b0, const spinor<R>* b1) { (*this)(LEAF, b0, b1); }
-  TREX_HD void operator()(int leaf, const spinor<R>* b0, const spinor<R>* b1) {
-#pragma unroll
-    for (int iv = 0; iv < 2; ++iv) { a0[leaf][iv] = row_col(b0[0], v[iv]); a1[leaf][iv] = row_col(b1[0], v[iv]); }
-  }
-};
 
 // Top line with TWO ordered sources (currents e1, e2 with momenta K1, K2 flowing into the line): the two orderings
 // A(1,2), A(2,1), each as (order 0, order 1 in kappa) for both antitop helicities: A12[order][v], A21[order][v].
@@ -294,54 +285,6 @@ TREX_HD void qq_close(const vec4<R>& eg, const rvec4<double>& Kg, const vec4<R>&
     res[th] = s;
   }
   out[0] = res[0]; out[1] = res[1];
-}
-
-// unit = (lam_row, lam_col, lam_g, lam_t) packed in 4 bits of `u` (bit0 row, bit1 col, bit2 gluon, bit3 top)
-template <class R, class RC>
-TREX_HD void qq_unit(const double* __restrict__ mom, long n, long e, QLineLegs L, int u, const ThetaPair& T, RC out[2]) {
-  const int lam_row = (u & 1) ? 1 : -1, lam_col = (u & 2) ? 1 : -1, lam_g = (u & 4) ? 1 : -1, lam_t = (u & 8) ? 1 : -1;
-  double pr[4], pc[4], pg[4], pt[4], ptb[4];
-  load_leg<double>(mom, n, e, L.lrow, pr); load_leg<double>(mom, n, e, L.lcol, pc); load_leg<double>(mom, n, e, L.lg, pg);
-  load_leg<double>(mom, n, e, 2, pt); load_leg<double>(mom, n, e, 3, ptb);
-  const bool row_in = L.lrow < 2, col_in = L.lcol < 2, g_in = L.lg < 2;
-  // light line ends: row = vbar (incoming antiquark) or ubar (outgoing quark); column = u (incoming) or v (outgoing)
-  spinor<R> w = cast<R>(row_in ? bar(spinor_v<double>(pr, lam_row, true)) : bar(spinor_u<double>(pr, lam_row, true)));
-  spinor<R> x = cast<R>(col_in ? spinor_u<double>(pc, lam_col, true) : spinor_v<double>(pc, lam_col, true));
-  rvec4<double> Kr, Kc, Kg, Kq;
-#pragma unroll
-  for (int mu = 0; mu < 4; ++mu) {
-    Kr.c[mu] = row_in ? pr[mu] : -pr[mu]; Kc.c[mu] = col_in ? pc[mu] : -pc[mu]; Kg.c[mu] = g_in ? pg[mu] : -pg[mu];
-    Kq.c[mu] = Kr.c[mu] + Kc.c[mu];
-  }
-  vec4<R> eg = cast<R>(polvec<double>(pg, lam_g, !g_in));
-  // quark-pair current  Jq = (w gamma^mu x) / Kq^2        [ (i g_s) * (-i / Kq^2) at g_s = 1 ]
-  vec4<R> Jq = bilinear(w, x);
-  { R s = R(1.0 / rdot(Kq, Kq));
-#pragma unroll
-    for (int i = 0; i < 4; ++i) Jq.c[i] = Jq.c[i] * s; }
-  // light line after radiating the gluon: W = w (i eslash)(i qslash)/q^2, q = -(Kr + Kg);  X = (i qslash)(i eslash) x / q^2, q = Kc + Kg
-  rvec4<double> Ptot = radd(Kq, Kg);
-  const double iP2 = 1.0 / rdot(Ptot, Ptot);
-  vec4<R> Jq3, Jq4;
-  { rvec4<double> q; for (int mu = 0; mu < 4; ++mu) q.c[mu] = -(Kr.c[mu] + Kg.c[mu]);
-    spinor<R> W = row_slash(row_slash(w, eg), cast<R>(q));
-    R s = R(-iP2 / rdot(q, q));
-    Jq3 = bilinear(W, x);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) Jq3.c[i] = Jq3.c[i] * s; }
-  { rvec4<double> q = radd(Kc, Kg);
-    spinor<R> X = slash_col(cast<R>(q), slash_col(eg, x));
-    R s = R(-iP2 / rdot(q, q));
-    Jq4 = bilinear(w, X);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) Jq4.c[i] = Jq4.c[i] * s; }
-
-  spinor<R> vtb[2] = {cast<R>(spinor_v<double>(ptb, -1, false)), cast<R>(spinor_v<double>(ptb, +1, false))};
-  spinor<R> ubar_t = cast<R>(bar(spinor_u<double>(pt, lam_t, false)));
-  rvec4<double> ptv;
-#pragma unroll
-  for (int mu = 0; mu < 4; ++mu) ptv.c[mu] = pt[mu];
-  qq_close<R, RC>(eg, Kg, Jq, Kq, Jq3, Jq4, Ptot, ubar_t, vtb, ptv, T, out);
 }
 
 // ---------------------------------------------------------------- e- e+ -> mu- mu+ (photon + Z), all 16 helicities
