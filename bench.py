@@ -26,6 +26,8 @@ from trex_inputs import make_config  # noqa: E402
 METRIC = "reweighted events/s (old+new |M|^2)"
 UNIT = "events/s"
 HEADLINE_CFG = 2
+HEADLINE_WORKLOAD = ("cfg2 gg->tt~ (+c_tG 0->0.5), 65536 seeded massive-RAMBO events per GPU "
+                     "(BASELINE.json configs[1]); inputs resident in HBM")
 
 # Algorithmic FP64 work per reweighted event of the dominant kernel of each config: thread-level DFMA/DMUL/DADD counted
 # by ncu (smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on.sum; DFMA = 2 flop) on the committed kernels,
@@ -139,7 +141,8 @@ def run_reference(args):
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": len(vals),
                       "warmup": args.warmup, "ms_per_step": 1e3 * n / v, "higher_is_better": True, "scaling": "weak",
                       "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": "cfg2 gg->tt~ (+c_tG 0->0.5), 65536 seeded RAMBO events (BASELINE.json configs[1])"},
+                      "config": {"workload": HEADLINE_WORKLOAD, "events_per_gpu": n,
+                                 "sample": "each step = the oracle on the whole 65536-event sample for a bounded time"},
                       "cpu_baseline": cb,
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
@@ -333,8 +336,7 @@ def main():
         line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": "cfg2 gg->tt~ (+c_tG 0->0.5), 65536 seeded massive-RAMBO events per GPU "
-                                       "(BASELINE.json configs[1]); inputs resident in HBM",
+                "config": {"workload": HEADLINE_WORKLOAD,
                            "l2": "256 MiB buffer written between timed iterations (L2 flush)",
                            "events_per_gpu": head["events"]},
                 "clocks": clocks, "e2e": head["e2e"], "gpu_launches": head["gpu_launches"],
