@@ -39,6 +39,8 @@ __global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(con
   constexpr int NW = TREX_GGTT_NW;                            // warps per block: 8 (one unit each) or 4 (two units each)
   __shared__ double wf[8][8][32];
   __shared__ double red[2][NW][32];
+  extern __shared__ __align__(16) double u1t_raw[];              // [8][16][32]: line state after ONE gluon, see phase A2
+  double (*u1t)[16][32] = reinterpret_cast<double (*)[16][32]>(u1t_raw);
   const EvIO io = resolve_io(a);
   if ((long)blockIdx.x * 32 >= io.n) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -61,6 +63,43 @@ __global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(con
       const spinor<double> w = leg == 2 ? bar(spinor_u<double>(p, lam, false)) : spinor_v<double>(p, lam, false);
 #pragma unroll
       for (int i = 0; i < 4; ++i) { wf[item][2 * i][lane] = w.c[i].re; wf[item][2 * i + 1][lane] = w.c[i].im; }
+    }
+  }
+  __syncthreads();
+  // ---- phase A2: U(a) = ubar Gamma(eps_a) S(p_t - K_a) depends on (gluon a, its helicity, lambda_t) only: 8 states per
+  // event where the 8 units x 2 orderings would form 16; one per warp, parked in shared memory
+  for (int item = warp; item < 8; item += NW) {
+    const int ga = item >> 2, ha = (item >> 1) & 1, lt = item & 1;
+    vec4<R> ea;
+    spinor<R> ubar;
+    rvec4<double> Ka, pt;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      ea.c[i] = cx<R>(R(wf[2 * ga + ha][2 * i][lane]), R(wf[2 * ga + ha][2 * i + 1][lane]));
+      ubar.c[i] = cx<R>(R(wf[4 + lt][2 * i][lane]), R(wf[4 + lt][2 * i + 1][lane]));
+      Ka.c[i] = pm[ga * 4 + i][lane]; pt.c[i] = pm[8 + i][lane];
+    }
+    spinor<R> c0, c1 = szero<R>();
+    ften<R> F = fzero<R>();
+    wedge_acc(F, cast<R>(Ka), ea);
+    const spinor<R> t0 = row_slash(ubar, ea);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) c0.c[i] = mul_i(t0.c[i]);
+    row_sigma_acc(c1, ubar, F);
+    const rvec4<double> qd = rsub(pt, Ka);
+    const double q2 = rdot(qd, qd);
+    const rvec4<R> q = cast<R>(qd);
+    const cx<double> den(q2 - a.T.mt[0] * a.T.mt[0], a.T.mGt[0]);
+    const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), den));
+    const spinor<R> s0 = row_slash(c0, q), s1 = row_slash(c1, q);
+    const R mtr = R(a.T.mt[0]);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      cx<R> n0 = s0.c[i]; cfma(n0, c0.c[i], mtr);
+      cx<R> n1 = s1.c[i]; cfma(n1, c1.c[i], mtr);
+      const cx<R> o0 = n0 * pr, o1 = n1 * pr;
+      u1t[item][2 * i][lane] = (double)o0.re; u1t[item][2 * i + 1][lane] = (double)o0.im;
+      u1t[item][8 + 2 * i][lane] = (double)o1.re; u1t[item][9 + 2 * i][lane] = (double)o1.im;
     }
   }
   __syncthreads();
@@ -112,35 +151,21 @@ __global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(con
   for (int ord = 0; ord < 2; ++ord) {
     // operands of this ordering (g_a next to the top, then g_b) come from shared memory / L1, not from register arrays
     const int ga = ord, gb = 1 - ord;
-    vec4<R> ea, eb;
-    rvec4<double> Ka, Kb;
+    vec4<R> eb;
+    rvec4<double> Kb;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      ea.c[i] = cx<R>(R(wf[wsel[ga]][2 * i][lane]), R(wf[wsel[ga]][2 * i + 1][lane]));
       eb.c[i] = cx<R>(R(wf[wsel[gb]][2 * i][lane]), R(wf[wsel[gb]][2 * i + 1][lane]));
-      Ka.c[i] = pm[ga * 4 + i][lane]; Kb.c[i] = pm[gb * 4 + i][lane];
+      Kb.c[i] = pm[gb * 4 + i][lane];
     }
-    // U(a) = ubar Gamma(eps_a) S(p_t - K_a)
+    // U(a) from phase A2
     dspinor<R> U1;
     {
-      spinor<R> c0, c1 = szero<R>();
-      ften<R> F = fzero<R>();
-      wedge_acc(F, cast<R>(Ka), ea);
-      const spinor<R> t0 = row_slash(ubar, ea);
-#pragma unroll
-      for (int i = 0; i < 4; ++i) c0.c[i] = mul_i(t0.c[i]);
-      row_sigma_acc(c1, ubar, F);
-      const rvec4<double> qd = rsub(pt, Ka);
-      const double q2 = rdot(qd, qd);
-      const rvec4<R> q = cast<R>(qd);
-      const cx<double> den(q2 - a.T.mt[0] * a.T.mt[0], a.T.mGt[0]);
-      const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), den));
-      const spinor<R> s0 = row_slash(c0, q), s1 = row_slash(c1, q);
+      const int it = (ga << 2) | (((gh >> ga) & 1) << 1) | lt;
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
-        cx<R> n0 = s0.c[i]; cfma(n0, c0.c[i], mt);
-        cx<R> n1 = s1.c[i]; cfma(n1, c1.c[i], mt);
-        U1.o0.c[i] = n0 * pr; U1.o1.c[i] = n1 * pr;
+        U1.o0.c[i] = cx<R>(R(u1t[it][2 * i][lane]), R(u1t[it][2 * i + 1][lane]));
+        U1.o1.c[i] = cx<R>(R(u1t[it][8 + 2 * i][lane]), R(u1t[it][9 + 2 * i][lane]));
       }
     }
     // bracket = +- (tuple term) + U(a) Gamma(eps_b)
@@ -193,7 +218,10 @@ __global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(con
 int TREX_TU_NAME(trex_tu_launch_n, TREX_TU_N, TREX_TU_MODE)(const ReweightArgs& a, int npass, unsigned grid, cudaStream_t s) {
 #if TREX_TU_N == 2
   if (npass == 1) {                                   // equal top mass and width at both parameter points
-    k_gg_tt<TuR, TuRC><<<grid, 32 * TREX_GGTT_NW, 0, s>>>(a);
+    constexpr int kU1Bytes = 8 * 16 * 32 * (int)sizeof(double);
+    static bool configured = false;
+    if (!configured) { cudaFuncSetAttribute(k_gg_tt<TuR, TuRC>, cudaFuncAttributeMaxDynamicSharedMemorySize, kU1Bytes); configured = true; }
+    k_gg_tt<TuR, TuRC><<<grid, 32 * TREX_GGTT_NW, kU1Bytes, s>>>(a);
     return (int)cudaGetLastError();
   }
 #endif
