@@ -311,7 +311,7 @@ template <int N> struct UTabIdx {
 template <class R, int N, int NFIX, int D, class Sink, int UT = 0, int STOP = 0> struct TabWalk {
   using I = TabIdx<N, NFIX>;
   static constexpr int NE = I::NE;
-  static_assert(UT == 0 || (NFIX == 0 && UT <= 2), "line-state tables: all helicities free, prefixes of length <= 2");
+  static_assert(UT <= 1 || (NFIX == 0 && UT == 2), "line-state tables: prefixes of length 1, or 2 with all helicities free");
   const R* tab; const int* off; const rvec4<double>* pset;
   R* utab; int nut, ubase, lt;        // line-state table (UT > 0 or STOP > 0)
   rvec4<double> pt;
@@ -328,7 +328,7 @@ template <class R, int N, int NFIX, int D, class Sink, int UT = 0, int STOP = 0>
   Sink* sink;
 
   template <int A> TREX_HD int uindex() const {
-    if constexpr (A == 1) return ubase + UTabIdx<N>::level1(s[0], cb, lt);
+    if constexpr (A == 1) return ubase + UTabIdx<N>::level1(s[0], fpos[1] ? cb : 0u, lt);   // a fixed helicity has no bit in cb
     else return ubase + UTabIdx<N>::level2(s[0], s[1], cb, lt);
   }
   // line state after the first A gluons: private, or from the per-event table

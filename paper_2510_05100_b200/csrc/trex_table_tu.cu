@@ -35,7 +35,7 @@ namespace {
 #define TREX_T3_MINB 3
 #endif
 #ifndef TREX_T3_UT
-#define TREX_T3_UT 0
+#define TREX_T3_UT 1
 #endif
 #ifndef TREX_T5_DMMA
 #define TREX_T5_DMMA 1
@@ -55,7 +55,7 @@ namespace {
 // UT: the top-line states of ordering prefixes up to this length are tabulated per event instead of being carried by
 // every walk thread (fewer registers per thread -> more warps, and no recomputation across tasks)
 template <int N> struct TabCfg;
-template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = TREX_T3_UT ? 3 : 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB, UT = TREX_T3_UT; };
+template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = TREX_T3_UT == 2 ? 3 : 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB, UT = TREX_T3_UT; };
 template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = TREX_T4_UT ? 4 : 2, TB = TREX_T4_TB, EPB = 1, MINB = TREX_T4_MINB, UT = TREX_T4_UT; };
 template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1, UT = 0; };
 
@@ -72,7 +72,7 @@ template <class R, class RC, int N> struct TabGeom {
   using Cfg = TabCfg<N>;
   using I = TabIdx<N, Cfg::NFIX>;
   static constexpr int NFIX = Cfg::NFIX, D = Cfg::D, TB = Cfg::TB, EPB = Cfg::EPB, GS = TB / EPB, UT = Cfg::UT;
-  static constexpr int NU = UTabIdx<N>::NU, NUT = 2 * NU;    // line-state table entries per parameter point / in all
+  static constexpr int NU = UTabIdx<N>::N1 + (UT == 2 ? UTabIdx<N>::N2 : 0), NUT = 2 * NU;   // line-state table entries per parameter point / in all
   static_assert(GS * EPB == TB && (GS == TB || GS == 32), "an event group is one warp or the whole block");
   static constexpr int NE = I::NE;
   static constexpr int NC = I::falling(N, N);
@@ -145,7 +145,11 @@ __device__ __forceinline__ void build_ustate(unsigned char* sb, const int* meta,
   NoSink none;
   const int lt = item & 1;
   unsigned bits;
-  if constexpr (L == 1) { bits = (item >> 1) & 1u; w.pref[0] = item >> 2; w.hfree = bits << w.pref[0]; }
+  if constexpr (L == 1) {
+    bits = (item >> 1) & 1u; w.pref[0] = item >> 2;
+    if (w.pref[0] < G::NFIX && bits) return;                 // a fixed helicity has one state per iteration
+    w.hfree = w.pref[0] >= G::NFIX ? bits << (w.pref[0] - G::NFIX) : 0u;
+  }
   else {
     bits = (item >> 1) & 3u;
     const int pr = item >> 3, g1 = pr / (N - 1), r = pr - g1 * (N - 1), g2 = r + (r >= g1 ? 1 : 0);
