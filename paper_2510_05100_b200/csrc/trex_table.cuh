@@ -299,11 +299,18 @@ TREX_HD void tab_build_level1(R* __restrict__ tab, const int* __restrict__ meta,
 // the ordering nor on the other helicities; they are tabulated once per event and parameter point (utab, built by
 // walks with STOP = 1 .. UT that store U[STOP] instead of descending) and the walk starts at level UT + 1.
 //   utab[comp * nut + ubase + index], comp = (order 0 / 1, spinor component, re / im) = 0..15
-//   index level 1: (g1 * 2 + hel) * 2 + lt;   level 2: 4 N + ((rank of (g1,g2) among ordered pairs) * 4 + hels) * 2 + lt
-template <int N> struct UTabIdx {
-  static constexpr int N1 = 4 * N, N2 = 8 * N * (N - 1), NU = N1 + N2;
-  TREX_HD static int level1(int g1, unsigned bits, int lt) { return (g1 * 2 + (int)(bits & 1u)) * 2 + lt; }
-  TREX_HD static int level2(int g1, int g2, unsigned bits, int lt) {
+//   index level 1: (state of (g1, hel)) * 2 + lt;   level 2: N1 + ((rank of (g1,g2) among ordered pairs) * 4 + hels) * 2 + lt
+template <int N, int NFIX> struct UTabIdx {
+  // level 1: one state per (gluon, helicity, lt); a gluon whose helicity the outer loop fixes has one helicity per iteration
+  static constexpr int N1 = 2 * (NFIX + 2 * (N - NFIX)), N2 = 8 * N * (N - 1), NU = N1 + N2;
+  TREX_HD static int level1(int g1, unsigned bits, int lt) {
+    return (g1 < NFIX ? g1 : NFIX + 2 * (g1 - NFIX) + (int)(bits & 1u)) * 2 + lt;
+  }
+  // inverse of level1 >> 1
+  TREX_HD static void level1_decode(int idx, int& g1, unsigned& bit) {
+    if (idx < NFIX) { g1 = idx; bit = 0u; } else { g1 = NFIX + ((idx - NFIX) >> 1); bit = (unsigned)((idx - NFIX) & 1); }
+  }
+  TREX_HD static int level2(int g1, int g2, unsigned bits, int lt) {     // NFIX = 0 only
     return N1 + ((g1 * (N - 1) + g2 - (g2 > g1 ? 1 : 0)) * 4 + (int)(bits & 3u)) * 2 + lt;
   }
 };
@@ -328,8 +335,8 @@ template <class R, int N, int NFIX, int D, class Sink, int UT = 0, int STOP = 0>
   Sink* sink;
 
   template <int A> TREX_HD int uindex() const {
-    if constexpr (A == 1) return ubase + UTabIdx<N>::level1(s[0], fpos[1] ? cb : 0u, lt);   // a fixed helicity has no bit in cb
-    else return ubase + UTabIdx<N>::level2(s[0], s[1], cb, lt);
+    if constexpr (A == 1) return ubase + UTabIdx<N, NFIX>::level1(s[0], fpos[1] ? cb : 0u, lt);   // a fixed helicity has no bit in cb
+    else return ubase + UTabIdx<N, NFIX>::level2(s[0], s[1], cb, lt);
   }
   // line state after the first A gluons: private, or from the per-event table
   template <int A> TREX_HD dspinor<R> state() const {

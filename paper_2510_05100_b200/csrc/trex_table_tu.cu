@@ -37,6 +37,9 @@ namespace {
 #ifndef TREX_T3_UT
 #define TREX_T3_UT 1
 #endif
+#ifndef TREX_T5_UT
+#define TREX_T5_UT 1
+#endif
 #ifndef TREX_T5_DMMA
 #define TREX_T5_DMMA 1
 #endif
@@ -57,7 +60,7 @@ namespace {
 template <int N> struct TabCfg;
 template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = TREX_T3_UT == 2 ? 3 : 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB, UT = TREX_T3_UT; };
 template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = TREX_T4_UT ? 4 : 2, TB = TREX_T4_TB, EPB = 1, MINB = TREX_T4_MINB, UT = TREX_T4_UT; };
-template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1, UT = 0; };
+template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1, UT = TREX_T5_UT; };
 
 template <int NC> struct FoldedC {
   // C'(i,j) = 0 (j < i), C_ii (j == i), 2 C_ij (j > i), stored by rows i for j >= RB floor(i/RB)
@@ -72,7 +75,8 @@ template <class R, class RC, int N> struct TabGeom {
   using Cfg = TabCfg<N>;
   using I = TabIdx<N, Cfg::NFIX>;
   static constexpr int NFIX = Cfg::NFIX, D = Cfg::D, TB = Cfg::TB, EPB = Cfg::EPB, GS = TB / EPB, UT = Cfg::UT;
-  static constexpr int NU = UTabIdx<N>::N1 + (UT == 2 ? UTabIdx<N>::N2 : 0), NUT = 2 * NU;   // line-state table entries per parameter point / in all
+  using UI = UTabIdx<N, Cfg::NFIX>;
+  static constexpr int NU = UI::N1 + (UT == 2 ? UI::N2 : 0), NUT = 2 * NU;   // line-state table entries per parameter point / in all
   static_assert(GS * EPB == TB && (GS == TB || GS == 32), "an event group is one warp or the whole block");
   static constexpr int NE = I::NE;
   static constexpr int NC = I::falling(N, N);
@@ -103,6 +107,7 @@ template <class R, class RC, int N> struct TabGeom {
   static constexpr size_t o_c = slot * EPB;
   static constexpr size_t o_meta = o_c + al(sizeof(RC) * FoldedC<NC>::size());
   static constexpr size_t bytes = o_meta + al(sizeof(int) * I::M_SIZE);
+  static_assert(bytes <= 232448, "one SM has 227 KB of shared memory");
 };
 
 // leaf sink of the walk: x_sigma = A0 + (kappa/g_s) A1 for both antitop helicities -> X tile
@@ -146,8 +151,7 @@ __device__ __forceinline__ void build_ustate(unsigned char* sb, const int* meta,
   const int lt = item & 1;
   unsigned bits;
   if constexpr (L == 1) {
-    bits = (item >> 1) & 1u; w.pref[0] = item >> 2;
-    if (w.pref[0] < G::NFIX && bits) return;                 // a fixed helicity has one state per iteration
+    G::UI::level1_decode(item >> 1, w.pref[0], bits);
     w.hfree = w.pref[0] >= G::NFIX ? bits << (w.pref[0] - G::NFIX) : 0u;
   }
   else {
@@ -175,7 +179,7 @@ __device__ __forceinline__ void build_levels(unsigned char* sb, const int* meta,
     const int e0 = meta[I::M_LVL + K], ntab = meta[I::M_LVL + K + 1] - e0;
     // the line states of the prefixes of length K - 1 need the table levels < K and the states of length K - 2: same phase
     constexpr int L = K - 1;
-    constexpr int nus = L <= G::UT ? (L == 1 ? UTabIdx<N>::N1 : UTabIdx<N>::N2) : 0;
+    constexpr int nus = L <= G::UT ? (L == 1 ? G::UI::N1 : G::UI::N2) : 0;
     for (int it = gtid; it < ntab + nus * NPASS; it += G::GS) {
       if (it < ntab) {
         tab_build_entry<R, N, G::NFIX, K>(reinterpret_cast<R*>(sb + G::o_tab), meta, reinterpret_cast<const rvec4<double>*>(sb + G::o_pset), e0 + it);
