@@ -145,11 +145,6 @@ int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_soa, int64_t 
 int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
                   const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
 
-/* Diagnostic: per-helicity colour-flow amplitudes J_c of ONE event (momenta_one: HOST [npar][4]), for parity at the
- * level of SURVEY.md I-4. out HOST [nhel][ncolor][2 orders in kappa][re,im], couplings included, order 1 per unit
- * kappa. Only for TREX_SP_GG_TT .. TREX_SP_GG_TTGGG. Synchronous. */
-int trex_debug_flow_amps(int subproc_id, const double* momenta_one, const double* theta, double* out);
-
 /* ---- reweighted cross section and propagated error:
  *   sigma' = C sum_i w'_i                                                  eq.(6)
  *   Delta sigma' = Delta sigma (1/N) sum_i w'_i / w_i + sigma std(w')      eq.(7), population standard deviation;
@@ -164,24 +159,11 @@ int trex_debug_flow_amps(int subproc_id, const double* momenta_one, const double
 int trex_xsec_moments(const double* w_in, const double* w_out, int64_t n, double* moments);
 int trex_xsec_finish(const double* moments, int nparts, double C, double sigma, double dsigma, double* out);
 
-/* Roofline denominator: enqueues ONE launch of a register-resident FMA chain kernel (blocks x 256 threads, 64 FMAs per
- * thread and iteration) on the library stream and returns the floating-point operations it executes (2 per FMA), or a
- * negative error code. fp32 != 0 exercises the FP32 pipe instead of the FP64 pipe. The caller times it with events
- * on that stream (no FP64 peak is provided, it has to be measured in the same run). */
-double trex_probe_fma(int fp32, int blocks, int iters);
-
 int trex_set_stream(void* cuda_stream);
 int trex_set_precision(int mode);      /* 0 = fp64 (default), 1 = mixed (amplitudes fp64, colour sum fp32,
                                           PAPER.md:1209 fptype m), 2 = fp32 */
 int trex_get_precision(void);
 int trex_set_poly_multi(int on);         /* 1 (default): trex_run_multi may use its polynomial path */
-/* Evaluation strategy of g g -> t t~ + (N-2) g: processes with N >= algo gluons (algo = 3, 4, 5; default 3) use the
- * fused current-table kernel (per-event shared-memory table of off-shell gluon currents shared by all helicities,
- * "helicity recycling"); the others, and all of them for algo = 0, use one thread per helicity unit walking every
- * ordering with private currents. Both evaluate the same colour-ordered recursion. */
-int trex_set_algorithm(int algo);
-/* kernels launched by this library since load (for bench.py's gpu_launches) */
-int64_t trex_launch_count(void);
 const char* trex_last_error(void);
 void trex_shutdown(void);
 

@@ -1,0 +1,49 @@
+/* rex_trex_diag.h -- diagnostics of librex_trex.so: probes, counters, kernel-selection knobs and per-flow dumps.
+ *
+ * NOT part of the product boundary (include/rex_trex.h is: SURVEY.md 8(b)). These entry points exist for tests/,
+ * bench.py's roofline denominator and profiles/; a user of the reweighting path never needs them.
+ */
+#ifndef REX_TREX_DIAG_H
+#define REX_TREX_DIAG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Per-helicity colour-flow amplitudes J_c of ONE event from the first-path walker (one thread per helicity walking
+ * every ordering with private currents; momenta_one: HOST [npar][4]), for parity at the level of SURVEY.md I-4.
+ * out HOST [nhel][ncolor][2 orders in kappa][re,im], couplings included, order 1 per unit kappa.
+ * Only for TREX_SP_GG_TT .. TREX_SP_GG_TTGGG. Synchronous. */
+int trex_debug_flow_amps(int subproc_id, const double* momenta_one, const double* theta, double* out);
+
+/* Roofline denominator: enqueues ONE launch of a register-resident FMA chain kernel (blocks x 256 threads, 64 FMAs per
+ * thread and iteration) on the library stream and returns the floating-point operations it executes (2 per FMA), or a
+ * negative error code. mode 0 / 1: FP64 / FP32 chains with two constant-bank operands (pipe peak); 2 / 3: three
+ * register operands; 4: FP64 tensor cores (mma.sync.m8n8k4.f64). The caller times it with events on that stream
+ * (no FP64 peak is provided, it has to be measured in the same run). */
+double trex_probe_fma(int mode, int blocks, int iters);
+
+/* Evaluation strategy of g g -> t t~ + (N-2) g: processes with N >= algo gluons (algo = 3, 4, 5; default 3) use the
+ * fused current-table kernel (per-event shared-memory table of off-shell gluon currents shared by all helicities,
+ * "helicity recycling"); the others, and all of them for algo = 0, use one thread per helicity unit walking every
+ * ordering with private currents. Both evaluate the same colour-ordered recursion; the second one is
+ * kept as an in-library cross-check of the first. */
+int trex_set_algorithm(int algo);
+
+/* kernels launched by this library since load (bench.py's gpu_launches) */
+int64_t trex_launch_count(void);
+/* trex_run calls served by replaying the captured CUDA graph since load (tests assert the replay branch was taken) */
+int64_t trex_graph_replays(void);
+
+/* Kernel timing for bench.py's roofline: while on, every |M|^2 launch (inside trex_reweight, trex_run, ...) is bracketed by
+ * CUDA events on the library stream and trex_run does not replay its CUDA graph. trex_kernel_time synchronises the
+ * stream, returns the summed duration [ms] and the number of launches recorded since its last call, and resets both. */
+int trex_kernel_timing(int on);
+int trex_kernel_time(double* total_ms, int64_t* launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* REX_TREX_DIAG_H */

@@ -50,6 +50,9 @@ _SIGNATURES = {
     "trex_set_poly_multi": (_int, [_int]),
     "trex_set_algorithm": (_int, [_int]),
     "trex_launch_count": (ctypes.c_int64, []),
+    "trex_graph_replays": (ctypes.c_int64, []),
+    "trex_kernel_timing": (_int, [_int]),
+    "trex_kernel_time": (_int, [_dp, ctypes.POINTER(ctypes.c_int64)]),
     "trex_last_error": (ctypes.c_char_p, []),
     "trex_shutdown": (None, []),
 }
@@ -60,7 +63,7 @@ def library_path():
 
 
 def exported_symbols():
-    """Names the binding expects the library to export (one per declaration in include/rex_trex.h)."""
+    """Names the binding expects the library to export (one per declaration in include/rex_trex.h and rex_trex_diag.h)."""
     return sorted(_SIGNATURES)
 
 
@@ -108,6 +111,22 @@ def _theta(th):
     if a.shape != (TREX_NTHETA,):
         raise TrexError("theta must have %d entries" % TREX_NTHETA)
     return a, a.ctypes.data_as(_dp)
+
+
+def _shapes(what, n, momenta_soa=None, keys=None, rows=(), mats=(), K=None):
+    """Every array of a path call must agree with n (and npar): a mismatch would be an out-of-bounds access on the device."""
+    if momenta_soa is not None:
+        sh = tuple(momenta_soa.shape)
+        if len(sh) != 3 or sh[1] != 4 or sh[2] != n or not 1 <= sh[0] <= 7:
+            raise TrexError("%s: momenta_soa must have shape (npar <= 7, 4, %d), got %s" % (what, n, sh))
+    if keys is not None and int(np.prod(keys.shape)) != n:
+        raise TrexError("%s: pdg_keys must have %d entries, got %s" % (what, n, tuple(keys.shape)))
+    for name, t in rows:
+        if t is not None and int(np.prod(t.shape)) != n:
+            raise TrexError("%s: %s must have %d entries, got %s" % (what, name, n, tuple(t.shape)))
+    for name, t in mats:
+        if t is not None and tuple(t.shape) != (K, n):
+            raise TrexError("%s: %s must have shape (%d, %d), got %s" % (what, name, K, n, tuple(t.shape)))
 
 
 # ---------------------------------------------------------------- host helpers
@@ -165,6 +184,21 @@ def trex_get_precision():
 
 def trex_launch_count():
     return int(lib().trex_launch_count())
+
+
+def trex_graph_replays():
+    return int(lib().trex_graph_replays())
+
+
+def trex_kernel_timing(on):
+    return _check(lib().trex_kernel_timing(int(bool(on))), "trex_kernel_timing")
+
+
+def trex_kernel_time():
+    """(summed duration [ms], launches) of the |M|^2 launches recorded since the last call (trex_kernel_timing on)."""
+    ms, cnt = ctypes.c_double(0.0), ctypes.c_int64(0)
+    _check(lib().trex_kernel_time(ctypes.byref(ms), ctypes.byref(cnt)), "trex_kernel_time")
+    return ms.value, cnt.value
 
 
 def trex_last_error():
@@ -231,6 +265,7 @@ def trex_reweight(subproc_id, momenta_soa, theta_old, theta_new, w_in, w_out=Non
         me2_old = torch.empty_like(w_in)
     if want_me2 and me2_new is None:
         me2_new = torch.empty_like(w_in)
+    _shapes("trex_reweight", n, rows=(("w_out", w_out), ("me2_old", me2_old), ("me2_new", me2_new)))
     to, pto = _theta(theta_old)
     tn, ptn = _theta(theta_new)
     f64 = torch.float64
@@ -251,6 +286,7 @@ def trex_run(pdg_keys, momenta_soa, theta_old, theta_new, w_in, w_out=None, me2_
         me2_old = torch.empty_like(w_in)
     if want_me2 and me2_new is None:
         me2_new = torch.empty_like(w_in)
+    _shapes("trex_run", n, momenta_soa, pdg_keys, rows=(("w_out", w_out), ("me2_old", me2_old), ("me2_new", me2_new)))
     to, pto = _theta(theta_old)
     tn, ptn = _theta(theta_new)
     f64 = torch.float64
@@ -283,6 +319,9 @@ def trex_run_pdg(pdg_soa, momenta_soa, n_in, theta_old, theta_new, w_in, w_out=N
         me2_old = torch.empty_like(w_in)
     if want_me2 and me2_new is None:
         me2_new = torch.empty_like(w_in)
+    _shapes("trex_run_pdg", n, momenta_soa, rows=(("w_out", w_out), ("me2_old", me2_old), ("me2_new", me2_new)))
+    if tuple(pdg_soa.shape) != (npar, n):
+        raise TrexError("trex_run_pdg: pdg_soa must have shape (%d, %d), got %s" % (npar, n, tuple(pdg_soa.shape)))
     to, pto = _theta(theta_old)
     tn, ptn = _theta(theta_new)
     f64 = torch.float64
@@ -306,8 +345,7 @@ def trex_run_multi(pdg_keys, momenta_soa, theta_old, thetas_new, w_in, w_out=Non
         me2_old = torch.empty_like(w_in)
     if want_me2 and me2_new is None:
         me2_new = torch.empty((K, n), dtype=torch.float64, device=w_in.device)
-    if tuple(w_out.shape) != (K, n) or (me2_new is not None and tuple(me2_new.shape) != (K, n)):
-        raise TrexError("trex_run_multi: w_out / me2_new must have shape [K, n]")
+    _shapes("trex_run_multi", n, momenta_soa, pdg_keys, rows=(("me2_old", me2_old),), mats=(("w_out", w_out), ("me2_new", me2_new)), K=K)
     to, pto = _theta(theta_old)
     f64 = torch.float64
     nb = _check(lib().trex_run_multi(_dev(pdg_keys, torch.int64, "pdg_keys"), _dev(momenta_soa, f64, "momenta_soa"), n, npar,
@@ -324,8 +362,10 @@ def _host(t, dtype, what):
         if t.dtype != dtype or not t.flags.c_contiguous:
             raise TrexError("%s must be a C-contiguous numpy array of dtype %s" % (what, dtype))
         return ctypes.c_void_p(t.ctypes.data)
-    if t.is_cuda or not t.is_contiguous():
-        raise TrexError("%s must be a contiguous host tensor" % what)
+    import torch
+    want = {np.float64: torch.float64, np.int64: torch.int64, np.uint64: torch.int64}[dtype]
+    if t.is_cuda or not t.is_contiguous() or t.dtype != want:
+        raise TrexError("%s must be a contiguous host tensor of dtype %s" % (what, want))
     return ctypes.c_void_p(t.data_ptr())
 
 
@@ -334,6 +374,7 @@ def trex_run_host(pdg_keys, momenta_soa, theta_old, theta_new, w_in, w_out, me2_
     _torch()
     n = int(np.prod(w_in.shape))
     npar = momenta_soa.shape[0]
+    _shapes("trex_run_host", n, momenta_soa, pdg_keys, rows=(("w_out", w_out), ("me2_old", me2_old), ("me2_new", me2_new)))
     to, pto = _theta(theta_old)
     tn, ptn = _theta(theta_new)
     f64 = np.float64

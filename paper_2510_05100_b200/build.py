@@ -18,7 +18,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 
 
 # headers each source depends on (besides itself)
-_KERNEL_HDRS = ["trex_math.cuh", "trex_ttng.cuh", "trex_proc.cuh", "trex_kernels.cuh", "trex_ctx.h", "../../include/rex_trex.h"]
+_KERNEL_HDRS = ["trex_math.cuh", "trex_ttng.cuh", "trex_proc.cuh", "trex_kernels.cuh", "trex_ctx.h", "../../include/rex_trex.h", "../../include/rex_trex_diag.h"]
 DEPS = {
     "trex_ttng_tu.cu": _KERNEL_HDRS,
     "trex_table_tu.cu": _KERNEL_HDRS + ["trex_table.cuh"],

@@ -407,7 +407,7 @@ __global__ void __launch_bounds__(256) k_keys(const int* __restrict__ pdg, int n
 __global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __restrict__ mom, const double* __restrict__ w_in, long n,
                              int nrows, const int* __restrict__ perm, double* __restrict__ blk, double* __restrict__ res,
                              const signed char* __restrict__ legmap) {
-  if (plan->single) return;
+  if (plan->single || plan->nb == 0) return;         // nb == 0: categorisation failed, perm was never written
   const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   const long p = perm[j];
@@ -425,7 +425,7 @@ __global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __r
 
 __global__ void k_run_scatter(const DevPlan* __restrict__ plan, const double* __restrict__ res, long n, const int* __restrict__ perm,
                               double* __restrict__ w_out, double* __restrict__ me2_old, double* __restrict__ me2_new) {
-  if (plan->single) return;
+  if (plan->single || plan->nb == 0) return;         // nb == 0: categorisation failed, perm was never written
   const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   const long p = perm[j];

@@ -328,6 +328,14 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
   a.T = T; a.sid = sid; a.q = sp->qlegs; a.C120 = c.C120;
   const unsigned grid32 = (unsigned)((nmax + 31) / 32);
   const int mode = c.precision;
+  cudaEvent_t kt[2] = {nullptr, nullptr};
+  if (c.ktiming) {
+    for (int i = 0; i < 2; ++i) {
+      if (!c.kev_pool.empty()) { kt[i] = c.kev_pool.back(); c.kev_pool.pop_back(); }
+      else TREX_CUDA_CHECK(cudaEventCreate(&kt[i]));
+    }
+    TREX_CUDA_CHECK(cudaEventRecord(kt[0], c.stream));
+  }
   if (sid == TREX_SP_EEMUMU) {
     const unsigned grid = (unsigned)((nmax + 127) / 128);
     if (mode == 2) k_eemumu<float><<<grid, 128, 0, c.stream>>>(a);
@@ -348,6 +356,10 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
   }
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());
+  if (c.ktiming) {
+    TREX_CUDA_CHECK(cudaEventRecord(kt[1], c.stream));
+    c.kev.push_back(kt[0]); c.kev.push_back(kt[1]);
+  }
   return 0;
 }
 
@@ -436,10 +448,10 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
   std::memcpy(key.th + TREX_NTHETA, theta_new, sizeof(double) * TREX_NTHETA);
   int64_t offsets[REX_MAX_BUCKETS + 1];
   // (not below trex_run_host: there the launches are issued while the input copies are still in flight, which hides them)
-  const bool may_replay = !c.in_host_run;
+  const bool may_replay = !c.in_host_run && !c.ktiming;
   if (may_replay && c.exec_valid && std::memcmp(&key, &c.exec_key, sizeof key) == 0) {
     TREX_CUDA_CHECK(cudaGraphLaunch(c.run_exec, c.stream));
-    c.launches += c.exec_launches;
+    c.launches += c.exec_launches; c.graph_replays += 1;
     return bucket_finish(offsets);
   }
   if (c.graphs_ok && std::getenv("TREX_NO_GRAPH")) c.graphs_ok = false;
@@ -461,7 +473,7 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
       c.run_exec = exec; c.exec_key = key; c.exec_valid = true; c.exec_launches = nl;
       cudaGraphDestroy(graph);
       TREX_CUDA_CHECK(cudaGraphLaunch(c.run_exec, c.stream));
-      c.launches += nl;
+      c.launches += nl; c.graph_replays += 1;
       return bucket_finish(offsets);
     }
     if (graph) cudaGraphDestroy(graph);
@@ -540,11 +552,10 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
     for (int k = 0; k < ntheta; ++k) u[k] = (kappa_of(theta_new + (size_t)k * TREX_NTHETA) - k0) / delta;
     TREX_CUDA_CHECK(cudaMemcpyAsync(du, u.data(), sizeof(double) * ntheta, cudaMemcpyHostToDevice, c.stream));
     // cudaMemcpyAsync from pageable memory returns after staging the source: u may go out of scope
-    double thp[2][TREX_NTHETA];
-    for (int s2 = 0; s2 < 2; ++s2) {
-      std::memcpy(thp[s2], theta_old, sizeof(double) * TREX_NTHETA);
-      thp[s2][TREX_TH_CTG] = (k0 + (s2 == 0 ? delta : -delta)) * std::sqrt(2.0) * theta_old[TREX_TH_LAMBDA] * theta_old[TREX_TH_LAMBDA] / theta_old[TREX_TH_VEV];
-    }
+    // support points kappa0 +- delta: kappa is carried into the kernel parameters directly (no round trip through c_tG,
+    // which would divide by vev)
+    const double gs0 = std::sqrt(4.0 * 3.14159265358979323846 * theta_old[TREX_TH_ALPHA_S]);
+    if (!std::isfinite(k0) || !std::isfinite(delta)) return fail(TREX_EINVAL, "trex_run_multi: non-finite kappa");
     if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar)) return rc;
     if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm, blk, res)) return rc;
     for (int s2 = 0; s2 < 2; ++s2) {
@@ -553,7 +564,8 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
       for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
         if (subproc_info(sid)->npar != npar) continue;
         ThetaPair Tp;
-        if (!make_theta_pair(sid, theta_old, thp[s2], Tp)) return fail(TREX_EINVAL, "trex_run_multi: theta outside its domain");
+        if (!make_theta_pair(sid, theta_old, theta_old, Tp)) return fail(TREX_EINVAL, "trex_run_multi: theta outside its domain");
+        Tp.kq[1] = gs0 > 0.0 ? (k0 + (s2 == 0 ? delta : -delta)) / gs0 : 0.0;
         ReweightArgs a;
         a.io = EvIO{momenta_soa, (long)n, (long)n, w_in, w_out, mo_out, mn_out};      // w_out row 0 doubles as a dummy here
         a.alt = EvIO{blk, (long)n, (long)n, blk + (size_t)nrows * n, res, res + n, res + 2 * (size_t)n};
@@ -658,6 +670,23 @@ extern "C" int trex_set_algorithm(int algo) {
   ctx().table_min_n = algo == 0 ? 99 : algo; return 0;
 }
 extern "C" int64_t trex_launch_count(void) { return ctx().launches; }
+extern "C" int64_t trex_graph_replays(void) { return ctx().graph_replays; }
+extern "C" int trex_kernel_timing(int on) { ctx().ktiming = on != 0; return 0; }
+extern "C" int trex_kernel_time(double* total_ms, int64_t* launches) {
+  Context& c = ctx();
+  if (!total_ms || !launches) return fail(TREX_EINVAL, "trex_kernel_time: null pointer");
+  TREX_CUDA_CHECK(cudaStreamSynchronize(c.stream));
+  double sum = 0.0;
+  for (size_t i = 0; i + 1 < c.kev.size(); i += 2) {
+    float ms = 0.f;
+    TREX_CUDA_CHECK(cudaEventElapsedTime(&ms, c.kev[i], c.kev[i + 1]));
+    sum += ms;
+  }
+  *total_ms = sum; *launches = (int64_t)(c.kev.size() / 2);
+  c.kev_pool.insert(c.kev_pool.end(), c.kev.begin(), c.kev.end());
+  c.kev.clear();
+  return 0;
+}
 extern "C" const char* trex_last_error(void) { return ctx().err; }
 extern "C" void trex_shutdown(void) {
   Context& c = ctx();
@@ -680,6 +709,9 @@ extern "C" void trex_shutdown(void) {
   if (c.xsec_scratch) cudaFree(c.xsec_scratch);
   if (c.xsec_host) cudaFreeHost(c.xsec_host);
   c.xsec_scratch = c.xsec_host = nullptr;
+  for (cudaEvent_t e : c.kev) cudaEventDestroy(e);
+  for (cudaEvent_t e : c.kev_pool) cudaEventDestroy(e);
+  c.kev.clear(); c.kev_pool.clear();
   if (c.run_exec) cudaGraphExecDestroy(c.run_exec);
   if (c.cap_stream) cudaStreamDestroy(c.cap_stream);
   c.run_exec = nullptr; c.cap_stream = nullptr; c.exec_valid = false; c.last_key_valid = false;

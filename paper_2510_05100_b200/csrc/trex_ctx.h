@@ -5,8 +5,10 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <vector>
 
 #include "../../include/rex_trex.h"
+#include "../../include/rex_trex_diag.h"
 
 namespace trex {
 
@@ -25,6 +27,10 @@ struct Context {
   int table_min_n = 3;               // gluon multiplicities >= this use the fused current-table kernel (trex_set_algorithm)
   int nsm = 0;                       // multiprocessors of the device
   int64_t launches = 0;
+  // diagnostics: CUDA events around every |M|^2 launch (trex_kernel_timing); implies no graph replay
+  bool ktiming = false;
+  std::vector<cudaEvent_t> kev;      // start/stop pairs recorded since the last trex_kernel_time
+  std::vector<cudaEvent_t> kev_pool; // events free for reuse
   char err[512] = {0};
   // rex_bucket scratch (device) and results of the last call (host)
   void* bucket_scratch = nullptr;
@@ -47,7 +53,7 @@ struct Context {
   bool in_host_run = false;
   RunKey last_key{}; bool last_key_valid = false;
   RunKey exec_key{}; bool exec_valid = false; bool graphs_ok = true;
-  cudaGraphExec_t run_exec = nullptr; int64_t exec_launches = 0;
+  cudaGraphExec_t run_exec = nullptr; int64_t exec_launches = 0; int64_t graph_replays = 0;
   cudaStream_t cap_stream = nullptr;
   DevPlan* plan = nullptr;           // device
   void* plan_keys = nullptr;         // device: key, leg count [2 NSUB] and process string [NSUB][8] of every compiled-in subprocess

@@ -55,6 +55,7 @@ inline bool make_theta_pair(int sid, const double* th_old, const double* th_new,
       const double gs = std::sqrt(4.0 * pi * as);
       const double kappa = th[TREX_TH_CTG] * th[TREX_TH_VEV] / (std::sqrt(2.0) * th[TREX_TH_LAMBDA] * th[TREX_TH_LAMBDA]);
       T.mt[k] = th[TREX_TH_MT]; T.mGt[k] = th[TREX_TH_MT] * th[TREX_TH_GAMMAT];
+      if (!std::isfinite(kappa) || !std::isfinite(th[TREX_TH_MT]) || !std::isfinite(th[TREX_TH_GAMMAT])) return false;
       T.kq[k] = gs > 0.0 ? kappa / gs : 0.0;      // alpha_s = 0: pref = 0, so |M|^2 = 0 exactly (zero guard applies)
       T.pref[k] = std::pow(gs, 2 * sp->nvert) / sp->navg;
       T.e2[k] = T.gL[k] = T.gR[k] = T.mZ2[k] = T.mZGZ[k] = 0.0;

@@ -21,10 +21,13 @@ def lib():
     return T.lib()
 
 
-def declared_functions():
-    text = open(os.path.join(ROOT, "include", "rex_trex.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b((?:rex|trex)_[a-z0-9_]+)\s*\(", text)))
+def declared_functions(headers=("rex_trex.h", "rex_trex_diag.h")):
+    names = set()
+    for h in headers:
+        text = open(os.path.join(ROOT, "include", h)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names |= set(re.findall(r"\b((?:rex|trex)_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_every_declared_symbol_is_exported_and_bound(lib):
@@ -36,8 +39,18 @@ def test_every_declared_symbol_is_exported_and_bound(lib):
 
 
 def test_no_torch_types_in_signatures():
-    text = open(os.path.join(ROOT, "include", "rex_trex.h")).read()
-    assert "torch" not in text and "at::" not in text and 'extern "C"' in text
+    for h in ("rex_trex.h", "rex_trex_diag.h"):
+        text = open(os.path.join(ROOT, "include", h)).read()
+        assert "torch" not in text and "at::" not in text and 'extern "C"' in text
+
+
+def test_product_header_carries_no_diagnostics():
+    """Probes, counters, debug dumps and kernel-selection knobs live in rex_trex_diag.h, not in the boundary."""
+    prod = declared_functions(("rex_trex.h",))
+    for name in ("trex_debug_flow_amps", "trex_probe_fma", "trex_launch_count", "trex_set_algorithm", "trex_graph_replays"):
+        assert name not in prod and name in declared_functions(("rex_trex_diag.h",))
+    for name in ("rex_bucket", "rex_gather", "trex_reweight", "trex_run", "trex_subproc_id", "rex_pack_key"):
+        assert name in prod
 
 
 def test_pack_key_matches_input_generator_and_alg1_semantics(lib):

@@ -1,0 +1,226 @@
+"""Host-visible behaviour of the CUDA path beyond plain parity (-m gpu): CUDA-graph replay, user streams, failure paths
+that must not touch memory, and all-event cross-checks between the kernel families at bench-like sizes."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from trex_inputs import make_config, REX_NPOS
+
+pytestmark = pytest.mark.gpu
+
+RTOL64 = 1e-11
+
+
+@pytest.fixture(scope="module")
+def T():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2510_05100_b200 as T
+    T.lib()
+    T.trex_set_stream(None)
+    T.trex_set_precision(0)
+    return T
+
+
+def dev(a):
+    import torch
+    a = np.ascontiguousarray(a)
+    if a.dtype == np.uint64:
+        a = a.view(np.int64)
+    return torch.from_numpy(a).cuda()
+
+
+def rel(a, b):
+    return np.abs(a - b) / np.abs(b)
+
+
+@pytest.mark.parametrize("cfg,n", [(3, 30011), (2, 65536), (3, 5000)])
+def test_graph_replay_is_taken_and_bit_equal(T, cfg, n):
+    """trex_run with the SAME buffers, sizes and parameter points replays the captured CUDA graph (the configuration
+    bench.py times): the replay must really be taken and give the bits of the plain launches."""
+    import torch
+    w = make_config(cfg, n=n)
+    keys = w.keys.copy()
+    if cfg == 3:
+        keys[5::131] = np.uint64(REX_NPOS)
+    dk, dm, dw = dev(keys), dev(w.momenta), dev(w.w_in)
+    first = T.trex_run(dk, dm, w.theta_old, w.theta_new, dw)                    # fresh outputs: plain launches
+    torch.cuda.synchronize()
+    ref = [x.clone() for x in first[:3]]
+    wo, mo, mn = (torch.full_like(dw, -1.0) for _ in range(3))
+    r0 = T.trex_graph_replays()
+    for it in range(4):
+        wo.fill_(-1.0); mo.fill_(-1.0); mn.fill_(-1.0)
+        _, _, _, nb = T.trex_run(dk, dm, w.theta_old, w.theta_new, dw, w_out=wo, me2_old=mo, me2_new=mn)
+        torch.cuda.synchronize()
+        assert nb == first[3]
+        assert torch.equal(wo, ref[0]) and torch.equal(mo, ref[1]) and torch.equal(mn, ref[2]), it
+    assert T.trex_graph_replays() - r0 >= 2                                      # call 2 captures + replays, 3 and 4 replay
+    # a changed size or parameter point must not replay the stale graph
+    r1 = T.trex_graph_replays()
+    m = n - 17
+    dk2, dm2, dw2 = dev(keys[:m]), dev(np.ascontiguousarray(w.momenta[:, :, :m])), dev(w.w_in[:m])
+    out2 = T.trex_run(dk2, dm2, w.theta_old, w.theta_new, dw2)
+    torch.cuda.synchronize()
+    assert T.trex_graph_replays() == r1
+    # (bucket order may differ for the prefix; compare per event)
+    assert torch.equal(out2[0], ref[0][:m])
+    th2 = w.theta_new.copy(); th2[7] = 0.77
+    out3 = T.trex_run(dk, dm, w.theta_old, th2, dw, w_out=wo, me2_old=mo, me2_new=mn)
+    torch.cuda.synchronize()
+    assert T.trex_graph_replays() == r1 and not torch.equal(wo, ref[0])
+    sp = w.classes[0]
+    idx = np.where(keys == sp.key)[0][:5]
+    rw, _, _ = O.reweight(sp.sid, np.ascontiguousarray(w.momenta[:, :, idx]), w.theta_old, th2, w.w_in[idx])
+    assert rel(wo.cpu().numpy()[idx], rw).max() < RTOL64
+
+
+def test_user_stream_including_graph_replay(T):
+    """The library enqueues on the stream given to trex_set_stream; the graph is captured on a private stream and
+    replayed on the user's."""
+    import torch
+    w = make_config(3, n=20000)
+    dk, dm, dw = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    ref = T.trex_run(dk, dm, w.theta_old, w.theta_new, dw)
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    wo, mo, mn = (torch.empty_like(dw) for _ in range(3))
+    T.trex_set_stream(s)
+    try:
+        r0 = T.trex_graph_replays()
+        with torch.cuda.stream(s):
+            for it in range(4):
+                wo.fill_(-1.0)
+                T.trex_run(dk, dm, w.theta_old, w.theta_new, dw, w_out=wo, me2_old=mo, me2_new=mn)
+                s.synchronize()
+                assert torch.equal(wo, ref[0]) and torch.equal(mn, ref[2]), it
+            assert T.trex_graph_replays() - r0 >= 2
+            # per-class call and the bucketing alone on the same stream
+            sel = np.where(w.keys == w.classes[0].key)[0]
+            o = T.trex_reweight(w.classes[0].sid, dev(np.ascontiguousarray(w.momenta[:, :, sel])), w.theta_old, w.theta_new,
+                                dev(w.w_in[sel]))
+            s.synchronize()
+            assert np.array_equal(o[0].cpu().numpy(), ref[0].cpu().numpy()[sel])
+            perm, offsets, _ = T.rex_bucket(dk)
+            rperm, roff, _ = O.bucket(w.keys)
+            assert np.array_equal(perm.cpu().numpy(), rperm) and np.array_equal(offsets, roff)
+    finally:
+        T.trex_set_stream(None)
+    again = T.trex_run(dk, dm, w.theta_old, w.theta_new, dw)
+    torch.cuda.synchronize()
+    assert torch.equal(again[0], ref[0])
+
+
+@pytest.mark.parametrize("n", [3000, 9000, 40000])
+def test_too_many_classes_after_a_larger_run_touches_no_memory(T, n):
+    """More than REX_MAX_BUCKETS keys: the categorisation fails on the device, so no permutation exists. The rest of the
+    already enqueued chain (transposition, |M|^2 kernels, transposition back) must then do nothing -- in particular not
+    gather / scatter through the stale permutation a larger earlier run left in the scratch buffer."""
+    import torch
+    big = make_config(3, n=120000)
+    T.trex_run(dev(big.keys), dev(big.momenta), big.theta_old, big.theta_new, dev(big.w_in))    # leaves indices up to 119999
+    torch.cuda.synchronize()
+    w = make_config(3, n=n)
+    keys = w.keys.copy()
+    keys[: T.REX_MAX_BUCKETS + 5] = np.arange(1, T.REX_MAX_BUCKETS + 6, dtype=np.uint64) * np.uint64(1000003)
+    pad = 4096
+    buf = torch.full((3 * n + 4 * pad,), -7.0, dtype=torch.float64, device="cuda")      # canaries around and between
+    wo = buf[pad:pad + n]
+    mo = buf[2 * pad + n:2 * pad + 2 * n]
+    mn = buf[3 * pad + 2 * n:3 * pad + 3 * n]
+    dm, dw = dev(w.momenta), dev(w.w_in)
+    with pytest.raises(T.TrexError):
+        T.trex_run(dev(keys), dm, w.theta_old, w.theta_new, dw, w_out=wo, me2_old=mo, me2_new=mn)
+    torch.cuda.synchronize()
+    assert bool((buf == -7.0).all())
+    th = np.tile(w.theta_new, (5, 1)); th[:, 7] = np.linspace(-1, 1, 5)
+    buf2 = torch.full((5 * n + 2 * pad,), -7.0, dtype=torch.float64, device="cuda")
+    with pytest.raises(T.TrexError):
+        T.trex_run_multi(dev(keys), dm, w.theta_old, th, dw, w_out=buf2[pad:pad + 5 * n].view(5, n), want_me2=False)
+    torch.cuda.synchronize()
+    assert bool((buf2[:pad] == -7.0).all()) and bool((buf2[pad + 5 * n:] == -7.0).all())
+    # the library stays usable and correct
+    out = T.trex_run(dev(w.keys), dm, w.theta_old, w.theta_new, dw)
+    torch.cuda.synchronize()
+    assert out[3] == 5 and bool((out[0] > 0).all())
+
+
+def test_binding_rejects_mismatched_shapes(T):
+    import torch
+    w = make_config(2, n=500)
+    dk, dm, dw = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    with pytest.raises(T.TrexError):
+        T.trex_run(dk, dm[:, :, :400].contiguous(), w.theta_old, w.theta_new, dw)
+    with pytest.raises(T.TrexError):
+        T.trex_run(dk[:300].contiguous(), dm, w.theta_old, w.theta_new, dw)
+    with pytest.raises(T.TrexError):
+        T.trex_run(dk, dm, w.theta_old, w.theta_new, dw, w_out=torch.empty(499, dtype=torch.float64, device="cuda"))
+    with pytest.raises(T.TrexError):
+        T.trex_run_host(w.keys, w.momenta.astype(np.float32), w.theta_old, w.theta_new, w.w_in, np.empty(w.n))
+    with pytest.raises(T.TrexError):
+        T.trex_run_host(w.keys, torch.from_numpy(w.momenta).float(), w.theta_old, w.theta_new, w.w_in, np.empty(w.n))
+
+
+def test_multi_polynomial_path_with_zero_vev_reference(T):
+    """theta_old with vev = 0 (kappa_old = 0 whatever c_tG is): the polynomial path carries kappa itself, no division by vev."""
+    import torch
+    w = make_config(2, n=3000)
+    tho = w.theta_old.copy(); tho[9] = 0.0; tho[7] = 0.4
+    thetas = []
+    for ctg in (-1.0, -0.3, 0.2, 0.45, 2.0):
+        th = w.theta_old.copy(); th[7] = ctg
+        thetas.append(th)
+    dk, dm, dw = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    wp = T.trex_run_multi(dk, dm, tho, thetas, dw)[0]
+    T.trex_set_poly_multi(False)
+    try:
+        wd = T.trex_run_multi(dk, dm, tho, thetas, dw)[0]
+    finally:
+        T.trex_set_poly_multi(True)
+    torch.cuda.synchronize()
+    a, b = wp.cpu().numpy(), wd.cpu().numpy()
+    assert np.all(np.isfinite(a)) and rel(a, b).max() < 1e-12
+
+
+# ---------------------------------------------------------------- all-event cross-checks at bench-like sizes
+@pytest.mark.parametrize("sid,cfg,n", [(3, 4, 65536), (4, 5, 4096), (2, 3, 200000)])
+def test_table_kernel_equals_first_path_on_every_event(T, sid, cfg, n):
+    """k_table (the kernel bench.py times) against the independent one-thread-per-helicity walk k_ttng on EVERY event of
+    a multi-wave launch (persistent blocks, strided events, ragged tail): catches stride / tail / reuse bugs that a
+    handful of oracle-sampled events cannot. A sample of the same launch is oracle-checked."""
+    import torch
+    w = make_config(cfg, n=n + 13)
+    if cfg == 3:
+        sel = np.where(w.keys == w.classes[0].key)[0]
+        mom, win = np.ascontiguousarray(w.momenta[:, :, sel]), w.w_in[sel]
+    else:
+        mom, win = w.momenta, w.w_in
+    dm, dw = dev(mom), dev(win)
+    a = T.trex_reweight(sid, dm, w.theta_old, w.theta_new, dw)
+    T.trex_set_algorithm(0)
+    try:
+        b = T.trex_reweight(sid, dm, w.theta_old, w.theta_new, dw)
+    finally:
+        T.trex_set_algorithm(3)
+    torch.cuda.synchronize()
+    for x, y in zip(a, b):
+        x, y = x.cpu().numpy(), y.cpu().numpy()
+        assert np.all(np.isfinite(x)) and rel(x, y).max() < 1e-12
+    idx = np.linspace(0, len(win) - 1, 7).astype(int)
+    rw, ro, rn = O.reweight(sid, np.ascontiguousarray(mom[:, :, idx]), w.theta_old, w.theta_new, win[idx])
+    assert rel(a[0].cpu().numpy()[idx], rw).max() < RTOL64 and rel(a[1].cpu().numpy()[idx], ro).max() < RTOL64
+
+
+def test_full_cfg3_run_equals_per_class_calls_on_every_event(T):
+    """trex_run on the full 1,048,576-event mixed sample against one trex_reweight per class on the class's events."""
+    import torch
+    w = make_config(3)
+    out = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    torch.cuda.synchronize()
+    got = [x.cpu().numpy() for x in out[:3]]
+    for sp in w.classes:
+        sel = np.where(w.keys == sp.key)[0]
+        ref = T.trex_reweight(sp.sid, dev(np.ascontiguousarray(w.momenta[:, :, sel])), w.theta_old, w.theta_new, dev(w.w_in[sel]))
+        torch.cuda.synchronize()
+        for g, r in zip(got, ref):
+            assert np.array_equal(g[sel], r.cpu().numpy()), sp.name

@@ -100,3 +100,35 @@ def test_two_rank_cross_section_equals_the_single_rank_definition():
     ref = O.xsec(w, wo, 0.1, 5.0, 0.2)
     assert res[0] == res[1]                                    # every rank holds the same numbers
     assert abs(res[0][0] / ref[0] - 1) < 1e-13 and abs(res[0][1] / ref[1] - 1) < 1e-12 and not res[0][2]
+
+
+def test_launcher_starts_two_ranks_that_shard_and_combine(tmp_path):
+    """bench.py --gpus N uses shard.launch_ranks when it is not already under torchrun: the same launcher, world_size 2,
+    gloo on CPU, running the package's shard self-check (slices, coverage all-reduce, eq.(6)-(7) all-gather)."""
+    import json
+    from oracle import oracle as O
+    from paper_2510_05100_b200.shard import launch_ranks
+    n = 1001
+    out = tmp_path / "shard.json"
+    rc = launch_ranks("paper_2510_05100_b200.shard", 2, [str(n), str(out)], module=True, timeout=300,
+                      env={"TREX_SHARD_BACKEND": "gloo", "CUDA_VISIBLE_DEVICES": ""})
+    assert rc == 0
+    res = json.loads(out.read_text())
+    assert res["world"] == 2 and res["backend"] == "gloo" and res["covered_once"] is True
+    rng = np.random.default_rng(21)
+    w = rng.lognormal(0, 0.5, n)
+    wo = w * rng.uniform(0.5, 2.0, n)
+    ref = O.xsec(w, wo, 0.1, 5.0, 0.2)
+    assert res["xsec"][0] == res["xsec"][1]
+    assert abs(res["xsec"][0][0] / ref[0] - 1) < 1e-13 and abs(res["xsec"][0][1] / ref[1] - 1) < 1e-12
+
+
+def test_shard_arrays_slices_the_event_axis():
+    from paper_2510_05100_b200.shard import shard_arrays
+    n = 37
+    keys = np.arange(n, dtype=np.uint64)
+    mom = np.arange(5 * 4 * n, dtype=np.float64).reshape(5, 4, n)
+    got = [shard_arrays(n, r, 3, keys, mom) for r in range(3)]
+    assert np.array_equal(np.concatenate([g[0] for g in got]), keys)
+    assert np.array_equal(np.concatenate([g[1] for g in got], axis=2), mom)
+    assert all(g[1].flags.c_contiguous for g in got)
