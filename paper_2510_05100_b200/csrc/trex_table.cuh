@@ -181,15 +181,25 @@ template <class R, int NE> TREX_HD sigF<R> tab_F(const R* __restrict__ tab, int 
   for (int i = 0; i < 6; ++i) f[i] = tab_get<R>(tab, (4 + i) * NE + e, sign);
   return F;
 }
-template <class R, int NE> TREX_HD void tab_store(R* __restrict__ tab, int e, const vec4<R>& J, const ften<R>& f) {
-#pragma unroll
-  for (int mu = 0; mu < 4; ++mu) tab_put<R>(tab, mu * NE + e, J.c[mu]);
+// -i * 2 sigma.F as the two 2x2 blocks the row-spinor product consumes
+template <class R> TREX_HD sigF<R> make_sigF(const ften<R>& f) {
   cx<R> xp[3], xm[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) { const cx<R> ie = mul_i(f.e[i]); xp[i] = R(2) * (f.b[i] + ie); xm[i] = R(2) * (f.b[i] - ie); }
-  const cx<R> out[6] = {xp[2], xp[0] + mul_i(xp[1]), xp[0] - mul_i(xp[1]), xm[2], xm[0] + mul_i(xm[1]), xm[0] - mul_i(xm[1])};
+  sigF<R> F;
+  F.p3 = mul_mi(xp[2]); F.pt = mul_mi(xp[0] + mul_i(xp[1])); F.pb = mul_mi(xp[0] - mul_i(xp[1]));
+  F.m3 = mul_mi(xm[2]); F.mt = mul_mi(xm[0] + mul_i(xm[1])); F.mb = mul_mi(xm[0] - mul_i(xm[1]));
+  return F;
+}
+template <class R, int NE> TREX_HD void tab_store(R* __restrict__ tab, int e, const vec4<R>& J, const sigF<R>& F) {
 #pragma unroll
-  for (int i = 0; i < 6; ++i) tab_put<R>(tab, (4 + i) * NE + e, mul_mi(out[i]));
+  for (int mu = 0; mu < 4; ++mu) tab_put<R>(tab, mu * NE + e, J.c[mu]);
+  const cx<R>* f = &F.p3;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) tab_put<R>(tab, (4 + i) * NE + e, f[i]);
+}
+template <class R, int NE> TREX_HD void tab_store(R* __restrict__ tab, int e, const vec4<R>& J, const ften<R>& f) {
+  tab_store<R, NE>(tab, e, J, make_sigF<R>(f));
 }
 // a -= b * c
 template <class R> TREX_HD void cfnma(cx<R>& a, cx<R> b, cx<R> c) {
@@ -248,26 +258,28 @@ template <class R, int N, int NFIX, int K> struct TabBuild {
       else if constexpr (J1 + 2 < K) v4_splits<J1 + 1, J1 + 2>(acc);
     }
   }
-  TREX_HD void run(R* tabw, int e) const {
+  TREX_HD void compute(vec4<R>& J, ften<R>& F) const {
     vec4<R> acc = vzero<R>();
-    ften<R> F = fzero<R>();
+    F = fzero<R>();
     v3_splits<1>(acc, F);
     v4_splits<1, 2>(acc);
     const rvec4<double>& P = pset[mask<K>(0)];
     // (-i/P^2) [(-i) V3 + (-i) V4] at g_s = 1; for K == N the propagator is that of the gluon feeding the t t~ line
     const R s = R(-1.0 / rdot(P, P));
-    vec4<R> J;
 #pragma unroll
     for (int i = 0; i < 4; ++i) J.c[i] = acc.c[i] * s;
     wedge_acc(F, cast<R>(P), J);
+  }
+  TREX_HD void run(R* tabw, int e) const {
+    vec4<R> J; ften<R> F;
+    compute(J, F);
     tab_store<R, NE>(tabw, e, J, F);
   }
 };
 
 template <class R, int N, int NFIX, int K>
-TREX_HD void tab_build_entry(R* __restrict__ tab, const int* __restrict__ meta, const rvec4<double>* __restrict__ pset, int e) {
+TREX_HD void tab_build_setup(TabBuild<R, N, NFIX, K>& b, const R* __restrict__ tab, const int* __restrict__ meta, const rvec4<double>* __restrict__ pset, int e) {
   using I = TabIdx<N, NFIX>;
-  TabBuild<R, N, NFIX, K> b;
   b.tab = tab; b.off = meta + I::M_OFF; b.pset = pset;
   const int cid = meta[I::M_CID + e];
   const int packed = meta[I::M_TUP + cid];
@@ -275,6 +287,11 @@ TREX_HD void tab_build_entry(R* __restrict__ tab, const int* __restrict__ meta, 
   b.fpos[0] = 0;
 #pragma unroll
   for (int i = 0; i < K; ++i) { b.t[i] = (packed >> (4 * i)) & 15; b.fpos[i + 1] = b.fpos[i] + (b.t[i] >= NFIX ? 1 : 0); }
+}
+template <class R, int N, int NFIX, int K>
+TREX_HD void tab_build_entry(R* __restrict__ tab, const int* __restrict__ meta, const rvec4<double>* __restrict__ pset, int e) {
+  TabBuild<R, N, NFIX, K> b;
+  tab_build_setup<R, N, NFIX, K>(b, tab, meta, pset, e);
   b.run(tab, e);
 }
 // level 1: J = polarisation vector, F = K ^ eps.  eps_all[(g * 2 + lambda) * 8 + (re, im per mu)]
@@ -290,6 +307,49 @@ TREX_HD void tab_build_level1(R* __restrict__ tab, const int* __restrict__ meta,
   ften<R> F = fzero<R>();
   wedge_acc(F, cast<R>(pset[1u << g]), J);
   tab_store<R, I::NE>(tab, e, J, F);
+}
+// the same, handing J and F back (W-form kernels contract them further)
+template <class R, int N, int NFIX>
+TREX_HD void tab_level1_JF(const int* __restrict__ meta, const rvec4<double>* __restrict__ pset, const double* __restrict__ eps_all,
+                           unsigned itbits, int e, vec4<R>& J, ften<R>& F) {
+  using I = TabIdx<N, NFIX>;
+  const int g = meta[I::M_CID + e];
+  const int lam = g < NFIX ? (int)((itbits >> g) & 1u) : e - meta[I::M_OFF + g];
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) J.c[mu] = cx<R>(R(eps_all[(g * 2 + lam) * 8 + 2 * mu]), R(eps_all[(g * 2 + lam) * 8 + 2 * mu + 1]));
+  F = fzero<R>();
+  wedge_acc(F, cast<R>(pset[1u << g]), J);
+}
+
+// ---------------------------------------------------------------- suffix contractions ("W form", N = 4)
+// The last vertex of an ordering closes the line with v(p_tbar): for a table entry e (the gluon tuple that ends the
+// ordering) the column spinors   Wj_e = i Jslash_e v,   Wf_e = i (-i 2 sigma.F_e) v   do not depend on the rest of the
+// ordering, so the leaf amplitude is a sum of row x column products  U_A . W_e  (12 complex multiply-adds per term and
+// antitop helicity) instead of a row x matrix product per term followed by the closing. With U_0 = ubar(p_t) the A = 0
+// term is the entry's own scalar  S_e = ubar W_e; likewise the A = 0 row of an inner node, ubar Gamma(J_e), is tabulated.
+// (M v) for M = -i 2 sigma.F in the block form of row_sigma_acc_x: (r M)_0 = r0 p3 + r1 pt, (r M)_1 = r0 pb - r1 p3, ...
+template <class R> TREX_HD spinor<R> sig_col(const sigF<R>& F, const spinor<R>& v) {
+  spinor<R> o;
+  o.c[0] = F.p3 * v.c[0]; cfma(o.c[0], F.pb, v.c[1]);
+  o.c[1] = F.pt * v.c[0]; cfnma(o.c[1], F.p3, v.c[1]);
+  o.c[2] = F.m3 * v.c[2]; cfma(o.c[2], F.mb, v.c[3]);
+  o.c[3] = F.mt * v.c[2]; cfnma(o.c[3], F.m3, v.c[3]);
+  return o;
+}
+template <class R> TREX_HD spinor<R> spinor_from(const double* __restrict__ p) {
+  spinor<R> s;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) s.c[i] = cx<R>(R(p[2 * i]), R(p[2 * i + 1]));
+  return s;
+}
+// 8 complex components of one record, component-major with `stride` records per component
+template <class R> TREX_HD void rec_put(R* __restrict__ t, int stride, int idx, const spinor<R>& a, const spinor<R>& b) {
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { tab_put<R>(t, i * stride + idx, a.c[i]); tab_put<R>(t, (4 + i) * stride + idx, b.c[i]); }
+}
+template <class R> TREX_HD void rec_get(const R* __restrict__ t, int stride, int idx, int sign, spinor<R>& a, spinor<R>& b) {
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { a.c[i] = tab_get<R>(t, i * stride + idx, sign); b.c[i] = tab_get<R>(t, (4 + i) * stride + idx, sign); }
 }
 
 // ---------------------------------------------------------------- phase 2: depth-first walk of the top line
