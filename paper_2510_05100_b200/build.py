@@ -21,7 +21,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 _KERNEL_HDRS = ["trex_math.cuh", "trex_ttng.cuh", "trex_proc.cuh", "trex_kernels.cuh", "trex_ctx.h", "../../include/rex_trex.h", "../../include/rex_trex_diag.h"]
 DEPS = {
     "trex_ttng_tu.cu": _KERNEL_HDRS,
-    "trex_table_tu.cu": _KERNEL_HDRS + ["trex_table.cuh"],
+    "trex_table_tu.cu": _KERNEL_HDRS + ["trex_table.cuh", "trex_table4.cuh"],
     "trex_api.cu": _KERNEL_HDRS + ["trex_ctx.h", "trex_host.h", "trex_colour.h", "../../include/rex_trex.h"],
     "rex_bucket.cu": ["trex_ctx.h", "../../include/rex_trex.h"],
     "trex_probe.cu": ["trex_ctx.h", "../../include/rex_trex.h"],

@@ -95,7 +95,24 @@ template <int N, int NFIX> struct TabIdx {
   static constexpr int M_LVL = M_OFF + NCID + 1;   // [N + 2]: index K = first entry of level K, K = 1 .. N+1
   static constexpr int M_TUP = M_LVL + N + 2;      // [NCID]
   static constexpr int M_CID = M_TUP + NCID;       // [NE]
-  static constexpr int M_SIZE = M_CID + NE;
+  // walk recipes (N <= 4, all helicities free): per ordering, in lexicographic order, four ints = the table references
+  // of the seven tuples a walk task touches, 16 bits each: entry offset of the canonical tuple (bits 0-8), tuple is
+  // reversed (bit 9: helicity bits are bit-reversed), sign -1 (bit 10); then the ordering itself and the rank of
+  // (s1, s2) among ordered pairs:  w0 = (s1 s2 s3) | (s2 s3) << 16,  w1 = (s3) | (s1 s2 s3 s4) << 16,
+  // w2 = (s2 s3 s4) | (s3 s4) << 16,  w3 = (s4) | (s1 | s2 << 2 | s3 << 4 | s4 << 6 | pair << 8) << 16
+  static constexpr int M_REC = (M_CID + NE + 3) / 4 * 4;
+  static constexpr int NREC = (N == 4 && NFIX == 0) ? 4 * 24 : 0;
+  static constexpr int M_SIZE = M_REC + NREC;
+  static int host_ref(const int* meta, const int* t, int L) {
+    const bool fwd = L == 1 || t[0] < t[L - 1];
+    int tt[8];
+    for (int i = 0; i < L; ++i) tt[i] = fwd ? t[i] : t[L - 1 - i];
+    int cid = tt[0];
+    if (L == 2) cid = cid_base(2) + canon_id<2>(tt);
+    if (L == 3) cid = cid_base(3) + canon_id<3>(tt);
+    if (L == 4) cid = cid_base(4) + canon_id<4>(tt);
+    return meta[M_OFF + cid] | (fwd ? 0 : 0x200) | ((fwd || (L & 1)) ? 0 : 0x400);
+  }
   static void build_meta(int* meta) {
     int e = 0, cid = 0;
     for (int K = 1; K <= N; ++K) {
@@ -113,6 +130,19 @@ template <int N, int NFIX> struct TabIdx {
     meta[M_OFF + cid] = e;
     meta[M_LVL + N + 1] = e;
     meta[M_LVL] = 0;
+    if constexpr (NREC > 0) {
+      int rank = 0;
+      for (int s1 = 0; s1 < 4; ++s1) for (int s2 = 0; s2 < 4; ++s2) for (int s3 = 0; s3 < 4; ++s3) for (int s4 = 0; s4 < 4; ++s4) {
+        if (s1 == s2 || s1 == s3 || s1 == s4 || s2 == s3 || s2 == s4 || s3 == s4) continue;
+        const int s[4] = {s1, s2, s3, s4};
+        int* w = meta + M_REC + 4 * rank++;
+        w[0] = host_ref(meta, s, 3) | host_ref(meta, s + 1, 2) << 16;
+        w[1] = host_ref(meta, s + 2, 1) | host_ref(meta, s, 4) << 16;
+        w[2] = host_ref(meta, s + 1, 3) | host_ref(meta, s + 2, 2) << 16;
+        const int pair = s1 * 3 + s2 - (s2 > s1 ? 1 : 0);
+        w[3] = host_ref(meta, s + 3, 1) | (s1 | s2 << 2 | s3 << 4 | s4 << 6 | pair << 8) << 16;
+      }
+    }
   }
 };
 
@@ -223,16 +253,20 @@ template <class R> TREX_HD void row_sigma_acc_x(spinor<R>& acc, const spinor<R>&
 
 // ---------------------------------------------------------------- phase 1: one table entry of level K >= 2
 // t[0..K) canonical tuple, fpos[i] = free gluons among t[0..i), fb = helicity bits of the free gluons in position order
-template <class R, int N, int NFIX, int K> struct TabBuild {
+// TS: entries per table component; PL, poff: references to entries of level <= PL are shifted by poff (the pipelined
+// N = 4 kernel keeps two copies of its lowest levels, one per event parity)
+template <class R, int N, int NFIX, int K, int TS = TabIdx<N, NFIX>::NE, int PL = 0> struct TabBuild {
   using I = TabIdx<N, NFIX>;
-  static constexpr int NE = I::NE;
+  static constexpr int NE = TS, KK = K;
   const R* tab; const int* off; const rvec4<double>* pset;
   int t[K], fpos[K + 1]; unsigned fb;
+  int poff = 0;
 
   template <int L> TREX_HD vec4<R> sub(int a) const {
     int sign;
     const int nf = fpos[a + L] - fpos[a];
-    const int e = tab_entry<N, NFIX, L>(off, t + a, (fb >> fpos[a]) & ((1u << nf) - 1u), nf, sign);
+    int e = tab_entry<N, NFIX, L>(off, t + a, (fb >> fpos[a]) & ((1u << nf) - 1u), nf, sign);
+    if constexpr (L <= PL) e += poff;
     return tab_J<R, NE>(tab, e, sign);
   }
   template <int L> TREX_HD unsigned mask(int a) const {
@@ -277,8 +311,8 @@ template <class R, int N, int NFIX, int K> struct TabBuild {
   }
 };
 
-template <class R, int N, int NFIX, int K>
-TREX_HD void tab_build_setup(TabBuild<R, N, NFIX, K>& b, const R* __restrict__ tab, const int* __restrict__ meta, const rvec4<double>* __restrict__ pset, int e) {
+template <class R, int N, int NFIX, int K, class B>
+TREX_HD void tab_build_setup(B& b, const R* __restrict__ tab, const int* __restrict__ meta, const rvec4<double>* __restrict__ pset, int e) {
   using I = TabIdx<N, NFIX>;
   b.tab = tab; b.off = meta + I::M_OFF; b.pset = pset;
   const int cid = meta[I::M_CID + e];

@@ -58,6 +58,9 @@ namespace {
 #ifndef TREX_T4_WFORM
 #define TREX_T4_WFORM 1
 #endif
+#ifndef TREX_T4_PIPE
+#define TREX_T4_PIPE 1
+#endif
 #ifndef TREX_T4_DMMA
 #define TREX_T4_DMMA 1
 #endif
@@ -378,30 +381,35 @@ __device__ __forceinline__ void walk_wform(unsigned char* sb, const int* meta, i
   const R* ubt = reinterpret_cast<const R*>(sb + G::o_ub);
   const rvec4<double>* pset = reinterpret_cast<const rvec4<double>*>(sb + G::o_pset);
   cx<RC>* xs = reinterpret_cast<cx<RC>*>(sb + G::o_x);
-  const int* off = meta + I::M_OFF;
   for (int task = gtid; task < 384 * NPASS; task += G::GS) {
     const int pass = task / 384, r = task - pass * 384;
     const int prank = r >> 4, lt = r & 1;
     const unsigned hp = (unsigned)(r >> 1) & 7u;             // helicities of s1, s2, s3 (bit i: s_{i+1})
-    int s[4];
-    prefix_of_rank<4, 4>(prank, s);
+    // table references of this ordering (TabIdx::M_REC): no index arithmetic on the critical path of the loads
+    const int4 rc = reinterpret_cast<const int4*>(meta + I::M_REC)[prank];
+    const auto ref = [](unsigned rf, unsigned bits, int nf, int& sign) {
+      sign = (rf & 0x400u) ? -1 : 1;
+      return (int)(rf & 0x1FFu) + (int)((rf & 0x200u) ? I::bitrev(bits, nf) : bits);
+    };
+    const unsigned sp = (unsigned)rc.w >> 16;
+    const int s[4] = {(int)(sp & 3u), (int)((sp >> 2) & 3u), (int)((sp >> 4) & 3u), (int)((sp >> 6) & 3u)};
     const int ubase = pass * G::NU;
     dspinor<R> U1, U2, U3;
     rec_get<R>(utab, G::NUT, ubase + UI::level1(s[0], hp & 1u, lt), 1, U1.o0, U1.o1);
-    rec_get<R>(utab, G::NUT, ubase + UI::level2(s[0], s[1], hp & 3u, lt), 1, U2.o0, U2.o1);
+    rec_get<R>(utab, G::NUT, ubase + UI::N1 + (((int)(sp >> 8) * 4 + (int)(hp & 3u)) * 2 + lt), 1, U2.o0, U2.o1);
     // ---- node 3: U3 = [ ubar Gamma(J(s1 s2 s3)) + U1 Gamma(J(s2 s3)) + U2 Gamma(J(s3)) ] S(p_t - K(s1 s2 s3))
     {
       spinor<R> s0, s1;
       int sign;
-      int e = tab_entry<N, 0, 3>(off, s, hp, 3, sign);
+      int e = ref((unsigned)rc.x & 0xFFFFu, hp, 3, sign);
       rec_get<R>(ubt, G::NUB, (e - G::E3) * 2 + lt, sign, s0, s1);
-      e = tab_entry<N, 0, 2>(off, s + 1, hp >> 1, 2, sign);
+      e = ref((unsigned)rc.x >> 16, hp >> 1, 2, sign);
       {
         const vec4<R> J = tab_J<R, NE>(tab, e, sign);
         row_slash_acc(s0, U1.o0, J); row_slash_acc(s1, U1.o1, J);
         row_sigma_acc_x(s1, U1.o0, tab_F<R, NE>(tab, e, sign));
       }
-      e = tab_entry<N, 0, 1>(off, s + 2, hp >> 2, 1, sign);
+      e = ref((unsigned)rc.y & 0xFFFFu, hp >> 2, 1, sign);
       {
         const vec4<R> J = tab_J<R, NE>(tab, e, sign);
         row_slash_acc(s0, U2.o0, J); row_slash_acc(s1, U2.o1, J);
@@ -409,7 +417,7 @@ __device__ __forceinline__ void walk_wform(unsigned char* sb, const int* meta, i
       }
 #pragma unroll
       for (int i = 0; i < 4; ++i) { s0.c[i] = mul_i(s0.c[i]); s1.c[i] = mul_i(s1.c[i]); }
-      const rvec4<double> qd = rsub(pt, pset[(1u << s[0]) | (1u << s[1]) | (1u << s[2])]);
+      const rvec4<double> qd = rsub(pt, pset[15u ^ (1u << s[3])]);
       const double q2 = rdot(qd, qd), mt = a.T.mt[pass];
       const rvec4<R> q = cast<R>(qd);
       const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), cx<double>(q2 - mt * mt, a.T.mGt[pass])));
@@ -427,10 +435,10 @@ __device__ __forceinline__ void walk_wform(unsigned char* sb, const int* meta, i
     for (unsigned h4 = 0; h4 < 2; ++h4) {
       const unsigned hp4 = hp | (h4 << 3);
       int sg0, sg1, sg2, sg3;
-      const int e4 = tab_entry<N, 0, 4>(off, s, hp4, 4, sg0);
-      const int e1 = tab_entry<N, 0, 3>(off, s + 1, hp4 >> 1, 3, sg1);
-      const int e2 = tab_entry<N, 0, 2>(off, s + 2, hp4 >> 2, 2, sg2);
-      const int e3 = tab_entry<N, 0, 1>(off, s + 3, hp4 >> 3, 1, sg3);
+      const int e4 = ref((unsigned)rc.y >> 16, hp4, 4, sg0);
+      const int e1 = ref((unsigned)rc.z & 0xFFFFu, hp4 >> 1, 3, sg1);
+      const int e2 = ref((unsigned)rc.z >> 16, hp4 >> 2, 2, sg2);
+      const int e3 = ref((unsigned)rc.w & 0xFFFFu, hp4 >> 3, 1, sg3);
       unsigned hfree = 0;
 #pragma unroll
       for (int i = 0; i < 4; ++i) hfree |= ((hp4 >> i) & 1u) << s[i];
@@ -453,6 +461,83 @@ __device__ __forceinline__ void walk_wform(unsigned char* sb, const int* meta, i
         }
       }
     }
+  }
+}
+
+// ---- phase 3 of k_table: x^dagger C x of every X column added into the event's partial-sum slots
+template <class R, class RC, int N>
+__device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, const RC* __restrict__ Cs, double* __restrict__ part, int tid, int gtid) {
+  using G = TabGeom<R, RC, N>;
+  using F = FoldedC<G::NC>;
+  constexpr int XS = G::XS, GS = G::GS;
+  // ---- phase 3: x^dagger C x of every X column, 8-row register blocks, row blocks paired (p, NB-1-p) for balance.
+  // A work item is always handled by the same thread, so its partial sum accumulates race-free in shared memory.
+  constexpr int RB = F::RB, NB = F::NB;
+  if constexpr (G::DMMA) {
+    // FP64 tensor cores (mma.sync m8n8k4, measured 37 TFLOP/s against 24.7 for register-operand DFMA): the tile is a
+    // real [NC x 2 NCOLT] matrix X (re/im interleaved); T = C'^T X is formed in 8 x 8 tiles (row block J of 8 flows,
+    // column block of 4 complex columns), k runs over the flows i < 8 J + 8 in steps of 4; the accumulator layout
+    // (lane: row lane/4, columns 2 (lane%4), +1) puts (Re, Im) of t_j for one complex column into one lane, which
+    // closes it with x_j. A warp owns one column block and walks the row-block pairs (p, NB-1-p).
+    const int lane = tid & 31, wrp = tid >> 5;
+    const int fr = lane >> 2, fc = lane & 3;
+    const double* xr = reinterpret_cast<const double*>(xs);
+    constexpr int XR = 2 * XS, NCB = G::NCOLT / 4;
+    double accl = 0.0;
+    // a warp owns one column block; row blocks go four at a time (J0 .. J0+3) so that one X fragment feeds four
+    // independent accumulator chains
+    for (int cb = wrp; cb < NCB; cb += GS / 32) {
+      for (int J0 = 0; J0 < NB; J0 += 4) {
+        double d[4][2];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { d[q][0] = 0.0; d[q][1] = 0.0; }
+        const int Jm = min(J0 + 3, NB - 1);
+        for (int ks = 0; ks < 2 * (Jm + 1); ++ks) {
+          const int i = 4 * ks + fc, bi = i >> 3;
+          const double bv = xr[i * XR + 8 * cb + fr];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const int J = J0 + q;
+            if (J < NB && bi <= J) {
+              // C' is stored in fragment order: fragment (J, ks) = the 8 x 4 block C'(4 ks + fc, 8 J + fr), lane-major
+              const double av = Cs[(J * (J + 1) + ks) * 32 + lane];
+              asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                           : "+d"(d[q][0]), "+d"(d[q][1]) : "d"(av), "d"(bv));
+            }
+          }
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const int J = J0 + q;
+          if (J < NB) { const cx<RC> xj = xs[(8 * J + fr) * XS + 4 * cb + fc]; accl += xj.re * d[q][0] + xj.im * d[q][1]; }
+        }
+      }
+    }
+    part[tid] += accl;                                  // slot parity = lane parity = column parity = theta
+  } else
+  for (int item = gtid; item < G::NCI0; item += GS) {
+    const int c = item % G::NCOLT, p = item / G::NCOLT;
+    RC accl = RC(0);
+    for (int side = 0; side < 2; ++side) {
+      const int b = side == 0 ? p : NB - 1 - p;
+      if (side == 1 && b == p) break;
+      cx<RC> t[RB];
+#pragma unroll
+      for (int r = 0; r < RB; ++r) t[r] = cx<RC>(RC(0), RC(0));
+      const RC* row = Cs;
+      const int iend = RB * b + RB;
+#pragma unroll 2
+      for (int i = 0; i < iend; ++i) {
+        const cx<RC> xi = xs[i * XS + c];
+        const RC* cr = row + (RB * b - RB * (i / RB));
+#pragma unroll
+        for (int r = 0; r < RB; ++r) cfma(t[r], xi, cr[r]);
+        row += F::row_len(i);
+      }
+#pragma unroll
+      for (int r = 0; r < RB; ++r) { const cx<RC> xj = xs[(RB * b + r) * XS + c]; accl += xj.re * t[r].re + xj.im * t[r].im; }
+    }
+    part[item] += (double)accl;
   }
 }
 
@@ -581,75 +666,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
       group_sync<GS>();
       PHASE_TICK(2);
 
-      // ---- phase 3: x^dagger C x of every X column, 8-row register blocks, row blocks paired (p, NB-1-p) for balance.
-      // A work item is always handled by the same thread, so its partial sum accumulates race-free in shared memory.
-      constexpr int RB = F::RB, NB = F::NB;
-      if constexpr (G::DMMA) {
-        // FP64 tensor cores (mma.sync m8n8k4, measured 37 TFLOP/s against 24.7 for register-operand DFMA): the tile is a
-        // real [NC x 2 NCOLT] matrix X (re/im interleaved); T = C'^T X is formed in 8 x 8 tiles (row block J of 8 flows,
-        // column block of 4 complex columns), k runs over the flows i < 8 J + 8 in steps of 4; the accumulator layout
-        // (lane: row lane/4, columns 2 (lane%4), +1) puts (Re, Im) of t_j for one complex column into one lane, which
-        // closes it with x_j. A warp owns one column block and walks the row-block pairs (p, NB-1-p).
-        const int lane = tid & 31, wrp = tid >> 5;
-        const int fr = lane >> 2, fc = lane & 3;
-        const double* xr = reinterpret_cast<const double*>(xs);
-        constexpr int XR = 2 * XS, NCB = G::NCOLT / 4;
-        double accl = 0.0;
-        // a warp owns one column block; row blocks go four at a time (J0 .. J0+3) so that one X fragment feeds four
-        // independent accumulator chains
-        for (int cb = wrp; cb < NCB; cb += GS / 32) {
-          for (int J0 = 0; J0 < NB; J0 += 4) {
-            double d[4][2];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) { d[q][0] = 0.0; d[q][1] = 0.0; }
-            const int Jm = min(J0 + 3, NB - 1);
-            for (int ks = 0; ks < 2 * (Jm + 1); ++ks) {
-              const int i = 4 * ks + fc, bi = i >> 3;
-              const double bv = xr[i * XR + 8 * cb + fr];
-#pragma unroll
-              for (int q = 0; q < 4; ++q) {
-                const int J = J0 + q;
-                if (J < NB && bi <= J) {
-                  // C' is stored in fragment order: fragment (J, ks) = the 8 x 4 block C'(4 ks + fc, 8 J + fr), lane-major
-                  const double av = Cs[(J * (J + 1) + ks) * 32 + lane];
-                  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                               : "+d"(d[q][0]), "+d"(d[q][1]) : "d"(av), "d"(bv));
-                }
-              }
-            }
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              const int J = J0 + q;
-              if (J < NB) { const cx<RC> xj = xs[(8 * J + fr) * XS + 4 * cb + fc]; accl += xj.re * d[q][0] + xj.im * d[q][1]; }
-            }
-          }
-        }
-        part[tid] += accl;                                  // slot parity = lane parity = column parity = theta
-      } else
-      for (int item = gtid; item < G::NCI0; item += GS) {
-        const int c = item % G::NCOLT, p = item / G::NCOLT;
-        RC accl = RC(0);
-        for (int side = 0; side < 2; ++side) {
-          const int b = side == 0 ? p : NB - 1 - p;
-          if (side == 1 && b == p) break;
-          cx<RC> t[RB];
-#pragma unroll
-          for (int r = 0; r < RB; ++r) t[r] = cx<RC>(RC(0), RC(0));
-          const RC* row = Cs;
-          const int iend = RB * b + RB;
-#pragma unroll 2
-          for (int i = 0; i < iend; ++i) {
-            const cx<RC> xi = xs[i * XS + c];
-            const RC* cr = row + (RB * b - RB * (i / RB));
-#pragma unroll
-            for (int r = 0; r < RB; ++r) cfma(t[r], xi, cr[r]);
-            row += F::row_len(i);
-          }
-#pragma unroll
-          for (int r = 0; r < RB; ++r) { const cx<RC> xj = xs[(RB * b + r) * XS + c]; accl += xj.re * t[r].re + xj.im * t[r].im; }
-        }
-        part[item] += (double)accl;
-      }
+      colour_phase<R, RC, N>(xs, Cs, part, tid, gtid);
 #ifdef TREX_PHASE_CLOCKS
       group_sync<GS>();
       PHASE_TICK(3);
@@ -685,6 +702,10 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
 #endif
 }
 
+#if TREX_TU_N == 4
+#include "trex_table4.cuh"
+#endif
+
 }  // namespace
 
 // meta block and folded colour matrix sizes (host allocates and fills them once)
@@ -717,6 +738,23 @@ int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const Reweight
                                                                   int nsm, cudaStream_t s) {
   constexpr int N = TREX_TU_N;
   using G = TabGeom<TuR, TuRC, N>;
+#if TREX_TU_N == 4 && TREX_T4_PIPE && TREX_T4_WFORM
+  {
+    // software-pipelined W-form kernel (trex_table4.cuh): one persistent 384-thread block per SM
+    using W = W4<TuR, TuRC>;
+    static bool ready = false;
+    if (!ready) {
+      if (cudaFuncSetAttribute(k_table4w<TuR, TuRC, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)W::bytes) != cudaSuccess ||
+          cudaFuncSetAttribute(k_table4w<TuR, TuRC, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)W::bytes) != cudaSuccess)
+        return (int)cudaGetLastError();
+      ready = true;
+    }
+    const unsigned grid = (unsigned)(nmax < (long)nsm ? nmax : (long)nsm);
+    if (npass == 1) k_table4w<TuR, TuRC, 1><<<grid, W::TB, W::bytes, s>>>(a, meta, Cfold);
+    else k_table4w<TuR, TuRC, 2><<<grid, W::TB, W::bytes, s>>>(a, meta, Cfold);
+    return (int)cudaGetLastError();
+  }
+#endif
   static int blocks_per_sm = 0;
   if (!blocks_per_sm) {
     cudaFuncSetAttribute(k_table<TuR, TuRC, N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::bytes);
