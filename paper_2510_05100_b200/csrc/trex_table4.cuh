@@ -324,35 +324,57 @@ __device__ __forceinline__ void w4_walk(const W4Ptr<R>& p, const typename W4<R, 
       }
       U3 = w4_propagate<R>(s0, s1, rsub(pt, sm.pset[15u ^ (1u << s3i)]), a.T.mt[pass], a.T.mGt[pass]);
     }
-    // ---- leaves: both helicities of s4, both antitop helicities
-#pragma unroll 1
-    for (unsigned h4 = 0; h4 < 2; ++h4) {
-      const unsigned hp4 = hp | (h4 << 3);
-      int sg0, sg1, sg2, sg3;
-      const int e4 = ref((unsigned)rc.y >> 16, hp4, 4, sg0);
-      const int e1 = ref((unsigned)rc.z & 0xFFFFu, hp4 >> 1, 3, sg1);
-      const int e2 = ref((unsigned)rc.z >> 16, hp4 >> 2, 2, sg2) + poffw;     // W records of levels 1, 2: parity copy
-      const int e3 = ref((unsigned)rc.w & 0xFFFFu, hp4 >> 3, 1, sg3) + poffw;
+    // ---- leaves: the four (helicity of s4, lambda_tbar) combinations c = 2 h4 + ltb are closed together,
+    //   a0[c] = S0 + sum_A U_A.o0 . Wj_A[c],   a1[c] = S1 + sum_A (U_A.o1 . Wj_A[c] + U_A.o0 . Wf_A[c]),
+    // component by component, so that one line-state component multiplies eight table numbers in a row (the FP64 pipe
+    // reads such a repeated operand from its reuse cache: two register reads per DFMA instead of three). The sign of a
+    // reversed tuple depends on the ordering only and is folded into the line state once.
+    int sg0, sg1, sg2, sg3;
+    const int b4 = ref((unsigned)rc.y >> 16, 0u, 4, sg0), b1 = ref((unsigned)rc.z & 0xFFFFu, 0u, 3, sg1);
+    const int b2 = ref((unsigned)rc.z >> 16, 0u, 2, sg2), b3 = ref((unsigned)rc.w & 0xFFFFu, 0u, 1, sg3);
+    const bool r4 = ((unsigned)rc.y >> 16) & 0x200u, r1 = (unsigned)rc.z & 0x200u, r2 = ((unsigned)rc.z >> 16) & 0x200u;
+    cx<R> a0[4], a1[4];
+    int rec1[4], rec2[4], rec3[4], colc[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      const unsigned h4 = (unsigned)c >> 1, hp4 = hp | (h4 << 3);
+      const int ltb = c & 1;
+      const int e4 = b4 + (int)(r4 ? I::bitrev(hp4, 4) : hp4);
+      a0[c] = tab_get<R>(p.tab, ((lt * 2 + ltb) * 2 + 0) * TS + e4, sg0);
+      a1[c] = tab_get<R>(p.tab, ((lt * 2 + ltb) * 2 + 1) * TS + e4, sg0);
+      rec1[c] = (b1 + (int)(r1 ? I::bitrev(hp4 >> 1, 3) : hp4 >> 1)) * 2 + ltb;
+      rec2[c] = (b2 + (int)(r2 ? I::bitrev(hp4 >> 2, 2) : hp4 >> 2) + poffw) * 2 + ltb;
+      rec3[c] = (b3 + (int)h4 + poffw) * 2 + ltb;
       unsigned hfree = 0;
 #pragma unroll
       for (int i = 0; i < 4; ++i) hfree |= ((hp4 >> i) & 1u) << ((sp >> (2 * i)) & 3u);
+      colc[c] = (((int)hfree * 2 + lt) * 2 + ltb) * 2;
+    }
+    const auto close_with = [&](const dspinor<R>& U, int sign, const int* rec) {
 #pragma unroll
-      for (int ltb = 0; ltb < 2; ++ltb) {
-        cx<R> a0 = tab_get<R>(p.tab, ((lt * 2 + ltb) * 2 + 0) * TS + e4, sg0);
-        cx<R> a1 = tab_get<R>(p.tab, ((lt * 2 + ltb) * 2 + 1) * TS + e4, sg0);
-        w4_leaf_term<R>(a0, a1, U1, p.wtab, W::NWR, e1 * 2 + ltb, sg1);
-        w4_leaf_term<R>(a0, a1, U2, p.wtab, W::NWR, e2 * 2 + ltb, sg2);
-        w4_leaf_term<R>(a0, a1, U3, p.wtab, W::NWR, e3 * 2 + ltb, sg3);
-        const int col = (((int)hfree * 2 + lt) * 2 + ltb) * 2;
-        if constexpr (NPASS == 1) {
-          cx<R> x = a0; cfma(x, a1, kq0);
-          cx<R> y = a0; cfma(y, a1, kq1);
-          xs[prank * XS + col] = cx<RC>(RC(x.re), RC(x.im));
-          xs[prank * XS + col + 1] = cx<RC>(RC(y.re), RC(y.im));
-        } else {
-          cx<R> x = a0; cfma(x, a1, pass == 0 ? kq0 : kq1);
-          xs[prank * XS + col + pass] = cx<RC>(RC(x.re), RC(x.im));
+      for (int i = 0; i < 4; ++i) {
+        const cx<R> u0(with_sign(U.o0.c[i].re, sign), with_sign(U.o0.c[i].im, sign));
+        const cx<R> u1(with_sign(U.o1.c[i].re, sign), with_sign(U.o1.c[i].im, sign));
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const cx<R> wj = tab_get<R>(p.wtab, i * W::NWR + rec[c], 1), wf = tab_get<R>(p.wtab, (4 + i) * W::NWR + rec[c], 1);
+          cfma(a0[c], u0, wj); cfma(a1[c], u0, wf); cfma(a1[c], u1, wj);
         }
+      }
+    };
+    close_with(U1, sg1, rec1);
+    close_with(U2, sg2, rec2);
+    close_with(U3, sg3, rec3);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      if constexpr (NPASS == 1) {
+        cx<R> x = a0[c]; cfma(x, a1[c], kq0);
+        cx<R> y = a0[c]; cfma(y, a1[c], kq1);
+        xs[prank * XS + colc[c]] = cx<RC>(RC(x.re), RC(x.im));
+        xs[prank * XS + colc[c] + 1] = cx<RC>(RC(y.re), RC(y.im));
+      } else {
+        cx<R> x = a0[c]; cfma(x, a1[c], pass == 0 ? kq0 : kq1);
+        xs[prank * XS + colc[c] + pass] = cx<RC>(RC(x.re), RC(x.im));
       }
     }
   }
@@ -388,19 +410,28 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
   w4_build3<R, RC, NPASS>(p, small[0], a, 0, tid);
   __syncthreads();
   int par = 0;
+#ifdef TREX_PHASE_CLOCKS
+  long long pc[4] = {0, 0, 0, 0}, t0 = clock64();
+#define W4_TICK(k) do { if (tid == 0) { const long long t1 = clock64(); pc[k] += t1 - t0; t0 = t1; } } while (0)
+#else
+#define W4_TICK(k) do { } while (0)
+#endif
   for (long e = e_first; e < io.n; e += e_step, par ^= 1) {
     const bool more = e + e_step < io.n;
     // ---- phase B: level-4 entries of this event | prep of the next one
     if (wrp < 6) w4_top<R, RC>(p, small[par], W::E4 + tid, par);
     else if (wrp < 8 && more) w4_prep<R, RC, NPASS>(p, small[par ^ 1], io, a, e + e_step, par ^ 1, wrp - 6, lane);
     __syncthreads();
+    W4_TICK(0);
     // ---- phase C: top-line walk
     w4_walk<R, RC, NPASS>(p, small[par], xs, a, par, tid);
     __syncthreads();
+    W4_TICK(1);
     // ---- phase D: colour sum of this event | level 3 of the next one
     colour_phase<R, RC, 4>(xs, Cs, part, tid, tid);
     if (more) w4_build3<R, RC, NPASS>(p, small[par ^ 1], a, par ^ 1, tid);
     __syncthreads();
+    W4_TICK(2);
     // ---- fixed-order reduction of the partial sums (slot parity = theta) + epilogue by the first warp, which clears
     // what it has read; the other warps already work on the next event
     if (wrp == 0) {
@@ -417,5 +448,9 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
         if (io.me2_new) io.me2_new[e] = mn;
       }
     }
+    W4_TICK(3);
   }
+#ifdef TREX_PHASE_CLOCKS
+  if (tid == 0 && blockIdx.x == 0) printf("k_table4w phases [cycles of block 0]: B (level 4 | prep) %lld  C (walk) %lld  D (colour | level 3) %lld  epilogue %lld\n", pc[0], pc[1], pc[2], pc[3]);
+#endif
 }
