@@ -18,6 +18,13 @@ extern "C" {
  * Only for TREX_SP_GG_TT .. TREX_SP_GG_TTGGG. Synchronous. */
 int trex_debug_flow_amps(int subproc_id, const double* momenta_one, const double* theta, double* out);
 
+/* The same for the PRODUCTION kernels (the ones trex_reweight launches and bench.py times: k_gg_tt, k_table<3>,
+ * k_table4w, k_table<5>): one event is run through the regular launch with a side buffer that receives the operand of
+ * the colour sum. out HOST [nhel][ncolor][2: theta_old, theta_new][re, im] = J_c(theta) = g_s^N (A0 + (kappa/g_s) A1),
+ * flows in lexicographic order of the gluon ordering, h as above. fp64 mode; when top mass or width differ between the
+ * two parameter points the two-pass kernels are the ones exercised. Synchronous. */
+int trex_debug_xtile(int subproc_id, const double* momenta_one, const double* theta_old, const double* theta_new, double* out);
+
 /* Roofline denominator: enqueues ONE launch of a register-resident FMA chain kernel (blocks x 256 threads, 64 FMAs per
  * thread and iteration) on the library stream and returns the floating-point operations it executes (2 per FMA), or a
  * negative error code. mode 0 / 1: FP64 / FP32 chains with two constant-bank operands (pipe peak); 2 / 3: three

@@ -41,6 +41,7 @@ _SIGNATURES = {
     "trex_run_multi": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _int, _vp, _vp, _vp, _vp]),
     "trex_run_host": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_debug_flow_amps": (_int, [_int, _dp, _dp, _dp]),
+    "trex_debug_xtile": (_int, [_int, _dp, _dp, _dp, _dp]),
     "trex_probe_fma": (ctypes.c_double, [_int, _int, _int]),
     "trex_xsec_moments": (_int, [_vp, _vp, ctypes.c_int64, _vp]),
     "trex_xsec_finish": (_int, [_vp, _int, ctypes.c_double, ctypes.c_double, ctypes.c_double, _vp]),
@@ -420,4 +421,16 @@ def trex_debug_flow_amps(subproc_id, momenta_one, theta):
     th, pth = _theta(theta)
     out = np.empty((nh, nc, 2, 2))
     _check(lib().trex_debug_flow_amps(subproc_id, m.ctypes.data_as(_dp), pth, out.ctypes.data_as(_dp)), "trex_debug_flow_amps")
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def trex_debug_xtile(subproc_id, momenta_one, theta_old, theta_new):
+    """Colour-flow amplitudes of one event from the PRODUCTION kernel: complex array [nhel, ncolor, 2 (theta_old, theta_new)]."""
+    _torch()
+    npar, nc, nh = trex_npar(subproc_id), trex_ncolor(subproc_id), trex_nhel(subproc_id)
+    m = np.ascontiguousarray(momenta_one, dtype=np.float64).reshape(npar, 4)
+    to, pto = _theta(theta_old)
+    tn, ptn = _theta(theta_new)
+    out = np.empty((nh, nc, 2, 2))
+    _check(lib().trex_debug_xtile(subproc_id, m.ctypes.data_as(_dp), pto, ptn, out.ctypes.data_as(_dp)), "trex_debug_xtile")
     return out[..., 0] + 1j * out[..., 1]

@@ -243,6 +243,7 @@ const TtngUploadFn kUpload[4][3] = {
 const TableLaunchFn kTableLaunch[3][3] = TREX_TAB_ROW(trex_tu_table_launch_n);
 const TableMetaFn kTableMeta[3][3] = TREX_TAB_ROW(trex_tu_table_meta_n);
 const TableFoldFn kTableFold[3][3] = TREX_TAB_ROW(trex_tu_table_fold_n);
+const TableGeomFn kTableGeom[3][3] = TREX_TAB_ROW(trex_tu_table_geom_n);
 #undef TREX_TAB_ROW
 
 int ensure_colour() {
@@ -325,7 +326,7 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
   Context& c = ctx();
   const SubprocInfo* sp = subproc_info(sid);
   if (int rc = ensure_colour()) return rc;
-  a.T = T; a.sid = sid; a.q = sp->qlegs; a.C120 = c.C120;
+  a.T = T; a.sid = sid; a.q = sp->qlegs; a.C120 = c.C120; a.dbg = c.dbg_out;
   const unsigned grid32 = (unsigned)((nmax + 31) / 32);
   const int mode = c.precision;
   cudaEvent_t kt[2] = {nullptr, nullptr};
@@ -655,6 +656,66 @@ extern "C" int trex_debug_flow_amps(int sid, const double* momenta_one, const do
   cudaError_t e3 = cudaStreamSynchronize(c.stream);
   cudaFree(d_mom); cudaFree(d_out);
   TREX_CUDA_CHECK(e1); TREX_CUDA_CHECK(e2); TREX_CUDA_CHECK(e3);
+  return 0;
+}
+
+// Colour-flow amplitudes of ONE event as the PRODUCTION kernels form them (k_gg_tt, k_table<3>, k_table4w, k_table<5>):
+// the kernel that trex_reweight launches copies its X tile (the operand of the colour sum) for event 0 to a scratch
+// buffer; here the columns are sorted into the full helicity index h (bit `leg` of h = helicity of that leg, process
+// order) and the couplings g_s^N are restored. out HOST [nhel][ncolor][2: theta_old, theta_new][re, im].
+extern "C" int trex_debug_xtile(int sid, const double* momenta_one, const double* theta_old, const double* theta_new, double* out) {
+  Context& c = ctx();
+  const SubprocInfo* sp = subproc_info(sid);
+  if (!sp || sid < TREX_SP_GG_TT || sid > TREX_SP_GG_TTGGG) return fail(TREX_EUNKNOWN_SUBPROC, "trex_debug_xtile: only g g > t t~ (+g..)");
+  if (!momenta_one || !theta_old || !theta_new || !out) return fail(TREX_EINVAL, "trex_debug_xtile: null pointer");
+  if (c.precision != 0) return fail(TREX_EINVAL, "trex_debug_xtile: fp64 mode only");
+  ThetaPair T;
+  if (!make_theta_pair(sid, theta_old, theta_new, T)) return fail(TREX_EINVAL, "trex_debug_xtile: theta outside its domain");
+  const int N = sp->npar - 2, nhel = sp->nhel, nc = sp->ncolor;
+  int geom[5] = {0, 1, 1, 2, 0};
+  if (N >= 3) kTableGeom[N - 3][0](geom);
+  const int NFIX = geom[0], NIT = geom[1], NLT = geom[2], NCOLT = geom[4];
+  const size_t ndump = N == 2 ? (size_t)8 * 2 * 2 * 2 : (size_t)NIT * NLT * nc * NCOLT;
+  double *d_mom = nullptr, *d_w = nullptr, *d_dbg = nullptr;
+  TREX_CUDA_CHECK(cudaMalloc((void**)&d_mom, sizeof(double) * 4 * sp->npar));
+  TREX_CUDA_CHECK(cudaMalloc((void**)&d_w, sizeof(double) * 4));
+  TREX_CUDA_CHECK(cudaMalloc((void**)&d_dbg, sizeof(double) * 2 * ndump));
+  const double one[4] = {1.0, 0.0, 0.0, 0.0};
+  cudaMemcpyAsync(d_mom, momenta_one, sizeof(double) * 4 * sp->npar, cudaMemcpyHostToDevice, c.stream);
+  cudaMemcpyAsync(d_w, one, sizeof one, cudaMemcpyHostToDevice, c.stream);
+  cudaMemsetAsync(d_dbg, 0, sizeof(double) * 2 * ndump, c.stream);
+  c.dbg_out = d_dbg;
+  ReweightArgs a;
+  a.io = EvIO{d_mom, 1, 1, d_w, d_w + 1, d_w + 2, d_w + 3};
+  a.alt = a.io; a.plan = nullptr;
+  const int rc = launch_reweight(sid, a, 1, T);
+  c.dbg_out = nullptr;
+  std::vector<double> dump(2 * ndump);
+  cudaError_t e1 = cudaMemcpyAsync(dump.data(), d_dbg, sizeof(double) * 2 * ndump, cudaMemcpyDeviceToHost, c.stream);
+  cudaError_t e2 = cudaStreamSynchronize(c.stream);
+  cudaFree(d_mom); cudaFree(d_w); cudaFree(d_dbg);
+  if (rc < 0) return rc;
+  TREX_CUDA_CHECK(e1); TREX_CUDA_CHECK(e2);
+  const double pi = 3.14159265358979323846;
+  const double gsN[2] = {std::pow(std::sqrt(4.0 * pi * theta_old[TREX_TH_ALPHA_S]), N), std::pow(std::sqrt(4.0 * pi * theta_new[TREX_TH_ALPHA_S]), N)};
+  for (int h = 0; h < nhel; ++h) {
+    const int lt = (h >> 2) & 1, ltb = (h >> 3) & 1;
+    unsigned gbits = 0;                                   // bit g = helicity of gluon g (legs 0, 1, 4, 5, ..)
+    for (int g = 0; g < N; ++g) gbits |= (unsigned)((h >> (g < 2 ? g : g + 2)) & 1) << g;
+    for (int s = 0; s < nc; ++s)
+      for (int th = 0; th < 2; ++th) {
+        size_t src;
+        if (N == 2) src = (size_t)((((gbits * 2 + lt) * 2 + s) * 2 + ltb) * 2 + th);
+        else {
+          const unsigned itb = gbits & ((1u << NFIX) - 1u), hfree = gbits >> NFIX;
+          const int lti = NLT == 2 ? lt : 0;
+          const int col = NLT == 2 ? (int)((hfree * 2 + ltb) * 2 + th) : (int)(((hfree * 2 + lt) * 2 + ltb) * 2 + th);
+          src = (((size_t)itb * NLT + lti) * nc + s) * NCOLT + col;
+        }
+        double* o = out + (((size_t)h * nc + s) * 2 + th) * 2;
+        o[0] = dump[2 * src] * gsN[th]; o[1] = dump[2 * src + 1] * gsN[th];
+      }
+  }
   return 0;
 }
 

@@ -28,6 +28,7 @@ struct Context {
   int nsm = 0;                       // multiprocessors of the device
   int64_t launches = 0;
   // diagnostics: CUDA events around every |M|^2 launch (trex_kernel_timing); implies no graph replay
+  double* dbg_out = nullptr;         // device buffer of trex_debug_xtile while it runs, else nullptr
   bool ktiming = false;
   std::vector<cudaEvent_t> kev;      // start/stop pairs recorded since the last trex_kernel_time
   std::vector<cudaEvent_t> kev_pool; // events free for reuse

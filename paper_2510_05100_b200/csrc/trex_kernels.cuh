@@ -27,6 +27,9 @@ struct ReweightArgs {
   const double* C120;
   ThetaPair T;
   QLineLegs q;
+  // diagnostics (trex_debug_xtile): when set, the production kernels copy the colour-flow amplitudes of event 0 here
+  // before the colour sum -- [iteration][flow][column][re, im]; nullptr in every product call
+  double* dbg;
 };
 
 // which events this launch works on: decided on the device for trex_run (the host has not seen the bucket sizes)
@@ -103,10 +106,12 @@ TREX_TU_DECL(5, 0) TREX_TU_DECL(5, 1) TREX_TU_DECL(5, 2)
 using TableLaunchFn = int (*)(const ReweightArgs&, int npass, long nmax, const int* meta, const double* Cfold, int nsm, cudaStream_t);
 using TableMetaFn = int (*)(int* meta);                       // fills the meta block (if non-null), returns its size in ints
 using TableFoldFn = int (*)(const double* C, double* f);      // fills the folded colour matrix (if non-null), returns its size
+using TableGeomFn = int (*)(int* out);                        // {NFIX, iterations, lambda_t passes, flows, columns} of the X-tile dump
 #define TREX_TABLE_DECL(N, M)                                                                                       \
   int trex_tu_table_launch_n##N##_m##M(const ReweightArgs&, int npass, long nmax, const int* meta, const double* Cfold, int nsm, cudaStream_t); \
   int trex_tu_table_meta_n##N##_m##M(int* meta);                                                                    \
-  int trex_tu_table_fold_n##N##_m##M(const double* C, double* f);
+  int trex_tu_table_fold_n##N##_m##M(const double* C, double* f);                                                   \
+  int trex_tu_table_geom_n##N##_m##M(int* out);
 TREX_TABLE_DECL(3, 0) TREX_TABLE_DECL(3, 1) TREX_TABLE_DECL(3, 2)
 TREX_TABLE_DECL(4, 0) TREX_TABLE_DECL(4, 1) TREX_TABLE_DECL(4, 2)
 TREX_TABLE_DECL(5, 0) TREX_TABLE_DECL(5, 1) TREX_TABLE_DECL(5, 2)

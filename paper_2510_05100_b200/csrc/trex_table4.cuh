@@ -427,6 +427,12 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
     w4_walk<R, RC, NPASS>(p, small[par], xs, a, par, tid);
     __syncthreads();
     W4_TICK(1);
+    if (a.dbg && e == 0)                                    // diagnostics only (trex_debug_xtile)
+      for (int i = tid; i < W::NC * G::NCOLT; i += W::TB) {
+        const int row = i / G::NCOLT, col = i - row * G::NCOLT;
+        const cx<RC> x = xs[row * W::XS + col];
+        a.dbg[2 * i] = (double)x.re; a.dbg[2 * i + 1] = (double)x.im;
+      }
     // ---- phase D: colour sum of this event | level 3 of the next one
     colour_phase<R, RC, 4>(xs, Cs, part, tid, tid);
     if (more) w4_build3<R, RC, NPASS>(p, small[par ^ 1], a, par ^ 1, tid);

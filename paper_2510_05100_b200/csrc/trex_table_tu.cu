@@ -665,6 +665,13 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
       }
       group_sync<GS>();
       PHASE_TICK(2);
+      if (a.dbg && e == 0)                                  // diagnostics only (trex_debug_xtile)
+        for (int i = gtid; i < G::NC * G::NCOLT; i += GS) {
+          const int row = i / G::NCOLT, col = i - row * G::NCOLT;
+          const cx<RC> x = xs[row * XS + col];
+          double* d = a.dbg + 2 * ((((long)itb * G::NLT + lti) * G::NC + row) * G::NCOLT + col);
+          d[0] = (double)x.re; d[1] = (double)x.im;
+        }
 
       colour_phase<R, RC, N>(xs, Cs, part, tid, gtid);
 #ifdef TREX_PHASE_CLOCKS
@@ -732,6 +739,13 @@ int TREX_TU_NAME(trex_tu_table_fold_n, TREX_TU_N, TREX_TU_MODE)(const double* C,
     }
   }
   return F::size();
+}
+
+// layout of the diagnostic X-tile dump: {NFIX, iterations, lambda_t passes per iteration, flows, columns per pass}
+int TREX_TU_NAME(trex_tu_table_geom_n, TREX_TU_N, TREX_TU_MODE)(int* out) {
+  using G = TabGeom<TuR, TuRC, TREX_TU_N>;
+  out[0] = G::NFIX; out[1] = G::NIT; out[2] = G::NLT; out[3] = G::NC; out[4] = G::NCOLT;
+  return 0;
 }
 
 int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const ReweightArgs& a, int npass, long nmax, const int* meta, const double* Cfold,

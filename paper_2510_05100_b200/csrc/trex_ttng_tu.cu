@@ -196,6 +196,10 @@ __global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(con
         const cx<RC> y(RC(x.re), RC(x.im));
         acc[th] += cd * norm2(y) + co * (y.re * xprev[iv][th].re + y.im * xprev[iv][th].im);
         xprev[iv][th] = y;
+        if (a.dbg && e == 0) {                              // diagnostics only (trex_debug_xtile): [unit][ordering][ltb][theta]
+          double* d = a.dbg + 2 * (((unit * 2 + ord) * 2 + iv) * 2 + th);
+          d[0] = (double)y.re; d[1] = (double)y.im;
+        }
       }
     }
   }

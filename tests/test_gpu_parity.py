@@ -177,6 +177,25 @@ def test_debug_flow_amps_five_gluons_one_helicity(T):
         assert np.all(np.abs(got[h] - ref) <= 1e-12 * scale)
 
 
+@pytest.mark.parametrize("sid,cfg,hels", [(1, 2, None), (2, 3, None), (3, 4, None), (4, 5, (0, 37, 77, 90, 127))])
+def test_production_kernels_colour_flow_amplitudes_match_oracle(T, sid, cfg, hels):
+    """SURVEY.md I-4 on the kernels trex_reweight launches and bench.py times (k_gg_tt, k_table<3>, k_table4w,
+    k_table<5>): the operand of their colour sum, every flow J_c at theta_old and theta_new, against the oracle's
+    colour-ordered amplitudes J0 + kappa J1 -- finer than the helicity- and colour-summed |M|^2."""
+    w = make_config(cfg, n=64)
+    tho, thn = w.theta_old, w.theta_new
+    for e in (0, 9):
+        mom1 = np.ascontiguousarray(w.momenta[:, :, e:e + 1])
+        got = T.trex_debug_xtile(sid, mom1[:, :, 0], tho, thn)
+        assert np.all(np.isfinite(got)) and np.abs(got).max() > 0
+        scale = np.abs(got).max(axis=(0, 1))
+        for h in (range(T.trex_nhel(sid)) if hels is None else hels):
+            for k, th in enumerate((tho, thn)):
+                ref = O.ttng_amps(sid, mom1, th, h)
+                want = ref[:, 0] + O.kappa(th) * ref[:, 1]
+                assert np.all(np.abs(got[h, :, k] - want) <= 1e-12 * scale[k]), (e, h, k)
+
+
 # ---------------------------------------------------------------- properties that hold at any size / edge cases
 def test_unit_ratio_zero_guard_and_empty(T):
     import torch
@@ -499,4 +518,110 @@ def test_reduced_precision_modes_every_config(T, cfg, n, mode):
         T.trex_set_precision(0)
     for g, r0 in zip(got, ref):
         r = rel(g, r0)
+        assert np.median(r) < 5e-5 and r.max() < 1e-3, (cfg, mode, np.median(r), r.max())
+
+
+# ---------------------------------------------------------------- adversarial kinematics, long double oracle as adjudicator
+def _event(sqrt_s, finals, th_star, phi_star, mt=173.0):
+    """2 -> t t~ + massless partons with the partons' momenta GIVEN (list of (E, theta, phi)): the t t~ pair recoils
+    against them and decays with angles (th_star, phi_star) in its rest frame. Test-side construction only."""
+    ps = []
+    for E, th, ph in finals:
+        ps.append(np.array([E, E * np.sin(th) * np.cos(ph), E * np.sin(th) * np.sin(ph), E * np.cos(th)]))
+    tot = np.array([sqrt_s, 0.0, 0.0, 0.0]) - sum(ps, np.zeros(4))
+    M = np.sqrt(tot[0] ** 2 - tot[1:] @ tot[1:])
+    assert M > 2 * mt
+    pstar = np.sqrt(M * M / 4 - mt * mt)
+    d = np.array([np.sin(th_star) * np.cos(phi_star), np.sin(th_star) * np.sin(phi_star), np.cos(th_star)])
+    out = []
+    beta = tot[1:] / tot[0]
+    g = tot[0] / M
+    for sgn in (1.0, -1.0):
+        k = sgn * pstar * d
+        e = M / 2
+        bk = beta @ k
+        b2 = beta @ beta
+        kk = k + ((g - 1.0) * bk / b2 + g * e) * beta if b2 > 0 else k
+        out.append(np.concatenate([[g * (e + bk)], kk]))
+    mom = [np.array([sqrt_s / 2, 0, 0, sqrt_s / 2]), np.array([sqrt_s / 2, 0, 0, -sqrt_s / 2])] + out + ps
+    return np.ascontiguousarray(np.array(mom)[:, :, None])
+
+
+ADVERSARIAL = [
+    # (sid, label, sqrt_s, partons (E, theta, phi), th*, phi*)
+    (1, "tops along the beam", 500.0, [], 0.0, 0.0),
+    (1, "tops nearly along the beam", 500.0, [], 1e-9, 0.3),
+    (1, "tops at threshold", 2 * 173.0 * (1 + 1e-9), [], 0.7, 1.1),
+    # (a massless final-state parton EXACTLY on the beam axis sits on the collinear pole 1 / (2 k_in . k_out) = 1 / 0 of
+    # the amplitude itself: there is no finite value to compare; the cases below approach it)
+    (2, "gluon 1e-3 from +z", 900.0, [(120.0, 1e-3, 0.0)], 0.8, 0.4),
+    (2, "gluon 1e-3 from -z", 900.0, [(120.0, np.pi - 1e-3, 2.0)], 0.8, 0.4),
+    (2, "gluon 1e-5 from +z", 900.0, [(120.0, 1e-5, 2.0)], 0.8, 0.4),
+    (2, "soft gluon", 900.0, [(0.09, 1.1, 0.2)], 1.3, 2.4),
+    (2, "gluon collinear to the beam", 900.0, [(200.0, 1e-4, 1.0)], 1.3, 2.4),
+    (2, "t t~ pair at threshold", 900.0, [((900.0 ** 2 - (2 * 173.0 * (1 + 1e-8)) ** 2) / (2 * 900.0), 0.9, 0.1)], 0.5, 0.6),
+    (3, "one gluon 1e-3 from -z, one soft", 1500.0, [(300.0, np.pi - 1e-3, 0.0), (0.15, 0.7, 1.9)], 1.0, 0.2),
+    (3, "collinear gluon pair", 1500.0, [(250.0, 1.0, 0.5), (180.0, 1.0 + 1e-4, 0.5)], 1.0, 0.2),
+    (4, "one gluon 1e-3 from +z, collinear pair", 2000.0, [(200.0, 1e-3, 0.0), (250.0, 2.0, 0.5), (100.0, 2.0 + 1e-4, 0.5)], 1.0, 0.2),
+    (5, "q q~: gluon 1e-3 from +z", 900.0, [(120.0, 1e-3, 0.0)], 0.8, 0.4),
+    (7, "q g: final quark 1e-3 from -z", 900.0, [(120.0, np.pi - 1e-3, 0.0)], 0.8, 0.4),
+    (8, "g q~: soft final antiquark", 900.0, [(0.09, 1.1, 0.2)], 0.8, 0.4),
+]
+
+
+@pytest.mark.parametrize("sid,label,sqrt_s,partons,ths,phs", ADVERSARIAL, ids=[a[1] for a in ADVERSARIAL])
+def test_adversarial_kinematics_against_long_double_oracle(T, sid, label, sqrt_s, partons, ths, phs):
+    """Degenerate phase-space corners (SURVEY P-13): tops on the beam axis (the pT -> 0 branch of the two-spinors),
+    final-state partons close to it, soft and collinear emissions, tops at threshold. The adjudicator is the
+    oracle in long double; the bar is 1e-11 where the double-precision oracle itself reaches it, else ten times the
+    oracle's own double-precision deviation (both sides then lose the same digits to the physical cancellation)."""
+    mom = _event(sqrt_s, partons, ths, phs)
+    tho, thn = default_theta(), default_theta()
+    thn[TH_CTG] = 0.8
+    if sid in (3, 4):
+        tho[TH_GAMMAT], thn[TH_GAMMAT] = 1.5, 1.35
+    w = np.array([1.7])
+    got = gpu_reweight(T, sid, mom, tho, thn, w)
+    ld = O.reweight(sid, mom, tho, thn, w, long_double=True)
+    db = O.reweight(sid, mom, tho, thn, w)
+    K = mom[:, :, 0].copy()
+    K[2:] *= -1.0                                            # all-incoming convention
+    light = [i for i in range(K.shape[0]) if i not in (2, 3)]
+    cond = 1.0
+    for i in light:
+        for j in light:
+            if i < j:
+                P = K[i] + K[j]
+                cond = max(cond, (abs(K[i, 0]) + abs(K[j, 0])) ** 2 / abs(P[0] ** 2 - P[1:] @ P[1:]))
+    for k, (g, a, b) in enumerate(zip(got, ld, db)):
+        assert np.all(np.isfinite(g)) and np.all(a > 0)
+        bar = max(RTOL64, 10.0 * float(rel(b, a).max()), 4 * 2.2e-16 * cond)
+        assert rel(g, a).max() < bar, (label, rel(g, a).max(), rel(b, a).max(), cond)
+    # the weight ratio is well conditioned wherever |M|^2 itself is finite
+    assert rel(got[0], ld[0]).max() < max(RTOL64, 10.0 * float(rel(db[0], ld[0]).max())), label
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 2048), (2, 4096), (3, 1536), (4, 96), (5, 12)])
+@pytest.mark.parametrize("mode", [1, 2])
+def test_reduced_precision_modes_against_the_oracle(T, cfg, n, mode):
+    """fptype m / f on every configuration against the ORACLE (not against the library's own fp64 result): median 5e-5,
+    maximum 1e-3 (north star)."""
+    w = make_config(cfg, n=n)
+    k, m, wi = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    T.trex_set_precision(mode)
+    try:
+        got = [x.cpu().numpy() for x in T.trex_run(k, m, w.theta_old, w.theta_new, wi)[:3]]
+    finally:
+        T.trex_set_precision(0)
+    ref = [np.zeros(n), np.zeros(n), np.zeros(n)]
+    for sp in w.classes:
+        sel = np.where(w.keys == sp.key)[0]
+        if sp.sid >= 5:
+            sel = sel[:24]                                   # explicit-colour engine: a sample of the quark channels
+        r = O.reweight(sp.sid, np.ascontiguousarray(w.momenta[:, :, sel]), w.theta_old, w.theta_new, w.w_in[sel])
+        for a, b in zip(ref, r):
+            a[sel] = b
+    ok = ref[1] != 0
+    for g, r0 in zip(got, ref):
+        r = rel(g[ok], r0[ok])
         assert np.median(r) < 5e-5 and r.max() < 1e-3, (cfg, mode, np.median(r), r.max())

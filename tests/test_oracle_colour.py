@@ -81,6 +81,19 @@ def test_colour_ordered_engine_equals_brute_force_with_four_gluon_vertex():
     assert relclose(a, b, rtol=1e-11), (a, b)
 
 
+def test_colour_ordered_engine_equals_brute_force_at_five_gluons():
+    """gg -> tt~ggg, one helicity: the explicit-colour engine E2 needs 8^5 x 9 colour assignments (five minutes on one
+    core), so its (A, B, D) are stored by tests/golden/make_e2_n5.py (a committed script that calls only oracle/). E1 is
+    the engine every n = 5 parity test uses; this is its only pin that is neither a symmetry nor E1 itself."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "e2_n5_single_helicity.txt")
+    ref = np.array([float(x) for x in [l for l in open(path) if not l.startswith("#")][0].split()])
+    w = make_config(5, n=8)
+    a = O.abd(4, w.momenta[:, :, :1], default_theta(), engine=1, hel_only=77)[0]
+    assert relclose(a, ref, rtol=1e-11), (a, ref)
+    assert np.all(ref > 0) and ref[1] ** 2 <= 4 * ref[0] * ref[2]
+
+
 def test_helicity_sum_is_sum_of_single_helicities():
     th = default_theta()
     w = make_config(2, n=2)
