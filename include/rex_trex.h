@@ -120,6 +120,22 @@ int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int
  * their event order; the identity for events no subprocess claims. Asynchronous on the library stream. */
 int rex_keys(const int32_t* pdg_soa, int npar, int n_in, int64_t n, uint64_t* keys, int8_t* legmap);
 
+/* Flavour keys under a comparator with a status filter (eventComparatorConfig::set_status_filter; the two
+ * comparators of Alg.1): only partons whose status is in status_filter (HOST [nfilter], values out of
+ * {-1, 1, 2}; nfilter == 0: no filtering) take part; two events get the same key iff those partons agree as unordered
+ * (status, PDG code) collections. pdg_soa DEVICE int32 [nlegs][n], status_soa DEVICE int8 [nlegs][n], nlegs <= 16 (all
+ * partons of the event record, intermediate ones included); keys DEVICE [n] out. Layout: kept partons with status -1
+ * first, then status 1, then status 2, each group sorted ascending by PDG code, one byte each as in rex_pack_key; byte 7 =
+ * n_intermediate << 6 | n_in << 4 | n_out -- for the filter {-1, 1} and no intermediate partons this is rex_pack_key's
+ * key, for {1} the two events of Alg.1 (g g > t t~, u u~ > t t~) fall into one class. More than 7 kept partons, |pdg| >
+ * 127, or (without a filter) a status outside {-1, 1, 2} give REX_NPOS. Feed the keys to rex_bucket / trex_run as usual.
+ * Relative tolerances on double-valued traits are not offered: such a comparison is not an equivalence
+ * relation, its classes depend on the order in which representatives are met. Asynchronous on the library stream. */
+int rex_keys_filtered(const int32_t* pdg_soa, const int8_t* status_soa, int nlegs, int64_t n, const int32_t* status_filter,
+                      int nfilter, uint64_t* keys);
+/* HOST helper: the same key for one event (pdg, status HOST [nlegs]). */
+uint64_t rex_pack_key_filtered(const int32_t* pdg, const int8_t* status, int nlegs, const int32_t* status_filter, int nfilter);
+
 /* trex_run for events given by PDG codes in arbitrary parton order: rex_keys, then the path of trex_run with the
  * transposition re-indexing every event's legs to the process-string order. momenta_soa [npar][4][n] in the events'
  * own leg order. Same outputs and return value as trex_run. */

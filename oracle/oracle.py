@@ -215,6 +215,36 @@ def flavour_key(pdg, n_in):
     return np.uint64(key)
 
 
+def comparator_equal(pdg1, status1, pdg2, status2, status_filter=(-1, 1)):
+    """The event comparison an eventComparatorConfig with set_pdg(true) and the given status_filter defines
+    (PAPER.md:227-231): only partons whose status is in status_filter take part (an empty filter means no filtering),
+    and two events are equal iff those partons agree as unordered (status, PDG code) collections (the default comparator
+    compares unordered external legs; Alg.1). Written out as the definition."""
+    def legs(pdg, status):
+        return sorted((int(s), int(p)) for p, s in zip(pdg, status) if len(status_filter) == 0 or int(s) in status_filter)
+    return legs(pdg1, status1) == legs(pdg2, status2)
+
+
+def flavour_key_filtered(pdg, status, status_filter=(-1, 1)):
+    """Key of one event under the comparator above: the partons the filter keeps, incoming (status < 0) first, then
+    final (status 1), then everything else (intermediate: 2, 3, ...), each group sorted ascending by PDG code; one byte
+    per parton as in flavour_key; byte 7 = n_other << 6 | n_in << 4 | n_out. More than 7 kept partons, more than 3
+    incoming or intermediate ones, statuses outside {-1, 1, 2}, or |pdg| > 127 give REX_NPOS. For events without
+    intermediate partons and the filter {-1, 1} this is flavour_key."""
+    keep = [(int(s), int(p)) for p, s in zip(pdg, status) if len(status_filter) == 0 or int(s) in status_filter]
+    ini = sorted(p for s, p in keep if s == -1)
+    fin = sorted(p for s, p in keep if s == 1)
+    oth = sorted(p for s, p in keep if s == 2)
+    legs = ini + fin + oth
+    if (len(legs) != len(keep) or len(legs) > 7 or len(ini) > 3 or len(oth) > 3 or any(abs(p) > 127 for p in legs)):
+        return np.uint64(0xFFFFFFFFFFFFFFFF)
+    key = 0
+    for i, p in enumerate(legs):
+        key |= ((abs(p) & 0x7F) | (0x80 if p < 0 else 0)) << (8 * i)
+    key |= ((len(oth) << 6) | (len(ini) << 4) | len(fin)) << 56
+    return np.uint64(key)
+
+
 def keys_and_legmap(pdg, n_in, process_strings):
     """pdg int [npar, n]; process_strings: the PDG tuples of the compiled-in subprocesses in process-string order.
     Returns (keys uint64 [n], legmap int8 [npar, n]): legmap[pos, i] = the leg of event i that plays position `pos` of the

@@ -25,6 +25,8 @@ _vp, _i64, _i32, _int = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.
 _dp = ctypes.POINTER(ctypes.c_double)
 _SIGNATURES = {
     "rex_pack_key": (ctypes.c_uint64, [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int8), _int]),
+    "rex_pack_key_filtered": (ctypes.c_uint64, [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int8), _int, ctypes.POINTER(ctypes.c_int32), _int]),
+    "rex_keys_filtered": (_int, [_vp, _vp, _int, _i64, ctypes.POINTER(ctypes.c_int32), _int, _vp]),
     "rex_bucket": (_int, [_vp, _i64, _vp, ctypes.POINTER(ctypes.c_int64)]),
     "rex_bucket_keys": (_int, [ctypes.POINTER(ctypes.c_uint64)]),
     "rex_gather": (_int, [_vp, _i64, _vp, _i64, _int, _vp]),
@@ -136,6 +138,14 @@ def rex_pack_key(pdg, status):
     s = np.ascontiguousarray(status, dtype=np.int8)
     return int(lib().rex_pack_key(p.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
                                   s.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)), len(p)))
+
+
+def rex_pack_key_filtered(pdg, status, status_filter=(-1, 1)):
+    p = np.ascontiguousarray(pdg, dtype=np.int32)
+    s = np.ascontiguousarray(status, dtype=np.int8)
+    f = np.ascontiguousarray(list(status_filter), dtype=np.int32)
+    return int(lib().rex_pack_key_filtered(p.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), s.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)),
+                                           len(p), f.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), len(f)))
 
 
 def trex_subproc_id(key):
@@ -307,6 +317,20 @@ def rex_keys(pdg_soa, n_in, want_legmap=True):
     _check(lib().rex_keys(_dev(pdg_soa, torch.int32, "pdg_soa"), npar, int(n_in), n, _dev(keys, torch.int64, "keys"),
                           _dev(legmap, torch.int8, "legmap")), "rex_keys")
     return keys, legmap
+
+
+def rex_keys_filtered(pdg_soa, status_soa, status_filter=(-1, 1)):
+    """Flavour keys under a comparator with a status filter: pdg_soa int32 [nlegs, n], status_soa int8 [nlegs, n] CUDA
+    tensors; returns the keys (int64 view of the uint64 keys) [n]."""
+    torch = _torch()
+    nlegs, n = int(pdg_soa.shape[0]), int(pdg_soa.shape[1])
+    if tuple(status_soa.shape) != (nlegs, n):
+        raise TrexError("rex_keys_filtered: status_soa must have shape (%d, %d)" % (nlegs, n))
+    f = np.ascontiguousarray(list(status_filter), dtype=np.int32)
+    keys = torch.empty(n, dtype=torch.int64, device=pdg_soa.device)
+    _check(lib().rex_keys_filtered(_dev(pdg_soa, torch.int32, "pdg_soa"), _dev(status_soa, torch.int8, "status_soa"), nlegs, n,
+                                   f.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), len(f), _dev(keys, torch.int64, "keys")), "rex_keys_filtered")
+    return keys
 
 
 def trex_run_pdg(pdg_soa, momenta_soa, n_in, theta_old, theta_new, w_in, w_out=None, me2_old=None, me2_new=None, want_me2=True):

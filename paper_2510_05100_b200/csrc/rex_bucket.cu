@@ -403,6 +403,42 @@ __global__ void __launch_bounds__(256) k_keys(const int* __restrict__ pdg, int n
   }
 }
 
+// flavour key under a comparator with a status filter (Alg.1 :419-444): the partons whose status the
+// filter keeps -- incoming (-1) first, then final (1), then intermediate (2), each group sorted ascending by PDG code --
+// one byte per parton as in rex_pack_key; byte 7 = n_other << 6 | n_in << 4 | n_out. fmask: bit 0 keeps status -1,
+// bit 1 status 1, bit 2 status 2, bit 3 = no filtering at all (then any other status makes the event "no class").
+__host__ __device__ inline unsigned long long filtered_key(const int* pdg, const signed char* status, int nlegs, long stride, unsigned fmask) {
+  int grp[3][8];
+  int cnt[3] = {0, 0, 0};
+  bool bad = false;
+  for (int l = 0; l < nlegs; ++l) {
+    const int st = status[(long)l * stride], q = pdg[(long)l * stride];
+    const int g = st == -1 ? 0 : (st == 1 ? 1 : (st == 2 ? 2 : -1));
+    if (g < 0) { bad = bad || (fmask & 8u); continue; }
+    if (!(fmask & 8u) && !((fmask >> g) & 1u)) continue;
+    if (cnt[g] >= 7 || q > 127 || q < -127) { bad = true; continue; }
+    int b = cnt[g]++;
+    while (b > 0 && grp[g][b - 1] > q) { grp[g][b] = grp[g][b - 1]; --b; }      // insertion sort inside the group
+    grp[g][b] = q;
+  }
+  if (bad || cnt[0] + cnt[1] + cnt[2] > 7 || cnt[0] > 3 || cnt[2] > 3) return REX_NPOS;
+  unsigned long long key = 0;
+  int pos = 0;
+  for (int g = 0; g < 3; ++g)
+    for (int i = 0; i < cnt[g]; ++i) {
+      const int q = grp[g][i];
+      key |= (unsigned long long)(((q < 0 ? -q : q) & 0x7F) | (q < 0 ? 0x80 : 0)) << (8 * pos++);
+    }
+  return key | (unsigned long long)((cnt[2] << 6) | (cnt[0] << 4) | cnt[1]) << 56;
+}
+
+__global__ void __launch_bounds__(256) k_keys_filtered(const int* __restrict__ pdg, const signed char* __restrict__ status, int nlegs, long n,
+                                                       unsigned fmask, unsigned long long* __restrict__ keys) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  keys[i] = filtered_key(pdg + i, status + i, nlegs, n, fmask);
+}
+
 // momenta rows + weights into bucketed order; result rows cleared (classes nobody claims keep zero weights)
 __global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __restrict__ mom, const double* __restrict__ w_in, long n,
                              int nrows, const int* __restrict__ perm, double* __restrict__ blk, double* __restrict__ res,
@@ -557,6 +593,36 @@ extern "C" int rex_keys(const int32_t* pdg_soa, int npar, int n_in, int64_t n, u
   if (int rc = ensure_plan()) return rc;
   k_keys<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(pdg_soa, npar, n_in, n, (const unsigned long long*)c.plan_keys,
                                                            (unsigned long long*)keys, (signed char*)legmap);
+  c.launches += 1;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return 0;
+}
+
+static bool filter_mask(const int32_t* status_filter, int nfilter, unsigned& fmask) {
+  if (nfilter < 0 || (nfilter > 0 && !status_filter)) return false;
+  fmask = nfilter == 0 ? 8u : 0u;
+  for (int k = 0; k < nfilter; ++k) {
+    const int st = status_filter[k];
+    if (st == -1) fmask |= 1u; else if (st == 1) fmask |= 2u; else if (st == 2) fmask |= 4u; else return false;
+  }
+  return true;
+}
+
+extern "C" uint64_t rex_pack_key_filtered(const int32_t* pdg, const int8_t* status, int nlegs, const int32_t* status_filter, int nfilter) {
+  unsigned fmask = 0;
+  if (!pdg || !status || nlegs < 0 || nlegs > 16 || !filter_mask(status_filter, nfilter, fmask)) return REX_NPOS;
+  return filtered_key(pdg, (const signed char*)status, nlegs, 1, fmask);
+}
+
+extern "C" int rex_keys_filtered(const int32_t* pdg_soa, const int8_t* status_soa, int nlegs, int64_t n, const int32_t* status_filter,
+                                 int nfilter, uint64_t* keys) {
+  Context& c = ctx();
+  unsigned fmask = 0;
+  if (n < 0 || nlegs < 1 || nlegs > 16) return fail(TREX_EINVAL, "rex_keys_filtered: bad size (1 <= nlegs <= 16)");
+  if (!filter_mask(status_filter, nfilter, fmask)) return fail(TREX_EINVAL, "rex_keys_filtered: the filter may hold the statuses -1, 1, 2");
+  if (n == 0) return 0;
+  if (!pdg_soa || !status_soa || !keys) return fail(TREX_EINVAL, "rex_keys_filtered: null device pointer");
+  k_keys_filtered<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(pdg_soa, (const signed char*)status_soa, nlegs, n, fmask, (unsigned long long*)keys);
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());
   return 0;

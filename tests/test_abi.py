@@ -118,3 +118,31 @@ def test_argument_errors_do_not_crash(lib):
     off = (ctypes.c_int64 * 257)()
     assert lib.rex_bucket(None, 0, None, off) == 0 and off[0] == 0
     assert lib.rex_bucket(None, 5, None, off) == -1
+
+
+def test_filtered_key_host_helper_matches_the_oracle_comparator(lib):
+    """rex_pack_key_filtered against the oracle's key AND against the comparator definition (Alg.1)."""
+    from oracle import oracle as O
+    rng = np.random.default_rng(4)
+    flav = [21, 2, -2, 1, 6, -6, 23, 25]
+    evs = []
+    for _ in range(80):
+        n = int(rng.integers(3, 9))
+        st = [-1, -1] + [int(x) for x in rng.choice([1, 1, 1, 2], size=n - 2)]
+        evs.append(([int(x) for x in rng.choice(flav, size=n)], st))
+    for filt in ((-1, 1), (1,), (), (1, 2), (-1,)):
+        keys = []
+        for p, s in evs:
+            k = T.rex_pack_key_filtered(p, s, filt)
+            assert k == int(O.flavour_key_filtered(p, s, status_filter=filt))
+            keys.append(k)
+        for i in range(len(evs)):
+            for j in range(i):
+                if keys[i] != T.REX_NPOS and keys[j] != T.REX_NPOS:
+                    assert (keys[i] == keys[j]) == O.comparator_equal(*evs[i], *evs[j], status_filter=filt)
+    # Alg.1: the two events differ under the external-leg comparator and are equal under the final-state one
+    a, b = ([21, 21, 6, -6], [-1, -1, 1, 1]), ([2, -2, 6, -6], [-1, -1, 1, 1])
+    assert T.rex_pack_key_filtered(*a, (-1, 1)) != T.rex_pack_key_filtered(*b, (-1, 1))
+    assert T.rex_pack_key_filtered(*a, (1,)) == T.rex_pack_key_filtered(*b, (1,))
+    assert T.rex_pack_key_filtered(*a, (-1, 1)) == T.rex_pack_key(*a)
+    assert T.rex_pack_key_filtered(*a, (7,)) == T.REX_NPOS                      # a status the filter cannot hold

@@ -625,3 +625,30 @@ def test_reduced_precision_modes_against_the_oracle(T, cfg, n, mode):
     for g, r0 in zip(got, ref):
         r = rel(g[ok], r0[ok])
         assert np.median(r) < 5e-5 and r.max() < 1e-3, (cfg, mode, np.median(r), r.max())
+
+
+def test_status_filter_comparators_on_the_device(T):
+    """NEXT-3 (Alg.1 :419-444): keys under comparators with a status filter, bit-exact against the
+    oracle; under the final-state-only comparator g g > t t~ g and q q~ > t t~ g fall into one class, and rex_bucket
+    orders the classes by first appearance as ever."""
+    import torch
+    w = make_config(3, n=20011)
+    pdg, mom, n_in = shuffled_legs(w, 17, unknown_every=0)
+    rng = np.random.default_rng(8)
+    nl = w.npar + 1                                          # one intermediate parton (status 2) per event record
+    pdg2 = np.vstack([pdg, rng.choice([23, 25, 6], size=(1, w.n)).astype(np.int32)])
+    st = np.vstack([np.full((2, w.n), -1), np.ones((w.npar - 2, w.n)), np.full((1, w.n), 2)]).astype(np.int8)
+    col = rng.permuted(np.tile(np.arange(nl)[:, None], (1, w.n)), axis=0)         # records in arbitrary parton order
+    pdg2, st = np.take_along_axis(pdg2, col, 0), np.take_along_axis(st, col, 0)
+    dp, ds = torch.from_numpy(np.ascontiguousarray(pdg2)).cuda(), torch.from_numpy(np.ascontiguousarray(st)).cuda()
+    for filt in ((-1, 1), (1,), (), (1, 2)):
+        keys = T.rex_keys_filtered(dp, ds, filt).cpu().numpy().view(np.uint64)
+        ref = np.array([O.flavour_key_filtered(pdg2[:, i], st[:, i], status_filter=filt) for i in range(w.n)], dtype=np.uint64)
+        assert np.array_equal(keys, ref), filt
+        perm, offsets, bkeys = T.rex_bucket(dev(keys))
+        rperm, roff, rkeys = O.bucket(ref)
+        assert np.array_equal(perm.cpu().numpy(), rperm) and np.array_equal(offsets, roff) and np.array_equal(bkeys, rkeys)
+    ext = T.rex_keys_filtered(dp, ds, (-1, 1)).cpu().numpy().view(np.uint64)
+    fin = T.rex_keys_filtered(dp, ds, (1,)).cpu().numpy().view(np.uint64)
+    assert np.array_equal(ext, w.keys)                       # the external-leg comparator is the default key
+    assert len(np.unique(ext)) == 5 and len(np.unique(fin)) == 3          # t t~ g | t t~ u | t t~ u~

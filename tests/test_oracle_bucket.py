@@ -62,3 +62,39 @@ def test_gather_is_the_soa_transpose():
     for j in range(37):
         assert np.array_equal(dst[:, :, j], src[:, :, perm[j]])
     assert sorted(perm.tolist()) == list(range(37))
+
+
+# ---------------------------------------------------------------- comparators with a status filter (Alg.1)
+def test_alg1_example_both_halves():
+    """Alg.1: g g > t t~ and u u~ > t t~ DIFFER under the comparator over all external legs and are
+    EQUAL under the comparator over final-state particles only."""
+    ev1 = ([21, 21, 6, -6], [-1, -1, 1, 1])
+    ev2 = ([2, -2, 6, -6], [-1, -1, 1, 1])
+    assert not O.comparator_equal(*ev1, *ev2, status_filter=(-1, 1))
+    assert O.comparator_equal(*ev1, *ev2, status_filter=(1,))
+    assert O.flavour_key_filtered(*ev1, status_filter=(-1, 1)) != O.flavour_key_filtered(*ev2, status_filter=(-1, 1))
+    assert O.flavour_key_filtered(*ev1, status_filter=(1,)) == O.flavour_key_filtered(*ev2, status_filter=(1,))
+    # with the external-leg filter and no intermediate partons the key is the default one
+    assert O.flavour_key_filtered(*ev1) == O.flavour_key(ev1[0], 2)
+
+
+def test_filtered_key_equality_is_exactly_the_comparator():
+    """Brute force: for random small events (statuses -1, 1, 2; a few flavours) and every filter, two keys are equal iff
+    the comparator -- written out as the paper's definition -- calls the events equal."""
+    rng = np.random.default_rng(12)
+    flav = [21, 2, -2, 6, -6, 23]
+    evs = []
+    for _ in range(60):
+        n = int(rng.integers(3, 7))
+        st = [-1, -1] + [int(x) for x in rng.choice([1, 1, 1, 2], size=n - 2)]
+        evs.append(([int(x) for x in rng.choice(flav, size=n)], st))
+    for filt in ((-1, 1), (1,), (-1,), (), (1, 2), (-1, 1, 2)):
+        keys = [int(O.flavour_key_filtered(p, s, status_filter=filt)) for p, s in evs]
+        assert all(k != 0xFFFFFFFFFFFFFFFF for k in keys)
+        for i in range(len(evs)):
+            for j in range(i):
+                assert (keys[i] == keys[j]) == O.comparator_equal(*evs[i], *evs[j], status_filter=filt), (filt, evs[i], evs[j])
+    # what the key cannot hold is "no class"
+    assert int(O.flavour_key_filtered([21] * 9, [-1, -1] + [1] * 7)) == 0xFFFFFFFFFFFFFFFF
+    assert int(O.flavour_key_filtered([21, 21, 1000022], [-1, -1, 1])) == 0xFFFFFFFFFFFFFFFF
+    assert int(O.flavour_key_filtered([21, 21, 6], [-1, -1, -2], status_filter=())) == 0xFFFFFFFFFFFFFFFF
