@@ -34,7 +34,7 @@ HEADLINE_EVENTS = 1048576
 L2_NOTE = "256 MiB buffer written between timed iterations (L2 flush)"
 SID_OF_CFG = {1: 0, 2: 1, 4: 3, 5: 4}
 KERNEL_OF_CFG = {1: "k_eemumu<double>", 2: "k_gg_tt<double,double>", 3: "k_table<double,double,3,1> + k_qq<double,double>",
-                 4: "k_table<double,double,4,2>", 5: "k_table<double,double,5,1>"}
+                 4: "k_table4w<double,double,2>", 5: "k_table<double,double,5,1>", 6: "k_table<double,double,3,1> + k_qq<double,double>"}
 # nominal FP64 vector peak of B200: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
@@ -106,7 +106,7 @@ class ClockSampler:
 
 # seeded sample of each workload the oracle is timed on (about 10-30 s of host work; the rate is per event, so the
 # sample size only sets the resolution)
-ORACLE_SAMPLE = {1: 4096, 2: 65536, 3: 2048, 4: 4096, 5: 384}
+ORACLE_SAMPLE = {1: 4096, 2: 65536, 3: 2048, 4: 4096, 5: 384, 6: 4096}
 
 
 def cpu_oracle_rate(cfg, budget_s=20.0, n_sample=None):
@@ -117,7 +117,7 @@ def cpu_oracle_rate(cfg, budget_s=20.0, n_sample=None):
     w = make_config(cfg, n=n_sample)
     O.reweight(SID_OF_CFG.get(cfg, 2), np.ascontiguousarray(w.momenta[:, :, :8]), w.theta_old, w.theta_new, w.w_in[:8])  # load + colour tables
     cores = os.cpu_count()
-    if cfg == 3:
+    if cfg in (3, 6):
         t_class = {}
         for sp in w.classes:
             sel = np.where(w.keys == sp.key)[0]
@@ -130,8 +130,8 @@ def cpu_oracle_rate(cfg, budget_s=20.0, n_sample=None):
         frac = {sp.sid: float(np.mean(w.keys == sp.key)) for sp in w.classes}
         per_event = sum(frac[s] * t_class[s] for s in frac)
         return {"value": 1.0 / per_event, "unit": UNIT, "cores": cores, "kind": "oracle",
-                "sample": "cfg3 seeded sample of %d events; per-class time per event weighted by class fraction "
-                          "(quark channels on 1/64 of their events)" % n_sample}
+                "sample": "cfg%d seeded sample of %d events; per-class time per event weighted by class fraction "
+                          "(quark channels on 1/64 of their events)" % (cfg, n_sample)}
     done, t0 = 0, time.perf_counter()
     while True:
         O.reweight(SID_OF_CFG[cfg], w.momenta, w.theta_old, w.theta_new, w.w_in)
@@ -391,7 +391,7 @@ def main():
 
     configs = {}
     if args.configs == "all":
-        for cfg, warm, steps in ((1, 3, 20), (2, 3, 20), (3, 3, 10), (5, 3, 10)):
+        for cfg, warm, steps in ((1, 3, 20), (2, 3, 20), (3, 3, 10), (5, 3, 10), (6, 3, 10)):
             configs["cfg%d" % cfg] = measure(cfg, warm, steps, with_e2e=(cfg != 1))
         configs["cfg4_mixed"] = measure(4, 3, 10, precision=1)
         configs["cfg4_fp32"] = measure(4, 3, 10, precision=2)
@@ -407,7 +407,7 @@ def main():
     if rank == 0 and not args.no_cpu_baseline:
         cpu = cpu_oracle_rate(HEADLINE_CFG)
         if args.configs == "all" and world == 1:
-            for cfg in (1, 2, 3, 5):
+            for cfg in (1, 2, 3, 5, 6):
                 configs["cfg%d" % cfg]["cpu_baseline"] = cpu_oracle_rate(cfg, budget_s=8.0)
 
     if rank == 0:

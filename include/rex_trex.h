@@ -54,7 +54,13 @@ enum { TREX_SP_EEMUMU = 0,   /* e- e+ > mu- mu+   (photon + Z)          */
        TREX_SP_DDX_TTG = 6,  /* d d~ > t t~ g                           */
        TREX_SP_UG_TTU = 7,   /* u g > t t~ u                            */
        TREX_SP_GUX_TTUX = 8, /* g u~ > t t~ u~                          */
-       TREX_NSUBPROC = 9 };
+       TREX_SP_RESERVED = 9, /* no kernel (keeps the numbering of the ids below free of gaps elsewhere)          */
+       /* the same three one-light-line channels for the other massless flavours (QCD does not see the flavour; the two
+        * beam orders of a channel share one flavour key and are re-indexed by trex_run_pdg)                        */
+       TREX_SP_SSX_TTG = 10, TREX_SP_CCX_TTG = 11, TREX_SP_BBX_TTG = 12,                         /* q q~ > t t~ g   */
+       TREX_SP_DG_TTD = 13, TREX_SP_SG_TTS = 14, TREX_SP_CG_TTC = 15, TREX_SP_BG_TTB = 16,       /* q g > t t~ q    */
+       TREX_SP_GDX_TTDX = 17, TREX_SP_GSX_TTSX = 18, TREX_SP_GCX_TTCX = 19, TREX_SP_GBX_TTBX = 20, /* g q~ > t t~ q~ */
+       TREX_NSUBPROC = 21 };
 
 /* ---- flavour keys (PAPER.md:334 default comparator: unordered PDG codes of external legs, initial and final state
  * kept apart; Alg.1).

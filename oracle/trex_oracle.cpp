@@ -736,9 +736,17 @@ template <class R> ABD<R> e2_abd(const Event<R>& ev, const Params<R>& P, int kin
 
 // ---------------------------------------------------------------- subprocess dispatch (ids of include/rex_trex.h)
 // 0 e-e+->mu-mu+ ; 1..4 gg->tt~+{0,1,2,3}g (E1) ; 5,6 q q~->tt~g ; 7 u g->tt~u ; 8 g u~->tt~u~ (E2)
-// 9 (oracle only, for the closed-form pin F-4): u u~ -> t t~
-inline int npar_of(int sid) { static const int t[10] = {4, 4, 5, 6, 7, 5, 5, 5, 5, 4}; return (sid >= 0 && sid < 10) ? t[sid] : -1; }
-inline int kind_of(int sid) { return sid <= 4 ? K_TTNG : ((sid <= 6 || sid == 9) ? K_QQB : (sid == 7 ? K_QG : K_GQB)); }
+// 9 (oracle only, for the closed-form pin F-4): u u~ -> t t~ ; 10..20: further flavours, see npar_of
+// 10..20: the same three one-light-line channels for the other massless flavours -- QCD does not see the flavour, it only
+// labels the class: 10, 11, 12 = s s~, c c~, b b~ > t t~ g ; 13..16 = d g, s g, c g, b g > t t~ q ; 17..20 = g d~, g s~,
+// g c~, g b~ > t t~ q~
+inline int npar_of(int sid) {
+  static const int t[10] = {4, 4, 5, 6, 7, 5, 5, 5, 5, 4};
+  if (sid >= 0 && sid < 10) return t[sid];
+  return (sid >= 10 && sid <= 20) ? 5 : -1; }
+inline int kind_of(int sid) {
+  if (sid >= 10) return sid <= 12 ? K_QQB : (sid <= 16 ? K_QG : K_GQB);
+  return sid <= 4 ? K_TTNG : ((sid <= 6 || sid == 9) ? K_QQB : (sid == 7 ? K_QG : K_GQB)); }
 
 template <class R> R me2_one(int sid, const Event<R>& ev, const double* theta) {
   Params<R> P(theta);

@@ -13,6 +13,9 @@ TREX_NTHETA = 16
 SUBPROCESS_IDS = {
     "e- e+ > mu- mu+": 0, "g g > t t~": 1, "g g > t t~ g": 2, "g g > t t~ g g": 3, "g g > t t~ g g g": 4,
     "u u~ > t t~ g": 5, "d d~ > t t~ g": 6, "u g > t t~ u": 7, "g u~ > t t~ u~": 8,
+    "s s~ > t t~ g": 10, "c c~ > t t~ g": 11, "b b~ > t t~ g": 12,
+    "d g > t t~ d": 13, "s g > t t~ s": 14, "c g > t t~ c": 15, "b g > t t~ b": 16,
+    "g d~ > t t~ d~": 17, "g s~ > t t~ s~": 18, "g c~ > t t~ c~": 19, "g b~ > t t~ b~": 20,
 }
 
 

@@ -29,20 +29,38 @@ namespace {
 //   phase A2: the 10 light-line currents (Jq[c]; Jq3[c][lambda_g], Jq4[c][lambda_g]: the line after radiating the gluon at
 //             its row / column end), one per warp
 //   phase B : warp = unit: top line (qq_close) with operands read back (lane = event: conflict-free)
+// per class: legs of the light line and 1 / N_avg (0 for ids that are not quark channels)
+__constant__ QLineLegs c_qlegs[TREX_NSUBPROC];
+__constant__ double c_qinvnavg[TREX_NSUBPROC];
+
 template <class R, class RC>
 __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightArgs a) {
   static_assert(WARPS == 8, "one allowed helicity unit per warp");
   __shared__ double pm[20][32];
   __shared__ double wf[10][8][32];
   __shared__ double cur[10][8][32];
-  const EvIO io = resolve_io(a);
-  if ((long)blockIdx.x * 32 >= io.n) return;
+  // which class this block belongs to: given by the call (trex_reweight), or found in the device plan when one launch
+  // serves every quark-channel class of a run (blocks are dealt to the classes in id order, 32 events each)
+  int sid = a.sid;
+  long blk = blockIdx.x;
+  if (a.plan && a.qfamily) {
+    sid = -1;
+    for (int s = 0; s < TREX_NSUBPROC; ++s) {
+      if (c_qinvnavg[s] == 0.0) continue;
+      const long nb = (a.plan->cnt[s] + 31) >> 5;
+      if (blk < nb) { sid = s; break; }
+      blk -= nb;
+    }
+    if (sid < 0) return;
+  }
+  const EvIO io = resolve_io(a, sid);
+  if (blk * 32 >= io.n) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long e = (long)blockIdx.x * 32 + lane;
+  const long e = blk * 32 + lane;
   const long ev = e < io.n ? e : io.n - 1;
   for (int r = warp; r < 20; r += WARPS) pm[r][lane] = io.mom[(long)r * io.ld + ev];
   __syncthreads();
-  const QLineLegs L = a.q;
+  const QLineLegs L = c_qlegs[sid];
   const bool row_in = L.lrow < 2, col_in = L.lcol < 2, g_in = L.lg < 2;
   auto leg = [&](int l, double p[4]) {
 #pragma unroll
@@ -157,7 +175,7 @@ __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightA
     double s0 = 0.0, s1 = 0.0;
 #pragma unroll
     for (int w = 0; w < WARPS; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
-    const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
+    const double mo = s0 * (a.T.gs2nv[0] * c_qinvnavg[sid]), mn = s1 * (a.T.gs2nv[1] * c_qinvnavg[sid]);
     const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
     io.w_out[e] = io.w_in[e] * norm * mn;                      // evaluate + append_wgts
     if (io.me2_old) io.me2_old[e] = mo;
@@ -273,6 +291,15 @@ int ensure_colour() {
       TREX_CUDA_CHECK(cudaMemcpy(c.C120, C.data(), sizeof(double) * C.size(), cudaMemcpyHostToDevice));
     }
   }
+  QLineLegs ql[TREX_NSUBPROC];
+  double qi[TREX_NSUBPROC];
+  for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
+    const SubprocInfo* sp = subproc_info(sid);
+    ql[sid] = sp ? sp->qlegs : QLineLegs{0, 0, 0};
+    qi[sid] = (sp && is_quark_channel(sid)) ? 1.0 / sp->navg : 0.0;
+  }
+  TREX_CUDA_CHECK(cudaMemcpyToSymbol(c_qlegs, ql, sizeof ql));
+  TREX_CUDA_CHECK(cudaMemcpyToSymbol(c_qinvnavg, qi, sizeof qi));
   c.colour_ready = true;
   return 0;
 }
@@ -285,6 +312,7 @@ using namespace trex;
 extern "C" int trex_subproc_id(uint64_t key) {
   for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
     const SubprocInfo* sp = subproc_info(sid);
+    if (!sp) continue;
     int8_t status[7];
     for (int i = 0; i < sp->npar; ++i) status[i] = i < 2 ? -1 : 1;
     if (rex_pack_key(sp->pdg, status, sp->npar) == key) return sid;
@@ -327,6 +355,7 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
   const SubprocInfo* sp = subproc_info(sid);
   if (int rc = ensure_colour()) return rc;
   a.T = T; a.sid = sid; a.q = sp->qlegs; a.C120 = c.C120; a.dbg = c.dbg_out;
+  if (!a.plan || !is_quark_channel(sid)) a.qfamily = 0;
   const unsigned grid32 = (unsigned)((nmax + 31) / 32);
   const int mode = c.precision;
   cudaEvent_t kt[2] = {nullptr, nullptr};
@@ -351,9 +380,11 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
       return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
   } else {
-    if (mode == 0) k_qq<double, double><<<grid32, WARPS * 32, 0, c.stream>>>(a);
-    else if (mode == 1) k_qq<double, float><<<grid32, WARPS * 32, 0, c.stream>>>(a);
-    else k_qq<float, float><<<grid32, WARPS * 32, 0, c.stream>>>(a);
+    // a family launch (trex_run) serves every quark-channel class: each class rounds its events up to whole blocks
+    const unsigned gq = a.qfamily ? grid32 + (unsigned)TREX_NSUBPROC : grid32;
+    if (mode == 0) k_qq<double, double><<<gq, WARPS * 32, 0, c.stream>>>(a);
+    else if (mode == 1) k_qq<double, float><<<gq, WARPS * 32, 0, c.stream>>>(a);
+    else k_qq<float, float><<<gq, WARPS * 32, 0, c.stream>>>(a);
   }
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());
@@ -375,7 +406,7 @@ extern "C" int trex_reweight(int sid, const double* momenta_soa, int64_t n, cons
   if (!make_theta_pair(sid, theta_old, theta_new, T)) return fail(TREX_EINVAL, "trex_reweight: theta outside its domain");
   ReweightArgs a;
   a.io = EvIO{momenta_soa, (long)n, (long)n, w_in, w_out, me2_old, me2_new};
-  a.alt = a.io; a.plan = nullptr;
+  a.alt = a.io; a.plan = nullptr; a.qfamily = 0;
   return launch_reweight(sid, a, n, T);
 }
 
@@ -386,6 +417,7 @@ int trex::ensure_plan() {
   unsigned long long sub[2 * TREX_NSUBPROC + 8 * TREX_NSUBPROC] = {0};
   for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
     const SubprocInfo* sp = subproc_info(sid);
+    if (!sp) { sub[2 * sid] = REX_NPOS; sub[2 * sid + 1] = 0; continue; }
     int8_t status[7];
     for (int i = 0; i < sp->npar; ++i) status[i] = i < 2 ? -1 : 1;
     sub[2 * sid] = rex_pack_key(sp->pdg, status, sp->npar);
@@ -413,7 +445,7 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
   // parameter points first: nothing is enqueued if theta is unusable
   ThetaPair T[TREX_NSUBPROC];
   for (int sid = 0; sid < TREX_NSUBPROC; ++sid)
-    if (subproc_info(sid)->npar == npar && !make_theta_pair(sid, theta_old, theta_new, T[sid]))
+    if (npar_of_sid(sid) == npar && !make_theta_pair(sid, theta_old, theta_new, T[sid]))
       return fail(TREX_EINVAL, "trex_run: theta outside its domain");
   if (int rc = ensure_plan()) return rc;
   if (int rc = ensure_colour()) return rc;
@@ -429,12 +461,14 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
     double* res = blk + (size_t)(nrows + 1) * n;      // [3][n]: w_out, me2_old, me2_new   -- in bucketed order
     if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar)) return rc;
     if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm, blk, res)) return rc;
+    bool quark_done = false;                          // ONE launch serves all quark-channel classes (k_qq finds the class in the plan)
     for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
-      if (subproc_info(sid)->npar != npar) continue;
+      if (npar_of_sid(sid) != npar) continue;
+      if (is_quark_channel(sid)) { if (quark_done) continue; quark_done = true; }
       ReweightArgs a;
       a.io = EvIO{momenta_soa, (long)n, (long)n, w_in, w_out, me2_old, me2_new};
       a.alt = EvIO{blk, (long)n, (long)n, blk + (size_t)nrows * n, res, res + n, res + 2 * (size_t)n};
-      a.plan = c.plan;
+      a.plan = c.plan; a.qfamily = is_quark_channel(sid) ? 1 : 0;
       if (int rc = launch_reweight(sid, a, n, T[sid])) return rc;
     }
     return run_scatter(res, n, (const int32_t*)c.run_perm, w_out, me2_old, me2_new);
@@ -520,7 +554,7 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
   std::vector<ThetaPair> T((size_t)ntheta * TREX_NSUBPROC);
   for (int k = 0; k < ntheta; ++k)
     for (int sid = 0; sid < TREX_NSUBPROC; ++sid)
-      if (subproc_info(sid)->npar == npar &&
+      if (npar_of_sid(sid) == npar &&
           !make_theta_pair(sid, theta_old, theta_new + (size_t)k * TREX_NTHETA, T[(size_t)k * TREX_NSUBPROC + sid]))
         return fail(TREX_EINVAL, "trex_run_multi: theta_new[%d] outside its domain", k);
   if (int rc = ensure_plan()) return rc;
@@ -562,15 +596,17 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
     for (int s2 = 0; s2 < 2; ++s2) {
       double* mo_out = s2 == 0 ? tmp : nullptr;
       double* mn_out = tmp + (size_t)(1 + s2) * n;
+      bool quark_done = false;
       for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
-        if (subproc_info(sid)->npar != npar) continue;
+        if (npar_of_sid(sid) != npar) continue;
+        if (is_quark_channel(sid)) { if (quark_done) continue; quark_done = true; }
         ThetaPair Tp;
         if (!make_theta_pair(sid, theta_old, theta_old, Tp)) return fail(TREX_EINVAL, "trex_run_multi: theta outside its domain");
         Tp.kq[1] = gs0 > 0.0 ? (k0 + (s2 == 0 ? delta : -delta)) / gs0 : 0.0;
         ReweightArgs a;
         a.io = EvIO{momenta_soa, (long)n, (long)n, w_in, w_out, mo_out, mn_out};      // w_out row 0 doubles as a dummy here
         a.alt = EvIO{blk, (long)n, (long)n, blk + (size_t)nrows * n, res, res + n, res + 2 * (size_t)n};
-        a.plan = c.plan;
+        a.plan = c.plan; a.qfamily = is_quark_channel(sid) ? 1 : 0;
         if (int rc = launch_reweight(sid, a, n, Tp)) return rc;
       }
       if (int rc = run_scatter(res, n, (const int32_t*)c.run_perm, w_out, mo_out, mn_out)) return rc;
@@ -588,12 +624,14 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
     double* wk = w_out + (size_t)k * n;
     double* mok = k == 0 ? me2_old : nullptr;                   // |M(theta_old)|^2 is the same for every k
     double* mnk = me2_new ? me2_new + (size_t)k * n : nullptr;
+    bool quark_done = false;
     for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
-      if (subproc_info(sid)->npar != npar) continue;
+      if (npar_of_sid(sid) != npar) continue;
+      if (is_quark_channel(sid)) { if (quark_done) continue; quark_done = true; }
       ReweightArgs a;
       a.io = EvIO{momenta_soa, (long)n, (long)n, w_in, wk, mok, mnk};
       a.alt = EvIO{blk, (long)n, (long)n, blk + (size_t)nrows * n, res, res + n, res + 2 * (size_t)n};
-      a.plan = c.plan;
+      a.plan = c.plan; a.qfamily = is_quark_channel(sid) ? 1 : 0;
       if (int rc = launch_reweight(sid, a, n, T[(size_t)k * TREX_NSUBPROC + sid])) return rc;
     }
     if (int rc = run_scatter(res, n, (const int32_t*)c.run_perm, wk, mok, mnk)) return rc;
@@ -687,7 +725,7 @@ extern "C" int trex_debug_xtile(int sid, const double* momenta_one, const double
   c.dbg_out = d_dbg;
   ReweightArgs a;
   a.io = EvIO{d_mom, 1, 1, d_w, d_w + 1, d_w + 2, d_w + 3};
-  a.alt = a.io; a.plan = nullptr;
+  a.alt = a.io; a.plan = nullptr; a.qfamily = 0;
   const int rc = launch_reweight(sid, a, 1, T);
   c.dbg_out = nullptr;
   std::vector<double> dump(2 * ndump);

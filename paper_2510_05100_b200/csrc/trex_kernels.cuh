@@ -24,6 +24,7 @@ struct ReweightArgs {
   EvIO alt;                // trex_run's scratch in bucketed order (mom, w_in, results), ld = sample size
   const DevPlan* plan;     // trex_run: device-resident bucket ranges; nullptr for trex_reweight
   int sid;
+  int qfamily;             // k_qq inside trex_run: one launch serves every quark-channel class of the plan
   const double* C120;
   ThetaPair T;
   QLineLegs q;
@@ -33,10 +34,11 @@ struct ReweightArgs {
 };
 
 // which events this launch works on: decided on the device for trex_run (the host has not seen the bucket sizes)
-__device__ __forceinline__ EvIO resolve_io(const ReweightArgs& a) {
+__device__ __forceinline__ EvIO resolve_io(const ReweightArgs& a, int sid = -1) {
   EvIO io = a.io;
+  if (sid < 0) sid = a.sid;
   if (a.plan) {
-    const long off = a.plan->off[a.sid], cnt = a.plan->cnt[a.sid];
+    const long off = a.plan->off[sid], cnt = a.plan->cnt[sid];
     if (!a.plan->single) {
       io = a.alt;
       io.mom += off; io.w_in += off; io.w_out += off; io.me2_old += off; io.me2_new += off;

@@ -17,6 +17,7 @@ struct ThetaPair {           // index 0 = theta_old, 1 = theta_new
   double mt[2], mGt[2];      // top mass, m_t * Gamma_t
   double kq[2];              // kappa / g_s
   double pref[2];            // g_s^(2 nv) / N_avg
+  double gs2nv[2];           // g_s^(2 nv) alone (the quark-channel family kernel divides by its class's N_avg itself)
   // electroweak (e- e+ -> mu- mu+)
   double e2[2], gL[2], gR[2], mZ2[2], mZGZ[2];
 };

@@ -253,3 +253,50 @@ def test_repeated_launches_are_bit_identical(T, sid, cfg, n):
         else:
             for x, y in zip(out, ref):
                 assert torch.equal(x, y), rep
+
+
+def test_multi_channel_sample_one_quark_family_launch(T):
+    """cfg6 (NEXT-4): a p p -> t t~ + parton sample with all 16 one-light-line classes (5 massless flavours). The whole path
+    takes ONE launch for the gluonic channel and ONE for every quark-channel class together (the kernel finds its class in
+    the device plan): weights against the oracle per class, launch count independent of the number of classes, and
+    every event equal to a per-class trex_reweight call."""
+    import torch
+    w = make_config(6, n=60000)
+    assert len(w.classes) == 16
+    dk, dm, dw = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    l0 = T.trex_launch_count()
+    wo, mo, mn, nb = T.trex_run(dk, dm, w.theta_old, w.theta_new, dw)
+    torch.cuda.synchronize()
+    launches = T.trex_launch_count() - l0
+    assert nb == 16 and launches <= 10, launches          # 6 bucketing + gather + k_table<3> + k_qq + scatter
+    got = [x.cpu().numpy() for x in (wo, mo, mn)]
+    assert np.all(got[0] > 0) and np.all(np.isfinite(got[0]))
+    for sp in w.classes:
+        sel = np.where(w.keys == sp.key)[0]
+        ref = T.trex_reweight(sp.sid, dev(np.ascontiguousarray(w.momenta[:, :, sel])), w.theta_old, w.theta_new, dev(w.w_in[sel]))
+        torch.cuda.synchronize()
+        for g, r in zip(got, ref):
+            assert np.array_equal(g[sel], r.cpu().numpy()), sp.name
+        idx = sel[:3]
+        rw, ro, rn = O.reweight(sp.sid, np.ascontiguousarray(w.momenta[:, :, idx]), w.theta_old, w.theta_new, w.w_in[idx])
+        assert rel(got[0][idx], rw).max() < RTOL64 and rel(got[1][idx], ro).max() < RTOL64 and rel(got[2][idx], rn).max() < RTOL64, sp.name
+    # a sample that holds quark channels only, and one with a single quark class (reweighted in place, no transposition)
+    for keep in ([sp.key for sp in w.classes if sp.sid != 2], [w.classes[5].key]):
+        sel = np.where(np.isin(w.keys, np.array(keep, dtype=np.uint64)))[0]
+        out = T.trex_run(dev(w.keys[sel]), dev(np.ascontiguousarray(w.momenta[:, :, sel])), w.theta_old, w.theta_new, dev(w.w_in[sel]))
+        torch.cuda.synchronize()
+        assert out[3] == len(keep) and np.array_equal(out[0].cpu().numpy(), got[0][sel])
+
+
+def test_both_beam_orders_reach_the_same_class_through_the_parton_reindexing(T):
+    """q g and g q (q q~ and q~ q, ...) share one flavour key -- legs are compared unordered -- and
+    trex_run_pdg brings either order to the process string: cfg6 with shuffled legs gives the canonical weights."""
+    import torch
+    from trex_inputs import shuffled_legs
+    w = make_config(6, n=30000)
+    pdg, mom, n_in = shuffled_legs(w, 23)
+    assert (pdg[0] != np.array([w.classes[0].pdg[0]] * w.n)).any()
+    wo, _, _, nb = T.trex_run_pdg(torch.from_numpy(pdg).cuda(), dev(mom), n_in, w.theta_old, w.theta_new, dev(w.w_in))
+    w0, _, _, nb0 = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    torch.cuda.synchronize()
+    assert nb == nb0 == 16 and rel(wo.cpu().numpy(), w0.cpu().numpy()).max() < 1e-12

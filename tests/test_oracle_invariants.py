@@ -121,3 +121,22 @@ def test_flop_counter_counts_the_same_evaluation():
         assert c1 == c2 and c1["flop"] == c1["add"] + c1["mul"] + c1["div"] + c1["sqrt"]
         counts.append(c1["flop"])
     assert 1e5 < counts[0] < 1e7 and counts[0] * 5 < counts[1] and counts[1] * 5 < counts[2]
+
+
+# ---------------------------------------------------------------- the other massless flavours (ids 10..20)
+def test_flavour_of_the_light_line_does_not_change_the_matrix_element():
+    """QCD does not see the flavour of a massless quark: ids 10..20 are ids 5, 7, 8 under another label."""
+    from trex_inputs import SUBPROCESSES
+    w = make_config(3, n=8)
+    mom = np.ascontiguousarray(w.momenta[:, :, :2])
+    th = w.theta_new.copy()
+    ref = {False: None}
+    want = {"qq": O.me2(5, mom, th), "qg": O.me2(7, mom, th), "gqb": O.me2(8, mom, th)}
+    seen = 0
+    for sp in SUBPROCESSES:
+        if sp.sid < 10:
+            continue
+        kind = "qq" if 21 not in sp.pdg[:2] else ("qg" if sp.pdg[1] == 21 else "gqb")
+        assert np.array_equal(O.me2(sp.sid, mom, th), want[kind]), sp.name
+        seen += 1
+    assert seen == 11

@@ -41,7 +41,7 @@ def test_identical_particles_keep_their_event_order_and_unknown_events_map_to_id
     ev = np.array([[21], [21], [21], [-6], [6], [21]], dtype=np.int32)          # g g > g t~ t g
     _, lm = O.keys_and_legmap(ev, 2, STRINGS)
     assert list(lm[:, 0]) == [0, 1, 4, 3, 2, 5]                                 # g g > t t~ g g: gluons 2 and 5 in event order
-    ev = np.array([[3], [-3], [6], [-6], [21]], dtype=np.int32)
+    ev = np.array([[3], [-4], [6], [-6], [21]], dtype=np.int32)             # s c~ > ...: no such class
     keys, lm = O.keys_and_legmap(ev, 2, STRINGS)
     assert list(lm[:, 0]) == [0, 1, 2, 3, 4] and all(keys[0] != sp.key for sp in SUBPROCESSES)
 

@@ -78,6 +78,25 @@ SUBPROCESSES = (
 )
 
 
+def _light_line_channels():
+    """The one-light-line channels for the other massless flavours (labels only; QCD does not see the flavour): ids
+    10, 11, 12 = s s~, c c~, b b~ > t t~ g; 13..16 = d g, s g, c g, b g > t t~ q; 17..20 = g d~, g s~, g c~, g b~ > t t~ q~.
+    (The two beam orders of a channel share one flavour key -- legs are compared unordered, PAPER.md:334 -- and are
+    brought to the order of the process string by the parton re-indexing of trex_run_pdg.)"""
+    name = {1: "d", 2: "u", 3: "s", 4: "c", 5: "b"}
+    out, sid = [], 10
+    for f in (3, 4, 5):
+        out.append(Subprocess(sid, "%s %s~ > t t~ g" % (name[f], name[f]), (f, -f, 6, -6, 21), (-1, -1, 1, 1, 1), (2, 3))); sid += 1
+    for f in (1, 3, 4, 5):
+        out.append(Subprocess(sid, "%s g > t t~ %s" % (name[f], name[f]), (f, 21, 6, -6, f), (-1, -1, 1, 1, 1), (2, 3))); sid += 1
+    for f in (1, 3, 4, 5):
+        out.append(Subprocess(sid, "g %s~ > t t~ %s~" % (name[f], name[f]), (21, -f, 6, -6, -f), (-1, -1, 1, 1, 1), (2, 3))); sid += 1
+    return tuple(out)
+
+
+SUBPROCESSES = SUBPROCESSES + _light_line_channels()
+
+
 def subprocess_by_name(name):
     for sp in SUBPROCESSES:
         if sp.name == name:
@@ -197,6 +216,38 @@ def make_config(cfg, n=None):
         sp = SUBPROCESSES[4]
         return Workload(5, "cfg5 gg -> tt~ggg", n, 7, np.full(n, sp.key, dtype=np.uint64),
                         mom, np.ones(n), th_old, th_new, (sp,))
+    if cfg == 6:
+        # multi-channel p p -> t t~ + 1 parton sample with every one-light-line channel (16 classes; the paper's QCD sample has
+        # 65 distinct parton configurations): g g > t t~ g 45 %, the rest shared among the quark channels with
+        # parton-density-like weights (u : d : s : c : b = 8 : 4 : 2 : 1 : 1; q g twice as likely as q q~; antiquark-initiated
+        # channels half as likely as quark-initiated ones). Same recipe as cfg 3 otherwise.
+        n = 1048576 if n is None else n
+        rng = np.random.default_rng(6)
+        classes = tuple(sp for sp in SUBPROCESSES if sp.npar == 5)
+        fw = {1: 4.0, 2: 8.0, 3: 2.0, 4: 1.0, 5: 1.0}
+        wts = []
+        for sp in classes:
+            ini = sp.pdg[:2]
+            if ini == (21, 21):
+                wts.append(0.0)
+                continue
+            f = [abs(x) for x in ini if x != 21][0]
+            kind_w = 2.0 if 21 in ini else 1.0
+            anti_w = 0.5 if (21 in ini and min(ini) < 0) else 1.0
+            wts.append(fw[f] * kind_w * anti_w)
+        wts = np.array(wts)
+        fr = 0.55 * wts / wts.sum()
+        fr[[i for i, sp in enumerate(classes) if sp.pdg[:2] == (21, 21)][0]] = 0.45
+        counts = largest_remainder(fr, n)
+        labels = np.concatenate([np.full(int(c), i, dtype=np.int64) for i, c in enumerate(counts)])
+        labels = rng.permutation(labels)
+        class_keys = np.array([sp.key for sp in classes], dtype=np.uint64)
+        keys = class_keys[labels]
+        mom = _two_to_n(rng, n, (500.0, 3000.0), [mt, mt, 0.0], True)
+        w = rng.lognormal(0.0, 0.5, n)
+        th_new[TH_CTG] = 1.0
+        present = tuple(sp for sp, c in zip(classes, counts) if c > 0)
+        return Workload(6, "cfg6 multi-channel pp -> tt~ + 1 parton, 16 classes", n, 5, keys, mom, w, th_old, th_new, present)
     raise ValueError(f"unknown config {cfg}")
 
 
@@ -204,7 +255,7 @@ def shuffled_legs(w, seed, unknown_every=0):
     """LHE-like view of a workload: per-event PDG codes [npar, n] (int32) and momenta whose legs were shuffled inside
     the initial state and inside the final state with a seeded permutation per event (an LHE file does not promise the
     parton order of the process string: PAPER.md:227-242). Returns (pdg, momenta, n_in). `unknown_every` > 0 turns
-    every k-th event into a class no subprocess claims (s s~ > ...). No method arithmetic here: only labels move."""
+    every k-th event into a class no subprocess claims (s c~ > ...). No method arithmetic here: only labels move."""
     rng = np.random.default_rng(seed)
     npar, n = w.npar, w.n
     n_in = 2
@@ -224,5 +275,5 @@ def shuffled_legs(w, seed, unknown_every=0):
     mom = np.ascontiguousarray(mom[order, :, cols].transpose(0, 2, 1))     # [npar, n, 4] -> [npar, 4, n]
     if unknown_every:
         pdg[0, ::unknown_every] = 3
-        pdg[1, ::unknown_every] = -3
+        pdg[1, ::unknown_every] = -4
     return pdg, mom, n_in
