@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(1024) k_scan(unsigned* __restrict__ counts, lo
 }
 
 __global__ void __launch_bounds__(WARPS * 32) k_scatter(const unsigned long long* __restrict__ keys, long n, long wch, long nchunks,
-                                                      Table t, const unsigned* __restrict__ base, int* __restrict__ perm) {
+                                                      Table t, const unsigned* __restrict__ base, int* __restrict__ perm, int* __restrict__ inv) {
   __shared__ SmemTable tab;
   __shared__ unsigned pos[WARPS][NBMAX];
   const int nb = t.meta[3];
@@ -217,7 +217,9 @@ __global__ void __launch_bounds__(WARPS * 32) k_scatter(const unsigned long long
       const int b = tab.lookup(keys[i], nb - 1);
       const unsigned peers = __match_any_sync(active, b);
       const unsigned rank = __popc(peers & ((1u << lane) - 1u));
-      perm[pos[warp][b] + rank] = (int)i;
+      const unsigned dst = pos[warp][b] + rank;
+      perm[dst] = (int)i;
+      if (inv) inv[i] = (int)dst;                            // inverse permutation: coalesced, for the transposition
       __syncwarp(active);
       if (rank == 0) pos[warp][b] += __popc(peers);
     }
@@ -250,7 +252,7 @@ constexpr long SMALL_N = 8192;      // beyond this one SM's load latency loses a
 constexpr int SB_WARPS = 32;
 
 __global__ void __launch_bounds__(1024) k_bucket_small(const unsigned long long* __restrict__ keys, long n, int* __restrict__ perm,
-                                                       BucketResult* __restrict__ res, const unsigned long long* __restrict__ sub,
+                                                       int* __restrict__ inv, BucketResult* __restrict__ res, const unsigned long long* __restrict__ sub,
                                                        int npar, DevPlan* __restrict__ plan, int force_gather) {
   __shared__ unsigned long long sk[TS];
   __shared__ unsigned sf[TS];
@@ -345,7 +347,9 @@ __global__ void __launch_bounds__(1024) k_bucket_small(const unsigned long long*
         const int b = lookup(keys[i]);
         const unsigned peers = __match_any_sync(active, b);
         const unsigned rank = __popc(peers & ((1u << lane) - 1u));
-        perm[boff[b] + cnt[warp][b] + rank] = (int)i;
+        const long dst = boff[b] + cnt[warp][b] + rank;
+        perm[dst] = (int)i;
+        if (inv) inv[i] = (int)dst;
         __syncwarp(active);
         if (rank == 0) cnt[warp][b] += (unsigned short)__popc(peers);
       }
@@ -439,24 +443,27 @@ __global__ void __launch_bounds__(256) k_keys_filtered(const int* __restrict__ p
   keys[i] = filtered_key(pdg + i, status + i, nlegs, n, fmask);
 }
 
-// momenta rows + weights into bucketed order; result rows cleared (classes nobody claims keep zero weights)
+// momenta rows + weights into bucketed order; result rows cleared (classes nobody claims keep zero weights).
+// A thread owns one event of the INPUT order and sends it to position inv[i]: the reads are fully coalesced and the
+// 8-byte writes of neighbouring events of a class land in the same 32-byte sectors while those are still in L2, so the
+// transposition moves its algorithmic bytes (reading at perm[j] instead fetched a whole sector per 8 bytes).
 __global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __restrict__ mom, const double* __restrict__ w_in, long n,
-                             int nrows, const int* __restrict__ perm, double* __restrict__ blk, double* __restrict__ res,
+                             int nrows, const int* __restrict__ inv, double* __restrict__ blk, double* __restrict__ res,
                              const signed char* __restrict__ legmap) {
   if (plan->single || plan->nb == 0) return;         // nb == 0: categorisation failed, perm was never written
-  const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= n) return;
-  const long p = perm[j];
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const long j = inv[i];
   if (legmap) {
     // parton re-indexing: position `leg` of the process string is played by leg legmap[leg] of the event
     for (int leg = 0; leg < nrows / 4; ++leg) {
-      const int src = legmap[(long)leg * n + p];
-      for (int mu = 0; mu < 4; ++mu) blk[(long)(leg * 4 + mu) * n + j] = mom[(long)(src * 4 + mu) * n + p];
+      const int src = legmap[(long)leg * n + i];
+      for (int mu = 0; mu < 4; ++mu) blk[(long)(leg * 4 + mu) * n + j] = mom[(long)(src * 4 + mu) * n + i];
     }
   } else
-  for (int r = 0; r < nrows; ++r) blk[(long)r * n + j] = mom[(long)r * n + p];
-  blk[(long)nrows * n + j] = w_in[p];
-  res[j] = 0.0; res[n + j] = 0.0; res[2 * n + j] = 0.0;
+  for (int r = 0; r < nrows; ++r) blk[(long)r * n + j] = mom[(long)r * n + i];
+  blk[(long)nrows * n + j] = w_in[i];
+  res[i] = 0.0; res[n + i] = 0.0; res[2 * n + i] = 0.0;
 }
 
 __global__ void k_run_scatter(const DevPlan* __restrict__ plan, const double* __restrict__ res, long n, const int* __restrict__ perm,
@@ -513,7 +520,7 @@ int trex::bucket_reserve(int64_t n) {
   return 0;
 }
 
-int trex::bucket_enqueue(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int npar) {
+int trex::bucket_enqueue(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int npar, int32_t* inv) {
   Context& c = ctx();
   const BucketLayout L = bucket_layout(n);
   const long wch = L.wch, nchunks = L.nchunks;
@@ -525,7 +532,7 @@ int trex::bucket_enqueue(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int
   const unsigned long long* keys = (const unsigned long long*)pdg_keys;
 
   if (n <= SMALL_N) {
-    k_bucket_small<<<1, 1024, 0, c.stream>>>(keys, n, perm, res, (const unsigned long long*)c.plan_keys, npar, c.plan, c.legmap ? 1 : 0);
+    k_bucket_small<<<1, 1024, 0, c.stream>>>(keys, n, perm, inv, res, (const unsigned long long*)c.plan_keys, npar, c.plan, c.legmap ? 1 : 0);
     c.launches += 1;
     TREX_CUDA_CHECK(cudaGetLastError());
     TREX_CUDA_CHECK(cudaMemcpyAsync(c.bucket_host, res, sizeof(BucketResult), cudaMemcpyDeviceToHost, c.stream));
@@ -540,7 +547,7 @@ int trex::bucket_enqueue(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int
   const unsigned cblk = (unsigned)((nchunks + WARPS - 1) / WARPS);
   k_hist<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts);
   k_scan<<<1, 1024, 0, c.stream>>>(counts, nchunks, n, t, res, (const unsigned long long*)c.plan_keys, npar, c.plan, c.legmap ? 1 : 0);
-  k_scatter<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts, perm);
+  k_scatter<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts, perm, inv);
   c.launches += 6;
   TREX_CUDA_CHECK(cudaGetLastError());
   TREX_CUDA_CHECK(cudaMemcpyAsync(c.bucket_host, res, sizeof(BucketResult), cudaMemcpyDeviceToHost, c.stream));
@@ -565,13 +572,13 @@ extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, in
   c.last_nbuckets = 0;
   if (n == 0) { offsets[0] = 0; return 0; }
   if (int rc = bucket_reserve(n)) return rc;
-  if (int rc = bucket_enqueue(pdg_keys, n, perm, 0)) return rc;
+  if (int rc = bucket_enqueue(pdg_keys, n, perm, 0, nullptr)) return rc;
   return bucket_finish(offsets);
 }
 
-int trex::run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* perm, double* blk, double* res) {
+int trex::run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* inv, double* blk, double* res) {
   Context& c = ctx();
-  k_run_gather<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, mom, w_in, n, nrows, perm, blk, res, (const signed char*)c.legmap);
+  k_run_gather<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, mom, w_in, n, nrows, inv, blk, res, (const signed char*)c.legmap);
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());
   return 0;

@@ -450,7 +450,7 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
   if (int rc = ensure_plan()) return rc;
   if (int rc = ensure_colour()) return rc;
   const int nrows = 4 * npar;
-  if (int rc = ensure_scratch(&c.run_perm, &c.run_perm_bytes, sizeof(int32_t) * (size_t)n)) return rc;
+  if (int rc = ensure_scratch(&c.run_perm, &c.run_perm_bytes, 2 * sizeof(int32_t) * (size_t)n)) return rc;
   if (int rc = ensure_scratch(&c.run_blocks, &c.run_blocks_bytes, sizeof(double) * (size_t)n * (nrows + 1 + 3))) return rc;
   if (int rc = bucket_reserve(n)) return rc;
   c.last_nbuckets = 0;
@@ -459,8 +459,8 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
   auto enqueue = [&]() -> int {
     double* blk = (double*)c.run_blocks;              // [4 npar][n] momenta, [1][n] w_in  -- in bucketed order
     double* res = blk + (size_t)(nrows + 1) * n;      // [3][n]: w_out, me2_old, me2_new   -- in bucketed order
-    if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar)) return rc;
-    if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm, blk, res)) return rc;
+    if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar, (int32_t*)c.run_perm + n)) return rc;
+    if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
     bool quark_done = false;                          // ONE launch serves all quark-channel classes (k_qq finds the class in the plan)
     for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
       if (npar_of_sid(sid) != npar) continue;
@@ -560,7 +560,7 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
   if (int rc = ensure_plan()) return rc;
   if (int rc = ensure_colour()) return rc;
   const int nrows = 4 * npar;
-  if (int rc = ensure_scratch(&c.run_perm, &c.run_perm_bytes, sizeof(int32_t) * (size_t)n)) return rc;
+  if (int rc = ensure_scratch(&c.run_perm, &c.run_perm_bytes, 2 * sizeof(int32_t) * (size_t)n)) return rc;
   if (int rc = ensure_scratch(&c.run_blocks, &c.run_blocks_bytes, sizeof(double) * (size_t)n * (nrows + 1 + 3))) return rc;
   if (int rc = bucket_reserve(n)) return rc;
   c.last_nbuckets = 0;
@@ -591,8 +591,8 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
     // which would divide by vev)
     const double gs0 = std::sqrt(4.0 * 3.14159265358979323846 * theta_old[TREX_TH_ALPHA_S]);
     if (!std::isfinite(k0) || !std::isfinite(delta)) return fail(TREX_EINVAL, "trex_run_multi: non-finite kappa");
-    if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar)) return rc;
-    if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm, blk, res)) return rc;
+    if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar, (int32_t*)c.run_perm + n)) return rc;
+    if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
     for (int s2 = 0; s2 < 2; ++s2) {
       double* mo_out = s2 == 0 ? tmp : nullptr;
       double* mn_out = tmp + (size_t)(1 + s2) * n;
@@ -618,8 +618,8 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
     int64_t offs[REX_MAX_BUCKETS + 1];
     return bucket_finish(offs);
   }
-  if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar)) return rc;
-  if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm, blk, res)) return rc;
+  if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar, (int32_t*)c.run_perm + n)) return rc;
+  if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
   for (int k = 0; k < ntheta; ++k) {
     double* wk = w_out + (size_t)k * n;
     double* mok = k == 0 ? me2_old : nullptr;                   // |M(theta_old)|^2 is the same for every k

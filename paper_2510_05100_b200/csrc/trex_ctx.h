@@ -72,11 +72,11 @@ Context& ctx();
 // rex_bucket in two halves (rex_bucket.cu): enqueue the kernel chain (+ the device plan for a run over `npar`-leg events,
 // if sub_keys != nullptr), then fetch sizes and keys -- the only point where the host waits for the device
 int bucket_reserve(int64_t n);          // (re)allocates the scratch of bucket_enqueue; never called while capturing
-int bucket_enqueue(const uint64_t* keys, int64_t n, int32_t* perm, int npar);
+int bucket_enqueue(const uint64_t* keys, int64_t n, int32_t* perm, int npar, int32_t* inv);   // inv (nullable): inverse permutation
 int ensure_plan();                      // uploads the subprocess registry the device plan and rex_keys need (trex_api.cu)
 int bucket_finish(int64_t* offsets);
 // transposition kernels of trex_run driven by the device plan (both are no-ops for a single-class sample)
-int run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* perm, double* blk, double* res);
+int run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* inv, double* blk, double* res);
 int run_scatter(const double* res, int64_t n, const int32_t* perm, double* w_out, double* me2_old, double* me2_new);
 
 inline int fail(int code, const char* fmt, ...) {
