@@ -447,7 +447,7 @@ __global__ void __launch_bounds__(256) k_keys_filtered(const int* __restrict__ p
 // A thread owns one event of the INPUT order and sends it to position inv[i]: the reads are fully coalesced and the
 // 8-byte writes of neighbouring events of a class land in the same 32-byte sectors while those are still in L2, so the
 // transposition moves its algorithmic bytes (reading at perm[j] instead fetched a whole sector per 8 bytes).
-__global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __restrict__ mom, const double* __restrict__ w_in, long n,
+__global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __restrict__ mom, long ld, const double* __restrict__ w_in, long n,
                              int nrows, const int* __restrict__ inv, double* __restrict__ blk, double* __restrict__ res,
                              const signed char* __restrict__ legmap) {
   if (plan->single || plan->nb == 0) return;         // nb == 0: categorisation failed, perm was never written
@@ -458,10 +458,10 @@ __global__ void k_run_gather(const DevPlan* __restrict__ plan, const double* __r
     // parton re-indexing: position `leg` of the process string is played by leg legmap[leg] of the event
     for (int leg = 0; leg < nrows / 4; ++leg) {
       const int src = legmap[(long)leg * n + i];
-      for (int mu = 0; mu < 4; ++mu) blk[(long)(leg * 4 + mu) * n + j] = mom[(long)(src * 4 + mu) * n + i];
+      for (int mu = 0; mu < 4; ++mu) blk[(long)(leg * 4 + mu) * n + j] = mom[(long)(src * 4 + mu) * ld + i];
     }
   } else
-  for (int r = 0; r < nrows; ++r) blk[(long)r * n + j] = mom[(long)r * n + i];
+  for (int r = 0; r < nrows; ++r) blk[(long)r * n + j] = mom[(long)r * ld + i];
   blk[(long)nrows * n + j] = w_in[i];
   res[i] = 0.0; res[n + i] = 0.0; res[2 * n + i] = 0.0;
 }
@@ -576,9 +576,9 @@ extern "C" int rex_bucket(const uint64_t* pdg_keys, int64_t n, int32_t* perm, in
   return bucket_finish(offsets);
 }
 
-int trex::run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* inv, double* blk, double* res) {
+int trex::run_gather(const double* mom, int64_t ld, const double* w_in, int64_t n, int nrows, const int32_t* inv, double* blk, double* res) {
   Context& c = ctx();
-  k_run_gather<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, mom, w_in, n, nrows, inv, blk, res, (const signed char*)c.legmap);
+  k_run_gather<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(c.plan, mom, ld, w_in, n, nrows, inv, blk, res, (const signed char*)c.legmap);
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());
   return 0;

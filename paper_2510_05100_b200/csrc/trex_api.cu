@@ -435,8 +435,17 @@ int trex::ensure_plan() {
 // compiled-in subprocess with the right number of legs gets one launch sized for the whole sample whose blocks beyond its
 // bucket exit at once, and a single-class sample is reweighted in place (gather / scatter return immediately). The
 // host waits once, at the end, to read the number of buckets it has to return.
+static int run_core(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int64_t ld, int npar, const double* theta_old,
+                    const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new);
+
 extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
                         const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new) {
+  return run_core(pdg_keys, momenta_soa, n, n, npar, theta_old, theta_new, w_in, w_out, me2_old, me2_new);
+}
+
+// ld: row stride of momenta_soa (== n for a caller's block; trex_run_host hands in column ranges of a larger block)
+static int run_core(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int64_t ld, int npar, const double* theta_old,
+                    const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new) {
   Context& c = ctx();
   if (n < 0 || npar < 1 || npar > 7 || !theta_old || !theta_new) return fail(TREX_EINVAL, "trex_run: bad size or null theta");
   if (n == 0) return 0;
@@ -460,13 +469,13 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
     double* blk = (double*)c.run_blocks;              // [4 npar][n] momenta, [1][n] w_in  -- in bucketed order
     double* res = blk + (size_t)(nrows + 1) * n;      // [3][n]: w_out, me2_old, me2_new   -- in bucketed order
     if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar, (int32_t*)c.run_perm + n)) return rc;
-    if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
+    if (int rc = run_gather(momenta_soa, ld, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
     bool quark_done = false;                          // ONE launch serves all quark-channel classes (k_qq finds the class in the plan)
     for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
       if (npar_of_sid(sid) != npar) continue;
       if (is_quark_channel(sid)) { if (quark_done) continue; quark_done = true; }
       ReweightArgs a;
-      a.io = EvIO{momenta_soa, (long)n, (long)n, w_in, w_out, me2_old, me2_new};
+      a.io = EvIO{momenta_soa, (long)n, (long)ld, w_in, w_out, me2_old, me2_new};
       a.alt = EvIO{blk, (long)n, (long)n, blk + (size_t)nrows * n, res, res + n, res + 2 * (size_t)n};
       a.plan = c.plan; a.qfamily = is_quark_channel(sid) ? 1 : 0;
       if (int rc = launch_reweight(sid, a, n, T[sid])) return rc;
@@ -478,7 +487,7 @@ extern "C" int trex_run(const uint64_t* pdg_keys, const double* momenta_soa, int
   // of a streamed sample) replays it as one CUDA graph
   Context::RunKey key{};
   key.ptr[0] = pdg_keys; key.ptr[1] = momenta_soa; key.ptr[2] = w_in; key.ptr[3] = w_out; key.ptr[4] = me2_old; key.ptr[5] = me2_new;
-  key.n = n; key.npar = npar; key.precision = c.precision; key.table_min_n = c.table_min_n;
+  key.n = n; key.ld = ld; key.npar = npar; key.precision = c.precision; key.table_min_n = c.table_min_n;
   std::memcpy(key.th, theta_old, sizeof(double) * TREX_NTHETA);
   std::memcpy(key.th + TREX_NTHETA, theta_new, sizeof(double) * TREX_NTHETA);
   int64_t offsets[REX_MAX_BUCKETS + 1];
@@ -551,6 +560,7 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
   if (n == 0 || ntheta == 0) return 0;
   if (!pdg_keys || !momenta_soa || !w_in || !w_out) return fail(TREX_EINVAL, "trex_run_multi: null device pointer");
   if (n >= (int64_t(1) << 31)) return fail(TREX_EINVAL, "trex_run_multi: n must be < 2^31");
+  const int64_t ld = n;
   std::vector<ThetaPair> T((size_t)ntheta * TREX_NSUBPROC);
   for (int k = 0; k < ntheta; ++k)
     for (int sid = 0; sid < TREX_NSUBPROC; ++sid)
@@ -592,7 +602,7 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
     const double gs0 = std::sqrt(4.0 * 3.14159265358979323846 * theta_old[TREX_TH_ALPHA_S]);
     if (!std::isfinite(k0) || !std::isfinite(delta)) return fail(TREX_EINVAL, "trex_run_multi: non-finite kappa");
     if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar, (int32_t*)c.run_perm + n)) return rc;
-    if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
+    if (int rc = run_gather(momenta_soa, ld, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
     for (int s2 = 0; s2 < 2; ++s2) {
       double* mo_out = s2 == 0 ? tmp : nullptr;
       double* mn_out = tmp + (size_t)(1 + s2) * n;
@@ -619,7 +629,7 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
     return bucket_finish(offs);
   }
   if (int rc = bucket_enqueue(pdg_keys, n, (int32_t*)c.run_perm, npar, (int32_t*)c.run_perm + n)) return rc;
-  if (int rc = run_gather(momenta_soa, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
+  if (int rc = run_gather(momenta_soa, ld, w_in, n, nrows, (const int32_t*)c.run_perm + n, blk, res)) return rc;
   for (int k = 0; k < ntheta; ++k) {
     double* wk = w_out + (size_t)k * n;
     double* mok = k == 0 ? me2_old : nullptr;                   // |M(theta_old)|^2 is the same for every k
@@ -640,7 +650,11 @@ extern "C" int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_so
   return bucket_finish(offsets);
 }
 
-// the same with HOST buffers: copies in, runs, copies out, synchronises (bench.py's end-to-end figure)
+// the same with HOST buffers (bench.py's end-to-end figure). Events are independent, so the sample is cut into column
+// ranges ("chunks") that go through the whole path one after the other on the library stream while a second stream
+// copies the NEXT chunk in and the PREVIOUS chunk's weights out: the transfers hide behind the kernels. Per-event results
+// do not depend on the cut; the number of buckets returned is that of the whole sample (union of the chunks' keys, in
+// order of first appearance, REX_NPOS last).
 extern "C" int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
                              const double* theta_new, const double* w_in, double* w_out, double* me2_old, double* me2_new) {
   Context& c = ctx();
@@ -649,23 +663,62 @@ extern "C" int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa
   if (!pdg_keys || !momenta_soa || !w_in || !w_out) return fail(TREX_EINVAL, "trex_run_host: null pointer");
   const size_t nn = (size_t)n, rows = (size_t)4 * npar;
   if (int rc = ensure_scratch(&c.host_io, &c.host_io_bytes, 8 * nn * (1 + rows + 1 + 3))) return rc;
+  if (!c.copy_stream) {
+    TREX_CUDA_CHECK(cudaStreamCreateWithFlags(&c.copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) TREX_CUDA_CHECK(cudaEventCreateWithFlags(&c.copy_ev[i], cudaEventDisableTiming));
+  }
   uint64_t* d_keys = (uint64_t*)c.host_io;
   double* d_mom = (double*)c.host_io + nn;
   double* d_win = d_mom + rows * nn;
   double* d_out = d_win + nn;
-  TREX_CUDA_CHECK(cudaMemcpyAsync(d_keys, pdg_keys, 8 * nn, cudaMemcpyHostToDevice, c.stream));
-  TREX_CUDA_CHECK(cudaMemcpyAsync(d_mom, momenta_soa, 8 * nn * rows, cudaMemcpyHostToDevice, c.stream));
-  TREX_CUDA_CHECK(cudaMemcpyAsync(d_win, w_in, 8 * nn, cudaMemcpyHostToDevice, c.stream));
+  const int nchunk = (int)std::max<int64_t>(1, std::min<int64_t>(8, n / 65536));
+  const auto lo_of = [&](int k) { return (size_t)(nn * (size_t)k / (size_t)nchunk); };
+  const auto copy_in = [&](int k) -> int {
+    const size_t lo = lo_of(k), w = lo_of(k + 1) - lo;
+    TREX_CUDA_CHECK(cudaMemcpyAsync(d_keys + lo, pdg_keys + lo, 8 * w, cudaMemcpyHostToDevice, c.copy_stream));
+    TREX_CUDA_CHECK(cudaMemcpy2DAsync(d_mom + lo, 8 * nn, momenta_soa + lo, 8 * nn, 8 * w, rows, cudaMemcpyHostToDevice, c.copy_stream));
+    TREX_CUDA_CHECK(cudaMemcpyAsync(d_win + lo, w_in + lo, 8 * w, cudaMemcpyHostToDevice, c.copy_stream));
+    TREX_CUDA_CHECK(cudaEventRecord(c.copy_ev[k & 1], c.copy_stream));
+    return 0;
+  };
+  // the caller's earlier work on the library stream comes first
+  TREX_CUDA_CHECK(cudaEventRecord(c.copy_ev[1], c.stream));
+  TREX_CUDA_CHECK(cudaStreamWaitEvent(c.copy_stream, c.copy_ev[1], 0));
+  if (int rc = copy_in(0)) return rc;
+  uint64_t keys_seen[REX_MAX_BUCKETS + 1];
+  int nseen = 0;
+  bool npos_seen = false;
   c.in_host_run = true;
-  const int rc = trex_run(d_keys, d_mom, n, npar, theta_old, theta_new, d_win, d_out, me2_old ? d_out + nn : nullptr,
-                          me2_new ? d_out + 2 * nn : nullptr);
+  int rc = 0;
+  for (int k = 0; k < nchunk && rc >= 0; ++k) {
+    const size_t lo = lo_of(k), w = lo_of(k + 1) - lo;
+    if (k + 1 < nchunk) { if (int r2 = copy_in(k + 1)) { rc = r2; break; } }
+    if (cudaStreamWaitEvent(c.stream, c.copy_ev[k & 1], 0) != cudaSuccess) { rc = fail(TREX_ECUDA, "trex_run_host: cudaStreamWaitEvent failed"); break; }
+    // run_core returns after the chunk's kernels have finished (it reads the bucket sizes back)
+    rc = run_core(d_keys + lo, d_mom + lo, (int64_t)w, n, npar, theta_old, theta_new, d_win + lo, d_out + lo,
+                  me2_old ? d_out + nn + lo : nullptr, me2_new ? d_out + 2 * nn + lo : nullptr);
+    if (rc < 0) break;
+    for (int b = 0; b < c.last_nbuckets; ++b) {
+      const uint64_t key = c.last_keys[b];
+      if (key == REX_NPOS) { npos_seen = true; continue; }
+      bool have = false;
+      for (int j = 0; j < nseen && !have; ++j) have = keys_seen[j] == key;
+      if (!have && nseen <= REX_MAX_BUCKETS) keys_seen[nseen++] = key;
+    }
+    cudaMemcpyAsync(w_out + lo, d_out + lo, 8 * w, cudaMemcpyDeviceToHost, c.copy_stream);
+    if (me2_old) cudaMemcpyAsync(me2_old + lo, d_out + nn + lo, 8 * w, cudaMemcpyDeviceToHost, c.copy_stream);
+    if (me2_new) cudaMemcpyAsync(me2_new + lo, d_out + 2 * nn + lo, 8 * w, cudaMemcpyDeviceToHost, c.copy_stream);
+  }
   c.in_host_run = false;
+  cudaError_t e1 = cudaStreamSynchronize(c.copy_stream), e2 = cudaStreamSynchronize(c.stream);
   if (rc < 0) return rc;
-  TREX_CUDA_CHECK(cudaMemcpyAsync(w_out, d_out, 8 * nn, cudaMemcpyDeviceToHost, c.stream));
-  if (me2_old) TREX_CUDA_CHECK(cudaMemcpyAsync(me2_old, d_out + nn, 8 * nn, cudaMemcpyDeviceToHost, c.stream));
-  if (me2_new) TREX_CUDA_CHECK(cudaMemcpyAsync(me2_new, d_out + 2 * nn, 8 * nn, cudaMemcpyDeviceToHost, c.stream));
-  TREX_CUDA_CHECK(cudaStreamSynchronize(c.stream));
-  return rc;
+  TREX_CUDA_CHECK(e1); TREX_CUDA_CHECK(e2); TREX_CUDA_CHECK(cudaGetLastError());
+  const int total = nseen + (npos_seen ? 1 : 0);
+  if (total > REX_MAX_BUCKETS) return fail(TREX_EINVAL, "rex_bucket: more than %d distinct flavour keys", REX_MAX_BUCKETS);
+  for (int j = 0; j < nseen; ++j) c.last_keys[j] = keys_seen[j];
+  if (npos_seen) c.last_keys[nseen] = REX_NPOS;
+  c.last_nbuckets = total;
+  return total;
 }
 
 extern "C" int trex_debug_flow_amps(int sid, const double* momenta_one, const double* theta, double* out) {
@@ -811,6 +864,7 @@ extern "C" void trex_shutdown(void) {
   for (cudaEvent_t e : c.kev) cudaEventDestroy(e);
   for (cudaEvent_t e : c.kev_pool) cudaEventDestroy(e);
   c.kev.clear(); c.kev_pool.clear();
+  if (c.copy_stream) { cudaStreamDestroy(c.copy_stream); cudaEventDestroy(c.copy_ev[0]); cudaEventDestroy(c.copy_ev[1]); c.copy_stream = nullptr; }
   if (c.run_exec) cudaGraphExecDestroy(c.run_exec);
   if (c.cap_stream) cudaStreamDestroy(c.cap_stream);
   c.run_exec = nullptr; c.cap_stream = nullptr; c.exec_valid = false; c.last_key_valid = false;

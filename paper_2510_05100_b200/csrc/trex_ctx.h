@@ -49,13 +49,14 @@ struct Context {
   void* xsec_scratch = nullptr; void* xsec_host = nullptr;   // trex_xsec_moments: block partials (device), result (pinned)
   // trex_run replayed as a CUDA graph when it is called again with the same buffers, sizes and parameter points
   struct RunKey {
-    const void* ptr[6]; int64_t n; int npar, precision, table_min_n; double th[2 * TREX_NTHETA];
+    const void* ptr[6]; int64_t n, ld; int npar, precision, table_min_n; double th[2 * TREX_NTHETA];
   };
   bool in_host_run = false;
   RunKey last_key{}; bool last_key_valid = false;
   RunKey exec_key{}; bool exec_valid = false; bool graphs_ok = true;
   cudaGraphExec_t run_exec = nullptr; int64_t exec_launches = 0; int64_t graph_replays = 0;
   cudaStream_t cap_stream = nullptr;
+  cudaStream_t copy_stream = nullptr; cudaEvent_t copy_ev[2] = {nullptr, nullptr};   // trex_run_host: transfers beside the kernels
   DevPlan* plan = nullptr;           // device
   void* plan_keys = nullptr;         // device: key, leg count [2 NSUB] and process string [NSUB][8] of every compiled-in subprocess
   const int8_t* legmap = nullptr;    // trex_run_pdg: per-event leg order (device [npar][n]); forces the transposition
@@ -76,7 +77,7 @@ int bucket_enqueue(const uint64_t* keys, int64_t n, int32_t* perm, int npar, int
 int ensure_plan();                      // uploads the subprocess registry the device plan and rex_keys need (trex_api.cu)
 int bucket_finish(int64_t* offsets);
 // transposition kernels of trex_run driven by the device plan (both are no-ops for a single-class sample)
-int run_gather(const double* mom, const double* w_in, int64_t n, int nrows, const int32_t* inv, double* blk, double* res);
+int run_gather(const double* mom, int64_t ld, const double* w_in, int64_t n, int nrows, const int32_t* inv, double* blk, double* res);   // ld: row stride of mom
 int run_scatter(const double* res, int64_t n, const int32_t* perm, double* w_out, double* me2_old, double* me2_new);
 
 inline int fail(int code, const char* fmt, ...) {

@@ -18,7 +18,9 @@ template <class R, class RC> struct W4 {
   using UI = UTabIdx<4, 0>;
   using G = TabGeom<R, RC, 4>;
   static constexpr int NE = I::NE, PE = I::entries_below(3), E4 = I::entries_below(4);
-  static constexpr int TS = NE + PE;                    // table stride (entries per component)
+  // table stride (entries per component); odd, so that the closed scalars of lambda_t = -/+ (4 components apart, read by
+  // the lanes of one warp in one instruction) fall into different halves of a 128-byte bank line
+  static constexpr int TS = NE + PE + 1;
   static constexpr int NWR = 2 * (E4 + PE);             // W records: (entry below level 4, lambda_tbar)
   static constexpr int NUB = 2 * (E4 - PE);             // A = 0 rows of the level-3 entries: (entry, lambda_t)
   static constexpr int N1 = UI::N1, N2 = UI::N2, NU = N1 + N2, NUT = 2 * NU, US = NUT + 2 * N1;   // line-state records

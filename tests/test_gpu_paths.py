@@ -300,3 +300,27 @@ def test_both_beam_orders_reach_the_same_class_through_the_parton_reindexing(T):
     w0, _, _, nb0 = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
     torch.cuda.synchronize()
     assert nb == nb0 == 16 and rel(wo.cpu().numpy(), w0.cpu().numpy()).max() < 1e-12
+
+
+def test_host_entry_point_pipelines_chunks_without_changing_a_bit(T):
+    """trex_run_host cuts large samples into column ranges whose transfers overlap the kernels: per-event results and the
+    number of buckets must be those of one trex_run over the whole sample (unknown classes and REX_NPOS included)."""
+    import torch
+    w = make_config(3, n=300001)
+    keys = w.keys.copy()
+    keys[3::1001] = np.uint64(REX_NPOS)
+    keys[250000:] = np.where(keys[250000:] == w.classes[1].key, np.uint64(424242), keys[250000:])   # a class that first appears late
+    ref = T.trex_run(dev(keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))
+    torch.cuda.synchronize()
+    out, mo, mn = np.full(w.n, -1.0), np.full(w.n, -1.0), np.full(w.n, -1.0)
+    nb = T.trex_run_host(keys, w.momenta, w.theta_old, w.theta_new, w.w_in, out, mo, mn)
+    assert nb == ref[3] == 7
+    assert np.array_equal(out, ref[0].cpu().numpy()) and np.array_equal(mo, ref[1].cpu().numpy()) and np.array_equal(mn, ref[2].cpu().numpy())
+    # pinned torch tensors, single-class sample (reweighted in place on the staged block: row stride != chunk length)
+    w4 = make_config(4, n=140000)
+    r4 = T.trex_run(dev(w4.keys), dev(w4.momenta), w4.theta_old, w4.theta_new, dev(w4.w_in))
+    hk = torch.from_numpy(w4.keys.view(np.int64)).pin_memory()
+    hm, hw = torch.from_numpy(w4.momenta).pin_memory(), torch.from_numpy(w4.w_in).pin_memory()
+    ho = torch.empty(w4.n, dtype=torch.float64).pin_memory()
+    assert T.trex_run_host(hk, hm, w4.theta_old, w4.theta_new, hw, ho) == 1
+    assert np.array_equal(ho.numpy(), r4[0].cpu().numpy())
