@@ -25,6 +25,10 @@ template <class R, class RC> struct W4 {
   static constexpr int NUB = 2 * (E4 - PE);             // A = 0 rows of the level-3 entries: (entry, lambda_t)
   static constexpr int N1 = UI::N1, N2 = UI::N2, NU = N1 + N2, NUT = 2 * NU, US = NUT + 2 * N1;   // line-state records
   static constexpr int TB = 384, XS = G::XS, NC = 24;
+#ifndef TREX_T4_NCW
+#define TREX_T4_NCW 6
+#endif
+  static constexpr int NCW = TREX_T4_NCW;               // warps that take the tensor-core colour sum in phase D
   struct Small {                                        // per-event constants, one block per parity
     rvec4<double> pset[16];
     double eps[64], spin[32], pm[24];
@@ -190,12 +194,12 @@ __device__ __forceinline__ void w4_prep(const W4Ptr<R>& p, typename W4<R, RC>::S
 
 // ---- level-3 entries and the line states after two gluons of one event (needs its prep)
 template <class R, class RC, int NPASS>
-__device__ __forceinline__ void w4_build3(const W4Ptr<R>& p, const typename W4<R, RC>::Small& sm, const ReweightArgs& a, int par, int tid) {
+__device__ __forceinline__ void w4_build3(const W4Ptr<R>& p, const typename W4<R, RC>::Small& sm, const ReweightArgs& a, int par, int tid, int nthreads) {
   using W = W4<R, RC>;
   using I = typename W::I;
   constexpr int N = 4, NL3 = W::E4 - W::PE;
   const int poff = par ? W::NE : 0;
-  for (int it = tid; it < NL3 + W::N2 * NPASS; it += W::TB) {
+  for (int it = tid; it < NL3 + W::N2 * NPASS; it += nthreads) {
     if (it < NL3) {
       const int e = W::PE + it;
       TabBuild<R, N, 0, 3, W::TS, 2> b;
@@ -409,7 +413,7 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
   // pipeline prologue: prep and level 3 of the block's first event
   if (wrp == 6 || wrp == 7) w4_prep<R, RC, NPASS>(p, small[0], io, a, e_first, 0, wrp - 6, lane);
   __syncthreads();
-  w4_build3<R, RC, NPASS>(p, small[0], a, 0, tid);
+  w4_build3<R, RC, NPASS>(p, small[0], a, 0, tid, W::TB);
   __syncthreads();
   int par = 0;
 #ifdef TREX_PHASE_CLOCKS
@@ -435,14 +439,22 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
         const cx<RC> x = xs[row * W::XS + col];
         a.dbg[2 * i] = (double)x.re; a.dbg[2 * i + 1] = (double)x.im;
       }
-    // ---- phase D: colour sum of this event | level 3 of the next one
-    colour_phase<R, RC, 4>(xs, Cs, part, tid, tid);
-    if (more) w4_build3<R, RC, NPASS>(p, small[par ^ 1], a, par ^ 1, tid);
+    // ---- phase D: colour sum of this event | level 3 of the next one. With the colour sum on the tensor cores three
+    // warps take it (384 mma for 32 column blocks) while the other nine build the 96 level-3 entries and the U2 states of
+    // the next event on the FP64 pipe -- the two pipes work side by side; the FMA colour sum (mixed / fp32 modes) is done
+    // by all warps before they turn to level 3.
+    if constexpr (G::DMMA) {
+      if (wrp < W::NCW) colour_phase<R, RC, 4>(xs, Cs, part, tid, tid, W::NCW);
+      else if (more) w4_build3<R, RC, NPASS>(p, small[par ^ 1], a, par ^ 1, tid - 32 * W::NCW, W::TB - 32 * W::NCW);
+    } else {
+      colour_phase<R, RC, 4>(xs, Cs, part, tid, tid);
+      if (more) w4_build3<R, RC, NPASS>(p, small[par ^ 1], a, par ^ 1, tid, W::TB);
+    }
     __syncthreads();
     W4_TICK(2);
-    // ---- fixed-order reduction of the partial sums (slot parity = theta) + epilogue by the first warp, which clears
-    // what it has read; the other warps already work on the next event
-    if (wrp == 0) {
+    // ---- fixed-order reduction of the partial sums (slot parity = theta) + epilogue by warp 8, which has nothing to do
+    // in phase B and clears what it has read; the other warps already work on the next event
+    if (wrp == 8) {
       double v = 0.0;
       for (int i = lane; i < G::NCI; i += 32) { v += part[i]; part[i] = 0.0; }
 #pragma unroll

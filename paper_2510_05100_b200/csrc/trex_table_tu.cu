@@ -466,7 +466,8 @@ __device__ __forceinline__ void walk_wform(unsigned char* sb, const int* meta, i
 
 // ---- phase 3 of k_table: x^dagger C x of every X column added into the event's partial-sum slots
 template <class R, class RC, int N>
-__device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, const RC* __restrict__ Cs, double* __restrict__ part, int tid, int gtid) {
+// ncw > 0 (tensor-core form only): the first ncw warps of the group share the column blocks, the others do not take part
+__device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, const RC* __restrict__ Cs, double* __restrict__ part, int tid, int gtid, int ncw = 0) {
   using G = TabGeom<R, RC, N>;
   using F = FoldedC<G::NC>;
   constexpr int XS = G::XS, GS = G::GS;
@@ -486,7 +487,9 @@ __device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, cons
     double accl = 0.0;
     // a warp owns one column block; row blocks go four at a time (J0 .. J0+3) so that one X fragment feeds four
     // independent accumulator chains
-    for (int cb = wrp; cb < NCB; cb += GS / 32) {
+    const int cstep = ncw > 0 ? ncw : GS / 32;
+    if (wrp >= cstep) return;
+    for (int cb = wrp; cb < NCB; cb += cstep) {
       for (int J0 = 0; J0 < NB; J0 += 4) {
         double d[4][2];
 #pragma unroll
