@@ -43,7 +43,7 @@ template <class R, class RC> struct W4 {
   static constexpr size_t o_part = o_utab + al(sizeof(R) * 16 * US);
   static constexpr size_t o_small = o_part + al(sizeof(double) * G::NCI);
   static constexpr size_t o_c = o_small + 2 * al(sizeof(Small));
-  static constexpr size_t o_meta = o_c + al(sizeof(RC) * FoldedC<NC>::size());
+  static constexpr size_t o_meta = o_c + al(sizeof(RC) * G::CN);
   static constexpr size_t bytes = o_meta + al(sizeof(int) * I::M_SIZE);
   static_assert(bytes <= 232448, "one SM has 227 KB of shared memory");
   __device__ static int uidx1(int pass, int idx, int par) { return par ? NUT + pass * N1 + idx : pass * NU + idx; }
@@ -407,7 +407,7 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
   const long e_first = blockIdx.x, e_step = gridDim.x;
   if (e_first >= io.n) return;
   for (int i = tid; i < I::M_SIZE; i += W::TB) meta[i] = gmeta[i];
-  for (int i = tid; i < F::size(); i += W::TB) Cs[i] = RC(Cfold[i]);
+  for (int i = tid; i < G::CN; i += W::TB) Cs[i] = RC(Cfold[i]);
   for (int i = tid; i < G::NCI; i += W::TB) part[i] = 0.0;
   __syncthreads();
   // pipeline prologue: prep and level 3 of the block's first event
@@ -443,7 +443,7 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
     // warps take it (384 mma for 32 column blocks) while the other nine build the 96 level-3 entries and the U2 states of
     // the next event on the FP64 pipe -- the two pipes work side by side; the FMA colour sum (mixed / fp32 modes) is done
     // by all warps before they turn to level 3.
-    if constexpr (G::DMMA) {
+    if constexpr (G::DMMA || G::TF32) {
       if (wrp < W::NCW) colour_phase<R, RC, 4>(xs, Cs, part, tid, tid, W::NCW);
       else if (more) w4_build3<R, RC, NPASS>(p, small[par ^ 1], a, par ^ 1, tid - 32 * W::NCW, W::TB - 32 * W::NCW);
     } else {

@@ -61,6 +61,9 @@ namespace {
 #ifndef TREX_T4_PIPE
 #define TREX_T4_PIPE 1
 #endif
+#ifndef TREX_TF32_COLOUR
+#define TREX_TF32_COLOUR 1
+#endif
 #ifndef TREX_T4_DMMA
 #define TREX_T4_DMMA 1
 #endif
@@ -106,12 +109,23 @@ template <class R, class RC, int N> struct TabGeom {
   // row stride of the X tile in complex numbers: odd for the vector colour sum; = 4 mod 8 for the tensor-core one, so
   // that the four k rows of an mma fragment (stride 2 XS doubles = 8 mod 16) land in disjoint banks
   static constexpr bool DMMA_CFG = sizeof(RC) == 8 && EPB == 1 && ((TREX_T5_DMMA && NC == 120) || (TREX_T4_DMMA && NC == 24));
-  static constexpr int XS = DMMA_CFG ? NCOLT + 4 : NCOLT + 1;
+  // fp32 colour arithmetic (mixed / fp32 modes) on the tensor cores: mma.sync.m16n8k8 with TF32 operands.
+  // The folded colour matrix times 54 (ncol = 24) / 324 (ncol = 120) consists of integers with at most 11 significant
+  // bits: exact in TF32; X is split into two TF32 numbers (hi + lo), so the products keep fp32 accuracy.
+  // Measured (profiles/r02_kernels.md): wins for ncol = 120 (+2.4 % mixed, +5.8 % fp32 on the kernel), loses for ncol = 24
+  // (-9 %: the FMA form there is a fraction of one pipelined phase) -> ncol = 120 only.
+  static constexpr bool TF32 = TREX_TF32_COLOUR && sizeof(RC) == 4 && EPB == 1 && NC == 120;
+  static constexpr int TF32_DEN = NC == 24 ? 54 : 324;
+  static constexpr int NMT = (NC + 15) / 16, NKB = NC / 8;   // 16-row tiles of T = C'^T X, 8-flow k blocks
+  __host__ __device__ static constexpr int tf32_kb(int J) { return 2 * J + 2 < NKB ? 2 * J + 2 : NKB; }   // k blocks with i <= 16 J + 15
+  __host__ __device__ static constexpr int tf32_frag0(int J) { int f = 0; for (int j = 0; j < J; ++j) f += tf32_kb(j); return f; }
+  static constexpr int CN = TF32 ? tf32_frag0(NMT) * 128 : FoldedC<NC>::size();       // numbers in the colour-matrix block
+  static constexpr int XS = (DMMA_CFG || TF32) ? NCOLT + 4 : NCOLT + 1;
   static constexpr int NSUB = 1 << N;
   // colour sum on the FP64 tensor cores: fp64 colour arithmetic, ncol = 120 (and 24), one partial-sum slot per thread
   static constexpr bool DMMA = DMMA_CFG;
   static constexpr int NCI0 = NCOLT * FoldedC<NC>::NPAIR;    // colour-sum work items of the FMA form
-  static constexpr int NCI = (DMMA && NCI0 < TB) ? TB : NCI0;  // partial-sum slots per event
+  static constexpr int NCI = ((DMMA || TF32) && NCI0 < TB) ? TB : NCI0;  // partial-sum slots per event
   // shared-memory carve-up (bytes, every region 16-byte aligned): EPB event slots, then the block-wide constants
   static constexpr size_t al(size_t x) { return (x + 15) / 16 * 16; }
   static constexpr size_t o_tab = 0;
@@ -136,7 +150,7 @@ template <class R, class RC, int N> struct TabGeom {
   static constexpr int NROW = 4 * (N + 2);                   // momentum rows of one event
   static constexpr size_t slot = o_pm + al(sizeof(double) * NROW);
   static constexpr size_t o_c = slot * EPB;
-  static constexpr size_t o_meta = o_c + al(sizeof(RC) * FoldedC<NC>::size());
+  static constexpr size_t o_meta = o_c + al(sizeof(RC) * CN);
   static constexpr size_t bytes = o_meta + al(sizeof(int) * I::M_SIZE);
   static_assert(bytes <= 232448, "one SM has 227 KB of shared memory");
 };
@@ -517,6 +531,41 @@ __device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, cons
       }
     }
     part[tid] += accl;                                  // slot parity = lane parity = column parity = theta
+  } else if constexpr (G::TF32) {
+    // TF32 tensor cores (mma.sync m16n8k8, fp32 accumulators): T = C'^T X in 16 x 8 tiles (16 flows j, 4 complex columns),
+    // k over the flows i <= 16 J + 15 in blocks of 8; A = the integer colour matrix (exact in TF32), B = X as hi + lo.
+    // Accumulator layout: rows g = lane / 4 and g + 8, columns 2 (lane % 4), + 1 = (Re, Im) of t_j for one complex column.
+    const int lane = tid & 31, wrp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const float* xr = reinterpret_cast<const float*>(xs);
+    constexpr int XR = 2 * XS, NCB = G::NCOLT / 4;
+    const int cstep = ncw > 0 ? ncw : GS / 32;
+    if (wrp >= cstep) return;
+    float accl = 0.f;
+    const auto tf32 = [](float x) { unsigned r; asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x)); return r; };
+    for (int cb = wrp; cb < NCB; cb += cstep) {
+#pragma unroll 1
+      for (int J = 0; J < G::NMT; ++J) {
+        float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f;
+        const int nkb = G::tf32_kb(J);
+        const float4* af = reinterpret_cast<const float4*>(Cs) + (size_t)G::tf32_frag0(J) * 32 + lane;
+        for (int kb = 0; kb < nkb; ++kb) {
+          const float4 av = af[kb * 32];
+          const unsigned a0 = __float_as_uint(av.x), a1 = __float_as_uint(av.y), a2 = __float_as_uint(av.z), a3 = __float_as_uint(av.w);
+          const float x0 = xr[(8 * kb + t) * XR + 8 * cb + g], x1 = xr[(8 * kb + t + 4) * XR + 8 * cb + g];
+          const unsigned h0 = tf32(x0), h1 = tf32(x1);
+          const unsigned l0 = tf32(x0 - __uint_as_float(h0)), l1 = tf32(x1 - __uint_as_float(h1));
+          asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                       : "+f"(d0), "+f"(d1), "+f"(d2), "+f"(d3) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(h0), "r"(h1));
+          asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                       : "+f"(d0), "+f"(d1), "+f"(d2), "+f"(d3) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(l0), "r"(l1));
+        }
+        const int j0 = 16 * J + g;
+        if (j0 < G::NC) { const cx<RC> xj = xs[j0 * XS + 4 * cb + t]; accl += xj.re * d0 + xj.im * d1; }
+        if (j0 + 8 < G::NC) { const cx<RC> xj = xs[(j0 + 8) * XS + 4 * cb + t]; accl += xj.re * d2 + xj.im * d3; }
+      }
+    }
+    part[tid] += (double)accl * (1.0 / G::TF32_DEN);        // slot parity = lane parity = column parity = theta
   } else
   for (int item = gtid; item < G::NCI0; item += GS) {
     const int c = item % G::NCOLT, p = item / G::NCOLT;
@@ -565,7 +614,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
 
   const EvIO io = resolve_io(a);
   for (int i = tid; i < I::M_SIZE; i += TB) meta[i] = gmeta[i];
-  for (int i = tid; i < F::size(); i += TB) Cs[i] = RC(Cfold[i]);
+  for (int i = tid; i < G::CN; i += TB) Cs[i] = RC(Cfold[i]);
   for (int i = gtid; i < G::NCI; i += GS) part[i] = 0.0;
   __syncthreads();
 
@@ -730,7 +779,19 @@ int TREX_TU_NAME(trex_tu_table_fold_n, TREX_TU_N, TREX_TU_MODE)(const double* C,
   const auto folded = [&](int i, int j) { return j < i ? 0.0 : (j == i ? C[i * NC + i] : 2.0 * C[i * NC + j]); };
   if (f) {
     int k = 0;
-    if (TabGeom<TuR, TuRC, TREX_TU_N>::DMMA) {
+    using G = TabGeom<TuR, TuRC, TREX_TU_N>;
+    if (G::TF32) {
+      // mma.m16n8k8 A fragments (row-major 16 x 8, A[m = j][k = i] = C'(i, j) x TF32_DEN, integers): per (J, kb) 32 lanes x
+      // (a0, a1, a2, a3) = rows g / g + 8, columns t / t + 4 with g = lane / 4, t = lane % 4; flows beyond ncol are zero
+      const auto A = [&](int i, int j) { return (i < NC && j < NC) ? folded(i, j) * G::TF32_DEN : 0.0; };
+      for (int J = 0; J < G::NMT; ++J)
+        for (int kb = 0; kb < G::tf32_kb(J); ++kb)
+          for (int lane = 0; lane < 32; ++lane) {
+            const int g = lane >> 2, t = lane & 3;
+            f[k++] = std::nearbyint(A(8 * kb + t, 16 * J + g));     f[k++] = std::nearbyint(A(8 * kb + t, 16 * J + g + 8));
+            f[k++] = std::nearbyint(A(8 * kb + t + 4, 16 * J + g)); f[k++] = std::nearbyint(A(8 * kb + t + 4, 16 * J + g + 8));
+          }
+    } else if (TabGeom<TuR, TuRC, TREX_TU_N>::DMMA) {
       // tensor-core colour sum: mma A fragments in the order the kernel consumes them, (J, ks) -> 32 lanes
       // (lane = 4 fr + fc holds C'(4 ks + fc, 8 J + fr)); sum_J 2 (J + 1) fragments of 32 = F::size() numbers again
       for (int J = 0; J < F::NB; ++J)
@@ -741,7 +802,7 @@ int TREX_TU_NAME(trex_tu_table_fold_n, TREX_TU_N, TREX_TU_MODE)(const double* C,
         for (int j = F::RB * (i / F::RB); j < NC; ++j) f[k++] = folded(i, j);
     }
   }
-  return F::size();
+  return TabGeom<TuR, TuRC, TREX_TU_N>::CN;
 }
 
 // layout of the diagnostic X-tile dump: {NFIX, iterations, lambda_t passes per iteration, flows, columns per pass}
