@@ -146,7 +146,9 @@ __device__ __forceinline__ void w4_prep(const W4Ptr<R>& p, typename W4<R, RC>::S
       vec4<R> J; ften<R> Fw;
       tab_level1_JF<R, N, 0>(p.meta, sm.pset, sm.eps, 0u, lane, J, Fw);
       w4_finish<R, RC, 1>(p, sm, lane, poff, J, make_sigF<R>(Fw));
-    } else if (lane < 12) {                                // bilinears of the closed line (see wform_bilinears)
+    } else if (lane < 12) {
+      // bilinears of the closed line, per (lambda_t, lambda_tbar): i ubar Aslash v = sum_k c_k (a+, a-, at, ab)_k with
+      // a+- = a0 +- a3, at/ab = a1 +- i a2, and i ubar (-i 2 sigma.F) v = sum_k c_k (p3, pt, pb, m3, mt, mb)_k (w4_top)
       const int combo = lane - 8, lt = combo >> 1, ltb = combo & 1;
       const spinor<R> r = spinor_from<R>(sm.spin + lt * 8), v = spinor_from<R>(sm.spin + (2 + ltb) * 8);
       cx<R> c[10];

@@ -58,9 +58,6 @@ namespace {
 #ifndef TREX_T4_WFORM
 #define TREX_T4_WFORM 1
 #endif
-#ifndef TREX_T4_PIPE
-#define TREX_T4_PIPE 1
-#endif
 #ifndef TREX_TF32_COLOUR
 #define TREX_TF32_COLOUR 1
 #endif
@@ -73,14 +70,12 @@ namespace {
 // UT: the top-line states of ordering prefixes up to this length are tabulated per event instead of being carried by
 // every walk thread (fewer registers per thread -> more warps, and no recomputation across tasks)
 template <int N> struct TabCfg;
-// WFORM (N = 4): leaf amplitudes as row x column products against tabulated suffix contractions (trex_table.cuh, "W form");
-// a walk task is (ordering, helicities of its first three gluons, lambda_t, parameter point) and closes both helicities of
-// the last gluon and both antitop helicities from one line state
+// (N = 4 runs the W-form event pipeline of trex_table4.cuh unless TREX_T4_WFORM = 0 selects the kernel of this file)
 // LTSPLIT: walk + colour sum run once per top helicity, the X tile holds the columns of one lambda_t only (half the tile:
 // room for a second resident block per SM)
-template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = TREX_T3_UT == 2 ? 3 : 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB, UT = TREX_T3_UT, LTSPLIT = 0, WFORM = 0; };
-template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = TREX_T4_UT ? 4 : 2, TB = TREX_T4_TB, EPB = 1, MINB = TREX_T4_MINB, UT = TREX_T4_UT, LTSPLIT = TREX_T4_LTSPLIT, WFORM = TREX_T4_WFORM; };
-template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1, UT = TREX_T5_UT, LTSPLIT = 0, WFORM = 0; };
+template <> struct TabCfg<3> { static constexpr int NFIX = 0, D = TREX_T3_UT == 2 ? 3 : 2, TB = TREX_T3_TB, EPB = TREX_T3_EPB, MINB = TREX_T3_MINB, UT = TREX_T3_UT, LTSPLIT = 0; };
+template <> struct TabCfg<4> { static constexpr int NFIX = 0, D = TREX_T4_UT ? 4 : 2, TB = TREX_T4_TB, EPB = 1, MINB = TREX_T4_MINB, UT = TREX_T4_UT, LTSPLIT = TREX_T4_LTSPLIT; };
+template <> struct TabCfg<5> { static constexpr int NFIX = 3, D = 3, TB = 256, EPB = 1, MINB = 1, UT = TREX_T5_UT, LTSPLIT = 0; };
 
 template <int NC> struct FoldedC {
   // C'(i,j) = 0 (j < i), C_ii (j == i), 2 C_ij (j > i), stored by rows i for j >= RB floor(i/RB)
@@ -135,18 +130,7 @@ template <class R, class RC, int N> struct TabGeom {
   static constexpr size_t o_spin = o_eps + al(sizeof(double) * 16 * N);
   static constexpr size_t o_part = o_spin + al(sizeof(double) * 8 * 4);
   static constexpr size_t o_utab = o_part + al(sizeof(double) * NCI);
-  // W form: suffix contractions of the entries below level N, (entry, lambda_tbar) records; A = 0 rows of the level N - 1
-  // entries, (entry, lambda_t) records; the level-N entries keep only their closed scalars, in the table's own slots
-  static constexpr bool WFORM = Cfg::WFORM != 0;
-  static_assert(!WFORM || (N == 4 && NFIX == 0 && UT == 2 && Cfg::LTSPLIT == 0 && EPB == 1), "W form is written for N = 4");
-  static constexpr int E3 = I::entries_below(N - 1), E4 = I::entries_below(N);
-  static constexpr int NWE = 2 * E4, NUB = 2 * (E4 - E3);
-  static constexpr size_t o_w = o_utab + (UT ? al(sizeof(R) * 16 * NUT) : 0);
-  static constexpr size_t o_ub = o_w + (WFORM ? al(sizeof(R) * 16 * NWE) : 0);
-  // bilinears of the closed line, per (lambda_t, lambda_tbar): i ubar Aslash v = sum_k cA_k (a+, a-, at, ab)_k and
-  // i ubar (-i 2 sigma.F) v = sum_k cF_k (p3, pt, pb, m3, mt, mb)_k : [4 combos][10 complex]
-  static constexpr size_t o_bil = o_ub + (WFORM ? al(sizeof(R) * 16 * NUB) : 0);
-  static constexpr size_t o_pm = o_bil + (WFORM ? al(sizeof(R) * 2 * 40) : 0);
+  static constexpr size_t o_pm = o_utab + (UT ? al(sizeof(R) * 16 * NUT) : 0);
   static constexpr int NROW = 4 * (N + 2);                   // momentum rows of one event
   static constexpr size_t slot = o_pm + al(sizeof(double) * NROW);
   static constexpr size_t o_c = slot * EPB;
@@ -235,246 +219,6 @@ __device__ __forceinline__ void build_levels(unsigned char* sb, const int* meta,
     }
     group_sync<G::GS>();
     build_levels<R, RC, N, NPASS, K + 1>(sb, meta, gtid, a, pt);
-  }
-}
-
-#ifdef TREX_PHASE_CLOCKS
-__device__ long long g_lvl_clk[8], g_lvl_t0;     // block 0 only (instrumented build)
-#endif
-// ---------------------------------------------------------------- W form (N = 4)
-// what a finished table entry of level K leaves behind: J and -i 2 sigma.F (K < N), its suffix contractions W (K < N),
-// its A = 0 rows ubar Gamma(J) (K = N - 1), or nothing but its closed scalars S = ubar W (K = N)
-template <class R, class RC, int N, int K>
-__device__ __forceinline__ void wform_finish(unsigned char* sb, int e, const vec4<R>& J, const sigF<R>& F) {
-  using G = TabGeom<R, RC, N>;
-  constexpr int NE = G::NE;
-  R* tab = reinterpret_cast<R*>(sb + G::o_tab);
-  const double* spin = reinterpret_cast<const double*>(sb + G::o_spin);
-  static_assert(K < N, "level-N entries only leave their closed scalars (wform_top)");
-  tab_store<R, NE>(tab, e, J, F);
-#pragma unroll
-  for (int ltb = 0; ltb < 2; ++ltb) {
-    const spinor<R> v = spinor_from<R>(spin + (2 + ltb) * 8);
-    spinor<R> wj = slash_col(J, v), wf = sig_col(F, v);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) { wj.c[i] = mul_i(wj.c[i]); wf.c[i] = mul_i(wf.c[i]); }
-    rec_put<R>(reinterpret_cast<R*>(sb + G::o_w), G::NWE, e * 2 + ltb, wj, wf);
-  }
-  if constexpr (K == N - 1) {
-#pragma unroll
-    for (int lt = 0; lt < 2; ++lt) {
-      const spinor<R> ub = spinor_from<R>(spin + lt * 8);
-      spinor<R> s0 = szero<R>(), s1 = szero<R>();
-      row_slash_acc(s0, ub, J);
-      row_sigma_acc_x(s1, ub, F);
-      rec_put<R>(reinterpret_cast<R*>(sb + G::o_ub), G::NUB, (e - G::E3) * 2 + lt, s0, s1);
-    }
-  }
-}
-
-// bilinear coefficients of one (lambda_t, lambda_tbar) combination (see TabGeom::o_bil)
-template <class R, class RC, int N>
-__device__ __forceinline__ void wform_bilinears(unsigned char* sb, int combo) {
-  using G = TabGeom<R, RC, N>;
-  const double* spin = reinterpret_cast<const double*>(sb + G::o_spin);
-  const int lt = combo >> 1, ltb = combo & 1;
-  const spinor<R> r = spinor_from<R>(spin + lt * 8), v = spinor_from<R>(spin + (2 + ltb) * 8);
-  cx<R> c[10];
-  c[0] = r.c[2] * v.c[0]; cfma(c[0], r.c[1], v.c[3]);        // a+ = a0 + a3
-  c[1] = r.c[3] * v.c[1]; cfma(c[1], r.c[0], v.c[2]);        // a- = a0 - a3
-  c[2] = r.c[3] * v.c[0]; cfnma(c[2], r.c[1], v.c[2]);       // at = a1 + i a2
-  c[3] = r.c[2] * v.c[1]; cfnma(c[3], r.c[0], v.c[3]);       // ab = a1 - i a2
-  c[4] = r.c[0] * v.c[0]; cfnma(c[4], r.c[1], v.c[1]);       // p3
-  c[5] = r.c[1] * v.c[0];                                    // pt
-  c[6] = r.c[0] * v.c[1];                                    // pb
-  c[7] = r.c[2] * v.c[2]; cfnma(c[7], r.c[3], v.c[3]);       // m3
-  c[8] = r.c[3] * v.c[2];                                    // mt
-  c[9] = r.c[2] * v.c[3];                                    // mb
-  R* bil = reinterpret_cast<R*>(sb + G::o_bil);
-#pragma unroll
-  for (int k = 0; k < 10; ++k) tab_put<R>(bil, combo * 10 + k, mul_i(c[k]));
-}
-
-// a level-N entry: J and F stay in registers and are closed with the bilinears into S0 = i ubar Jslash v,
-// S1 = i ubar (-i 2 sigma.F) v for the four (lambda_t, lambda_tbar), stored in the entry's own table slots
-template <class R, class RC, int N>
-__device__ __forceinline__ void wform_top(unsigned char* sb, const int* meta, int e) {
-  using G = TabGeom<R, RC, N>;
-  constexpr int NE = G::NE;
-  const rvec4<double>* pset = reinterpret_cast<const rvec4<double>*>(sb + G::o_pset);
-  TabBuild<R, N, G::NFIX, N> b;
-  tab_build_setup<R, N, G::NFIX, N>(b, reinterpret_cast<const R*>(sb + G::o_tab), meta, pset, e);
-  vec4<R> acc = vzero<R>();
-  ften<R> Fc = fzero<R>();
-  b.template v3_splits<1>(acc, Fc);
-  b.template v4_splits<1, 2>(acc);
-  const rvec4<double>& P = pset[(1u << N) - 1u];
-  const R sc = R(-1.0 / rdot(P, P));
-  vec4<R> J;
-#pragma unroll
-  for (int i = 0; i < 4; ++i) J.c[i] = acc.c[i] * sc;
-  wedge_acc(Fc, cast<R>(P), J);
-  const sigF<R> F = make_sigF<R>(Fc);
-  const cx<R> a4[4] = {J.c[0] + J.c[3], J.c[0] - J.c[3], J.c[1] + mul_i(J.c[2]), J.c[1] - mul_i(J.c[2])};
-  const cx<R>* f6 = &F.p3;
-  const R* bil = reinterpret_cast<const R*>(sb + G::o_bil);
-  R* dst = reinterpret_cast<R*>(sb + G::o_tab);
-  const int stride = NE, idx = e;
-#pragma unroll
-  for (int combo = 0; combo < 4; ++combo) {
-    cx<R> s0 = tab_get<R>(bil, combo * 10, 1) * a4[0];
-#pragma unroll
-    for (int k = 1; k < 4; ++k) cfma(s0, tab_get<R>(bil, combo * 10 + k, 1), a4[k]);
-    cx<R> s1 = tab_get<R>(bil, combo * 10 + 4, 1) * f6[0];
-#pragma unroll
-    for (int k = 1; k < 6; ++k) cfma(s1, tab_get<R>(bil, combo * 10 + 4 + k, 1), f6[k]);
-    tab_put<R>(dst, (combo * 2 + 0) * stride + idx, s0);
-    tab_put<R>(dst, (combo * 2 + 1) * stride + idx, s1);
-  }
-}
-
-template <class R, class RC, int N, int NPASS, int K>
-__device__ __forceinline__ void build_levels_w(unsigned char* sb, const int* meta, int gtid, const ReweightArgs& a, const rvec4<double>& pt) {
-  using G = TabGeom<R, RC, N>;
-  using I = typename G::I;
-  if constexpr (K <= N) {
-    const int e0 = meta[I::M_LVL + K], ntab = meta[I::M_LVL + K + 1] - e0;
-    constexpr int L = K - 1;
-    constexpr int nus = (L >= 1 && L <= G::UT) ? (L == 1 ? G::UI::N1 : G::UI::N2) : 0;
-    if constexpr (K == N) {
-      for (int it = gtid; it < ntab; it += G::GS) wform_top<R, RC, N>(sb, meta, e0 + it);
-    } else
-    for (int it = gtid; it < ntab + nus * NPASS + (K == 1 ? 4 : 0); it += G::GS) {
-      if constexpr (K == 1) { if (it >= ntab) { wform_bilinears<R, RC, N>(sb, it - ntab); continue; } }
-      if (it < ntab) {
-        vec4<R> J; ften<R> Fw;
-        if constexpr (K == 1) tab_level1_JF<R, N, G::NFIX>(meta, reinterpret_cast<const rvec4<double>*>(sb + G::o_pset),
-                                                           reinterpret_cast<const double*>(sb + G::o_eps), 0u, e0 + it, J, Fw);
-        else {
-          TabBuild<R, N, G::NFIX, K> b;
-          tab_build_setup<R, N, G::NFIX, K>(b, reinterpret_cast<const R*>(sb + G::o_tab), meta, reinterpret_cast<const rvec4<double>*>(sb + G::o_pset), e0 + it);
-          b.compute(J, Fw);
-        }
-        wform_finish<R, RC, N, K>(sb, e0 + it, J, make_sigF<R>(Fw));
-      } else if constexpr (nus > 0) {
-        const int u = it - ntab, pass = u / nus;
-        build_ustate<R, RC, N, L>(sb, meta, a, pt, u - pass * nus, pass);
-      }
-    }
-    group_sync<G::GS>();
-#ifdef TREX_PHASE_CLOCKS
-    if (threadIdx.x == 0) { const long long t = clock64(); g_lvl_clk[K] += t - g_lvl_t0; g_lvl_t0 = t; }
-#endif
-    build_levels_w<R, RC, N, NPASS, K + 1>(sb, meta, gtid, a, pt);
-  }
-}
-
-// U . W terms of one leaf: a0 += sign U.o0 . Wj,  a1 += sign (U.o1 . Wj + U.o0 . Wf)
-template <class R> __device__ __forceinline__ void leaf_term(cx<R>& a0, cx<R>& a1, const dspinor<R>& U, const R* __restrict__ wtab, int nwe, int rec, int sign) {
-  spinor<R> wj, wf;
-  rec_get<R>(wtab, nwe, rec, 1, wj, wf);
-  cx<R> t0 = U.o0.c[0] * wj.c[0], t1 = U.o1.c[0] * wj.c[0];
-#pragma unroll
-  for (int i = 1; i < 4; ++i) { cfma(t0, U.o0.c[i], wj.c[i]); cfma(t1, U.o1.c[i], wj.c[i]); }
-#pragma unroll
-  for (int i = 0; i < 4; ++i) cfma(t1, U.o0.c[i], wf.c[i]);
-  a0 += cx<R>(with_sign(t0.re, sign), with_sign(t0.im, sign));
-  a1 += cx<R>(with_sign(t1.re, sign), with_sign(t1.im, sign));
-}
-
-template <class R, class RC, int NPASS>
-__device__ __forceinline__ void walk_wform(unsigned char* sb, const int* meta, int gtid, const ReweightArgs& a, const rvec4<double>& pt) {
-  constexpr int N = 4;
-  using G = TabGeom<R, RC, N>;
-  using I = typename G::I;
-  using UI = typename G::UI;
-  constexpr int NE = G::NE, XS = G::XS;
-  const R* tab = reinterpret_cast<const R*>(sb + G::o_tab);
-  const R* utab = reinterpret_cast<const R*>(sb + G::o_utab);
-  const R* wtab = reinterpret_cast<const R*>(sb + G::o_w);
-  const R* ubt = reinterpret_cast<const R*>(sb + G::o_ub);
-  const rvec4<double>* pset = reinterpret_cast<const rvec4<double>*>(sb + G::o_pset);
-  cx<RC>* xs = reinterpret_cast<cx<RC>*>(sb + G::o_x);
-  for (int task = gtid; task < 384 * NPASS; task += G::GS) {
-    const int pass = task / 384, r = task - pass * 384;
-    const int prank = r >> 4, lt = r & 1;
-    const unsigned hp = (unsigned)(r >> 1) & 7u;             // helicities of s1, s2, s3 (bit i: s_{i+1})
-    // table references of this ordering (TabIdx::M_REC): no index arithmetic on the critical path of the loads
-    const int4 rc = reinterpret_cast<const int4*>(meta + I::M_REC)[prank];
-    const auto ref = [](unsigned rf, unsigned bits, int nf, int& sign) {
-      sign = (rf & 0x400u) ? -1 : 1;
-      return (int)(rf & 0x1FFu) + (int)((rf & 0x200u) ? I::bitrev(bits, nf) : bits);
-    };
-    const unsigned sp = (unsigned)rc.w >> 16;
-    const int s[4] = {(int)(sp & 3u), (int)((sp >> 2) & 3u), (int)((sp >> 4) & 3u), (int)((sp >> 6) & 3u)};
-    const int ubase = pass * G::NU;
-    dspinor<R> U1, U2, U3;
-    rec_get<R>(utab, G::NUT, ubase + UI::level1(s[0], hp & 1u, lt), 1, U1.o0, U1.o1);
-    rec_get<R>(utab, G::NUT, ubase + UI::N1 + (((int)(sp >> 8) * 4 + (int)(hp & 3u)) * 2 + lt), 1, U2.o0, U2.o1);
-    // ---- node 3: U3 = [ ubar Gamma(J(s1 s2 s3)) + U1 Gamma(J(s2 s3)) + U2 Gamma(J(s3)) ] S(p_t - K(s1 s2 s3))
-    {
-      spinor<R> s0, s1;
-      int sign;
-      int e = ref((unsigned)rc.x & 0xFFFFu, hp, 3, sign);
-      rec_get<R>(ubt, G::NUB, (e - G::E3) * 2 + lt, sign, s0, s1);
-      e = ref((unsigned)rc.x >> 16, hp >> 1, 2, sign);
-      {
-        const vec4<R> J = tab_J<R, NE>(tab, e, sign);
-        row_slash_acc(s0, U1.o0, J); row_slash_acc(s1, U1.o1, J);
-        row_sigma_acc_x(s1, U1.o0, tab_F<R, NE>(tab, e, sign));
-      }
-      e = ref((unsigned)rc.y & 0xFFFFu, hp >> 2, 1, sign);
-      {
-        const vec4<R> J = tab_J<R, NE>(tab, e, sign);
-        row_slash_acc(s0, U2.o0, J); row_slash_acc(s1, U2.o1, J);
-        row_sigma_acc_x(s1, U2.o0, tab_F<R, NE>(tab, e, sign));
-      }
-#pragma unroll
-      for (int i = 0; i < 4; ++i) { s0.c[i] = mul_i(s0.c[i]); s1.c[i] = mul_i(s1.c[i]); }
-      const rvec4<double> qd = rsub(pt, pset[15u ^ (1u << s[3])]);
-      const double q2 = rdot(qd, qd), mt = a.T.mt[pass];
-      const rvec4<R> q = cast<R>(qd);
-      const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), cx<double>(q2 - mt * mt, a.T.mGt[pass])));
-      const spinor<R> n0 = row_slash(s0, q), n1 = row_slash(s1, q);
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        cx<R> x0 = n0.c[i]; cfma(x0, s0.c[i], R(mt));
-        cx<R> x1 = n1.c[i]; cfma(x1, s1.c[i], R(mt));
-        U3.o0.c[i] = x0 * pr; U3.o1.c[i] = x1 * pr;
-      }
-    }
-    // ---- leaves: both helicities of s4, both antitop helicities
-    const R kq0 = R(a.T.kq[0]), kq1 = R(a.T.kq[1]);
-#pragma unroll 1
-    for (unsigned h4 = 0; h4 < 2; ++h4) {
-      const unsigned hp4 = hp | (h4 << 3);
-      int sg0, sg1, sg2, sg3;
-      const int e4 = ref((unsigned)rc.y >> 16, hp4, 4, sg0);
-      const int e1 = ref((unsigned)rc.z & 0xFFFFu, hp4 >> 1, 3, sg1);
-      const int e2 = ref((unsigned)rc.z >> 16, hp4 >> 2, 2, sg2);
-      const int e3 = ref((unsigned)rc.w & 0xFFFFu, hp4 >> 3, 1, sg3);
-      unsigned hfree = 0;
-#pragma unroll
-      for (int i = 0; i < 4; ++i) hfree |= ((hp4 >> i) & 1u) << s[i];
-#pragma unroll
-      for (int ltb = 0; ltb < 2; ++ltb) {
-        cx<R> a0 = tab_get<R>(tab, ((lt * 2 + ltb) * 2 + 0) * NE + e4, sg0);
-        cx<R> a1 = tab_get<R>(tab, ((lt * 2 + ltb) * 2 + 1) * NE + e4, sg0);
-        leaf_term<R>(a0, a1, U1, wtab, G::NWE, e1 * 2 + ltb, sg1);
-        leaf_term<R>(a0, a1, U2, wtab, G::NWE, e2 * 2 + ltb, sg2);
-        leaf_term<R>(a0, a1, U3, wtab, G::NWE, e3 * 2 + ltb, sg3);
-        const int col = (((int)hfree * 2 + lt) * 2 + ltb) * 2;
-        if constexpr (NPASS == 1) {
-          cx<R> x = a0; cfma(x, a1, kq0);
-          cx<R> y = a0; cfma(y, a1, kq1);
-          xs[prank * XS + col] = cx<RC>(RC(x.re), RC(x.im));
-          xs[prank * XS + col + 1] = cx<RC>(RC(y.re), RC(y.im));
-        } else {
-          cx<R> x = a0; cfma(x, a1, pass == 0 ? kq0 : kq1);
-          xs[prank * XS + col + pass] = cx<RC>(RC(x.re), RC(x.im));
-        }
-      }
-    }
   }
 }
 
@@ -677,21 +421,13 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
     for (int mu = 0; mu < 4; ++mu) ptop.c[mu] = pm[2 * 4 + mu];
     for (unsigned itb = 0; itb < (unsigned)G::NIT; ++itb) {
       // ---- phase 1: current table of this helicity iteration (+ line states of short prefixes, if tabulated)
-#ifdef TREX_PHASE_CLOCKS
-      if (tid == 0) g_lvl_t0 = clock64();
-#endif
-      if constexpr (G::WFORM) build_levels_w<R, RC, N, NPASS, 1>(sb, meta, gtid, a, ptop);
-      else {
-        for (int e1 = gtid; e1 < meta[I::M_LVL + 2]; e1 += GS) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
-        group_sync<GS>();
-        build_levels<R, RC, N, NPASS, 2>(sb, meta, gtid, a, ptop);
-      }
+      for (int e1 = gtid; e1 < meta[I::M_LVL + 2]; e1 += GS) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
+      group_sync<GS>();
+      build_levels<R, RC, N, NPASS, 2>(sb, meta, gtid, a, ptop);
       PHASE_TICK(1);
 
       for (int lti = 0; lti < G::NLT; ++lti) {
       // ---- phase 2: top-line walk
-      if constexpr (G::WFORM) { if constexpr (N == 4) walk_wform<R, RC, NPASS>(sb, meta, gtid, a, ptop); }
-      else
       for (int task = gtid; task < G::NTASK * NPASS; task += GS) {
         const int pass = task / G::NTASK, r = task - pass * G::NTASK;
         const int hli = r % G::NHL, prank = r / G::NHL;
@@ -756,7 +492,6 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
     PHASE_TICK(4);
   }
 #ifdef TREX_PHASE_CLOCKS
-  if (tid == 0 && blockIdx.x == 0 && G::WFORM) printf("   table levels 1..4: %lld %lld %lld %lld\n", g_lvl_clk[1], g_lvl_clk[2], g_lvl_clk[3], g_lvl_clk[4]);
   if (tid == 0 && blockIdx.x == 0) printf("k_table N=%d phases [cycles of block 0]: setup %lld  table %lld  walk %lld  colour %lld  epilogue %lld\n", N, pc[0], pc[1], pc[2], pc[3], pc[4]);
 #endif
 }
@@ -816,7 +551,7 @@ int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const Reweight
                                                                   int nsm, cudaStream_t s) {
   constexpr int N = TREX_TU_N;
   using G = TabGeom<TuR, TuRC, N>;
-#if TREX_TU_N == 4 && TREX_T4_PIPE && TREX_T4_WFORM
+#if TREX_TU_N == 4 && TREX_T4_WFORM
   {
     // software-pipelined W-form kernel (trex_table4.cuh): one persistent 384-thread block per SM
     using W = W4<TuR, TuRC>;
@@ -832,7 +567,7 @@ int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const Reweight
     else k_table4w<TuR, TuRC, 2><<<grid, W::TB, W::bytes, s>>>(a, meta, Cfold);
     return (int)cudaGetLastError();
   }
-#endif
+#else
   static int blocks_per_sm = 0;
   if (!blocks_per_sm) {
     cudaFuncSetAttribute(k_table<TuR, TuRC, N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::bytes);
@@ -848,6 +583,7 @@ int TREX_TU_NAME(trex_tu_table_launch_n, TREX_TU_N, TREX_TU_MODE)(const Reweight
   if (npass == 1) k_table<TuR, TuRC, N, 1><<<grid, G::TB, G::bytes, s>>>(a, meta, Cfold);
   else k_table<TuR, TuRC, N, 2><<<grid, G::TB, G::bytes, s>>>(a, meta, Cfold);
   return (int)cudaGetLastError();
+#endif
 }
 
 }  // namespace trex
