@@ -30,7 +30,7 @@ struct Table {
   unsigned long long* keys;   // [TS]
   unsigned* first;            // [TS] index of first appearance
   int* bid;                   // [TS] bucket id
-  int* meta;                  // [0] ndistinct, [1] has_npos, [2] overflow, [3] nb
+  int* meta;                  // [0] ndistinct, [1] has_npos, [2] overflow, [3] nb, [4] single known class: chain finished by k_rank
   unsigned* npos_first;       // [1]
 };
 
@@ -39,7 +39,7 @@ __device__ __forceinline__ unsigned hash_key(unsigned long long k) { return (uns
 __global__ void k_init(Table t) {
   int i = threadIdx.x;
   t.keys[i] = EMPTY; t.first[i] = 0xFFFFFFFFu; t.bid[i] = -1;
-  if (i < 4) t.meta[i] = 0;
+  if (i < 8) t.meta[i] = 0;
   if (i == 0) *t.npos_first = 0xFFFFFFFFu;
 }
 
@@ -88,7 +88,10 @@ __global__ void __launch_bounds__(256) k_discover(const unsigned long long* __re
   }
 }
 
-__global__ void __launch_bounds__(TS) k_rank(Table t, BucketResult* res) {
+// (trex_run only, npar > 0) A sample of ONE class that a compiled-in subprocess claims is reweighted in place: no
+// permutation is needed, so the plan is written here and histogram, scan and scatter return at once (meta[4]).
+__global__ void __launch_bounds__(TS) k_rank(Table t, BucketResult* res, long n, const unsigned long long* __restrict__ sub, int npar,
+                                             DevPlan* __restrict__ plan, int force_gather) {
   __shared__ unsigned sf[NBMAX + 1];
   __shared__ int s_cnt;
   const int s = threadIdx.x;
@@ -114,6 +117,20 @@ __global__ void __launch_bounds__(TS) k_rank(Table t, BucketResult* res) {
     res->err = bad ? 1 : 0;
     if (!bad && has_npos) res->keys[nd] = EMPTY;
   }
+  if (npar <= 0 || bad || nd != 1 || has_npos || force_gather) return;       // uniform over the block
+  __shared__ unsigned long long the_key;
+  __shared__ int claimed;
+  if (s == 0) claimed = 0;
+  if (k != EMPTY) the_key = k;
+  __syncthreads();
+  if (s < TREX_NSUBPROC && (int)sub[2 * s + 1] == npar && sub[2 * s] == the_key) claimed = 1;
+  __syncthreads();
+  if (!claimed) return;
+  if (s < TREX_NSUBPROC) {
+    const bool mine = (int)sub[2 * s + 1] == npar && sub[2 * s] == the_key;
+    plan->off[s] = 0; plan->cnt[s] = mine ? n : 0;
+  }
+  if (s == 0) { plan->single = 1; plan->nb = 1; res->offsets[0] = 0; res->offsets[1] = n; t.meta[4] = 1; }
 }
 
 // shared-memory copy of the key -> bucket table for the lookups of hist / scatter
@@ -139,7 +156,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_hist(const unsigned long long* _
   __shared__ SmemTable tab;
   __shared__ unsigned hist[WARPS][NBMAX];
   const int nb = t.meta[3];
-  if (nb == 0) return;
+  if (nb == 0 || t.meta[4]) return;
   tab.load(t);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   for (int i = lane; i < nb; i += 32) hist[warp][i] = 0;
@@ -155,6 +172,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_hist(const unsigned long long* _
 __global__ void __launch_bounds__(1024) k_scan(unsigned* __restrict__ counts, long nchunks, long n, Table t, BucketResult* res,
                                                const unsigned long long* __restrict__ sub, int npar, DevPlan* __restrict__ plan, int force_gather) {
   __shared__ unsigned long long part[1024];
+  if (t.meta[4]) return;
   const int nb = t.meta[3];
   const long total = (long)nb * nchunks;
   const long seg = (total + 1023) / 1024;
@@ -200,7 +218,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_scatter(const unsigned long long
   __shared__ SmemTable tab;
   __shared__ unsigned pos[WARPS][NBMAX];
   const int nb = t.meta[3];
-  if (nb == 0) return;
+  if (nb == 0 || t.meta[4]) return;
   tab.load(t);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const long chunk = (long)blockIdx.x * WARPS + warp;
@@ -499,7 +517,7 @@ BucketLayout bucket_layout(int64_t n) {
   while ((n + L.wch - 1) / L.wch > 4096) L.wch *= 2;
   L.nchunks = (n + L.wch - 1) / L.wch;
   L.off_keys = 0; L.off_first = align_up(L.off_keys + TS * 8); L.off_bid = align_up(L.off_first + TS * 4);
-  L.off_meta = align_up(L.off_bid + TS * 4); L.off_npos = align_up(L.off_meta + 16); L.off_res = align_up(L.off_npos + 4);
+  L.off_meta = align_up(L.off_bid + TS * 4); L.off_npos = align_up(L.off_meta + 32); L.off_res = align_up(L.off_npos + 4);
   L.off_counts = align_up(L.off_res + sizeof(BucketResult));
   L.total = align_up(L.off_counts + (size_t)NBMAX * L.nchunks * 4);
   return L;
@@ -543,7 +561,7 @@ int trex::bucket_enqueue(const uint64_t* pdg_keys, int64_t n, int32_t* perm, int
   while (per_block < 8192 && (n + per_block - 1) / per_block > 592) per_block *= 2;
   const unsigned nblk = (unsigned)((n + per_block - 1) / per_block);
   k_discover<<<nblk, 256, 0, c.stream>>>(keys, n, per_block, t);
-  k_rank<<<1, TS, 0, c.stream>>>(t, res);
+  k_rank<<<1, TS, 0, c.stream>>>(t, res, (long)n, (const unsigned long long*)c.plan_keys, npar, c.plan, c.legmap ? 1 : 0);
   const unsigned cblk = (unsigned)((nchunks + WARPS - 1) / WARPS);
   k_hist<<<cblk, WARPS * 32, 0, c.stream>>>(keys, n, wch, nchunks, t, counts);
   k_scan<<<1, 1024, 0, c.stream>>>(counts, nchunks, n, t, res, (const unsigned long long*)c.plan_keys, npar, c.plan, c.legmap ? 1 : 0);
