@@ -6,8 +6,9 @@
 //   phase B(i): level-4 entries of event i (warps 0-5)  |  "prep" of event i+1 (warps 6, 7): momenta, subset momenta,
 //               polarisations, spinors, bilinears, table levels 1 and 2 with their W records, line states U1
 //   phase C(i): top-line walk of event i (all warps)
-//   phase D(i): colour sum of event i (tensor cores for fp64)  |  level-3 entries + line states U2 of event i+1
-//   epilogue(i) by warp 0 while the others start phase B(i+1)
+//   phase D(i): colour sum of event i (fp64: six warps on the tensor cores)  |  level-3 entries + line states U2 of
+//               event i+1 (the other six warps; all warps do both when the colour sum is in FFMA form)
+//   epilogue(i) by warp 8, which is idle in phase B, while the others start phase B(i+1)
 // Three block barriers per event. What prep writes is double-buffered by event parity: the per-event constants are two
 // small blocks; the table entries of levels 1 and 2 (indices < PE), their W records and the U1 states have a second copy
 // at the end of their arrays (index + poff). Which references are of level <= 2 is known at compile time.
