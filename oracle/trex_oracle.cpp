@@ -686,8 +686,8 @@ template <class R> ABD<R> e2_abd(const Event<R>& ev, const Params<R>& P, int kin
     std::vector<int> gl;     // gluon legs
     if (kind == K_TTNG) { gl = {0, 1}; for (int l = 4; l < ev.npar; ++l) gl.push_back(l); }
     else if (kind == K_QQB) { for (int l = 4; l < ev.npar; ++l) gl.push_back(l); }
-    else if (kind == K_QG) gl = {1};
-    else gl = {0};
+    else if (kind == K_QG) { gl = {1}; for (int l = 5; l < ev.npar; ++l) gl.push_back(l); }     // leg 4 is the outgoing quark
+    else { gl = {0}; for (int l = 5; l < ev.npar; ++l) gl.push_back(l); }
     e.ns = 0;
     for (int leg : gl) {
       bool inc = leg < 2; int s = e.ns++;
@@ -730,8 +730,8 @@ template <class R> ABD<R> e2_abd(const Event<R>& ev, const Params<R>& P, int kin
   }
   R navg;
   if (kind == K_TTNG) { int n = ev.npar - 2; R fact = 1; for (int k = 2; k <= n - 2; ++k) fact *= k; navg = R(4) * R(64) * fact; }
-  else if (kind == K_QQB) navg = R(4) * R(9);
-  else navg = R(4) * R(24);
+  else if (kind == K_QQB) { R fact = 1; for (int k = 2; k <= ev.npar - 4; ++k) fact *= k; navg = R(4) * R(9) * fact; }   // identical final gluons
+  else { R fact = 1; for (int k = 2; k <= ev.npar - 5; ++k) fact *= k; navg = R(4) * R(24) * fact; }
   return ABD<R>{A / navg, B / navg, D / navg}; }
 
 // ---------------------------------------------------------------- subprocess dispatch (ids of include/rex_trex.h)
@@ -743,8 +743,10 @@ template <class R> ABD<R> e2_abd(const Event<R>& ev, const Params<R>& P, int kin
 inline int npar_of(int sid) {
   static const int t[10] = {4, 4, 5, 6, 7, 5, 5, 5, 5, 4};
   if (sid >= 0 && sid < 10) return t[sid];
+  if (sid >= 21 && sid <= 23) return 6;             // 21 u u~ > t t~ g g ; 22 u g > t t~ u g ; 23 g u~ > t t~ u~ g
   return (sid >= 10 && sid <= 20) ? 5 : -1; }
 inline int kind_of(int sid) {
+  if (sid >= 21) return sid == 21 ? K_QQB : (sid == 22 ? K_QG : K_GQB);
   if (sid >= 10) return sid <= 12 ? K_QQB : (sid <= 16 ? K_QG : K_GQB);
   return sid <= 4 ? K_TTNG : ((sid <= 6 || sid == 9) ? K_QQB : (sid == 7 ? K_QG : K_GQB)); }
 
