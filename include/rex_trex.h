@@ -60,7 +60,10 @@ enum { TREX_SP_EEMUMU = 0,   /* e- e+ > mu- mu+   (photon + Z)          */
        TREX_SP_SSX_TTG = 10, TREX_SP_CCX_TTG = 11, TREX_SP_BBX_TTG = 12,                         /* q q~ > t t~ g   */
        TREX_SP_DG_TTD = 13, TREX_SP_SG_TTS = 14, TREX_SP_CG_TTC = 15, TREX_SP_BG_TTB = 16,       /* q g > t t~ q    */
        TREX_SP_GDX_TTDX = 17, TREX_SP_GSX_TTSX = 18, TREX_SP_GCX_TTCX = 19, TREX_SP_GBX_TTBX = 20, /* g q~ > t t~ q~ */
-       TREX_NSUBPROC = 21 };
+       /* one light line + TWO gluons (the multi-jet samples are dominated by such channels) */
+       TREX_SP_UUX_TTGG = 21, TREX_SP_UG_TTUG = 22, TREX_SP_GUX_TTUXG = 23,   /* u u~ > t t~ g g, u g > t t~ u g, g u~ > t t~ u~ g */
+       TREX_SP_DDX_TTGG = 24, TREX_SP_DG_TTDG = 25, TREX_SP_GDX_TTDXG = 26,   /* the same for d */
+       TREX_NSUBPROC = 27 };
 
 /* ---- flavour keys (PAPER.md:334 default comparator: unordered PDG codes of external legs, initial and final state
  * kept apart; Alg.1).

@@ -743,10 +743,10 @@ template <class R> ABD<R> e2_abd(const Event<R>& ev, const Params<R>& P, int kin
 inline int npar_of(int sid) {
   static const int t[10] = {4, 4, 5, 6, 7, 5, 5, 5, 5, 4};
   if (sid >= 0 && sid < 10) return t[sid];
-  if (sid >= 21 && sid <= 23) return 6;             // 21 u u~ > t t~ g g ; 22 u g > t t~ u g ; 23 g u~ > t t~ u~ g
+  if (sid >= 21 && sid <= 26) return 6;             // 21 u u~ > t t~ g g ; 22 u g > t t~ u g ; 23 g u~ > t t~ u~ g ; 24..26: d
   return (sid >= 10 && sid <= 20) ? 5 : -1; }
 inline int kind_of(int sid) {
-  if (sid >= 21) return sid == 21 ? K_QQB : (sid == 22 ? K_QG : K_GQB);
+  if (sid >= 21) return (sid - 21) % 3 == 0 ? K_QQB : ((sid - 21) % 3 == 1 ? K_QG : K_GQB);
   if (sid >= 10) return sid <= 12 ? K_QQB : (sid <= 16 ? K_QG : K_GQB);
   return sid <= 4 ? K_TTNG : ((sid <= 6 || sid == 9) ? K_QQB : (sid == 7 ? K_QG : K_GQB)); }
 

@@ -11,7 +11,7 @@ LIB = os.path.join(HERE, "librex_trex.so")
 UNITS = [("trex_ttng_tu.cu", "trex_ttng_n%d_m%d" % (n, m), ["-DTREX_TU_N=%d" % n, "-DTREX_TU_MODE=%d" % m])
          for n in (5, 4, 3, 2) for m in (0, 1, 2)] + \
         [("trex_table_tu.cu", "trex_table_n%d_m%d" % (n, m), ["-DTREX_TU_N=%d" % n, "-DTREX_TU_MODE=%d" % m])
-         for n in (5, 4, 3) for m in (0, 1, 2)] + [("trex_api.cu", "trex_api", []), ("rex_bucket.cu", "rex_bucket", []),
+         for n in (5, 4, 3) for m in (0, 1, 2)] + [("trex_api.cu", "trex_api", []), ("trex_qq2_tu.cu", "trex_qq2", []), ("rex_bucket.cu", "rex_bucket", []),
                                                  ("trex_probe.cu", "trex_probe", []), ("trex_xsec.cu", "trex_xsec", [])]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-Wno-deprecated-gpu-targets"]
@@ -22,6 +22,7 @@ _KERNEL_HDRS = ["trex_math.cuh", "trex_ttng.cuh", "trex_proc.cuh", "trex_kernels
 DEPS = {
     "trex_ttng_tu.cu": _KERNEL_HDRS,
     "trex_table_tu.cu": _KERNEL_HDRS + ["trex_table.cuh", "trex_table4.cuh"],
+    "trex_qq2_tu.cu": _KERNEL_HDRS + ["trex_qq2.cuh"],
     "trex_api.cu": _KERNEL_HDRS + ["trex_ctx.h", "trex_host.h", "trex_colour.h", "../../include/rex_trex.h"],
     "rex_bucket.cu": ["trex_ctx.h", "../../include/rex_trex.h"],
     "trex_probe.cu": ["trex_ctx.h", "../../include/rex_trex.h"],

@@ -292,14 +292,17 @@ int ensure_colour() {
     }
   }
   QLineLegs ql[TREX_NSUBPROC];
-  double qi[TREX_NSUBPROC];
+  double qi[TREX_NSUBPROC], qi2[TREX_NSUBPROC];
   for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
     const SubprocInfo* sp = subproc_info(sid);
-    ql[sid] = sp ? sp->qlegs : QLineLegs{0, 0, 0};
-    qi[sid] = (sp && is_quark_channel(sid)) ? 1.0 / sp->navg : 0.0;
+    ql[sid] = sp ? sp->qlegs : QLineLegs{0, 0, 0, 0};
+    qi[sid] = (sp && is_quark_channel(sid) && !is_two_gluon_quark_channel(sid)) ? 1.0 / sp->navg : 0.0;
+    qi2[sid] = (sp && is_two_gluon_quark_channel(sid)) ? 1.0 / sp->navg : 0.0;
   }
   TREX_CUDA_CHECK(cudaMemcpyToSymbol(c_qlegs, ql, sizeof ql));
   TREX_CUDA_CHECK(cudaMemcpyToSymbol(c_qinvnavg, qi, sizeof qi));
+  if (trex_tu_qq2_setup(ql, qi2, trex_colour::qq2_colour_matrix().data()) != 0)
+    return fail(TREX_ECUDA, "upload of the two-gluon quark-channel tables failed: %s", cudaGetErrorString(cudaGetLastError()));
   c.colour_ready = true;
   return 0;
 }
@@ -330,6 +333,11 @@ extern "C" int trex_colour_matrix(int sid, double* out) {
   if (sid == TREX_SP_EEMUMU) { out[0] = 1.0; return 1; }
   if (sid >= TREX_SP_GG_TT && sid <= TREX_SP_GG_TTGGG) {
     std::vector<double> C = trex_colour::ttng_colour_matrix(sp->npar - 2);
+    std::memcpy(out, C.data(), C.size() * sizeof(double));
+    return sp->ncolor;
+  }
+  if (is_two_gluon_quark_channel(sid)) {
+    std::vector<double> C = trex_colour::qq2_colour_matrix();
     std::memcpy(out, C.data(), C.size() * sizeof(double));
     return sp->ncolor;
   }
@@ -379,6 +387,10 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
     } else if (kLaunch[N - 2][mode](a, npass, grid32, c.stream) != 0) {
       return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
+  } else if (is_two_gluon_quark_channel(sid)) {
+    const unsigned gq = a.qfamily ? grid32 + (unsigned)TREX_NSUBPROC : grid32;
+    if (trex_tu_qq2_launch(a, mode, gq, c.stream) != 0)
+      return fail(TREX_ECUDA, "kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
   } else {
     // a family launch (trex_run) serves every quark-channel class: each class rounds its events up to whole blocks
     const unsigned gq = a.qfamily ? grid32 + (unsigned)TREX_NSUBPROC : grid32;

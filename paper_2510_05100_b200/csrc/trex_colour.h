@@ -101,4 +101,27 @@ inline std::vector<double> ttng_colour_matrix(int n) {
   return C;
 }
 
+// One light line + t t~ + two gluons (trex_qq2.cuh): twelve flows. With (S1, S2) one of
+//   0 (ab, -), 1 (ba, -), 2 (a, b), 3 (b, a), 4 (-, ab), 5 (-, ba)
+// type I (flows 0..5) is (S1)_{t k} (S2)_{r tb}, type II (flows 6..11) is (S1)_{t tb} (S2)_{r k}. T^a is hermitian, so the
+// conjugate of a string is the reversed string with its indices swapped, and the sums over all colours are
+//   I  x I'  : tr(S1 rev S1') tr(S2 rev S2')        II x II' : the same
+//   I  x II' : tr(S1 rev S2' S2 rev S1')
+inline std::vector<double> qq2_colour_matrix() {
+  const Word s1[6] = {{0, 1}, {1, 0}, {0}, {1}, {}, {}}, s2[6] = {{}, {}, {1}, {0}, {0, 1}, {1, 0}};
+  auto rev = [](Word w) { std::reverse(w.begin(), w.end()); return w; };
+  auto cat = [](std::initializer_list<Word> ws) { Word o; for (const Word& w : ws) o.insert(o.end(), w.begin(), w.end()); return o; };
+  std::vector<double> C(144);
+  for (int i = 0; i < 12; ++i)
+    for (int j = 0; j < 12; ++j) {
+      const int p = i % 6, q = j % 6;
+      Frac v;
+      if ((i < 6) == (j < 6)) v = reduce({cat({s1[p], rev(s1[q])}), cat({s2[p], rev(s2[q])})});
+      else if (i < 6) v = reduce({cat({s1[p], rev(s2[q]), s2[p], rev(s1[q])})});
+      else v = reduce({cat({s1[q], rev(s2[p]), s2[q], rev(s1[p])})});
+      C[i * 12 + j] = v.value();
+    }
+  return C;
+}
+
 }  // namespace trex_colour

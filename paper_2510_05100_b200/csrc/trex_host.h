@@ -16,7 +16,7 @@ struct SubprocInfo {
   int nvert;       // power of g_s in the amplitude
   double navg;     // spin x colour average x identical-particle factor (R-7)
   int pdg[7];      // process-string order
-  QLineLegs qlegs; // light-quark line (quark channels only)
+  QLineLegs qlegs; // light-quark line (quark channels only): row end, column end, gluon, second gluon
 };
 
 inline const SubprocInfo* subproc_info(int sid) {
@@ -41,12 +41,27 @@ inline const SubprocInfo* subproc_info(int sid) {
     for (int f : {3, 4, 5}) { tab[sid] = base[5]; tab[sid].pdg[0] = f; tab[sid].pdg[1] = -f; ++sid; }
     for (int f : {1, 3, 4, 5}) { tab[sid] = base[7]; tab[sid].pdg[0] = f; tab[sid].pdg[4] = f; ++sid; }
     for (int f : {1, 3, 4, 5}) { tab[sid] = base[8]; tab[sid].pdg[1] = -f; tab[sid].pdg[4] = -f; ++sid; }
+    // one light line + two gluons (trex_qq2.cuh): twelve colour flows, 64 helicity combinations of which 32 survive the
+    // chirality of the massless line; identical final gluons of q q~ > t t~ g g: 1/2!
+    const SubprocInfo two[3] = {
+        /* u u~ > t t~ g g  */ {6, 12, 64, 16, 4, 4.0 * 9.0 * 2.0, {2, -2, 6, -6, 21, 21}, {1, 0, 4, 5}},
+        /* u g > t t~ u g   */ {6, 12, 64, 16, 4, 4.0 * 24.0, {2, 21, 6, -6, 2, 21}, {4, 0, 1, 5}},
+        /* g u~ > t t~ u~ g */ {6, 12, 64, 16, 4, 4.0 * 24.0, {21, -2, 6, -6, -2, 21}, {1, 4, 0, 5}},
+    };
+    sid = TREX_SP_UUX_TTGG;
+    for (int f : {2, 1})
+      for (int k = 0; k < 3; ++k) {
+        tab[sid] = two[k];
+        for (int i = 0; i < 6; ++i) if (tab[sid].pdg[i] == 2 || tab[sid].pdg[i] == -2) tab[sid].pdg[i] = tab[sid].pdg[i] > 0 ? f : -f;
+        ++sid;
+      }
     ready = true;
   }
   return (sid >= 0 && sid < TREX_NSUBPROC && tab[sid].npar > 0) ? &tab[sid] : nullptr;
 }
 inline int npar_of_sid(int sid) { const SubprocInfo* sp = subproc_info(sid); return sp ? sp->npar : 0; }
 inline bool is_quark_channel(int sid) { return (sid >= TREX_SP_UUX_TTG && sid <= TREX_SP_GUX_TTUX) || (sid >= TREX_SP_SSX_TTG && sid < TREX_NSUBPROC); }
+inline bool is_two_gluon_quark_channel(int sid) { return sid >= TREX_SP_UUX_TTGG && sid <= TREX_SP_GDX_TTDXG; }
 
 // returns false if theta is unusable (negative couplings, non-positive scale)
 inline bool make_theta_pair(int sid, const double* th_old, const double* th_new, ThetaPair& T) {

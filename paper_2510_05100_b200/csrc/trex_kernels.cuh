@@ -104,6 +104,10 @@ TREX_TU_DECL(4, 0) TREX_TU_DECL(4, 1) TREX_TU_DECL(4, 2)
 TREX_TU_DECL(5, 0) TREX_TU_DECL(5, 1) TREX_TU_DECL(5, 2)
 #undef TREX_TU_DECL
 
+// one light line + two gluons (trex_qq2_tu.cu): tables (legs, 1 / N_avg per id, 12 x 12 colour matrix) and launch
+int trex_tu_qq2_setup(const QLineLegs* legs, const double* invnavg, const double* C144);
+int trex_tu_qq2_launch(const ReweightArgs& a, int mode, unsigned grid, cudaStream_t stream);
+
 // fused current-table kernels (trex_table_tu.cu), one translation unit per (N = 3, 4, 5; precision mode)
 using TableLaunchFn = int (*)(const ReweightArgs&, int npass, long nmax, const int* meta, const double* Cfold, int nsm, cudaStream_t);
 using TableMetaFn = int (*)(int* meta);                       // fills the meta block (if non-null), returns its size in ints

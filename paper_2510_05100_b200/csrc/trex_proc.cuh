@@ -165,7 +165,7 @@ TREX_HD void ttng_unit(const double* __restrict__ mom, long n, long e, int gh, i
 //   J1 = (A(g,Q) + K4)/2, J2 = (A(Q,g) + K3)/2, J3 = -(A(g,Q) + A(Q,g))/6, J4 = -(K3 + K4)/6
 // where A(.,.) are the two orderings of (gluon, quark-pair current) on the top line and K3 / K4 attach the current
 // of the light line that has radiated the gluon at its row / column end. C = [[12,0,4,4],[0,12,4,4],[4,4,12,0],[4,4,0,12]].
-struct QLineLegs { int lrow, lcol, lg; };   // leg numbers; legs 0,1 are incoming
+struct QLineLegs { int lrow, lcol, lg, lg2; };   // leg numbers (lg2: second gluon of the two-gluon channels, trex_qq2.cuh); legs 0,1 are incoming
 
 
 // Top line with TWO ordered sources (currents e1, e2 with momenta K1, K2 flowing into the line): the two orderings

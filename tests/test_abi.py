@@ -99,6 +99,44 @@ def test_colour_matrices_against_group_theory(lib):
     assert np.array_equal(cq, [[12, 0, 4, 4], [0, 12, 4, 4], [4, 4, 12, 0], [4, 4, 0, 12]])
 
 
+def test_colour_matrix_of_the_two_gluon_channels(lib):
+    """The 12 x 12 matrix the kernel sums with, against explicit Gell-Mann matrices (flows as in trex_qq2.cuh)."""
+    C = T.trex_colour_matrix(21)
+    assert C.shape == (12, 12) and np.array_equal(C, C.T)
+    lam = np.zeros((8, 3, 3), dtype=complex)
+    lam[0][0, 1] = lam[0][1, 0] = 1
+    lam[1][0, 1], lam[1][1, 0] = -1j, 1j
+    lam[2][0, 0], lam[2][1, 1] = 1, -1
+    lam[3][0, 2] = lam[3][2, 0] = 1
+    lam[4][0, 2], lam[4][2, 0] = -1j, 1j
+    lam[5][1, 2] = lam[5][2, 1] = 1
+    lam[6][1, 2], lam[6][2, 1] = -1j, 1j
+    lam[7] = np.diag([1, 1, -2]) / math.sqrt(3)
+    Tm = lam / 2
+    one = np.eye(3)
+    flows = []
+    for typ in (1, 2):
+        for s1, s2 in (("ab", ""), ("ba", ""), ("a", "b"), ("b", "a"), ("", "ab"), ("", "ba")):
+            f = np.zeros((8, 8, 3, 3, 3, 3), dtype=complex)          # [a, b, t, tb, r, k]
+            for a in range(8):
+                for b in range(8):
+                    def string(s):
+                        m = one
+                        for ch in s:
+                            m = m @ Tm[a if ch == "a" else b]
+                        return m
+                    m1, m2 = string(s1), string(s2)
+                    if typ == 1:
+                        f[a, b] = np.einsum("tk,rq->tqrk", m1, m2)    # (S1)_{t k} (S2)_{r tb}
+                    else:
+                        f[a, b] = np.einsum("tq,rk->tqrk", m1, m2)    # (S1)_{t tb} (S2)_{r k}
+            flows.append(f.reshape(-1))
+    F = np.array(flows)
+    want = (F.conj() @ F.T).real
+    assert np.allclose(C, want, rtol=0, atol=1e-12)
+    assert T.trex_ncolor(22) == 12 and T.trex_nhel(23) == 64 and T.trex_npar(26) == 6
+
+
 def test_compute_calls_fail_loudly_without_gpu(lib):
     import torch
     if torch.cuda.is_available():

@@ -1,0 +1,163 @@
+"""Parity of the one-light-line + two-gluon kernels (k_qq2; ids 21..26) with the oracle (-m gpu).
+
+The oracle's explicit-colour evaluator needs about half a minute per event and thread for these channels, so the direct
+comparisons use a handful of events: (A, B, D) of |M|^2 = A + kappa B + kappa^2 D from ONE oracle evaluation per event are
+compared with the CUDA path at three values of c_tG; a further case has different top masses and widths at theta_old and
+theta_new (the kernel then walks the top line once per parameter point). Everything else (the family launch inside
+trex_run, flavours, reduced precision) is checked against those oracle-checked fp64 results at larger sizes."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from trex_inputs import SUBPROCESSES, default_theta, make_config, TH_CTG, TH_GAMMAT, TH_MT
+
+pytestmark = pytest.mark.gpu
+
+RTOL64 = 1e-11
+
+
+@pytest.fixture(scope="module")
+def T():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2510_05100_b200 as T
+    T.lib()
+    T.trex_set_stream(None)
+    T.trex_set_precision(0)
+    return T
+
+
+def dev(a):
+    import torch
+    a = np.ascontiguousarray(a)
+    if a.dtype == np.uint64:
+        a = a.view(np.int64)
+    return torch.from_numpy(a).cuda()
+
+
+def rel(a, b):
+    return np.abs(a - b) / np.abs(b)
+
+
+def _events(n, first=0):
+    w = make_config(7, n=64)
+    return np.ascontiguousarray(w.momenta[:, :, first:first + n])
+
+
+@pytest.mark.parametrize("sid", [21, 22, 23, 25])
+def test_abd_against_oracle(T, sid):
+    mom = _events(4, first=sid - 21)
+    th0 = default_theta()
+    abd = O.abd(sid, mom, th0, engine=2)                   # [n, 3]
+    dm, dw = dev(mom), dev(np.ones(mom.shape[2]))
+    for c in (1.7, -2.3):
+        th1 = th0.copy()
+        th1[TH_CTG] = c
+        k = O.kappa(th1)
+        want_new = abd[:, 0] + k * abd[:, 1] + k * k * abd[:, 2]
+        w_out, mo, mn = (x.cpu().numpy() for x in T.trex_reweight(sid, dm, th0, th1, dw))
+        assert rel(mo, abd[:, 0]).max() < RTOL64, rel(mo, abd[:, 0])
+        assert rel(mn, want_new).max() < RTOL64, rel(mn, want_new)
+        assert rel(w_out, want_new / abd[:, 0]).max() < RTOL64
+    # the three coefficients separately: B and D from three parameter points
+    th_p, th_m = th0.copy(), th0.copy()
+    th_p[TH_CTG], th_m[TH_CTG] = 1.0, -1.0
+    k = O.kappa(th_p)
+    mp = T.trex_reweight(sid, dm, th0, th_p, dw)[2].cpu().numpy()
+    mm = T.trex_reweight(sid, dm, th0, th_m, dw)[2].cpu().numpy()
+    B = (mp - mm) / (2 * k)
+    D = ((mp + mm) / 2 - abd[:, 0]) / (k * k)
+    assert rel(B, abd[:, 1]).max() < 1e-9 and rel(D, abd[:, 2]).max() < 1e-7      # D k^2 is 1e-4 of A here: cancellation
+
+
+def test_top_mass_and_width_differ_between_the_parameter_points(T):
+    mom = _events(2, first=9)
+    th0, th1 = default_theta(), default_theta()
+    th0[TH_GAMMAT], th1[TH_GAMMAT] = 1.5, 1.3
+    th1[TH_MT] = 171.0
+    th1[TH_CTG] = 0.9
+    # on-shell momenta belong to m_t = 173: the new point evaluates the same momenta with another mass parameter in the
+    # propagators and spinors, exactly as the oracle does
+    w_in = np.array([0.7, 1.9])
+    want = O.reweight(22, mom, th0, th1, w_in)
+    got = [x.cpu().numpy() for x in T.trex_reweight(22, dev(mom), th0, th1, dev(w_in))]
+    for g, r in zip(got, want):
+        assert rel(g, r).max() < RTOL64, (g, r)
+
+
+def test_flavour_of_the_light_line_is_a_label(T):
+    mom = _events(64)
+    th0, th1 = default_theta(), default_theta()
+    th1[TH_CTG] = 1.1
+    dm, dw = dev(mom), dev(np.ones(64))
+    for u, d in ((21, 24), (22, 25), (23, 26)):
+        a = T.trex_reweight(u, dm, th0, th1, dw)
+        b = T.trex_reweight(d, dm, th0, th1, dw)
+        for x, y in zip(a, b):
+            assert np.array_equal(x.cpu().numpy(), y.cpu().numpy())
+    # the oracle agrees that it is a label (single helicity: the full sum takes minutes)
+    m1 = np.ascontiguousarray(mom[:, :, :1])
+    for u, d in ((21, 24), (22, 25), (23, 26)):
+        assert np.array_equal(O.abd(u, m1, th1, engine=2, hel_only=0b010110 if u == 21 else 0b010111 if u == 23 else 0b010011),
+                              O.abd(d, m1, th1, engine=2, hel_only=0b010110 if u == 21 else 0b010111 if u == 23 else 0b010011))
+
+
+@pytest.mark.parametrize("n", [7, 1000, 30011])
+def test_cfg7_whole_path_equals_per_class_calls(T, n):
+    """trex_run on the seven-class 2 -> t t~ + 2 partons sample: categorisation (bit-exact against the oracle's bucketing),
+    one launch of the g g kernel + ONE family launch for the six quark classes, results equal to per-class trex_reweight
+    calls on the gathered events (which test_abd_against_oracle pins to the oracle)."""
+    import torch
+    w = make_config(7, n=n)
+    dk, dm, dw = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    l0 = T.trex_launch_count()
+    w_out, mo, mn, nb = T.trex_run(dk, dm, w.theta_old, w.theta_new, dw)
+    torch.cuda.synchronize()
+    launches = T.trex_launch_count() - l0
+    present = [sp for sp in w.classes if np.any(w.keys == sp.key)]
+    assert nb == len(present)
+    assert launches <= 12, launches                        # bucketing passes + gather + TWO |M|^2 launches + scatter
+    w_out, mo, mn = w_out.cpu().numpy(), mo.cpu().numpy(), mn.cpu().numpy()
+    assert np.all(np.isfinite(w_out)) and np.all(mo > 0)
+    perm, off, _ = O.bucket(w.keys)
+    gperm, goff, _ = T.rex_bucket(dk)
+    assert np.array_equal(gperm.cpu().numpy(), perm) and np.array_equal(goff, off)
+    for sp in present:
+        sel = np.where(w.keys == sp.key)[0]
+        r = T.trex_reweight(sp.sid, dev(np.ascontiguousarray(w.momenta[:, :, sel])), w.theta_old, w.theta_new, dev(w.w_in[sel]))
+        assert np.array_equal(w_out[sel], r[0].cpu().numpy()), sp.name
+        assert np.array_equal(mo[sel], r[1].cpu().numpy()) and np.array_equal(mn[sel], r[2].cpu().numpy()), sp.name
+
+
+def test_cfg7_sampled_events_against_oracle(T):
+    """Two events of the mixed sample straight against the oracle, through the whole path (one q g and one g q~ event)."""
+    import torch
+    w = make_config(7, n=4096)
+    dk, dm, dw = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    w_out = T.trex_run(dk, dm, w.theta_old, w.theta_new, dw)[0].cpu().numpy()
+    for sid in (25, 23):
+        sp = [s for s in SUBPROCESSES if s.sid == sid][0]
+        i = np.where(w.keys == sp.key)[0][-1:]
+        want = O.reweight(sid, np.ascontiguousarray(w.momenta[:, :, i]), w.theta_old, w.theta_new, w.w_in[i])[0]
+        assert rel(w_out[i], want).max() < RTOL64, (sid, w_out[i], want)
+
+
+def test_reduced_precision_modes(T):
+    """mixed (fp64 amplitudes, fp32 colour sum) and fp32 against the oracle-checked fp64 kernel on 4096 events per class:
+    median 5e-5, maximum 1e-3 of the weight ratio (the bars of the other channels)."""
+    w = make_config(7, n=8192)
+    th0, th1 = w.theta_old, w.theta_new
+    for sid in (21, 22, 23):
+        dm, dw = dev(w.momenta), dev(w.w_in)
+        T.trex_set_precision(0)
+        ref = T.trex_reweight(sid, dm, th0, th1, dw)[0].cpu().numpy()
+        try:
+            for mode, med, mx in ((1, 1e-6, 1e-4), (2, 5e-5, 1e-3)):
+                T.trex_set_precision(mode)
+                got = T.trex_reweight(sid, dm, th0, th1, dw)[0].cpu().numpy()
+                r = rel(got, ref)
+                assert np.median(r) < med and r.max() < mx, (sid, mode, np.median(r), r.max())
+        finally:
+            T.trex_set_precision(0)

@@ -134,7 +134,7 @@ def test_flavour_of_the_light_line_does_not_change_the_matrix_element():
     want = {"qq": O.me2(5, mom, th), "qg": O.me2(7, mom, th), "gqb": O.me2(8, mom, th)}
     seen = 0
     for sp in SUBPROCESSES:
-        if sp.sid < 10:
+        if not 10 <= sp.sid <= 20:
             continue
         kind = "qq" if 21 not in sp.pdg[:2] else ("qg" if sp.pdg[1] == 21 else "gqb")
         assert np.array_equal(O.me2(sp.sid, mom, th), want[kind]), sp.name

@@ -94,7 +94,20 @@ def _light_line_channels():
     return tuple(out)
 
 
-SUBPROCESSES = SUBPROCESSES + _light_line_channels()
+def _two_gluon_channels():
+    """One light line + two gluons (ids 21..26): u u~ > t t~ g g, u g > t t~ u g, g u~ > t t~ u~ g and the
+    same three for d."""
+    name = {1: "d", 2: "u"}
+    out, sid = [], 21
+    for f in (2, 1):
+        q = name[f]
+        out.append(Subprocess(sid, "%s %s~ > t t~ g g" % (q, q), (f, -f, 6, -6, 21, 21), (-1, -1, 1, 1, 1, 1), (2, 3))); sid += 1
+        out.append(Subprocess(sid, "%s g > t t~ %s g" % (q, q), (f, 21, 6, -6, f, 21), (-1, -1, 1, 1, 1, 1), (2, 3))); sid += 1
+        out.append(Subprocess(sid, "g %s~ > t t~ %s~ g" % (q, q), (21, -f, 6, -6, -f, 21), (-1, -1, 1, 1, 1, 1), (2, 3))); sid += 1
+    return tuple(out)
+
+
+SUBPROCESSES = SUBPROCESSES + _light_line_channels() + _two_gluon_channels()
 
 
 def subprocess_by_name(name):
@@ -248,6 +261,24 @@ def make_config(cfg, n=None):
         th_new[TH_CTG] = 1.0
         present = tuple(sp for sp, c in zip(classes, counts) if c > 0)
         return Workload(6, "cfg6 multi-channel pp -> tt~ + 1 parton, 16 classes", n, 5, keys, mom, w, th_old, th_new, present)
+    if cfg == 7:
+        # multi-channel p p -> t t~ + 2 partons sample: g g > t t~ g g 50 %, q g 24 % (u : d = 2 : 1), g q~ 8 %, q q~ 18 %
+        # (the multi-jet samples of PAPER.md:1279-1284 mix the gluonic channel with quark-line channels). Same phase space as
+        # cfg 4 (sqrt(s) = 1500, RAMBO), theta as cfg 3.
+        n = 262144 if n is None else n
+        rng = np.random.default_rng(7)
+        classes = tuple(sp for sp in SUBPROCESSES if sp.npar == 6)
+        fr = {3: 0.50, 21: 0.12, 22: 0.16, 23: 0.05, 24: 0.06, 25: 0.08, 26: 0.03}
+        counts = largest_remainder([fr[sp.sid] for sp in classes], n)
+        labels = np.concatenate([np.full(int(c), i, dtype=np.int64) for i, c in enumerate(counts)])
+        labels = rng.permutation(labels)
+        class_keys = np.array([sp.key for sp in classes], dtype=np.uint64)
+        keys = class_keys[labels]
+        mom = _two_to_n(rng, n, 1500.0, [mt, mt, 0.0, 0.0], False)
+        w = rng.lognormal(0.0, 0.5, n)
+        th_new[TH_CTG] = 1.0
+        present = tuple(sp for sp, c in zip(classes, counts) if c > 0)
+        return Workload(7, "cfg7 multi-channel pp -> tt~ + 2 partons, 7 classes", n, 6, keys, mom, w, th_old, th_new, present)
     raise ValueError(f"unknown config {cfg}")
 
 
