@@ -17,6 +17,11 @@
 //     S_L = {x}    : Q(x|) and Q(|x), two orderings of (y, Q) each                    (two_source_line)
 //     S_L = {a, b} : Q(ab|) Q(ba|) Q(a|b) Q(b|a) Q(|ab) Q(|ba), single source        (one bracket each)
 // The 12 x 12 colour matrix comes from trex_colour.h (traces of the strings, exact rationals).
+//
+// Live state. The 12 x 2 x 2 complex flow amplitudes of a thread (96 numbers) are accumulated in SHARED memory (element i
+// of thread t at s[i * stride + t]: conflict-free), and the eleven light-line currents are formed right where they are used
+// instead of being kept (they cost a few hundred operations each, the top-line walks tens of thousands): what stays in
+// registers is the external wavefunctions and the walk itself.
 #pragma once
 #include "trex_proc.cuh"
 
@@ -24,30 +29,32 @@ namespace trex {
 
 constexpr int QQ2_NFLOW = 12;
 
-// amplitudes of one (light-line, gluon, top) helicity choice, both antitop helicities: F[flow][order in kappa][v]
-template <class R> struct Qq2Flows {
-  cx<R> F[QQ2_NFLOW][2][2];
-  TREX_HD void clear() {
-#pragma unroll
-    for (int f = 0; f < QQ2_NFLOW; ++f)
-#pragma unroll
-      for (int o = 0; o < 2; ++o) { F[f][o][0] = cx<R>(0, 0); F[f][o][1] = cx<R>(0, 0); }
+// flow amplitudes of one (light-line, gluon, top) helicity choice, both antitop helicities: element
+// ((flow * 2 + order in kappa) * 2 + v) * 2 + (re, im) of this thread at s[element * stride]
+template <class R> struct Qq2Acc {
+  R* s; int stride;
+  static constexpr int NEL = QQ2_NFLOW * 8;
+  TREX_HD R& at(int f, int o, int iv, int ri) const { return s[(((f * 2 + o) * 2 + iv) * 2 + ri) * stride]; }
+  TREX_HD void clear() const {
+#pragma unroll 8
+    for (int i = 0; i < NEL; ++i) s[i * stride] = R(0);
   }
   // one term: +1/2 to its type-I flow, -1/6 to its type-II flow
-  TREX_HD void add(int f1, int f2, const cx<R> A[2][2]) {
+  TREX_HD void add(int f1, int f2, const cx<R> A[2][2]) const {
 #pragma unroll
     for (int o = 0; o < 2; ++o)
 #pragma unroll
       for (int iv = 0; iv < 2; ++iv) {
-        cfma(F[f1][o][iv], A[o][iv], R(0.5));
-        cfma(F[6 + f2][o][iv], A[o][iv], R(-1.0 / 6.0));
+        at(f1, o, iv, 0) += R(0.5) * A[o][iv].re; at(f1, o, iv, 1) += R(0.5) * A[o][iv].im;
+        at(6 + f2, o, iv, 0) += R(-1.0 / 6.0) * A[o][iv].re; at(6 + f2, o, iv, 1) += R(-1.0 / 6.0) * A[o][iv].im;
       }
   }
+  TREX_HD cx<R> get(int f, int o, int iv) const { return cx<R>(at(f, o, iv, 0), at(f, o, iv, 1)); }
 };
 
 // sink of the three-source walk (sources 0 = a, 1 = b, 2 = Q; leaves in lexicographic order)
 template <class R> struct Qq2Sink3 {
-  Qq2Flows<R>* fl;
+  Qq2Acc<R> fl;
   const spinor<R>* v;
   template <int LEAF> TREX_HD void put(const spinor<R>* b0, const spinor<R>* b1) {
     // leaf: 0 (a,b,Q) 1 (a,Q,b) 2 (b,a,Q) 3 (b,Q,a) 4 (Q,a,b) 5 (Q,b,a)
@@ -56,186 +63,190 @@ template <class R> struct Qq2Sink3 {
     cx<R> A[2][2];
 #pragma unroll
     for (int iv = 0; iv < 2; ++iv) { A[0][iv] = row_col(b0[0], v[iv]); A[1][iv] = row_col(b1[0], v[iv]); }
-    fl->add(f1, f2, A);
+    fl.add(f1, f2, A);
   }
 };
 
-// the eleven currents of the light line for one choice of its helicity combination and of the gluon helicities
-template <class R> struct Qq2Currents {
-  vec4<R> Q0;            // no gluon absorbed
-  vec4<R> Qr[2], Qc[2];  // gluon x (0 = a, 1 = b) absorbed at the row / column end
-  vec4<R> Q2[6];         // both: (ab|) (ba|) (a|b) (b|a) (|ab) (|ba)
-};
+template <class R> TREX_HD vec4<R> qq2_scaled(const vec4<R>& j, double s) {
+  vec4<R> o; const R sr = R(s);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) o.c[i] = j.c[i] * sr;
+  return o;
+}
 
+// light line after ONE gluon (e, K) at its row end / column end:
+//   R_x = w (i eslash)(i qslash)/q^2 = -w eslash qslash / q^2, q = -(Kr + K);   C_x = -qslash eslash x / q^2, q = Kc + K
 template <class R>
-TREX_HD void qq2_light_line(const spinor<R>& w, const spinor<R>& x, const rvec4<double>& Kr, const rvec4<double>& Kc, const vec4<R> e[2],
-                            const rvec4<double> K[2], Qq2Currents<R>& out) {
-  const rvec4<double> Kq = radd(Kr, Kc);
-  auto scaled = [](const vec4<R>& j, double s) { vec4<R> o; const R sr = R(s);
+TREX_HD spinor<R> qq2_row1(const spinor<R>& w, const rvec4<double>& Kr, const vec4<R>& e, const rvec4<double>& K) {
+  rvec4<double> q;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) o.c[i] = j.c[i] * sr; return o; };
-  out.Q0 = scaled(bilinear(w, x), 1.0 / rdot(Kq, Kq));
-  // one gluon: R_x = w (i eslash)(i qslash)/q^2 = -w eslash qslash / q^2, q = -(Kr + Kx);  C_x = -qslash eslash x / q^2, q = Kc + Kx
-  spinor<R> Rx[2], Cx[2];
+  for (int mu = 0; mu < 4; ++mu) q.c[mu] = -(Kr.c[mu] + K.c[mu]);
+  const R s = R(-1.0 / rdot(q, q));
+  spinor<R> o = row_slash(row_slash(w, e), cast<R>(q));
 #pragma unroll
-  for (int g = 0; g < 2; ++g) {
-    rvec4<double> qr, qc;
+  for (int i = 0; i < 4; ++i) o.c[i] = o.c[i] * s;
+  return o;
+}
+template <class R>
+TREX_HD spinor<R> qq2_col1(const spinor<R>& x, const rvec4<double>& Kc, const vec4<R>& e, const rvec4<double>& K) {
+  const rvec4<double> q = radd(Kc, K);
+  const R s = R(-1.0 / rdot(q, q));
+  spinor<R> o = slash_col(cast<R>(q), slash_col(e, x));
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) { qr.c[mu] = -(Kr.c[mu] + K[g].c[mu]); qc.c[mu] = Kc.c[mu] + K[g].c[mu]; }
-    const R sr = R(-1.0 / rdot(qr, qr)), sc = R(-1.0 / rdot(qc, qc));
-    Rx[g] = row_slash(row_slash(w, e[g]), cast<R>(qr));
-    Cx[g] = slash_col(cast<R>(qc), slash_col(e[g], x));
+  for (int i = 0; i < 4; ++i) o.c[i] = o.c[i] * s;
+  return o;
+}
+
+// external wavefunctions and momenta of one (light-line combination, gluon helicities) choice
+template <class R> struct Qq2Ext {
+  spinor<R> w, x;                 // row / column spinor of the light line
+  vec4<R> e[2];                   // gluon polarisations
+  rvec4<double> Kr, Kc, K[2], pt; // incoming-convention momenta of the light-line ends and the gluons; top momentum
+};
+
+// single-source top-line amplitude of the current Q (momentum P into the line): A[order][v]
+template <class R>
+TREX_HD void qq2_single(const spinor<R>& ubar_t, const spinor<R> vtb[2], const vec4<R>& Q, const rvec4<R>& P, cx<R> A[2][2]) {
+  const spinor<R> c0 = row_slash(ubar_t, Q);
+  spinor<R> c1 = szero<R>();
+  ften<R> F = fzero<R>();
+  wedge_acc(F, P, Q);
+  row_sigma_acc(c1, ubar_t, F);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) { Rx[g].c[i] = Rx[g].c[i] * sr; Cx[g].c[i] = Cx[g].c[i] * sc; }
-    const rvec4<double> P = radd(Kq, K[g]);
-    const double iP2 = 1.0 / rdot(P, P);
-    out.Qr[g] = scaled(bilinear(Rx[g], x), iP2);
-    out.Qc[g] = scaled(bilinear(w, Cx[g]), iP2);
-  }
-  // both gluons: merged current of the tuple (a, b); the tuple (b, a) has the opposite sign
-  const rvec4<double> Kab = radd(K[0], K[1]);
-  vec4<R> Jab;
-  {
-    vec4<R> acc = vzero<R>();
-    v3_acc(acc, K[0], e[0], K[1], e[1]);
-    Jab = scaled(acc, -1.0 / rdot(Kab, Kab));
-  }
-  rvec4<double> qr, qc;
-#pragma unroll
-  for (int mu = 0; mu < 4; ++mu) { qr.c[mu] = -(Kr.c[mu] + Kab.c[mu]); qc.c[mu] = Kc.c[mu] + Kab.c[mu]; }
-  const R sr = R(-1.0 / rdot(qr, qr)), sc = R(-1.0 / rdot(qc, qc));
-  const rvec4<double> P = radd(Kq, Kab);
-  const double iP2 = 1.0 / rdot(P, P);
-  const spinor<R> wJ = row_slash(w, Jab), Jx = slash_col(Jab, x);
-#pragma unroll
-  for (int ord = 0; ord < 2; ++ord) {                       // ord 0: (a, b); 1: (b, a)
-    const int g1 = ord, g2 = 1 - ord;
-    const R sg = ord ? R(-1) : R(1);
-    // R_2 = -[ R_g1 eslash_g2 + w Jslash ] qslash / q^2
-    spinor<R> t = row_slash(Rx[g1], e[g2]);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) cfma(t.c[i], wJ.c[i], sg);
-    spinor<R> R2 = row_slash(t, cast<R>(qr));
-#pragma unroll
-    for (int i = 0; i < 4; ++i) R2.c[i] = R2.c[i] * sr;
-    out.Q2[ord] = scaled(bilinear(R2, x), iP2);
-    // (g1 | g2)
-    out.Q2[2 + ord] = scaled(bilinear(Rx[g1], Cx[g2]), iP2);
-    // C_2 (string g1 g2, g2 next to the column end) = -qslash [ eslash_g1 C_g2 + Jslash x ] / q^2
-    spinor<R> u = slash_col(e[g1], Cx[g2]);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) cfma(u.c[i], Jx.c[i], sg);
-    spinor<R> C2 = slash_col(cast<R>(qc), u);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) C2.c[i] = C2.c[i] * sc;
-    out.Q2[4 + ord] = scaled(bilinear(w, C2), iP2);
-  }
+  for (int iv = 0; iv < 2; ++iv) { A[0][iv] = mul_i(row_col(c0, vtb[iv])); A[1][iv] = row_col(c1, vtb[iv]); }
 }
 
 // all twelve flows for one top helicity and one parameter point's top line
 template <class R>
-TREX_HD void qq2_flows(const Qq2Currents<R>& Q, const vec4<R> e[2], const rvec4<double> K[2], const rvec4<double>& Kq, const spinor<R>& ubar_t,
-                       const spinor<R> vtb[2], const rvec4<double>& pt, double mt, double mGt, Qq2Flows<R>& fl) {
+TREX_HD void qq2_flows(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor<R> vtb[2], double mt, double mGt, const Qq2Acc<R>& fl) {
   fl.clear();
-  // S_L = {}: three sources
+  const rvec4<double> Kq = radd(X.Kr, X.Kc);
+  // S_L = {}: three sources (a, b, Q0), Q0 = (w gamma x) / Kq^2
   {
-    Qq2Sink3<R> sink{&fl, vtb};
+    Qq2Sink3<R> sink{fl, vtb};
     TTNGS<R, 3, 1, Qq2Sink3<R>> t;
-    t.K[0] = K[0]; t.K[1] = K[1]; t.K[2] = Kq;
-    t.eps[0] = e[0]; t.eps[1] = e[1]; t.eps[2] = Q.Q0;
-    t.pt = pt; t.ubar_t = ubar_t;
+    t.K[0] = X.K[0]; t.K[1] = X.K[1]; t.K[2] = Kq;
+    t.eps[0] = X.e[0]; t.eps[1] = X.e[1]; t.eps[2] = qq2_scaled(bilinear(X.w, X.x), 1.0 / rdot(Kq, Kq));
+    t.pt = X.pt; t.ubar_t = ubar_t;
     t.line[0].mt = mt; t.line[0].mGt = mGt;
     t.run(&sink);
   }
   // S_L = {x}: the other gluon y and Q(x|) / Q(|x)
-#pragma unroll
-  for (int xg = 0; xg < 2; ++xg) {
-    const int yg = 1 - xg;
-    const rvec4<double> Kqx = radd(Kq, K[xg]);
+#pragma unroll 1
+  for (int k = 0; k < 4; ++k) {
+    const int xg = k >> 1, yg = 1 - xg, col_end = k & 1;
+    const rvec4<double> Kqx = radd(Kq, X.K[xg]);
+    const double iP2 = 1.0 / rdot(Kqx, Kqx);
+    const vec4<R> ex = xg ? X.e[1] : X.e[0], ey = yg ? X.e[1] : X.e[0];
+    const rvec4<double> Kx = xg ? X.K[1] : X.K[0], Ky = yg ? X.K[1] : X.K[0];
+    const vec4<R> Q = col_end ? qq2_scaled(bilinear(X.w, qq2_col1(X.x, X.Kc, ex, Kx)), iP2)
+                              : qq2_scaled(bilinear(qq2_row1(X.w, X.Kr, ex, Kx), X.x), iP2);
     cx<R> A12[2][2], A21[2][2];                            // (y, Q'), (Q', y)
-    // pair numbers: (y; x) = 3 - ... : (a; b) = 2, (b; a) = 3
-    const int p_yx = yg == 0 ? 2 : 3, p_xy = xg == 0 ? 2 : 3;
-    const int p_0_xy = xg == 0 ? 4 : 5;                    // (-; x y)
-    const int p_yx_0 = yg == 0 ? 0 : 1;                    // (y x; -)
-    two_source_line<R>(ubar_t, pt, e[yg], K[yg], Q.Qr[xg], Kqx, mt, mGt, vtb, A12, A21);
-    fl.add(p_yx, p_yx, A12);
-    fl.add(p_0_xy, p_yx, A21);
-    two_source_line<R>(ubar_t, pt, e[yg], K[yg], Q.Qc[xg], Kqx, mt, mGt, vtb, A12, A21);
-    fl.add(p_yx_0, p_yx, A12);
-    fl.add(p_xy, p_yx, A21);
+    two_source_line<R>(ubar_t, X.pt, ey, Ky, Q, Kqx, mt, mGt, vtb, A12, A21);
+    // pair numbers: (a; b) = 2, (b; a) = 3, (-; x y) = 4 + xg, (y x; -) = yg
+    const int p_yx = 2 + yg, p_xy = 2 + xg;
+    fl.add(col_end ? yg : p_yx, p_yx, A12);
+    fl.add(col_end ? p_xy : 4 + xg, p_yx, A21);
   }
-  // S_L = {a, b}: single source
+  // S_L = {a, b}: single source; (ab|) (ba|) (a|b) (b|a) (|ab) (|ba) -> type I pairs 4 5 3 2 0 1, type II pairs 4 5 4 5 4 5
   {
-    const rvec4<double> Ptot = radd(Kq, radd(K[0], K[1]));
+    const rvec4<double> Kab = radd(X.K[0], X.K[1]);
+    const rvec4<double> Ptot = radd(Kq, Kab);
     const rvec4<R> Pr = cast<R>(Ptot);
-    // (ab|) (ba|) (a|b) (b|a) (|ab) (|ba): type I pair, type II pair
-    const int f1[6] = {4, 5, 3, 2, 0, 1}, f2[6] = {4, 5, 4, 5, 4, 5};
+    const double iP2 = 1.0 / rdot(Ptot, Ptot);
+    vec4<R> Jab;                                           // merged current of the tuple (a, b); (b, a) has the opposite sign
+    {
+      vec4<R> acc = vzero<R>();
+      v3_acc(acc, X.K[0], X.e[0], X.K[1], X.e[1]);
+      Jab = qq2_scaled(acc, -1.0 / rdot(Kab, Kab));
+    }
+    rvec4<double> qr, qc;
 #pragma unroll
-    for (int k = 0; k < 6; ++k) {
-      const spinor<R> c0 = row_slash(ubar_t, Q.Q2[k]);
-      spinor<R> c1 = szero<R>();
-      ften<R> F = fzero<R>();
-      wedge_acc(F, Pr, Q.Q2[k]);
-      row_sigma_acc(c1, ubar_t, F);
+    for (int mu = 0; mu < 4; ++mu) { qr.c[mu] = -(X.Kr.c[mu] + Kab.c[mu]); qc.c[mu] = X.Kc.c[mu] + Kab.c[mu]; }
+    const R sr = R(-1.0 / rdot(qr, qr)), sc = R(-1.0 / rdot(qc, qc));
+#pragma unroll 1
+    for (int ord = 0; ord < 2; ++ord) {                    // ord 0: strings (a, b); 1: (b, a)
+      const vec4<R> e1 = ord ? X.e[1] : X.e[0], e2 = ord ? X.e[0] : X.e[1];
+      const rvec4<double> K1 = ord ? X.K[1] : X.K[0], K2 = ord ? X.K[0] : X.K[1];
+      const R sg = ord ? R(-1) : R(1);
+      const spinor<R> R1 = qq2_row1(X.w, X.Kr, e1, K1), C2 = qq2_col1(X.x, X.Kc, e2, K2);
       cx<R> A[2][2];
+      // (g1 g2 |): R_2 = -[ R_g1 eslash_g2 + w Jslash ] qslash / q^2
+      {
+        spinor<R> t = row_slash(R1, e2);
+        const spinor<R> wJ = row_slash(X.w, Jab);
 #pragma unroll
-      for (int iv = 0; iv < 2; ++iv) { A[0][iv] = mul_i(row_col(c0, vtb[iv])); A[1][iv] = row_col(c1, vtb[iv]); }
-      fl.add(f1[k], f2[k], A);
+        for (int i = 0; i < 4; ++i) cfma(t.c[i], wJ.c[i], sg);
+        spinor<R> R2 = row_slash(t, cast<R>(qr));
+#pragma unroll
+        for (int i = 0; i < 4; ++i) R2.c[i] = R2.c[i] * sr;
+        qq2_single(ubar_t, vtb, qq2_scaled(bilinear(R2, X.x), iP2), Pr, A);
+        fl.add(4 + ord, 4 + ord, A);
+      }
+      // (g1 | g2)
+      qq2_single(ubar_t, vtb, qq2_scaled(bilinear(R1, C2), iP2), Pr, A);
+      fl.add(3 - ord, 4 + ord, A);
+      // (| g1 g2), g2 next to the column end: C = -qslash [ eslash_g1 C_g2 + Jslash x ] / q^2
+      {
+        spinor<R> u = slash_col(e1, C2);
+        const spinor<R> Jx = slash_col(Jab, X.x);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) cfma(u.c[i], Jx.c[i], sg);
+        spinor<R> Cc = slash_col(cast<R>(qc), u);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) Cc.c[i] = Cc.c[i] * sc;
+        qq2_single(ubar_t, vtb, qq2_scaled(bilinear(X.w, Cc), iP2), Pr, A);
+        fl.add(ord, 4 + ord, A);
+      }
     }
   }
 }
 
 // sum over the top helicity (and both antitop helicities) of x^dagger C x at theta_old and theta_new for one choice of the
-// light-line combination c and the gluon helicities; pm = momenta of the event [leg][mu]
+// light-line combination c and the gluon helicities; pm = momenta of the event [leg][mu]; fl = this thread's flow storage
 template <class R, class RC>
-TREX_HD void qq2_unit(const double (*pm)[4], const QLineLegs& L, int c, int la, int lb, const ThetaPair& T, RC out[2]) {
+TREX_HD void qq2_unit(const double (*pm)[4], const QLineLegs& L, int c, int la, int lb, const ThetaPair& T, const Qq2Acc<R>& fl, RC out[2]) {
   const bool row_in = L.lrow < 2, col_in = L.lcol < 2;
   // row spinor in the upper block for c = 1 (see k_qq)
   const bool row_upper = c != 0, col_upper = !row_upper;
-  spinor<R> w, x;
+  Qq2Ext<R> X;
   {
     const int lam = (row_in ? !row_upper : row_upper) ? 1 : -1;
-    w = cast<R>(row_in ? bar(spinor_v<double>(pm[L.lrow], lam, true)) : bar(spinor_u<double>(pm[L.lrow], lam, true)));
+    X.w = cast<R>(row_in ? bar(spinor_v<double>(pm[L.lrow], lam, true)) : bar(spinor_u<double>(pm[L.lrow], lam, true)));
     const int lamc = (col_in ? !col_upper : col_upper) ? 1 : -1;
-    x = cast<R>(col_in ? spinor_u<double>(pm[L.lcol], lamc, true) : spinor_v<double>(pm[L.lcol], lamc, true));
+    X.x = cast<R>(col_in ? spinor_u<double>(pm[L.lcol], lamc, true) : spinor_v<double>(pm[L.lcol], lamc, true));
   }
-  rvec4<double> Kr, Kc, K[2], pt;
-  vec4<R> e[2];
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) {
-    Kr.c[mu] = row_in ? pm[L.lrow][mu] : -pm[L.lrow][mu];
-    Kc.c[mu] = col_in ? pm[L.lcol][mu] : -pm[L.lcol][mu];
-    pt.c[mu] = pm[2][mu];
+    X.Kr.c[mu] = row_in ? pm[L.lrow][mu] : -pm[L.lrow][mu];
+    X.Kc.c[mu] = col_in ? pm[L.lcol][mu] : -pm[L.lcol][mu];
+    X.pt.c[mu] = pm[2][mu];
   }
 #pragma unroll
   for (int g = 0; g < 2; ++g) {
     const int lg = g == 0 ? L.lg : L.lg2;
     const bool g_in = lg < 2;
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) K[g].c[mu] = g_in ? pm[lg][mu] : -pm[lg][mu];
-    e[g] = cast<R>(polvec<double>(pm[lg], (g == 0 ? la : lb) ? 1 : -1, !g_in));
+    for (int mu = 0; mu < 4; ++mu) X.K[g].c[mu] = g_in ? pm[lg][mu] : -pm[lg][mu];
+    X.e[g] = cast<R>(polvec<double>(pm[lg], (g == 0 ? la : lb) ? 1 : -1, !g_in));
   }
-  Qq2Currents<R> Q;
-  qq2_light_line<R>(w, x, Kr, Kc, e, K, Q);
-  const rvec4<double> Kq = radd(Kr, Kc);
   const spinor<R> vtb[2] = {cast<R>(spinor_v<double>(pm[3], -1, false)), cast<R>(spinor_v<double>(pm[3], +1, false))};
   const bool same_line = (T.mt[0] == T.mt[1]) && (T.mGt[0] == T.mGt[1]);
   RC acc[2] = {RC(0), RC(0)};
 #pragma unroll 1
   for (int lt = 0; lt < 2; ++lt) {
     const spinor<R> ubar_t = cast<R>(bar(spinor_u<double>(pm[2], lt ? 1 : -1, false)));
-    Qq2Flows<R> fl;
 #pragma unroll 1
     for (int th = 0; th < 2; ++th) {
-      if (th == 0 || !same_line) qq2_flows<R>(Q, e, K, Kq, ubar_t, vtb, pt, T.mt[th], T.mGt[th], fl);
+      if (th == 0 || !same_line) qq2_flows<R>(X, ubar_t, vtb, T.mt[th], T.mGt[th], fl);
       const R kq = R(T.kq[th]);
-#pragma unroll
+#pragma unroll 1
       for (int iv = 0; iv < 2; ++iv) {
         cx<RC> xf[QQ2_NFLOW];
 #pragma unroll
         for (int f = 0; f < QQ2_NFLOW; ++f) {
-          cx<R> a = fl.F[f][0][iv];
-          cfma(a, fl.F[f][1][iv], kq);
+          cx<R> a = fl.get(f, 0, iv);
+          cfma(a, fl.get(f, 1, iv), kq);
           xf[f] = cx<RC>(RC(a.re), RC(a.im));
         }
         acc[th] += colour_quadform<RC, QQ2_NFLOW, 1>(xf, nullptr);
