@@ -13,7 +13,7 @@
 //     type II: (S1)_{t tb} (S2)_{r k}      -1/6 A      with S1 = L_T R_T, S2 = L R
 // (t, tb: colour of top / antitop; r, k: row / column end of the light line; S1, S2: ordered strings of T^a, T^b). The pair
 // (S1, S2) is numbered 0 (ab, -), 1 (ba, -), 2 (a, b), 3 (b, a), 4 (-, ab), 5 (-, ba); type II adds 6. Terms:
-//     S_L = {}     : six orderings of (a, b, Q) on the top line                      (TTNGS<3>)
+//     S_L = {}     : six orderings of (a, b, Q) on the top line                      (three_source_path)
 //     S_L = {x}    : Q(x|) and Q(|x), two orderings of (y, Q) each                    (two_source_line)
 //     S_L = {a, b} : Q(ab|) Q(ba|) Q(a|b) Q(b|a) Q(|ab) Q(|ba), single source        (one bracket each)
 // The 12 x 12 colour matrix comes from trex_colour.h (traces of the strings, exact rationals).
@@ -50,21 +50,6 @@ template <class R> struct Qq2Acc {
       }
   }
   TREX_HD cx<R> get(int f, int o, int iv) const { return cx<R>(at(f, o, iv, 0), at(f, o, iv, 1)); }
-};
-
-// sink of the three-source walk (sources 0 = a, 1 = b, 2 = Q; leaves in lexicographic order)
-template <class R> struct Qq2Sink3 {
-  Qq2Acc<R> fl;
-  const spinor<R>* v;
-  template <int LEAF> TREX_HD void put(const spinor<R>* b0, const spinor<R>* b1) {
-    // leaf: 0 (a,b,Q) 1 (a,Q,b) 2 (b,a,Q) 3 (b,Q,a) 4 (Q,a,b) 5 (Q,b,a)
-    constexpr int f1 = LEAF == 0 ? 0 : LEAF == 1 ? 2 : LEAF == 2 ? 1 : LEAF == 3 ? 3 : LEAF == 4 ? 4 : 5;
-    constexpr int f2 = (LEAF == 0 || LEAF == 1 || LEAF == 4) ? 0 : 1;
-    cx<R> A[2][2];
-#pragma unroll
-    for (int iv = 0; iv < 2; ++iv) { A[0][iv] = row_col(b0[0], v[iv]); A[1][iv] = row_col(b1[0], v[iv]); }
-    fl.add(f1, f2, A);
-  }
 };
 
 template <class R> TREX_HD vec4<R> qq2_scaled(const vec4<R>& j, double s) {
@@ -116,22 +101,134 @@ TREX_HD void qq2_single(const spinor<R>& ubar_t, const spinor<R> vtb[2], const v
   for (int iv = 0; iv < 2; ++iv) { A[0][iv] = mul_i(row_col(c0, vtb[iv])); A[1][iv] = row_col(c1, vtb[iv]); }
 }
 
-// all twelve flows for one top helicity and one parameter point's top line
+// the three groups of terms for one top helicity and one parameter point's top line. On the device they are separate
+// functions (not inlined): each gets the whole register file for its walk, and the caller's state is saved once around
+// the call instead of being spilled and reloaded piecemeal inside it.
+#if defined(__CUDA_ARCH__) && !defined(TREX_QQ2_INLINE)
+#define TREX_QQ2_FN __device__ __noinline__
+#else
+#define TREX_QQ2_FN TREX_HD
+#endif
+
+// Top line with THREE ordered sources (e[i], K[i]: current and momentum into the line), ONE ordering (0, 1, 2): the path
+// (0), (0 1), (0 1 2) of the prefix walk of trex_ttng.cuh written out -- merged currents J02 = (0 1), J13 = (1 2),
+// J03 = (0 1 2), line states U1, U2 -- and closed with both antitop spinors: A[order in kappa][v]. The caller loops over
+// the six orderings (rolled), so that only one path is alive at a time.
 template <class R>
-TREX_HD void qq2_flows(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor<R> vtb[2], double mt, double mGt, const Qq2Acc<R>& fl) {
-  fl.clear();
-  const rvec4<double> Kq = radd(X.Kr, X.Kc);
-  // S_L = {}: three sources (a, b, Q0), Q0 = (w gamma x) / Kq^2
+TREX_HD void three_source_path(const spinor<R>& ubar, const rvec4<double>& pt, const vec4<R>& e0, const rvec4<double>& K0,
+                               const vec4<R>& e1, const rvec4<double>& K1, const vec4<R>& e2, const rvec4<double>& K2, double mt_d,
+                               double mGt, const spinor<R> v[2], cx<R> A[2][2]) {
+  const R mt = R(mt_d);
+  auto propagate = [&](const spinor<R>& b0, const spinor<R>& b1, const rvec4<double>& qd, dspinor<R>& U) {
+    const double q2 = rdot(qd, qd);
+    const rvec4<R> q = cast<R>(qd);
+    const cx<R> pr = cast<R>(cdiv(cx<double>(0, 1), cx<double>(q2 - mt_d * mt_d, mGt)));
+    const spinor<R> s0 = row_slash(b0, q), s1 = row_slash(b1, q);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      cx<R> n0 = s0.c[i]; cfma(n0, b0.c[i], mt);
+      cx<R> n1 = s1.c[i]; cfma(n1, b1.c[i], mt);
+      U.o0.c[i] = n0 * pr; U.o1.c[i] = n1 * pr;
+    }
+  };
+  auto scale = [](const vec4<R>& a, double s) { vec4<R> o; const R sr = R(s);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) o.c[i] = a.c[i] * sr;
+    return o; };
+  // term of a bracket: b0 += i U.o0 Jslash, b1 += i U.o1 Jslash + U.o0 sigma.F
+  auto absorb = [](spinor<R>& b0, spinor<R>& b1, const dspinor<R>& U, const vec4<R>& J, const ften<R>& F) {
+    const spinor<R> t0 = row_slash(U.o0, J), t1 = row_slash(U.o1, J);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { b0.c[i] += mul_i(t0.c[i]); b1.c[i] += mul_i(t1.c[i]); }
+    row_sigma_acc(b1, U.o0, F);
+  };
+  auto absorb0 = [&](spinor<R>& b0, spinor<R>& b1, const vec4<R>& J, const ften<R>& F) {      // at the external spinor
+    const spinor<R> t0 = row_slash(ubar, J);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) b0.c[i] += mul_i(t0.c[i]);
+    row_sigma_acc(b1, ubar, F);
+  };
+  // level 1
+  dspinor<R> U1, U2;
   {
-    Qq2Sink3<R> sink{fl, vtb};
-    TTNGS<R, 3, 1, Qq2Sink3<R>> t;
-    t.K[0] = X.K[0]; t.K[1] = X.K[1]; t.K[2] = Kq;
-    t.eps[0] = X.e[0]; t.eps[1] = X.e[1]; t.eps[2] = qq2_scaled(bilinear(X.w, X.x), 1.0 / rdot(Kq, Kq));
-    t.pt = X.pt; t.ubar_t = ubar_t;
-    t.line[0].mt = mt; t.line[0].mGt = mGt;
-    t.run(&sink);
+    spinor<R> b0 = szero<R>(), b1 = szero<R>();
+    ften<R> F = fzero<R>();
+    wedge_acc(F, cast<R>(K0), e0);
+    absorb0(b0, b1, e0, F);
+    propagate(b0, b1, rsub(pt, K0), U1);
   }
-  // S_L = {x}: the other gluon y and Q(x|) / Q(|x)
+  // level 2
+  const rvec4<double> P02 = radd(K0, K1);
+  vec4<R> J02;
+  {
+    vec4<R> acc = vzero<R>();
+    v3_acc(acc, K0, e0, K1, e1);
+    J02 = scale(acc, -1.0 / rdot(P02, P02));
+  }
+  {
+    spinor<R> b0 = szero<R>(), b1 = szero<R>();
+    ften<R> F = fzero<R>();
+    wedge_acc(F, cast<R>(P02), J02); wedge_acc(F, e0, e1);
+    absorb0(b0, b1, J02, F);
+    F = fzero<R>();
+    wedge_acc(F, cast<R>(K1), e1);
+    absorb(b0, b1, U1, e1, F);
+    propagate(b0, b1, rsub(pt, P02), U2);
+  }
+  // level 3
+  const rvec4<double> P13 = radd(K1, K2), P03 = radd(P02, K2);
+  vec4<R> J13, J03;
+  {
+    vec4<R> acc = vzero<R>();
+    v3_acc(acc, K1, e1, K2, e2);
+    J13 = scale(acc, -1.0 / rdot(P13, P13));
+    acc = vzero<R>();
+    v3_acc(acc, K0, e0, P13, J13);
+    v3_acc(acc, P02, J02, K2, e2);
+    v4_acc(acc, e0, e1, e2);
+    J03 = scale(acc, -1.0 / rdot(P03, P03));
+  }
+  spinor<R> b0 = szero<R>(), b1 = szero<R>();
+  {
+    ften<R> F = fzero<R>();
+    wedge_acc(F, cast<R>(P03), J03); wedge_acc(F, e0, J13); wedge_acc(F, J02, e2);
+    absorb0(b0, b1, J03, F);
+    F = fzero<R>();
+    wedge_acc(F, cast<R>(P13), J13); wedge_acc(F, e1, e2);
+    absorb(b0, b1, U1, J13, F);
+    F = fzero<R>();
+    wedge_acc(F, cast<R>(K2), e2);
+    absorb(b0, b1, U2, e2, F);
+  }
+#pragma unroll
+  for (int iv = 0; iv < 2; ++iv) { A[0][iv] = row_col(b0, v[iv]); A[1][iv] = row_col(b1, v[iv]); }
+}
+
+// S_L = {}: three sources (a, b, Q0), Q0 = (w gamma x) / Kq^2, six orderings
+template <class R>
+TREX_QQ2_FN void qq2_group0(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor<R> vtb[2], double mt, double mGt, const Qq2Acc<R>& fl) {
+  const rvec4<double> Kq = radd(X.Kr, X.Kc);
+  const vec4<R> Q0 = qq2_scaled(bilinear(X.w, X.x), 1.0 / rdot(Kq, Kq));
+  auto src_e = [&](int i) { return i == 0 ? X.e[0] : (i == 1 ? X.e[1] : Q0); };
+  auto src_K = [&](int i) { return i == 0 ? X.K[0] : (i == 1 ? X.K[1] : Kq); };
+  // orderings in lexicographic order of (a, b, Q) = (0, 1, 2): (a,b,Q) (a,Q,b) (b,a,Q) (b,Q,a) (Q,a,b) (Q,b,a);
+  // type I pair = (gluons before Q; gluons after Q), type II pair = (all gluons in order; -)
+#pragma unroll 1
+  for (int o = 0; o < 6; ++o) {
+    const int i0 = o >> 1, r = o & 1;
+    const int i1 = i0 == 0 ? 1 + r : (i0 == 1 ? 2 * r : r), i2 = 3 - i0 - i1;
+    cx<R> A[2][2];
+    three_source_path<R>(ubar_t, X.pt, src_e(i0), src_K(i0), src_e(i1), src_K(i1), src_e(i2), src_K(i2), mt, mGt, vtb, A);
+    const int f1 = o == 0 ? 0 : o == 1 ? 2 : o == 2 ? 1 : o == 3 ? 3 : o == 4 ? 4 : 5;
+    const int f2 = (o == 0 || o == 1 || o == 4) ? 0 : 1;
+    fl.add(f1, f2, A);
+  }
+}
+
+// S_L = {x}: the other gluon y and Q(x|) / Q(|x)
+template <class R>
+TREX_QQ2_FN void qq2_group1(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor<R> vtb[2], double mt, double mGt, const Qq2Acc<R>& fl) {
+  const rvec4<double> Kq = radd(X.Kr, X.Kc);
 #pragma unroll 1
   for (int k = 0; k < 4; ++k) {
     const int xg = k >> 1, yg = 1 - xg, col_end = k & 1;
@@ -148,7 +245,12 @@ TREX_HD void qq2_flows(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor
     fl.add(col_end ? yg : p_yx, p_yx, A12);
     fl.add(col_end ? p_xy : 4 + xg, p_yx, A21);
   }
-  // S_L = {a, b}: single source; (ab|) (ba|) (a|b) (b|a) (|ab) (|ba) -> type I pairs 4 5 3 2 0 1, type II pairs 4 5 4 5 4 5
+}
+
+// S_L = {a, b}: single source; (ab|) (ba|) (a|b) (b|a) (|ab) (|ba) -> type I pairs 4 5 3 2 0 1, type II pairs 4 5 4 5 4 5
+template <class R>
+TREX_QQ2_FN void qq2_group2(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor<R> vtb[2], const Qq2Acc<R>& fl) {
+  const rvec4<double> Kq = radd(X.Kr, X.Kc);
   {
     const rvec4<double> Kab = radd(X.K[0], X.K[1]);
     const rvec4<double> Ptot = radd(Kq, Kab);
@@ -200,6 +302,15 @@ TREX_HD void qq2_flows(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor
       }
     }
   }
+}
+
+// all twelve flows
+template <class R>
+TREX_HD void qq2_flows(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor<R> vtb[2], double mt, double mGt, const Qq2Acc<R>& fl) {
+  fl.clear();
+  qq2_group0<R>(X, ubar_t, vtb, mt, mGt, fl);
+  qq2_group1<R>(X, ubar_t, vtb, mt, mGt, fl);
+  qq2_group2<R>(X, ubar_t, vtb, fl);
 }
 
 // sum over the top helicity (and both antitop helicities) of x^dagger C x at theta_old and theta_new for one choice of the

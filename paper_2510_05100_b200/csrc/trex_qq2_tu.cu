@@ -15,11 +15,14 @@ namespace {
 __constant__ QLineLegs c_q2legs[TREX_NSUBPROC];
 __constant__ double c_q2invnavg[TREX_NSUBPROC];      // 1 / N_avg; 0 for ids that are not two-gluon quark channels
 
+#ifndef TREX_QQ2_MINB
+#define TREX_QQ2_MINB 2
+#endif
 constexpr int Q2_WARPS = 4, Q2_TB = Q2_WARPS * 32;
 template <class R> constexpr size_t q2_smem() { return sizeof(R) * Qq2Acc<R>::NEL * Q2_TB; }
 
 template <class R, class RC>
-__global__ void __launch_bounds__(Q2_TB, 2) k_qq2(const ReweightArgs a) {
+__global__ void __launch_bounds__(Q2_TB, TREX_QQ2_MINB) k_qq2(const ReweightArgs a) {
   extern __shared__ __align__(16) unsigned char q2_raw[];
   __shared__ double red[2][Q2_WARPS][32];
   int sid = a.sid;
