@@ -165,6 +165,20 @@ int trex_run_pdg(const int32_t* pdg_soa, const double* momenta_soa, int64_t n, i
 int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
                    const double* theta_new, int ntheta, const double* w_in, double* w_out, double* me2_old, double* me2_new);
 
+/* trex_run with a PER-EVENT strong coupling (an LHE event carries its own alpha_s = AQCDUP at its renormalisation scale;
+ * Rex exposes g_S = sqrt(4 pi alpha_S) per event through gS()): alpha_s DEVICE [n] replaces
+ * theta[TREX_TH_ALPHA_S] of BOTH parameter points for that event; everything else as trex_run. With g_s factored out
+ * an amplitude with nv strong vertices is g_s^nv (A0 + (kappa / g_s) A1) (one dimension-6 insertion at most), so
+ *   |M(theta; alpha_s)|^2 = g_s^(2 nv) [ a + (kappa / g_s) b + (kappa / g_s)^2 d ]
+ * with a, b, d free of alpha_s: they are obtained per event and parameter point from three passes of the unchanged
+ * |M|^2 kernels at g_s = 1 (kappa / g_s = 0, +delta, -delta: the quadratic is exact), and one elementwise kernel applies
+ * the event's g_s. Cost: 1.5 x trex_run. e- e+ > mu- mu+ events do not depend on alpha_s and come out as from trex_run.
+ * An event with alpha_s = 0 has |M|^2 = 0 and weight 0 (zero guard); negative or non-finite alpha_s
+ * gives NaN for that event only. Returns the number of buckets. */
+int trex_run_alphas(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
+                    const double* theta_new, const double* alpha_s, const double* w_in, double* w_out, double* me2_old,
+                    double* me2_new);
+
 /* The same with HOST buffers (pinned or pageable): copies keys, momenta and weights to internal device scratch on the
  * stream, runs trex_run, copies the results back and synchronises the stream before returning. */
 int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,

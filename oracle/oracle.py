@@ -97,6 +97,20 @@ def reweight(sid, momenta, theta_old, theta_new, w_in, long_double=False):
     return w_out, mo, mn
 
 
+def reweight_alphas(sid, momenta, theta_old, theta_new, alpha_s, w_in):
+    """Reweighting with a per-event strong coupling (an LHE event carries its own alpha_s; g_S per event: PAPER.md:66-67,
+    104): for event i both parameter points are evaluated with theta[0] = alpha_s[i]. Written as its definition: one plain
+    `reweight` call per event with the two parameter vectors changed in that one entry."""
+    m, n = _mom(sid, momenta)
+    w_out, mo, mn = np.empty(n), np.empty(n), np.empty(n)
+    for i in range(n):
+        to = np.array(theta_old, dtype=np.float64)
+        tn = np.array(theta_new, dtype=np.float64)
+        to[0] = tn[0] = alpha_s[i]
+        w_out[i:i + 1], mo[i:i + 1], mn[i:i + 1] = reweight(sid, np.ascontiguousarray(m[:, :, i:i + 1]), to, tn, w_in[i:i + 1])
+    return w_out, mo, mn
+
+
 def ttng_amps(sid, momenta_one, theta, hel, gauge_gluon=-1):
     """Colour-flow amplitudes A_sigma (order 0 and order 1 in kappa) of one event and one helicity index.
     Returns complex array [n!, 2]; orderings lexicographic."""

@@ -44,6 +44,7 @@ _SIGNATURES = {
     "rex_keys": (_int, [_vp, _int, _int, _i64, _vp, _vp]),
     "trex_run_pdg": (_int, [_vp, _vp, _i64, _int, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_run_multi": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _int, _vp, _vp, _vp, _vp]),
+    "trex_run_alphas": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _vp, _vp, _vp, _vp, _vp]),
     "trex_run_host": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_debug_flow_amps": (_int, [_int, _dp, _dp, _dp]),
     "trex_debug_xtile": (_int, [_int, _dp, _dp, _dp, _dp]),
@@ -307,6 +308,29 @@ def trex_run(pdg_keys, momenta_soa, theta_old, theta_new, w_in, w_out=None, me2_
     nb = _check(lib().trex_run(_dev(pdg_keys, torch.int64, "pdg_keys"), _dev(momenta_soa, f64, "momenta_soa"), n, npar,
                                pto, ptn, _dev(w_in, f64, "w_in"), _dev(w_out, f64, "w_out"),
                                _dev(me2_old, f64, "me2_old"), _dev(me2_new, f64, "me2_new")), "trex_run")
+    return w_out, me2_old, me2_new, nb
+
+
+def trex_run_alphas(pdg_keys, momenta_soa, theta_old, theta_new, alpha_s, w_in, w_out=None, me2_old=None, me2_new=None, want_me2=True):
+    """trex_run with a per-event strong coupling: alpha_s (CUDA tensor [n]) replaces theta[0] of both parameter points for
+    that event. Returns (w_out, me2_old, me2_new, nbuckets)."""
+    torch = _torch()
+    n = w_in.numel()
+    npar = momenta_soa.shape[0]
+    if w_out is None:
+        w_out = torch.empty_like(w_in)
+    if want_me2 and me2_old is None:
+        me2_old = torch.empty_like(w_in)
+    if want_me2 and me2_new is None:
+        me2_new = torch.empty_like(w_in)
+    _shapes("trex_run_alphas", n, momenta_soa, pdg_keys,
+            rows=(("alpha_s", alpha_s), ("w_out", w_out), ("me2_old", me2_old), ("me2_new", me2_new)))
+    to, pto = _theta(theta_old)
+    tn, ptn = _theta(theta_new)
+    f64 = torch.float64
+    nb = _check(lib().trex_run_alphas(_dev(pdg_keys, torch.int64, "pdg_keys"), _dev(momenta_soa, f64, "momenta_soa"), n, npar,
+                                      pto, ptn, _dev(alpha_s, f64, "alpha_s"), _dev(w_in, f64, "w_in"), _dev(w_out, f64, "w_out"),
+                                      _dev(me2_old, f64, "me2_old"), _dev(me2_new, f64, "me2_new")), "trex_run_alphas")
     return w_out, me2_old, me2_new, nb
 
 

@@ -468,6 +468,12 @@ static int run_core(const uint64_t* pdg_keys, const double* momenta_soa, int64_t
   for (int sid = 0; sid < TREX_NSUBPROC; ++sid)
     if (npar_of_sid(sid) == npar && !make_theta_pair(sid, theta_old, theta_new, T[sid]))
       return fail(TREX_EINVAL, "trex_run: theta outside its domain");
+  if (c.unit_gs)                                      // a pass of trex_run_alphas: g_s = 1, the same kappa / g_s at both points
+    for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
+      const SubprocInfo* sp = subproc_info(sid);
+      if (!sp || sp->npar != npar || sid == TREX_SP_EEMUMU) continue;
+      for (int k = 0; k < 2; ++k) { T[sid].kq[k] = c.unit_gs_kq; T[sid].gs2nv[k] = 1.0; T[sid].pref[k] = 1.0 / sp->navg; }
+    }
   if (int rc = ensure_plan()) return rc;
   if (int rc = ensure_colour()) return rc;
   const int nrows = 4 * npar;
@@ -539,6 +545,72 @@ static int run_core(const uint64_t* pdg_keys, const double* momenta_soa, int64_t
   c.last_key = key; c.last_key_valid = true;
   if (int rc = enqueue()) return rc;
   return bucket_finish(offsets);
+}
+
+// |M|^2 = g_s^(2 nv) [a + x b + x^2 d], x = kappa / g_s, from its values m0, mp, mm at x = 0, +delta, -delta and g_s = 1
+__global__ void __launch_bounds__(256) k_alphas_weights(const unsigned long long* __restrict__ keys, unsigned long long eemumu_key, int nv,
+                                                        const double* __restrict__ alpha_s, const double* __restrict__ m /* [2][3][n] */,
+                                                        long n, double xo, double xn, const double* __restrict__ w_in,
+                                                        double* __restrict__ w_out, double* __restrict__ me2_old, double* __restrict__ me2_new) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double res[2];
+  const bool qcd = keys[i] != eemumu_key;
+  const double gs = sqrt(4.0 * 3.14159265358979323846 * alpha_s[i]);
+#pragma unroll
+  for (int p = 0; p < 2; ++p) {
+    const double m0 = m[(size_t)(3 * p) * n + i], mp = m[(size_t)(3 * p + 1) * n + i], mm = m[(size_t)(3 * p + 2) * n + i];
+    if (!qcd) { res[p] = m0; continue; }
+    const double b = 0.5 * (mp - mm), d = 0.5 * (mp + mm) - m0;
+    const double u = (p == 0 ? xo : xn) / gs;                 // (kappa / g_s) / delta
+    double g2 = 1.0;
+    for (int k = 0; k < nv; ++k) g2 *= gs * gs;
+    res[p] = gs == 0.0 ? 0.0 : g2 * (m0 + u * (b + u * d));
+  }
+  const double norm = (res[0] == 0.0) ? 0.0 : 1.0 / res[0];   // zero guard
+  w_out[i] = w_in[i] * norm * res[1];
+  if (me2_old) me2_old[i] = res[0];
+  if (me2_new) me2_new[i] = res[1];
+}
+
+extern "C" int trex_run_alphas(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,
+                               const double* theta_new, const double* alpha_s, const double* w_in, double* w_out, double* me2_old,
+                               double* me2_new) {
+  Context& c = ctx();
+  if (n < 0 || npar < 1 || npar > 7 || !theta_old || !theta_new) return fail(TREX_EINVAL, "trex_run_alphas: bad size or null theta");
+  if (n == 0) return 0;
+  if (!alpha_s || !pdg_keys || !momenta_soa || !w_in || !w_out) return fail(TREX_EINVAL, "trex_run_alphas: null device pointer");
+  const auto kappa_of = [](const double* th) { return th[TREX_TH_CTG] * th[TREX_TH_VEV] / (std::sqrt(2.0) * th[TREX_TH_LAMBDA] * th[TREX_TH_LAMBDA]); };
+  if (!(theta_old[TREX_TH_LAMBDA] > 0.0) || !(theta_new[TREX_TH_LAMBDA] > 0.0)) return fail(TREX_EINVAL, "trex_run_alphas: theta outside its domain");
+  const double ko = kappa_of(theta_old), kn = kappa_of(theta_new);
+  if (!std::isfinite(ko) || !std::isfinite(kn)) return fail(TREX_EINVAL, "trex_run_alphas: non-finite kappa");
+  // support points of the quadratic in x = kappa / g_s: of the size x takes for g_s of order one
+  double delta = std::fmax(std::fabs(ko), std::fabs(kn));
+  if (delta == 0.0) delta = 1.0;
+  if (int rc = ensure_scratch(&c.poly_tmp, &c.poly_tmp_bytes, sizeof(double) * 6 * (size_t)n)) return rc;
+  double* m = (double*)c.poly_tmp;                    // [old, new][x = 0, +delta, -delta][n]
+  // the passes read theta for everything but the strong coupling; alpha_s of theta must only be usable
+  double tho[TREX_NTHETA], thn[TREX_NTHETA];
+  std::memcpy(tho, theta_old, sizeof tho); std::memcpy(thn, theta_new, sizeof thn);
+  tho[TREX_TH_ALPHA_S] = thn[TREX_TH_ALPHA_S] = 1.0;
+  int rc = 0, nb = 0;
+  c.unit_gs = true; c.in_host_run = true;             // no graph replay: the key does not know about unit_gs_kq
+  for (int s = 0; s < 3 && rc >= 0; ++s) {
+    c.unit_gs_kq = s == 0 ? 0.0 : (s == 1 ? delta : -delta);
+    rc = run_core(pdg_keys, momenta_soa, n, n, npar, tho, thn, w_in, w_out, m + (size_t)s * n, m + (size_t)(3 + s) * n);
+    if (rc >= 0) nb = rc;
+  }
+  c.unit_gs = false; c.in_host_run = false;
+  if (rc < 0) return rc;
+  const SubprocInfo* ee = subproc_info(TREX_SP_EEMUMU);
+  int8_t status[4] = {-1, -1, 1, 1};
+  const unsigned long long eekey = rex_pack_key(ee->pdg, status, 4);
+  k_alphas_weights<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>((const unsigned long long*)pdg_keys, eekey, npar - 2, alpha_s, m, (long)n,
+                                                                      ko / delta, kn / delta, w_in, w_out, me2_old, me2_new);
+  c.launches += 1;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  TREX_CUDA_CHECK(cudaStreamSynchronize(c.stream));
+  return nb;
 }
 
 // The path for events that carry PDG codes in arbitrary parton order (an LHE file does not promise the order of the
