@@ -161,3 +161,48 @@ def test_reduced_precision_modes(T):
                 assert np.median(r) < med and r.max() < mx, (sid, mode, np.median(r), r.max())
         finally:
             T.trex_set_precision(0)
+
+
+def test_cfg7_events_in_arbitrary_parton_order(T):
+    """trex_run_pdg on the seven-class sample with shuffled legs: keys and leg maps bit-exact against
+    the oracle's, weights equal to those of the canonical sample (the order of the identical gluons does not matter), one
+    q q~ > t t~ g g event straight against the oracle on its re-indexed momenta, unknown classes zero."""
+    import torch
+    from trex_inputs import shuffled_legs
+    w = make_config(7, n=12007)
+    pdg, mom, n_in = shuffled_legs(w, 77, unknown_every=61)
+    keys, lm = T.rex_keys(torch.from_numpy(pdg).cuda(), n_in)
+    rk, rl = O.keys_and_legmap(pdg, n_in, [sp.pdg for sp in SUBPROCESSES])
+    assert np.array_equal(keys.cpu().numpy().view(np.uint64), rk) and np.array_equal(lm.cpu().numpy(), rl)
+    wo, mo, mn, nb = T.trex_run_pdg(torch.from_numpy(pdg).cuda(), dev(mom), n_in, w.theta_old, w.theta_new, dev(w.w_in))
+    wo = wo.cpu().numpy()
+    known = np.isin(rk, np.array([sp.key for sp in w.classes], dtype=np.uint64))
+    assert (~known).sum() > 0 and np.all(wo[~known] == 0) and np.all(wo[known] > 0)
+    assert nb == len(np.unique(rk))
+    w0 = T.trex_run(dev(w.keys), dev(w.momenta), w.theta_old, w.theta_new, dev(w.w_in))[0].cpu().numpy()
+    assert rel(wo[known], w0[known]).max() < 1e-12
+    sp = [s for s in SUBPROCESSES if s.sid == 21][0]
+    i = np.where(rk == sp.key)[0][:1]
+    canon = np.ascontiguousarray(mom[rl[:, i], :, i].transpose(0, 2, 1))
+    want = O.reweight(21, canon, w.theta_old, w.theta_new, w.w_in[i])[0]
+    assert rel(wo[i], want).max() < RTOL64
+
+
+def test_cfg7_many_parameter_points(T):
+    """trex_run_multi on the seven-class sample: the direct path equals trex_run row by row (bit for bit), the polynomial
+    path (exact quadratic in kappa) agrees with it to 1e-12."""
+    w = make_config(7, n=5000)
+    dk, dm, dw = dev(w.keys), dev(w.momenta), dev(w.w_in)
+    thetas = np.tile(w.theta_new, (6, 1))
+    thetas[:, TH_CTG] = np.linspace(-2.0, 3.0, 6)
+    T.trex_set_poly_multi(False)
+    try:
+        direct = T.trex_run_multi(dk, dm, w.theta_old, thetas, dw)
+    finally:
+        T.trex_set_poly_multi(True)
+    for k in (0, 3, 5):
+        one = T.trex_run(dk, dm, w.theta_old, thetas[k], dw)
+        assert np.array_equal(direct[0][k].cpu().numpy(), one[0].cpu().numpy())
+        assert np.array_equal(direct[2][k].cpu().numpy(), one[2].cpu().numpy())
+    poly = T.trex_run_multi(dk, dm, w.theta_old, thetas, dw)
+    assert rel(poly[0].cpu().numpy(), direct[0].cpu().numpy()).max() < 1e-12
