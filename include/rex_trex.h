@@ -198,6 +198,21 @@ int trex_run_host(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n
 int trex_xsec_moments(const double* w_in, const double* w_out, int64_t n, double* moments);
 int trex_xsec_finish(const double* moments, int nparts, double C, double sigma, double dsigma, double* out);
 
+/* trex_xsec_moments for callers that must not allocate (code under CUDA-graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same two fixed-order passes, but
+ *   - the block partials live in a file-scope `static __device__` array of 65.6 KB (8200 doubles) that every GPU
+ *     loading the library holds until exit, sized for n <= TREX_XSEC_NOALLOC_MAX_EVENTS events per call (larger n is
+ *     rejected with TREX_EINVAL and a message; split the shard and combine the parts with trex_xsec_finish);
+ *   - moments_dev is a DEVICE buffer [4] of the caller (N, sum w', sum w'/w, M2), written on the library stream; the call
+ *     is asynchronous and does not wait for the device.
+ * The call performs no cudaMalloc / cudaFree / cudaMallocHost and calls no allocating library routine. Every call on a
+ * device shares the one array: calls are ordered by the library stream; calls that overlap on the GPU (issued on
+ * different streams via trex_set_stream without an event between them, or from several host threads) race on it.
+ * Nothing in the array has to start at zero: each call overwrites what it reads. Summation order differs from
+ * trex_xsec_moments in the number of blocks, so the two agree to rounding (~1e-15 relative), not bit for bit. */
+#define TREX_XSEC_NOALLOC_MAX_EVENTS 16777216ll
+int trex_xsec_moments_noalloc(const double* w_in, const double* w_out, int64_t n, double* moments_dev);
+
 int trex_set_stream(void* cuda_stream);
 int trex_set_precision(int mode);      /* 0 = fp64 (default), 1 = mixed (amplitudes fp64, colour sum fp32,
                                           PAPER.md:1209 fptype m), 2 = fp32 */

@@ -50,6 +50,7 @@ _SIGNATURES = {
     "trex_debug_xtile": (_int, [_int, _dp, _dp, _dp, _dp]),
     "trex_probe_fma": (ctypes.c_double, [_int, _int, _int]),
     "trex_xsec_moments": (_int, [_vp, _vp, ctypes.c_int64, _vp]),
+    "trex_xsec_moments_noalloc": (_int, [_vp, _vp, ctypes.c_int64, _vp]),
     "trex_xsec_finish": (_int, [_vp, _int, ctypes.c_double, ctypes.c_double, ctypes.c_double, _vp]),
     "trex_set_stream": (_int, [_vp]),
     "trex_set_precision": (_int, [_int]),
@@ -444,6 +445,22 @@ def trex_xsec_moments(w_in, w_out):
     _check(lib().trex_xsec_moments(_dev(w_in, torch.float64, "w_in"), _dev(w_out, torch.float64, "w_out"), n,
                                    mom.ctypes.data_as(ctypes.c_void_p)), "trex_xsec_moments")
     return mom
+
+
+TREX_XSEC_NOALLOC_MAX_EVENTS = 16777216
+
+
+def trex_xsec_moments_noalloc(w_in, w_out, moments_out):
+    """trex_xsec_moments without any allocation inside the library: moments_out is a CUDA float64 tensor [4] of the
+    caller, filled asynchronously on the library stream (N, sum w', sum w'/w, M2). At most
+    TREX_XSEC_NOALLOC_MAX_EVENTS events per call."""
+    torch = _torch()
+    n = int(w_out.numel())
+    if int(w_in.numel()) != n or moments_out is None or int(moments_out.numel()) != 4:
+        raise TrexError("trex_xsec_moments_noalloc: w_in and w_out must have the same length and moments_out 4 entries")
+    _check(lib().trex_xsec_moments_noalloc(_dev(w_in, torch.float64, "w_in"), _dev(w_out, torch.float64, "w_out"), n,
+                                           _dev(moments_out, torch.float64, "moments_out")), "trex_xsec_moments_noalloc")
+    return moments_out
 
 
 def trex_xsec_finish(moments, C, sigma, dsigma):

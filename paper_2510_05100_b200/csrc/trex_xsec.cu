@@ -58,10 +58,84 @@ __global__ void __launch_bounds__(XB) k_xsec_m2(const double* __restrict__ w_out
   if (threadIdx.x == 0) part[blockIdx.x] = b;
 }
 
+// ---------------------------------------------------------------- the variant that allocates nothing
+// trex_xsec_moments_noalloc: the same two passes with the block partials in a file-scope device array instead of
+// cudaMalloc'd scratch, and the four moments written to a DEVICE buffer of the caller (no pinned staging buffer, no host
+// wait): usable under CUDA-graph capture and by callers that may not allocate. A block covers at most NA_EPB events, the
+// array holds the partials of NA_MAXBLK blocks: n <= NA_MAXBLK * NA_EPB = TREX_XSEC_NOALLOC_MAX_EVENTS.
+constexpr int NA_EPB = XB * 16;                 // events per block (16 per thread)
+constexpr int NA_MAXBLK = 4096;
+static_assert((long)NA_MAXBLK * NA_EPB == TREX_XSEC_NOALLOC_MAX_EVENTS, "header and kernel geometry must agree");
+// [2 NA_MAXBLK] block partials, [8] moments of the shard between the passes: 65.6 KB on every GPU that loads the library
+static __device__ __align__(256) double g_xsec_static[2 * NA_MAXBLK + 8];
+
+// one block: partials -> mom[first .. first + ncomp), fixed order (thread t sums partials t, t + XB, ..; then block_sum)
+__global__ void __launch_bounds__(XB) k_xsec_fold_wide(const double* __restrict__ part, int nblk, int stride, int ncomp, long n, double* __restrict__ mom, int first) {
+  __shared__ double sh[XB / 32];
+  for (int c = 0; c < ncomp; ++c) {
+    double s = 0.0;
+    for (int b = threadIdx.x; b < nblk; b += XB) s += part[stride * b + c];
+    const double t = block_sum(s, sh);
+    if (threadIdx.x == 0) mom[first + c] = t;
+  }
+  if (threadIdx.x == 0) mom[0] = (double)n;
+}
+__global__ void __launch_bounds__(32) k_xsec_emit(const double* __restrict__ mom, double* __restrict__ out) {
+  if (threadIdx.x < 4) out[threadIdx.x] = mom[threadIdx.x];
+}
+
+// device address of g_xsec_static on the CURRENT device (in host code the array's name is a host-side stand-in, not a
+// device address): asked for once per device, with that device current
+int xsec_static_ptr(double** out) {
+  constexpr int MAXDEV = 64;
+  static double* ptr[MAXDEV] = {nullptr};
+  int dev = -1;
+  TREX_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= MAXDEV) return fail(TREX_EINVAL, "trex_xsec_moments_noalloc: device ordinal %d out of range", dev);
+  if (!ptr[dev]) {
+    double* p = nullptr;
+    TREX_CUDA_CHECK(cudaGetSymbolAddress((void**)&p, g_xsec_static));
+    ptr[dev] = p;
+  }
+  *out = ptr[dev];
+  return 0;
+}
+
 }  // namespace
 }  // namespace trex
 
 using namespace trex;
+
+extern "C" int trex_xsec_moments_noalloc(const double* w_in, const double* w_out, int64_t n, double* moments_dev) {
+  Context& c = ctx();
+  if (n < 0 || !moments_dev) return fail(TREX_EINVAL, "trex_xsec_moments_noalloc: negative n or null output");
+  if (n > (int64_t)TREX_XSEC_NOALLOC_MAX_EVENTS)
+    return fail(TREX_EINVAL, "trex_xsec_moments_noalloc: n = %lld exceeds the static scratch (at most %lld events per call); "
+                "use trex_xsec_moments or split the shard and combine with trex_xsec_finish",
+                (long long)n, (long long)TREX_XSEC_NOALLOC_MAX_EVENTS);
+  if (n > 0 && (!w_in || !w_out)) return fail(TREX_EINVAL, "trex_xsec_moments_noalloc: null device pointer");
+  double* part = nullptr;
+  if (int rc = xsec_static_ptr(&part)) return rc;
+  double* mom = part + 2 * NA_MAXBLK;
+  if (n == 0) {                                          // zeros, as trex_xsec_moments gives
+    k_xsec_fold_wide<<<1, XB, 0, c.stream>>>(part, 0, 1, 3, 0, mom, 1);
+    k_xsec_emit<<<1, 32, 0, c.stream>>>(mom, moments_dev);
+    c.launches += 2;
+    TREX_CUDA_CHECK(cudaGetLastError());
+    return 0;
+  }
+  // every partial a fold reads and every moment is written by THIS call before it is read: nothing has to start at zero,
+  // whatever the previous call left in the array
+  const int nblk = (int)((n + NA_EPB - 1) / NA_EPB);
+  k_xsec_sums<<<nblk, XB, 0, c.stream>>>(w_in, w_out, n, part);
+  k_xsec_fold_wide<<<1, XB, 0, c.stream>>>(part, nblk, 2, 2, n, mom, 1);
+  k_xsec_m2<<<nblk, XB, 0, c.stream>>>(w_out, n, mom, part);
+  k_xsec_fold_wide<<<1, XB, 0, c.stream>>>(part, nblk, 1, 1, n, mom, 3);
+  k_xsec_emit<<<1, 32, 0, c.stream>>>(mom, moments_dev);
+  c.launches += 5;
+  TREX_CUDA_CHECK(cudaGetLastError());
+  return 0;
+}
 
 extern "C" int trex_xsec_moments(const double* w_in, const double* w_out, int64_t n, double* moments) {
   Context& c = ctx();
