@@ -25,6 +25,14 @@ int trex_debug_flow_amps(int subproc_id, const double* momenta_one, const double
  * two parameter points the two-pass kernels are the ones exercised. Synchronous. */
 int trex_debug_xtile(int subproc_id, const double* momenta_one, const double* theta_old, const double* theta_new, double* out);
 
+/* Per-helicity |M_h|^2 of the PRODUCTION quark-channel kernels (k_qq: one light line + one gluon; k_qq2: + two gluons):
+ * one event is run through the regular launch path, with the kernel template instantiated with its per-helicity dump
+ * compiled in (otherwise the same code), and a side buffer receives every helicity configuration's colour-summed value
+ * before the helicity sum. out HOST [nhel][2: theta_old, theta_new], h = sum_leg bit(leg) * (helicity
+ * of leg is +), couplings and 1 / N_avg included, so that sum_h out[h][.] is what trex_reweight returns as me2; the
+ * helicity configurations the massless line forbids are exact zeros. fp64 mode. Synchronous. */
+int trex_debug_helicity_me2(int subproc_id, const double* momenta_one, const double* theta_old, const double* theta_new, double* out);
+
 /* Roofline denominator: enqueues ONE launch of a register-resident FMA chain kernel (blocks x 256 threads, 64 FMAs per
  * thread and iteration) on the library stream and returns the floating-point operations it executes (2 per FMA), or a
  * negative error code. mode 0 / 1: FP64 / FP32 chains with two constant-bank operands (pipe peak); 2 / 3: three

@@ -48,6 +48,7 @@ _SIGNATURES = {
     "trex_run_host": (_int, [_vp, _vp, _i64, _int, _dp, _dp, _vp, _vp, _vp, _vp]),
     "trex_debug_flow_amps": (_int, [_int, _dp, _dp, _dp]),
     "trex_debug_xtile": (_int, [_int, _dp, _dp, _dp, _dp]),
+    "trex_debug_helicity_me2": (_int, [_int, _dp, _dp, _dp, _dp]),
     "trex_probe_fma": (ctypes.c_double, [_int, _int, _int]),
     "trex_xsec_moments": (_int, [_vp, _vp, ctypes.c_int64, _vp]),
     "trex_xsec_moments_noalloc": (_int, [_vp, _vp, ctypes.c_int64, _vp]),
@@ -490,6 +491,19 @@ def trex_debug_flow_amps(subproc_id, momenta_one, theta):
     out = np.empty((nh, nc, 2, 2))
     _check(lib().trex_debug_flow_amps(subproc_id, m.ctypes.data_as(_dp), pth, out.ctypes.data_as(_dp)), "trex_debug_flow_amps")
     return out[..., 0] + 1j * out[..., 1]
+
+
+def trex_debug_helicity_me2(subproc_id, momenta_one, theta_old, theta_new):
+    """Per-helicity |M_h|^2 of one event from the PRODUCTION quark-channel kernels: array [nhel, 2 (theta_old, theta_new)],
+    bit `leg` of h = helicity of that leg, couplings and average included."""
+    _torch()
+    npar, nh = trex_npar(subproc_id), trex_nhel(subproc_id)
+    m = np.ascontiguousarray(momenta_one, dtype=np.float64).reshape(npar, 4)
+    to, pto = _theta(theta_old)
+    tn, ptn = _theta(theta_new)
+    out = np.empty((nh, 2))
+    _check(lib().trex_debug_helicity_me2(subproc_id, m.ctypes.data_as(_dp), pto, ptn, out.ctypes.data_as(_dp)), "trex_debug_helicity_me2")
+    return out
 
 
 def trex_debug_xtile(subproc_id, momenta_one, theta_old, theta_new):

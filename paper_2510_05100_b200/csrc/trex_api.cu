@@ -33,7 +33,8 @@ namespace {
 __constant__ QLineLegs c_qlegs[TREX_NSUBPROC];
 __constant__ double c_qinvnavg[TREX_NSUBPROC];
 
-template <class R, class RC>
+// DBG: the instantiation trex_debug_helicity_me2 launches -- the same code with the per-helicity dump compiled in
+template <class R, class RC, bool DBG = false>
 __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightArgs a) {
   static_assert(WARPS == 8, "one allowed helicity unit per warp");
   __shared__ double pm[20][32];
@@ -165,7 +166,7 @@ __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightA
     const vec4<R> eg = get_vec(wf[4 + lg]), Jq = get_vec(cur[c]), Jq3 = get_vec(cur[2 + c * 2 + lg]), Jq4 = get_vec(cur[6 + c * 2 + lg]);
     const spinor<R> ubar_t = get_spinor(wf[6 + lt]);
     const spinor<R> vtb[2] = {get_spinor(wf[8]), get_spinor(wf[9])};
-    qq_close<R, RC>(eg, Kg, Jq, Kq, Jq3, Jq4, Ptot, ubar_t, vtb, pt, a.T, acc);
+    qq_close<R, RC>(eg, Kg, Jq, Kq, Jq3, Jq4, Ptot, ubar_t, vtb, pt, a.T, acc, (DBG && a.dbg && e == 0) ? a.dbg + warp * 4 : nullptr);
   }
   // fixed-order reduction over the 8 units (the light row spinors of phase A are dead: their slots carry the partial sums)
   double (*red)[8][32] = reinterpret_cast<double (*)[8][32]>(&wf[0][0][0]);
@@ -394,7 +395,8 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
   } else {
     // a family launch (trex_run) serves every quark-channel class: each class rounds its events up to whole blocks
     const unsigned gq = a.qfamily ? grid32 + (unsigned)TREX_NSUBPROC : grid32;
-    if (mode == 0) k_qq<double, double><<<gq, WARPS * 32, 0, c.stream>>>(a);
+    if (mode == 0 && a.dbg) k_qq<double, double, true><<<gq, WARPS * 32, 0, c.stream>>>(a);
+    else if (mode == 0) k_qq<double, double><<<gq, WARPS * 32, 0, c.stream>>>(a);
     else if (mode == 1) k_qq<double, float><<<gq, WARPS * 32, 0, c.stream>>>(a);
     else k_qq<float, float><<<gq, WARPS * 32, 0, c.stream>>>(a);
   }
@@ -890,6 +892,59 @@ extern "C" int trex_debug_xtile(int sid, const double* momenta_one, const double
         double* o = out + (((size_t)h * nc + s) * 2 + th) * 2;
         o[0] = dump[2 * src] * gsN[th]; o[1] = dump[2 * src + 1] * gsN[th];
       }
+  }
+  return 0;
+}
+
+// per-helicity |M_h|^2 of the quark-channel production kernels (k_qq, k_qq2): see include/rex_trex_diag.h
+extern "C" int trex_debug_helicity_me2(int sid, const double* momenta_one, const double* theta_old, const double* theta_new, double* out) {
+  Context& c = ctx();
+  const SubprocInfo* sp = subproc_info(sid);
+  if (!sp || !is_quark_channel(sid)) return fail(TREX_EUNKNOWN_SUBPROC, "trex_debug_helicity_me2: quark channels only");
+  if (!momenta_one || !theta_old || !theta_new || !out) return fail(TREX_EINVAL, "trex_debug_helicity_me2: null pointer");
+  if (c.precision != 0) return fail(TREX_EINVAL, "trex_debug_helicity_me2: fp64 mode only");
+  ThetaPair T;
+  if (!make_theta_pair(sid, theta_old, theta_new, T)) return fail(TREX_EINVAL, "trex_debug_helicity_me2: theta outside its domain");
+  const bool two = is_two_gluon_quark_channel(sid);
+  const size_t ndump = two ? 8 * 8 : 8 * 4;               // units x (lambda_t, lambda_tbar, theta) resp. (lambda_tbar, theta)
+  double *d_mom = nullptr, *d_w = nullptr, *d_dbg = nullptr;
+  TREX_CUDA_CHECK(cudaMalloc((void**)&d_mom, sizeof(double) * 4 * sp->npar));
+  TREX_CUDA_CHECK(cudaMalloc((void**)&d_w, sizeof(double) * 4));
+  TREX_CUDA_CHECK(cudaMalloc((void**)&d_dbg, sizeof(double) * ndump));
+  const double one[4] = {1.0, 0.0, 0.0, 0.0};
+  cudaMemcpyAsync(d_mom, momenta_one, sizeof(double) * 4 * sp->npar, cudaMemcpyHostToDevice, c.stream);
+  cudaMemcpyAsync(d_w, one, sizeof one, cudaMemcpyHostToDevice, c.stream);
+  cudaMemsetAsync(d_dbg, 0, sizeof(double) * ndump, c.stream);
+  c.dbg_out = d_dbg;
+  ReweightArgs a;
+  a.io = EvIO{d_mom, 1, 1, d_w, d_w + 1, d_w + 2, d_w + 3};
+  a.alt = a.io; a.plan = nullptr; a.qfamily = 0;
+  const int rc = launch_reweight(sid, a, 1, T);
+  c.dbg_out = nullptr;
+  std::vector<double> dump(ndump);
+  cudaError_t e1 = cudaMemcpyAsync(dump.data(), d_dbg, sizeof(double) * ndump, cudaMemcpyDeviceToHost, c.stream);
+  cudaError_t e2 = cudaStreamSynchronize(c.stream);
+  cudaFree(d_mom); cudaFree(d_w); cudaFree(d_dbg);
+  if (rc < 0) return rc;
+  TREX_CUDA_CHECK(e1); TREX_CUDA_CHECK(e2);
+  for (int i = 0; i < 2 * sp->nhel; ++i) out[i] = 0.0;
+  const QLineLegs L = sp->qlegs;
+  const bool row_in = L.lrow < 2, col_in = L.lcol < 2;
+  for (int u = 0; u < 8; ++u) {
+    // unit -> helicities: the light-line combination c fixes both ends (see k_qq / qq2_unit)
+    const int cc = two ? (u & 1) : ((u >> 2) & 1);
+    const bool row_upper = cc != 0, col_upper = !row_upper;
+    const int hrow = (row_in ? !row_upper : row_upper) ? 1 : 0, hcol = (col_in ? !col_upper : col_upper) ? 1 : 0;
+    for (int lt = 0; lt < 2; ++lt) {
+      if (!two && lt != ((u >> 1) & 1)) continue;
+      for (int iv = 0; iv < 2; ++iv) {
+        int h = (hrow << L.lrow) | (hcol << L.lcol) | (lt << 2) | (iv << 3);
+        size_t src;
+        if (two) { h |= (((u >> 1) & 1) << L.lg) | (((u >> 2) & 1) << L.lg2); src = (size_t)u * 8 + (lt * 2 + iv) * 2; }
+        else { h |= ((u & 1) << L.lg); src = (size_t)u * 4 + iv * 2; }
+        for (int th = 0; th < 2; ++th) out[2 * h + th] = dump[src + th] * T.gs2nv[th] / sp->navg;
+      }
+    }
   }
   return 0;
 }

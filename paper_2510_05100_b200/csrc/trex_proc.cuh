@@ -246,7 +246,7 @@ TREX_HD void two_source_line(const spinor<R>& ubar, const rvec4<double>& pt, con
 template <class R, class RC>
 TREX_HD void qq_close(const vec4<R>& eg, const rvec4<double>& Kg, const vec4<R>& Jq, const rvec4<double>& Kq, const vec4<R>& Jq3,
                       const vec4<R>& Jq4, const rvec4<double>& Ptot, const spinor<R>& ubar_t, const spinor<R> vtb[2],
-                      const rvec4<double>& pt, const ThetaPair& T, RC out[2]) {
+                      const rvec4<double>& pt, const ThetaPair& T, RC out[2], double* dbg = nullptr) {
   const spinor<R>* stv = vtb;
   // single-source brackets of K3, K4: ubar_t [ i Jslash + (kappa/g_s) 2 sigma(P ^ J) ]; they depend neither on theta nor on
   // the antitop helicity, so they are formed once
@@ -281,6 +281,7 @@ TREX_HD void qq_close(const vec4<R>& eg, const rvec4<double>& Kg, const vec4<R>&
       RC d = RC(12) * (norm2(J[0]) + norm2(J[1]) + norm2(J[2]) + norm2(J[3]));
       cx<RC> a = J[0] + J[1], b = J[2] + J[3];
       d += RC(8) * (a.re * b.re + a.im * b.im);
+      if (dbg) dbg[iv * 2 + th] = (double)d;                // diagnostics only (trex_debug_helicity_me2)
       s += d;
     }
     res[th] = s;

@@ -316,7 +316,8 @@ TREX_HD void qq2_flows(const Qq2Ext<R>& X, const spinor<R>& ubar_t, const spinor
 // sum over the top helicity (and both antitop helicities) of x^dagger C x at theta_old and theta_new for one choice of the
 // light-line combination c and the gluon helicities; pm = momenta of the event [leg][mu]; fl = this thread's flow storage
 template <class R, class RC>
-TREX_HD void qq2_unit(const double (*pm)[4], const QLineLegs& L, int c, int la, int lb, const ThetaPair& T, const Qq2Acc<R>& fl, RC out[2]) {
+TREX_HD void qq2_unit(const double (*pm)[4], const QLineLegs& L, int c, int la, int lb, const ThetaPair& T, const Qq2Acc<R>& fl, RC out[2],
+                      double* dbg = nullptr) {
   const bool row_in = L.lrow < 2, col_in = L.lcol < 2;
   // row spinor in the upper block for c = 1 (see k_qq)
   const bool row_upper = c != 0, col_upper = !row_upper;
@@ -360,7 +361,9 @@ TREX_HD void qq2_unit(const double (*pm)[4], const QLineLegs& L, int c, int la, 
           cfma(a, fl.get(f, 1, iv), kq);
           xf[f] = cx<RC>(RC(a.re), RC(a.im));
         }
-        acc[th] += colour_quadform<RC, QQ2_NFLOW, 1>(xf, nullptr);
+        const RC q = colour_quadform<RC, QQ2_NFLOW, 1>(xf, nullptr);
+        if (dbg) dbg[(lt * 2 + iv) * 2 + th] = (double)q;     // diagnostics only (trex_debug_helicity_me2)
+        acc[th] += q;
       }
     }
   }

@@ -21,7 +21,8 @@ __constant__ double c_q2invnavg[TREX_NSUBPROC];      // 1 / N_avg; 0 for ids tha
 constexpr int Q2_WARPS = 4, Q2_TB = Q2_WARPS * 32;
 template <class R> constexpr size_t q2_smem() { return sizeof(R) * Qq2Acc<R>::NEL * Q2_TB; }
 
-template <class R, class RC>
+// DBG: the instantiation trex_debug_helicity_me2 launches -- the same code with the per-helicity dump compiled in
+template <class R, class RC, bool DBG = false>
 __global__ void __launch_bounds__(Q2_TB, TREX_QQ2_MINB) k_qq2(const ReweightArgs a) {
   extern __shared__ __align__(16) unsigned char q2_raw[];
   __shared__ double red[2][Q2_WARPS][32];
@@ -53,7 +54,7 @@ __global__ void __launch_bounds__(Q2_TB, TREX_QQ2_MINB) k_qq2(const ReweightArgs
   for (int half = 0; half < 2; ++half) {
     const int u = warp + Q2_WARPS * half;                    // (c, lambda_a, lambda_b)
     RC o[2];
-    qq2_unit<R, RC>(pm, c_q2legs[sid], u & 1, (u >> 1) & 1, (u >> 2) & 1, a.T, fl, o);
+    qq2_unit<R, RC>(pm, c_q2legs[sid], u & 1, (u >> 1) & 1, (u >> 2) & 1, a.T, fl, o, (DBG && a.dbg && e == 0) ? a.dbg + u * 8 : nullptr);
     acc[0] += o[0]; acc[1] += o[1];
   }
   red[0][warp][lane] = (double)acc[0]; red[1][warp][lane] = (double)acc[1];
@@ -83,12 +84,14 @@ int trex_tu_qq2_launch(const ReweightArgs& a, int mode, unsigned grid, cudaStrea
   static bool ready = false;
   if (!ready) {
     if (cudaFuncSetAttribute(k_qq2<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)q2_smem<double>()) != cudaSuccess ||
+        cudaFuncSetAttribute(k_qq2<double, double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)q2_smem<double>()) != cudaSuccess ||
         cudaFuncSetAttribute(k_qq2<double, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)q2_smem<double>()) != cudaSuccess ||
         cudaFuncSetAttribute(k_qq2<float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)q2_smem<float>()) != cudaSuccess)
       return 1;
     ready = true;
   }
-  if (mode == 0) k_qq2<double, double><<<grid, Q2_TB, q2_smem<double>(), stream>>>(a);
+  if (mode == 0 && a.dbg) k_qq2<double, double, true><<<grid, Q2_TB, q2_smem<double>(), stream>>>(a);
+  else if (mode == 0) k_qq2<double, double><<<grid, Q2_TB, q2_smem<double>(), stream>>>(a);
   else if (mode == 1) k_qq2<double, float><<<grid, Q2_TB, q2_smem<double>(), stream>>>(a);
   else k_qq2<float, float><<<grid, Q2_TB, q2_smem<float>(), stream>>>(a);
   return cudaGetLastError() == cudaSuccess ? 0 : 1;

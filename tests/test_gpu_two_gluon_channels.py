@@ -206,3 +206,34 @@ def test_cfg7_many_parameter_points(T):
         assert np.array_equal(direct[2][k].cpu().numpy(), one[2].cpu().numpy())
     poly = T.trex_run_multi(dk, dm, w.theta_old, thetas, dw)
     assert rel(poly[0].cpu().numpy(), direct[0].cpu().numpy()).max() < 1e-12
+
+
+@pytest.mark.parametrize("sid", [5, 7, 8, 21, 22, 23])
+def test_every_helicity_of_the_production_kernels_against_the_oracle(T, sid):
+    """Per-helicity parity (SURVEY.md I-4 for the quark channels): the colour-summed |M_h|^2 of EVERY helicity configuration
+    as the production kernels (k_qq, k_qq2) form it, before their helicity sum, against the oracle's explicit-colour
+    evaluation of that one helicity. Compensating errors between helicities cannot hide here; forbidden helicities of the
+    massless line must be exact zeros on both sides."""
+    npar = T.trex_npar(sid)
+    w = make_config(7 if npar == 6 else 3, n=64)
+    mom1 = np.ascontiguousarray(w.momenta[:, :, 11:12])
+    th0, th1 = default_theta(), default_theta()
+    th1[TH_CTG] = 1.4
+    got = T.trex_debug_helicity_me2(sid, mom1[:, :, 0], th0, th1)          # [nhel, 2]
+    nhel = 1 << npar
+    assert got.shape == (nhel, 2)
+    k = O.kappa(th1)
+    hs = range(nhel) if npar == 5 else list(range(0, nhel, 3)) + [1, 2, 62]      # E2 at 6 legs: 0.4 s per helicity
+    nz = 0
+    for h in hs:
+        abd = O.abd(sid, mom1, th0, engine=2, hel_only=h)[0]
+        want = np.array([abd[0], abd[0] + k * abd[1] + k * k * abd[2]])
+        if abd[0] == 0.0:
+            assert np.all(got[h] == 0.0), (sid, bin(h), got[h])
+        else:
+            nz += 1
+            assert rel(got[h], want).max() < RTOL64, (sid, bin(h), got[h], want)
+    assert nz >= len(list(hs)) // 3
+    # and the helicity sum is what the kernel returns
+    r = T.trex_reweight(sid, dev(mom1), th0, th1, dev(np.ones(1)))
+    assert rel(got[:, 0].sum(), r[1].cpu().numpy()[0]) < 1e-13 and rel(got[:, 1].sum(), r[2].cpu().numpy()[0]) < 1e-13
