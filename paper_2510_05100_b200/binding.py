@@ -57,6 +57,7 @@ _SIGNATURES = {
     "trex_set_precision": (_int, [_int]),
     "trex_get_precision": (_int, []),
     "trex_set_poly_multi": (_int, [_int]),
+    "trex_set_helicity_symmetry": (_int, [_int]),
     "trex_set_algorithm": (_int, [_int]),
     "trex_launch_count": (ctypes.c_int64, []),
     "trex_graph_replays": (ctypes.c_int64, []),
@@ -189,6 +190,10 @@ def trex_set_precision(mode):
 
 def trex_set_algorithm(algo):
     return _check(lib().trex_set_algorithm(int(algo)), "trex_set_algorithm")
+
+
+def trex_set_helicity_symmetry(on):
+    return _check(lib().trex_set_helicity_symmetry(int(bool(on))), "trex_set_helicity_symmetry")
 
 
 def trex_set_poly_multi(on):

@@ -365,6 +365,8 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
   if (int rc = ensure_colour()) return rc;
   a.T = T; a.sid = sid; a.q = sp->qlegs; a.C120 = c.C120; a.dbg = c.dbg_out;
   if (!a.plan || !is_quark_channel(sid)) a.qfamily = 0;
+  // parity: |M_{-h}|^2 = |M_h|^2 when no propagator carries a width (R-20); the diagnostics dump every helicity
+  a.hsym = (c.hel_sym && !c.dbg_out && sid != TREX_SP_EEMUMU && T.mGt[0] == 0.0 && T.mGt[1] == 0.0) ? 1 : 0;
   const unsigned grid32 = (unsigned)((nmax + 31) / 32);
   const int mode = c.precision;
   cudaEvent_t kt[2] = {nullptr, nullptr};
@@ -507,7 +509,7 @@ static int run_core(const uint64_t* pdg_keys, const double* momenta_soa, int64_t
   // of a streamed sample) replays it as one CUDA graph
   Context::RunKey key{};
   key.ptr[0] = pdg_keys; key.ptr[1] = momenta_soa; key.ptr[2] = w_in; key.ptr[3] = w_out; key.ptr[4] = me2_old; key.ptr[5] = me2_new;
-  key.n = n; key.ld = ld; key.npar = npar; key.precision = c.precision; key.table_min_n = c.table_min_n;
+  key.n = n; key.ld = ld; key.npar = npar; key.precision = c.precision; key.table_min_n = c.table_min_n; key.hel_sym = c.hel_sym ? 1 : 0;
   std::memcpy(key.th, theta_old, sizeof(double) * TREX_NTHETA);
   std::memcpy(key.th + TREX_NTHETA, theta_new, sizeof(double) * TREX_NTHETA);
   int64_t offsets[REX_MAX_BUCKETS + 1];
@@ -956,6 +958,7 @@ extern "C" int trex_set_precision(int mode) {
 }
 extern "C" int trex_get_precision(void) { return ctx().precision; }
 extern "C" int trex_set_poly_multi(int on) { ctx().poly_multi = on != 0; return 0; }
+extern "C" int trex_set_helicity_symmetry(int on) { ctx().hel_sym = on != 0; return 0; }
 extern "C" int trex_set_algorithm(int algo) {
   if (algo != 0 && (algo < 3 || algo > 5)) return fail(TREX_EINVAL, "trex_set_algorithm: algo must be 0, 3, 4 or 5");
   ctx().table_min_n = algo == 0 ? 99 : algo; return 0;

@@ -46,10 +46,11 @@ struct Context {
   void* probe_out = nullptr;
   void* poly_tmp = nullptr; size_t poly_tmp_bytes = 0;   // trex_run_multi: |M|^2 at three kappa values + the u_k
   bool poly_multi = true;
+  bool hel_sym = true;               // trex_set_helicity_symmetry
   void* xsec_scratch = nullptr; void* xsec_host = nullptr;   // trex_xsec_moments: block partials (device), result (pinned)
   // trex_run replayed as a CUDA graph when it is called again with the same buffers, sizes and parameter points
   struct RunKey {
-    const void* ptr[6]; int64_t n, ld; int npar, precision, table_min_n; double th[2 * TREX_NTHETA];
+    const void* ptr[6]; int64_t n, ld; int npar, precision, table_min_n, hel_sym; double th[2 * TREX_NTHETA];
   };
   bool in_host_run = false;
   // trex_run_alphas: its three passes run the path at g_s = 1 with this kappa / g_s at both parameter points

@@ -50,9 +50,11 @@ __global__ void __launch_bounds__(Q2_TB, TREX_QQ2_MINB) k_qq2(const ReweightArgs
     for (int mu = 0; mu < 4; ++mu) pm[l][mu] = io.mom[(long)(l * 4 + mu) * io.ld + ev];
   const Qq2Acc<R> fl{reinterpret_cast<R*>(q2_raw) + threadIdx.x, Q2_TB};
   RC acc[2] = {RC(0), RC(0)};
+  // helicity symmetry (a.hsym): the four choices with light-line combination c = 0 stand for their parity partners
+  const int nhalf = (a.hsym && !DBG) ? 1 : 2;
 #pragma unroll 1
-  for (int half = 0; half < 2; ++half) {
-    const int u = warp + Q2_WARPS * half;                    // (c, lambda_a, lambda_b)
+  for (int half = 0; half < nhalf; ++half) {
+    const int u = nhalf == 1 ? 2 * warp : warp + Q2_WARPS * half;        // (c, lambda_a, lambda_b)
     RC o[2];
     qq2_unit<R, RC>(pm, c_q2legs[sid], u & 1, (u >> 1) & 1, (u >> 2) & 1, a.T, fl, o, (DBG && a.dbg && e == 0) ? a.dbg + u * 8 : nullptr);
     acc[0] += o[0]; acc[1] += o[1];
@@ -63,7 +65,8 @@ __global__ void __launch_bounds__(Q2_TB, TREX_QQ2_MINB) k_qq2(const ReweightArgs
     double s0 = 0.0, s1 = 0.0;
 #pragma unroll
     for (int w = 0; w < Q2_WARPS; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
-    const double mo = s0 * (a.T.gs2nv[0] * c_q2invnavg[sid]), mn = s1 * (a.T.gs2nv[1] * c_q2invnavg[sid]);
+    const double hs = nhalf == 1 ? 2.0 : 1.0;
+    const double mo = s0 * (a.T.gs2nv[0] * c_q2invnavg[sid] * hs), mn = s1 * (a.T.gs2nv[1] * c_q2invnavg[sid] * hs);
     const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
     io.w_out[e] = io.w_in[e] * norm * mn;                      // evaluate + append_wgts
     if (io.me2_old) io.me2_old[e] = mo;

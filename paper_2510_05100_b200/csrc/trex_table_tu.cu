@@ -419,7 +419,10 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
     rvec4<double> ptop;
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) ptop.c[mu] = pm[2 * 4 + mu];
-    for (unsigned itb = 0; itb < (unsigned)G::NIT; ++itb) {
+    // helicity symmetry (a.hsym): the iterations with the last fixed gluon at helicity - stand for their parity partners
+    const unsigned nit = (a.hsym && G::NIT >= 2 && !(a.dbg)) ? (unsigned)G::NIT / 2 : (unsigned)G::NIT;
+    const double hscale = nit < (unsigned)G::NIT ? 2.0 : 1.0;
+    for (unsigned itb = 0; itb < nit; ++itb) {
       // ---- phase 1: current table of this helicity iteration (+ line states of short prefixes, if tabulated)
       for (int e1 = gtid; e1 < meta[I::M_LVL + 2]; e1 += GS) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
       group_sync<GS>();
@@ -482,7 +485,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
       for (int o = 16; o >= 2; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
       const double s1 = __shfl_sync(0xFFFFFFFFu, v, 1);
       if (gtid == 0) {
-        const double mo = v * a.T.pref[0], mn = s1 * a.T.pref[1];
+        const double mo = v * (a.T.pref[0] * hscale), mn = s1 * (a.T.pref[1] * hscale);
         const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
         io.w_out[e] = io.w_in[e] * norm * mn;                        // evaluate + append_wgts
         if (io.me2_old) io.me2_old[e] = mo;
