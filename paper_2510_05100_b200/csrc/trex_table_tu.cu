@@ -225,7 +225,8 @@ __device__ __forceinline__ void build_levels(unsigned char* sb, const int* meta,
 // ---- phase 3 of k_table: x^dagger C x of every X column added into the event's partial-sum slots
 template <class R, class RC, int N>
 // ncw > 0 (tensor-core form only): the first ncw warps of the group share the column blocks, the others do not take part
-__device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, const RC* __restrict__ Cs, double* __restrict__ part, int tid, int gtid, int ncw = 0) {
+__device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, const RC* __restrict__ Cs, double* __restrict__ part, int tid, int gtid, int ncw = 0,
+                                             bool half_lt = false) {
   using G = TabGeom<R, RC, N>;
   using F = FoldedC<G::NC>;
   constexpr int XS = G::XS, GS = G::GS;
@@ -311,8 +312,11 @@ __device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, cons
     }
     part[tid] += (double)accl * (1.0 / G::TF32_DEN);        // slot parity = lane parity = column parity = theta
   } else
-  for (int item = gtid; item < G::NCI0; item += GS) {
-    const int c = item % G::NCOLT, p = item / G::NCOLT;
+  // half_lt (FMA form only): the columns of lambda_t = + [bit 2 of the column index] are not in use (helicity symmetry)
+  for (int item = gtid; item < (half_lt ? G::NCI0 / 2 : G::NCI0); item += GS) {
+    const int ncolt = half_lt ? G::NCOLT / 2 : G::NCOLT;
+    const int cc = item % ncolt, p = item / ncolt;
+    const int c = half_lt ? (((cc >> 2) << 3) | (cc & 3)) : cc;
     RC accl = RC(0);
     for (int side = 0; side < 2; ++side) {
       const int b = side == 0 ? p : NB - 1 - p;
@@ -360,6 +364,10 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
   for (int i = tid; i < I::M_SIZE; i += TB) meta[i] = gmeta[i];
   for (int i = tid; i < G::CN; i += TB) Cs[i] = RC(Cfold[i]);
   for (int i = gtid; i < G::NCI; i += GS) part[i] = 0.0;
+  // helicity symmetry (a.hsym, R-20) without a helicity loop to halve (N = 3): the walk tasks with lambda_t = -
+  // stand for their parity partners; the X columns of lambda_t = + are neither written nor read
+  constexpr bool HS_LT = G::NIT == 1 && G::NLT == 1 && !G::DMMA && !G::TF32;
+  const bool hs_lt = HS_LT && a.hsym && !a.dbg;
   __syncthreads();
 
 #ifdef TREX_PHASE_CLOCKS
@@ -421,7 +429,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
     for (int mu = 0; mu < 4; ++mu) ptop.c[mu] = pm[2 * 4 + mu];
     // helicity symmetry (a.hsym): the iterations with the last fixed gluon at helicity - stand for their parity partners
     const unsigned nit = (a.hsym && G::NIT >= 2 && !(a.dbg)) ? (unsigned)G::NIT / 2 : (unsigned)G::NIT;
-    const double hscale = nit < (unsigned)G::NIT ? 2.0 : 1.0;
+    const double hscale = (nit < (unsigned)G::NIT || hs_lt) ? 2.0 : 1.0;
     for (unsigned itb = 0; itb < nit; ++itb) {
       // ---- phase 1: current table of this helicity iteration (+ line states of short prefixes, if tabulated)
       for (int e1 = gtid; e1 < meta[I::M_LVL + 2]; e1 += GS) tab_build_level1<R, N, NFIX>(tab, meta, pset, eps_all, itb, e1);
@@ -431,9 +439,10 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
 
       for (int lti = 0; lti < G::NLT; ++lti) {
       // ---- phase 2: top-line walk
-      for (int task = gtid; task < G::NTASK * NPASS; task += GS) {
-        const int pass = task / G::NTASK, r = task - pass * G::NTASK;
-        const int hli = r % G::NHL, prank = r / G::NHL;
+      const int nhl = hs_lt ? G::NHL / 2 : G::NHL, ntask = G::NPREF * nhl;
+      for (int task = gtid; task < ntask * NPASS; task += GS) {
+        const int pass = task / ntask, r = task - pass * ntask;
+        const int hli = hs_lt ? 2 * (r % nhl) : r % nhl, prank = r / nhl;
         const int hl = G::NLT == 2 ? hli * 2 + lti : hli;
         using Store = TabLeafStore<R, RC, XS>;
         Store st;
@@ -464,7 +473,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
           d[0] = (double)x.re; d[1] = (double)x.im;
         }
 
-      colour_phase<R, RC, N>(xs, Cs, part, tid, gtid);
+      colour_phase<R, RC, N>(xs, Cs, part, tid, gtid, 0, hs_lt);
 #ifdef TREX_PHASE_CLOCKS
       group_sync<GS>();
       PHASE_TICK(3);
