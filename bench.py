@@ -50,7 +50,7 @@ def headline_config():
 def load_flops():
     """Algorithmic FP64 work per reweighted event of the |M|^2 kernels: thread-level DFMA/DMUL/DADD counted by ncu
     (DFMA = 2 flop) on the committed kernels / events of the launch (profiles/flops_per_event.json)."""
-    out = {"flops": {}, "tensor": {}, "traffic": {}, "oracle": {}}
+    out = {"flops": {}, "tensor": {}, "traffic": {}, "oracle": {}, "flops_hsym": {}, "tensor_hsym": {}}
     path = os.path.join(ROOT, "profiles", "flops_per_event.json")
     if os.path.exists(path):
         with open(path) as fh:
@@ -60,6 +60,9 @@ def load_flops():
                 out["flops"][int(k)] = v
         out["tensor"] = {int(k): v for k, v in d.get("tensor_flop_per_event", {}).items()}
         out["traffic"] = {int(k): v for k, v in d.get("traffic_bytes", {}).items()}
+        hs = d.get("helicity_symmetry", {})
+        out["flops_hsym"] = {int(k): v for k, v in hs.items() if k.isdigit()}
+        out["tensor_hsym"] = {int(k): v for k, v in hs.get("tensor_flop_per_event", {}).items()}
     opath = os.path.join(ROOT, "profiles", "oracle_flops_per_event.json")
     if os.path.exists(opath):
         with open(opath) as fh:
@@ -249,31 +252,34 @@ def main():
         barrier()
         return max_over_ranks([s.elapsed_time(e) for s, e in evs])
 
-    def roofline_of(cfg, n, kernel_ms, fp64_peak, dmma_peak):
+    def roofline_of(cfg, n, kernel_ms, fp64_peak, dmma_peak, hsym=True):
         """Executed FP64 flop of the |M|^2 kernel(s) of one step / their live CUDA-event duration, against the FP64 vector
         pipe peak measured in this run; tensor-pipe (DMMA) work is reported against its own peak, never summed in."""
-        fpe = F["flops"].get(cfg)
+        # with the helicity symmetry in use (library default; cfg 3, 5, 6, 7 have Gamma_t = 0) the kernels execute fewer operations
+        fpe = (F["flops_hsym"].get(cfg) if hsym else None) or F["flops"].get(cfg)
         if not fpe or not kernel_ms:
             return None
         ach = fpe * n / (kernel_ms * 1e-3) / 1e12
         r = {"bound": "alu", "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s", "frac": ach / fp64_peak,
              "traffic": F["traffic"].get(cfg), "kernel": KERNEL_OF_CFG[cfg], "kernel_ms": kernel_ms, "flop_per_event": fpe,
              "frac_of_nominal": ach / FP64_NOMINAL_TFLOPS}
-        tfe = F["tensor"].get(cfg)
+        tfe = (F["tensor_hsym"].get(cfg) if hsym else None) or F["tensor"].get(cfg)
         if tfe:
             tach = tfe * n / (kernel_ms * 1e-3) / 1e12
             r["tensor_pipe"] = {"achieved": tach, "peak": dmma_peak, "frac": tach / dmma_peak if dmma_peak else None,
                                 "flop_per_event": tfe, "note": "mma.sync.m8n8k4.f64 colour sum, separate pipe: not part of `achieved`"}
         return r
 
-    def measure(cfg, warm, steps, precision=0, with_e2e=False, kernel_in_region=False):
+    def measure(cfg, warm, steps, precision=0, with_e2e=False, kernel_in_region=False, hsym=True):
         """One config: whole-path step time (trex_run), the |M|^2 kernels' own time (CUDA events recorded by the library
         around every |M|^2 launch on its stream) and optionally the end-to-end number with host buffers."""
         w = make_config(cfg)
         keys, mom, win = dev(w.keys), dev(w.momenta), dev(w.w_in)
         wout = torch.empty_like(win)
         T.trex_set_precision(precision)
-        res = {"workload": w.name, "events": w.n, "steps": steps, "warmup": warm}
+        T.trex_set_helicity_symmetry(hsym)
+        res = {"workload": w.name, "events": w.n, "steps": steps, "warmup": warm,
+               "helicity_symmetry": bool(hsym and w.theta_old[6] == 0.0 and w.theta_new[6] == 0.0 and cfg in (3, 5, 6, 7))}
         run = lambda: T.trex_run(keys, mom, w.theta_old, w.theta_new, win, w_out=wout, want_me2=False)  # noqa: E731
         if kernel_in_region:
             # the kernel is timed inside the timed region itself (the chain is launched directly, not as a graph replay:
@@ -318,6 +324,7 @@ def main():
                           "d2h_bytes_per_step": int(ho.numel() * 8), "ms_median": float(np.median(ems)), "ms_min": float(min(ems))}
             assert bool(torch.isfinite(ho).all())
         T.trex_set_precision(0)
+        T.trex_set_helicity_symmetry(True)
         del keys, mom, win, wout
         return res
 
@@ -394,6 +401,9 @@ def main():
     if args.configs == "all":
         for cfg, warm, steps in ((1, 3, 20), (2, 3, 20), (3, 3, 10), (5, 3, 10), (6, 3, 10), (7, 3, 10)):
             configs["cfg%d" % cfg] = measure(cfg, warm, steps, with_e2e=(cfg != 1))
+        # the same samples with every helicity configuration evaluated (trex_set_helicity_symmetry(0)): the round-1 arithmetic
+        for cfg, warm, steps in ((3, 3, 10), (5, 3, 10), (7, 3, 10)):
+            configs["cfg%d_all_helicities" % cfg] = measure(cfg, warm, steps, hsym=False)
         configs["cfg4_mixed"] = measure(4, 3, 10, precision=1)
         configs["cfg4_fp32"] = measure(4, 3, 10, precision=2)
         configs["cfg3_multi8_direct"] = measure_multi(3, 8, False, 2, 5)
@@ -402,6 +412,8 @@ def main():
         for name, r in configs.items():
             if name[3:].isdigit():
                 r["roofline"] = roofline_of(int(name[3:]), r["events"], r.get("kernel_ms"), fp64_peak, dmma_peak)
+            elif name.endswith("_all_helicities"):
+                r["roofline"] = roofline_of(int(name[3]), r["events"], r.get("kernel_ms"), fp64_peak, dmma_peak, hsym=False)
     strong = measure_strong(HEADLINE_CFG, W, max(3, K // 2)) if world > 1 else None
 
     cpu = None
