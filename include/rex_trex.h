@@ -172,7 +172,8 @@ int trex_run_multi(const uint64_t* pdg_keys, const double* momenta_soa, int64_t 
  *   |M(theta; alpha_s)|^2 = g_s^(2 nv) [ a + (kappa / g_s) b + (kappa / g_s)^2 d ]
  * with a, b, d free of alpha_s: they are obtained per event and parameter point from three passes of the unchanged
  * |M|^2 kernels at g_s = 1 (kappa / g_s = 0, +delta, -delta: the quadratic is exact), and one elementwise kernel applies
- * the event's g_s. Cost: 1.5 x trex_run. e- e+ > mu- mu+ events do not depend on alpha_s and come out as from trex_run.
+ * the event's g_s. Cost: three trex_run passes; when top mass and width agree at the two parameter points a, b, d are
+ * common to both and two passes suffice (the two slots of a pass carry different kappa / g_s). e- e+ > mu- mu+ events do not depend on alpha_s and come out as from trex_run.
  * An event with alpha_s = 0 has |M|^2 = 0 and weight 0 (zero guard); negative or non-finite alpha_s
  * gives NaN for that event only. Returns the number of buckets. */
 int trex_run_alphas(const uint64_t* pdg_keys, const double* momenta_soa, int64_t n, int npar, const double* theta_old,

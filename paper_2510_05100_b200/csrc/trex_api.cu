@@ -472,11 +472,11 @@ static int run_core(const uint64_t* pdg_keys, const double* momenta_soa, int64_t
   for (int sid = 0; sid < TREX_NSUBPROC; ++sid)
     if (npar_of_sid(sid) == npar && !make_theta_pair(sid, theta_old, theta_new, T[sid]))
       return fail(TREX_EINVAL, "trex_run: theta outside its domain");
-  if (c.unit_gs)                                      // a pass of trex_run_alphas: g_s = 1, the same kappa / g_s at both points
+  if (c.unit_gs)                                      // a pass of trex_run_alphas: g_s = 1, prescribed kappa / g_s per slot
     for (int sid = 0; sid < TREX_NSUBPROC; ++sid) {
       const SubprocInfo* sp = subproc_info(sid);
       if (!sp || sp->npar != npar || sid == TREX_SP_EEMUMU) continue;
-      for (int k = 0; k < 2; ++k) { T[sid].kq[k] = c.unit_gs_kq; T[sid].gs2nv[k] = 1.0; T[sid].pref[k] = 1.0 / sp->navg; }
+      for (int k = 0; k < 2; ++k) { T[sid].kq[k] = c.unit_gs_kq[k]; T[sid].gs2nv[k] = 1.0; T[sid].pref[k] = 1.0 / sp->navg; }
     }
   if (int rc = ensure_plan()) return rc;
   if (int rc = ensure_colour()) return rc;
@@ -554,7 +554,7 @@ static int run_core(const uint64_t* pdg_keys, const double* momenta_soa, int64_t
 // |M|^2 = g_s^(2 nv) [a + x b + x^2 d], x = kappa / g_s, from its values m0, mp, mm at x = 0, +delta, -delta and g_s = 1
 __global__ void __launch_bounds__(256) k_alphas_weights(const unsigned long long* __restrict__ keys, unsigned long long eemumu_key, int nv,
                                                         const double* __restrict__ alpha_s, const double* __restrict__ m /* [2][3][n] */,
-                                                        long n, double xo, double xn, const double* __restrict__ w_in,
+                                                        int shared, long n, double xo, double xn, const double* __restrict__ w_in,
                                                         double* __restrict__ w_out, double* __restrict__ me2_old, double* __restrict__ me2_new) {
   const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -563,8 +563,11 @@ __global__ void __launch_bounds__(256) k_alphas_weights(const unsigned long long
   const double gs = sqrt(4.0 * 3.14159265358979323846 * alpha_s[i]);
 #pragma unroll
   for (int p = 0; p < 2; ++p) {
-    const double m0 = m[(size_t)(3 * p) * n + i], mp = m[(size_t)(3 * p + 1) * n + i], mm = m[(size_t)(3 * p + 2) * n + i];
-    if (!qcd) { res[p] = m0; continue; }
+    // shared: top mass and width agree at the two points, so a, b, d do; rows 0, 1, 2 = x = 0 (theta_old slot), +delta
+    // (theta_new slot), -delta. For e- e+ > mu- mu+ the two slots of the first pass are the two answers.
+    const int r0 = shared ? 0 : 3 * p;
+    const double m0 = m[(size_t)r0 * n + i], mp = m[(size_t)(r0 + 1) * n + i], mm = m[(size_t)(r0 + 2) * n + i];
+    if (!qcd) { res[p] = shared ? (p == 0 ? m0 : mp) : m0; continue; }
     const double b = 0.5 * (mp - mm), d = 0.5 * (mp + mm) - m0;
     const double u = (p == 0 ? xo : xn) / gs;                 // (kappa / g_s) / delta
     double g2 = 1.0;
@@ -598,18 +601,31 @@ extern "C" int trex_run_alphas(const uint64_t* pdg_keys, const double* momenta_s
   std::memcpy(tho, theta_old, sizeof tho); std::memcpy(thn, theta_new, sizeof thn);
   tho[TREX_TH_ALPHA_S] = thn[TREX_TH_ALPHA_S] = 1.0;
   int rc = 0, nb = 0;
+  // top mass and width equal at the two points (the usual case: only couplings move): a, b, d are common to both, and the
+  // two slots of a pass can carry different x -- two passes (x = 0 | +delta, then -delta) instead of three
+  const bool shared = theta_old[TREX_TH_MT] == theta_new[TREX_TH_MT] && theta_old[TREX_TH_GAMMAT] == theta_new[TREX_TH_GAMMAT];
   c.unit_gs = true; c.in_host_run = true;             // no graph replay: the key does not know about unit_gs_kq
-  for (int s = 0; s < 3 && rc >= 0; ++s) {
-    c.unit_gs_kq = s == 0 ? 0.0 : (s == 1 ? delta : -delta);
-    rc = run_core(pdg_keys, momenta_soa, n, n, npar, tho, thn, w_in, w_out, m + (size_t)s * n, m + (size_t)(3 + s) * n);
-    if (rc >= 0) nb = rc;
+  if (shared) {
+    c.unit_gs_kq[0] = 0.0; c.unit_gs_kq[1] = delta;
+    rc = run_core(pdg_keys, momenta_soa, n, n, npar, tho, thn, w_in, w_out, m, m + (size_t)n);
+    if (rc >= 0) {
+      nb = rc;
+      c.unit_gs_kq[0] = c.unit_gs_kq[1] = -delta;
+      rc = run_core(pdg_keys, momenta_soa, n, n, npar, tho, thn, w_in, w_out, m + 2 * (size_t)n, nullptr);
+    }
+  } else {
+    for (int s = 0; s < 3 && rc >= 0; ++s) {
+      c.unit_gs_kq[0] = c.unit_gs_kq[1] = s == 0 ? 0.0 : (s == 1 ? delta : -delta);
+      rc = run_core(pdg_keys, momenta_soa, n, n, npar, tho, thn, w_in, w_out, m + (size_t)s * n, m + (size_t)(3 + s) * n);
+      if (rc >= 0) nb = rc;
+    }
   }
   c.unit_gs = false; c.in_host_run = false;
   if (rc < 0) return rc;
   const SubprocInfo* ee = subproc_info(TREX_SP_EEMUMU);
   int8_t status[4] = {-1, -1, 1, 1};
   const unsigned long long eekey = rex_pack_key(ee->pdg, status, 4);
-  k_alphas_weights<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>((const unsigned long long*)pdg_keys, eekey, npar - 2, alpha_s, m, (long)n,
+  k_alphas_weights<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>((const unsigned long long*)pdg_keys, eekey, npar - 2, alpha_s, m, shared ? 1 : 0, (long)n,
                                                                       ko / delta, kn / delta, w_in, w_out, me2_old, me2_new);
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());

@@ -53,8 +53,8 @@ struct Context {
     const void* ptr[6]; int64_t n, ld; int npar, precision, table_min_n, hel_sym; double th[2 * TREX_NTHETA];
   };
   bool in_host_run = false;
-  // trex_run_alphas: its three passes run the path at g_s = 1 with this kappa / g_s at both parameter points
-  bool unit_gs = false; double unit_gs_kq = 0.0;
+  // trex_run_alphas: its passes run the path at g_s = 1 with these kappa / g_s in the theta_old / theta_new slots
+  bool unit_gs = false; double unit_gs_kq[2] = {0.0, 0.0};
   RunKey last_key{}; bool last_key_valid = false;
   RunKey exec_key{}; bool exec_valid = false; bool graphs_ok = true;
   cudaGraphExec_t run_exec = nullptr; int64_t exec_launches = 0; int64_t graph_replays = 0;
