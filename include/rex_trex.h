@@ -63,7 +63,10 @@ enum { TREX_SP_EEMUMU = 0,   /* e- e+ > mu- mu+   (photon + Z)          */
        /* one light line + TWO gluons (the multi-jet samples are dominated by such channels) */
        TREX_SP_UUX_TTGG = 21, TREX_SP_UG_TTUG = 22, TREX_SP_GUX_TTUXG = 23,   /* u u~ > t t~ g g, u g > t t~ u g, g u~ > t t~ u~ g */
        TREX_SP_DDX_TTGG = 24, TREX_SP_DG_TTDG = 25, TREX_SP_GDX_TTDXG = 26,   /* the same for d */
-       TREX_NSUBPROC = 27 };
+       TREX_SP_SSX_TTGG = 27, TREX_SP_SG_TTSG = 28, TREX_SP_GSX_TTSXG = 29,   /* s */
+       TREX_SP_CCX_TTGG = 30, TREX_SP_CG_TTCG = 31, TREX_SP_GCX_TTCXG = 32,   /* c */
+       TREX_SP_BBX_TTGG = 33, TREX_SP_BG_TTBG = 34, TREX_SP_GBX_TTBXG = 35,   /* b */
+       TREX_NSUBPROC = 36 };
 
 /* ---- flavour keys (PAPER.md:334 default comparator: unordered PDG codes of external legs, initial and final state
  * kept apart; Alg.1).

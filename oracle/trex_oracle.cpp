@@ -743,7 +743,7 @@ template <class R> ABD<R> e2_abd(const Event<R>& ev, const Params<R>& P, int kin
 inline int npar_of(int sid) {
   static const int t[10] = {4, 4, 5, 6, 7, 5, 5, 5, 5, 4};
   if (sid >= 0 && sid < 10) return t[sid];
-  if (sid >= 21 && sid <= 26) return 6;             // 21 u u~ > t t~ g g ; 22 u g > t t~ u g ; 23 g u~ > t t~ u~ g ; 24..26: d
+  if (sid >= 21 && sid <= 35) return 6;             // 21 u u~ > t t~ g g ; 22 u g > t t~ u g ; 23 g u~ > t t~ u~ g ; 24..35: d, s, c, b
   return (sid >= 10 && sid <= 20) ? 5 : -1; }
 inline int kind_of(int sid) {
   if (sid >= 21) return (sid - 21) % 3 == 0 ? K_QQB : ((sid - 21) % 3 == 1 ? K_QG : K_GQB);

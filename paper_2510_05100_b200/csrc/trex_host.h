@@ -49,7 +49,7 @@ inline const SubprocInfo* subproc_info(int sid) {
         /* g u~ > t t~ u~ g */ {6, 12, 64, 16, 4, 4.0 * 24.0, {21, -2, 6, -6, -2, 21}, {1, 4, 0, 5}},
     };
     sid = TREX_SP_UUX_TTGG;
-    for (int f : {2, 1})
+    for (int f : {2, 1, 3, 4, 5})
       for (int k = 0; k < 3; ++k) {
         tab[sid] = two[k];
         for (int i = 0; i < 6; ++i) if (tab[sid].pdg[i] == 2 || tab[sid].pdg[i] == -2) tab[sid].pdg[i] = tab[sid].pdg[i] > 0 ? f : -f;
@@ -61,7 +61,7 @@ inline const SubprocInfo* subproc_info(int sid) {
 }
 inline int npar_of_sid(int sid) { const SubprocInfo* sp = subproc_info(sid); return sp ? sp->npar : 0; }
 inline bool is_quark_channel(int sid) { return (sid >= TREX_SP_UUX_TTG && sid <= TREX_SP_GUX_TTUX) || (sid >= TREX_SP_SSX_TTG && sid < TREX_NSUBPROC); }
-inline bool is_two_gluon_quark_channel(int sid) { return sid >= TREX_SP_UUX_TTGG && sid <= TREX_SP_GDX_TTDXG; }
+inline bool is_two_gluon_quark_channel(int sid) { return sid >= TREX_SP_UUX_TTGG && sid <= TREX_SP_GBX_TTBXG; }
 
 // returns false if theta is unusable (negative couplings, non-positive scale)
 inline bool make_theta_pair(int sid, const double* th_old, const double* th_new, ThetaPair& T) {

@@ -134,7 +134,7 @@ def test_colour_matrix_of_the_two_gluon_channels(lib):
     F = np.array(flows)
     want = (F.conj() @ F.T).real
     assert np.allclose(C, want, rtol=0, atol=1e-12)
-    assert T.trex_ncolor(22) == 12 and T.trex_nhel(23) == 64 and T.trex_npar(26) == 6
+    assert T.trex_ncolor(22) == 12 and T.trex_nhel(23) == 64 and T.trex_npar(26) == 6 and T.trex_npar(35) == 6 and T.trex_npar(36) == -2
 
 
 def test_compute_calls_fail_loudly_without_gpu(lib):

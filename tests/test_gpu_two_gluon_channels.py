@@ -92,14 +92,15 @@ def test_flavour_of_the_light_line_is_a_label(T):
     th0, th1 = default_theta(), default_theta()
     th1[TH_CTG] = 1.1
     dm, dw = dev(mom), dev(np.ones(64))
-    for u, d in ((21, 24), (22, 25), (23, 26)):
+    for u in (21, 22, 23):
         a = T.trex_reweight(u, dm, th0, th1, dw)
-        b = T.trex_reweight(d, dm, th0, th1, dw)
-        for x, y in zip(a, b):
-            assert np.array_equal(x.cpu().numpy(), y.cpu().numpy())
+        for d in (u + 3, u + 6, u + 9, u + 12):               # d, s, c, b
+            b = T.trex_reweight(d, dm, th0, th1, dw)
+            for x, y in zip(a, b):
+                assert np.array_equal(x.cpu().numpy(), y.cpu().numpy())
     # the oracle agrees that it is a label (single helicity: the full sum takes minutes)
     m1 = np.ascontiguousarray(mom[:, :, :1])
-    for u, d in ((21, 24), (22, 25), (23, 26)):
+    for u, d in ((21, 24), (22, 31), (23, 35)):
         assert np.array_equal(O.abd(u, m1, th1, engine=2, hel_only=0b010110 if u == 21 else 0b010111 if u == 23 else 0b010011),
                               O.abd(d, m1, th1, engine=2, hel_only=0b010110 if u == 21 else 0b010111 if u == 23 else 0b010011))
 
@@ -186,6 +187,30 @@ def test_cfg7_events_in_arbitrary_parton_order(T):
     canon = np.ascontiguousarray(mom[rl[:, i], :, i].transpose(0, 2, 1))
     want = O.reweight(21, canon, w.theta_old, w.theta_new, w.w_in[i])[0]
     assert rel(wo[i], want).max() < RTOL64
+
+
+def test_all_fifteen_two_gluon_classes_through_the_whole_path(T):
+    """A 16-class sample (g g > t t~ g g + the fifteen one-light-line + two-gluon classes, all five flavours): ONE family launch
+    serves the fifteen; per-class results equal per-class trex_reweight calls, bucketing bit-exact."""
+    import torch
+    rng = np.random.default_rng(21)
+    w = make_config(7, n=9000)
+    classes = [sp for sp in SUBPROCESSES if sp.npar == 6]
+    assert len(classes) == 16
+    keys = np.array([sp.key for sp in classes], dtype=np.uint64)[rng.integers(0, 16, w.n)]
+    dk, dm, dw = dev(keys), dev(w.momenta), dev(w.w_in)
+    l0 = T.trex_launch_count()
+    w_out, mo, mn, nb = T.trex_run(dk, dm, w.theta_old, w.theta_new, dw)
+    torch.cuda.synchronize()
+    assert nb == 16 and T.trex_launch_count() - l0 <= 12
+    perm, off, _ = O.bucket(keys)
+    gperm, goff, _ = T.rex_bucket(dk)
+    assert np.array_equal(gperm.cpu().numpy(), perm) and np.array_equal(goff, off)
+    w_out = w_out.cpu().numpy()
+    for sp in classes:
+        sel = np.where(keys == sp.key)[0]
+        r = T.trex_reweight(sp.sid, dev(np.ascontiguousarray(w.momenta[:, :, sel])), w.theta_old, w.theta_new, dev(w.w_in[sel]))
+        assert np.array_equal(w_out[sel], r[0].cpu().numpy()), sp.name
 
 
 def test_cfg7_many_parameter_points(T):

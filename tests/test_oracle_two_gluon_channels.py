@@ -147,3 +147,15 @@ def test_collinear_limit_reproduces_the_one_gluon_channel(sid, parent_sid):
         ref = _sum_over(parent_sid, m5, th, fixed, [4])[:, 0]
         pred = sym * 8.0 * np.pi * th[0] / m45 ** 2 * split_fn * ref
         assert ref[0] > 0 and abs(acc[0] / pred[0] - 1.0) < tol, (sid, bin(fixed), acc / pred - 1)
+
+
+def test_flavour_labels_of_the_two_gluon_channels():
+    """ids 24..35 are ids 21, 22, 23 under another flavour label (d, s, c, b)."""
+    mom = _events(1)
+    th = default_theta()
+    th[7] = 0.5
+    for base, h in ((21, 0b010110), (22, 0b010011), (23, 0b010111)):
+        ref = O.abd(base, mom, th, engine=2, hel_only=h)
+        for k in (1, 2, 3, 4):
+            assert np.array_equal(O.abd(base + 3 * k, mom, th, engine=2, hel_only=h), ref)
+    assert O.lib().oracle_npar(35) == 6 and O.lib().oracle_npar(36) == -1

@@ -95,11 +95,11 @@ def _light_line_channels():
 
 
 def _two_gluon_channels():
-    """One light line + two gluons (ids 21..26): u u~ > t t~ g g, u g > t t~ u g, g u~ > t t~ u~ g and the
-    same three for d."""
-    name = {1: "d", 2: "u"}
+    """One light line + two gluons (ids 21..35): u u~ > t t~ g g, u g > t t~ u g, g u~ > t t~ u~ g and the
+    same three for d, s, c, b (labels only: QCD does not see the flavour of a massless quark)."""
+    name = {1: "d", 2: "u", 3: "s", 4: "c", 5: "b"}
     out, sid = [], 21
-    for f in (2, 1):
+    for f in (2, 1, 3, 4, 5):
         q = name[f]
         out.append(Subprocess(sid, "%s %s~ > t t~ g g" % (q, q), (f, -f, 6, -6, 21, 21), (-1, -1, 1, 1, 1, 1), (2, 3))); sid += 1
         out.append(Subprocess(sid, "%s g > t t~ %s g" % (q, q), (f, 21, 6, -6, f, 21), (-1, -1, 1, 1, 1, 1), (2, 3))); sid += 1
@@ -267,7 +267,7 @@ def make_config(cfg, n=None):
         # cfg 4 (sqrt(s) = 1500, RAMBO), theta as cfg 3.
         n = 262144 if n is None else n
         rng = np.random.default_rng(7)
-        classes = tuple(sp for sp in SUBPROCESSES if sp.npar == 6)
+        classes = tuple(sp for sp in SUBPROCESSES if sp.npar == 6 and sp.sid <= 26)
         fr = {3: 0.50, 21: 0.12, 22: 0.16, 23: 0.05, 24: 0.06, 25: 0.08, 26: 0.03}
         counts = largest_remainder([fr[sp.sid] for sp in classes], n)
         labels = np.concatenate([np.full(int(c), i, dtype=np.int64) for i, c in enumerate(counts)])
