@@ -365,7 +365,7 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
   if (int rc = ensure_colour()) return rc;
   a.T = T; a.sid = sid; a.q = sp->qlegs; a.C120 = c.C120; a.dbg = c.dbg_out;
   if (!a.plan || !is_quark_channel(sid)) a.qfamily = 0;
-  // parity: |M_{-h}|^2 = |M_h|^2 when no propagator carries a width (R-20); the diagnostics dump every helicity
+  // parity: |M_{-h}|^2 = |M_h|^2 when no propagator carries a width (R-21); the diagnostics dump every helicity
   a.hsym = (c.hel_sym && !c.dbg_out && sid != TREX_SP_EEMUMU && T.mGt[0] == 0.0 && T.mGt[1] == 0.0) ? 1 : 0;
   const unsigned grid32 = (unsigned)((nmax + 31) / 32);
   const int mode = c.precision;

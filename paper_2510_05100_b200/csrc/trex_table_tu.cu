@@ -364,7 +364,7 @@ __global__ void __launch_bounds__(TabCfg<N>::TB, TabCfg<N>::MINB) k_table(const 
   for (int i = tid; i < I::M_SIZE; i += TB) meta[i] = gmeta[i];
   for (int i = tid; i < G::CN; i += TB) Cs[i] = RC(Cfold[i]);
   for (int i = gtid; i < G::NCI; i += GS) part[i] = 0.0;
-  // helicity symmetry (a.hsym, R-20) without a helicity loop to halve (N = 3): the walk tasks with lambda_t = -
+  // helicity symmetry (a.hsym, R-21) without a helicity loop to halve (N = 3): the walk tasks with lambda_t = -
   // stand for their parity partners; the X columns of lambda_t = + are neither written nor read
   constexpr bool HS_LT = G::NIT == 1 && G::NLT == 1 && !G::DMMA && !G::TF32;
   const bool hs_lt = HS_LT && a.hsym && !a.dbg;

@@ -1,4 +1,4 @@
-"""Parity symmetry of the helicity sum (trex_set_helicity_symmetry; R-20): with Gamma_t = 0 the kernels that honour
+"""Parity symmetry of the helicity sum (trex_set_helicity_symmetry; R-21): with Gamma_t = 0 the kernels that honour
 the switch evaluate one helicity configuration of every pair {h, -h}; results must match the oracle (which sums every
 configuration) with the switch on AND off, and with a width the switch must change nothing, bit for bit."""
 import numpy as np
