@@ -34,12 +34,19 @@ __constant__ QLineLegs c_qlegs[TREX_NSUBPROC];
 __constant__ double c_qinvnavg[TREX_NSUBPROC];
 
 // DBG: the instantiation trex_debug_helicity_me2 launches -- the same code with the per-helicity dump compiled in
-template <class R, class RC, bool DBG = false>
+// HS (helicity symmetry, R-21; Gamma_t = 0): only the light-line combination c = 0 is evaluated (and doubled):
+// four units, eight wavefunctions and five currents per event, so the block takes TWO groups of 32 events, four warps each
+// (dynamic shared memory: the arrays below once per group)
+constexpr int QQ_SMEM_GROUP = (20 + 80 + 80) * 32 * (int)sizeof(double);
+template <class R, class RC, bool DBG = false, bool HS = false>
 __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightArgs a) {
   static_assert(WARPS == 8, "one allowed helicity unit per warp");
-  __shared__ double pm[20][32];
-  __shared__ double wf[10][8][32];
-  __shared__ double cur[10][8][32];
+  constexpr int NG = HS ? 2 : 1, NWG = WARPS / NG, EPB = 32 * NG;       // groups, warps per group, events per block
+  extern __shared__ __align__(16) unsigned char qq_raw[];
+  const int grp = HS ? (int)(threadIdx.x >> 7) : 0;
+  double (*pm)[32] = reinterpret_cast<double (*)[32]>(qq_raw + (size_t)grp * QQ_SMEM_GROUP);
+  double (*wf)[8][32] = reinterpret_cast<double (*)[8][32]>(pm + 20);
+  double (*cur)[8][32] = wf + 10;
   // which class this block belongs to: given by the call (trex_reweight), or found in the device plan when one launch
   // serves every quark-channel class of a run (blocks are dealt to the classes in id order, 32 events each)
   int sid = a.sid;
@@ -48,18 +55,18 @@ __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightA
     sid = -1;
     for (int s = 0; s < TREX_NSUBPROC; ++s) {
       if (c_qinvnavg[s] == 0.0) continue;
-      const long nb = (a.plan->cnt[s] + 31) >> 5;
+      const long nb = (a.plan->cnt[s] + EPB - 1) / EPB;
       if (blk < nb) { sid = s; break; }
       blk -= nb;
     }
     if (sid < 0) return;
   }
   const EvIO io = resolve_io(a, sid);
-  if (blk * 32 >= io.n) return;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long e = blk * 32 + lane;
+  if (blk * EPB >= io.n) return;
+  const int lane = threadIdx.x & 31, warp = (int)(threadIdx.x >> 5) - grp * NWG;       // warp within its group
+  const long e = blk * EPB + grp * 32 + lane;
   const long ev = e < io.n ? e : io.n - 1;
-  for (int r = warp; r < 20; r += WARPS) pm[r][lane] = io.mom[(long)r * io.ld + ev];
+  for (int r = warp; r < 20; r += NWG) pm[r][lane] = io.mom[(long)r * io.ld + ev];
   __syncthreads();
   const QLineLegs L = c_qlegs[sid];
   const bool row_in = L.lrow < 2, col_in = L.lcol < 2, g_in = L.lg < 2;
@@ -83,8 +90,9 @@ __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightA
     for (int i = 0; i < 4; ++i) o.c[i] = cx<R>(R(src[2 * i][lane]), R(src[2 * i + 1][lane]));
     return o;
   };
-  // ---- phase A
-  for (int item = warp; item < 10; item += WARPS) {
+  // ---- phase A (HS: the items of c = 0 only: 0, 2, 4 .. 9)
+  for (int it = warp; it < (HS ? 8 : 10); it += NWG) {
+    const int item = HS ? (it < 2 ? 2 * it : it + 2) : it;
     double p[4];
     if (item < 4) {
       const int c = item & 1;                               // row spinor sits in the upper block for c = 1
@@ -121,8 +129,9 @@ __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightA
     pt.c[mu] = pm[8 + mu][lane];
   }
   Ptot = radd(Kq, Kg);
-  // ---- phase A2
-  for (int item = warp; item < 10; item += WARPS) {
+  // ---- phase A2 (HS: Jq[0], Jq3[0][-/+], Jq4[0][-/+] = items 0, 2, 3, 6, 7)
+  for (int it = warp; it < (HS ? 5 : 10); it += NWG) {
+    const int item = HS ? (it == 0 ? 0 : (it < 3 ? it + 1 : it + 3)) : it;
     vec4<R> J;
     if (item < 2) {
       // quark-pair current  Jq = (w gamma^mu x) / Kq^2        [ (i g_s) * (-i / Kq^2) at g_s = 1 ]
@@ -160,13 +169,13 @@ __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightA
   }
   __syncthreads();
   // ---- phase B: unit = (lambda_g, lambda_t, light-line combination)
-  const int lg = warp & 1, lt = (warp >> 1) & 1, c = (warp >> 2) & 1;
+  const int lg = warp & 1, lt = (warp >> 1) & 1, c = HS ? 0 : (warp >> 2) & 1;
   RC acc[2];
   {
     const vec4<R> eg = get_vec(wf[4 + lg]), Jq = get_vec(cur[c]), Jq3 = get_vec(cur[2 + c * 2 + lg]), Jq4 = get_vec(cur[6 + c * 2 + lg]);
     const spinor<R> ubar_t = get_spinor(wf[6 + lt]);
     const spinor<R> vtb[2] = {get_spinor(wf[8]), get_spinor(wf[9])};
-    qq_close<R, RC>(eg, Kg, Jq, Kq, Jq3, Jq4, Ptot, ubar_t, vtb, pt, a.T, acc, (DBG && a.dbg && e == 0) ? a.dbg + warp * 4 : nullptr);
+    qq_close<R, RC>(eg, Kg, Jq, Kq, Jq3, Jq4, Ptot, ubar_t, vtb, pt, a.T, acc, (DBG && !HS && a.dbg && e == 0) ? a.dbg + warp * 4 : nullptr);
   }
   // fixed-order reduction over the 8 units (the light row spinors of phase A are dead: their slots carry the partial sums)
   double (*red)[8][32] = reinterpret_cast<double (*)[8][32]>(&wf[0][0][0]);
@@ -175,8 +184,9 @@ __global__ void __launch_bounds__(WARPS * 32, TREX_QQ_MINB) k_qq(const ReweightA
   if (warp == 0 && e < io.n) {
     double s0 = 0.0, s1 = 0.0;
 #pragma unroll
-    for (int w = 0; w < WARPS; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
-    const double mo = s0 * (a.T.gs2nv[0] * c_qinvnavg[sid]), mn = s1 * (a.T.gs2nv[1] * c_qinvnavg[sid]);
+    for (int w = 0; w < NWG; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
+    const double hs = HS ? 2.0 : 1.0;
+    const double mo = s0 * (a.T.gs2nv[0] * c_qinvnavg[sid] * hs), mn = s1 * (a.T.gs2nv[1] * c_qinvnavg[sid] * hs);
     const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
     io.w_out[e] = io.w_in[e] * norm * mn;                      // evaluate + append_wgts
     if (io.me2_old) io.me2_old[e] = mo;
@@ -397,10 +407,22 @@ static int launch_reweight(int sid, ReweightArgs& a, long nmax, const ThetaPair&
   } else {
     // a family launch (trex_run) serves every quark-channel class: each class rounds its events up to whole blocks
     const unsigned gq = a.qfamily ? grid32 + (unsigned)TREX_NSUBPROC : grid32;
-    if (mode == 0 && a.dbg) k_qq<double, double, true><<<gq, WARPS * 32, 0, c.stream>>>(a);
-    else if (mode == 0) k_qq<double, double><<<gq, WARPS * 32, 0, c.stream>>>(a);
-    else if (mode == 1) k_qq<double, float><<<gq, WARPS * 32, 0, c.stream>>>(a);
-    else k_qq<float, float><<<gq, WARPS * 32, 0, c.stream>>>(a);
+    static bool qq_ready = false;
+    if (!qq_ready) {
+      TREX_CUDA_CHECK(cudaFuncSetAttribute(k_qq<double, double, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * QQ_SMEM_GROUP));
+      TREX_CUDA_CHECK(cudaFuncSetAttribute(k_qq<double, float, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * QQ_SMEM_GROUP));
+      TREX_CUDA_CHECK(cudaFuncSetAttribute(k_qq<float, float, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * QQ_SMEM_GROUP));
+      qq_ready = true;
+    }
+    if (a.hsym && !a.dbg) {                                // two groups of 32 events per block
+      const unsigned gh = (a.qfamily ? (grid32 + 1) / 2 + (unsigned)TREX_NSUBPROC : (grid32 + 1) / 2);
+      if (mode == 0) k_qq<double, double, false, true><<<gh, WARPS * 32, 2 * QQ_SMEM_GROUP, c.stream>>>(a);
+      else if (mode == 1) k_qq<double, float, false, true><<<gh, WARPS * 32, 2 * QQ_SMEM_GROUP, c.stream>>>(a);
+      else k_qq<float, float, false, true><<<gh, WARPS * 32, 2 * QQ_SMEM_GROUP, c.stream>>>(a);
+    } else if (mode == 0 && a.dbg) k_qq<double, double, true><<<gq, WARPS * 32, QQ_SMEM_GROUP, c.stream>>>(a);
+    else if (mode == 0) k_qq<double, double><<<gq, WARPS * 32, QQ_SMEM_GROUP, c.stream>>>(a);
+    else if (mode == 1) k_qq<double, float><<<gq, WARPS * 32, QQ_SMEM_GROUP, c.stream>>>(a);
+    else k_qq<float, float><<<gq, WARPS * 32, QQ_SMEM_GROUP, c.stream>>>(a);
   }
   c.launches += 1;
   TREX_CUDA_CHECK(cudaGetLastError());
