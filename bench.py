@@ -255,7 +255,7 @@ def main():
     def roofline_of(cfg, n, kernel_ms, fp64_peak, dmma_peak, hsym=True):
         """Executed FP64 flop of the |M|^2 kernel(s) of one step / their live CUDA-event duration, against the FP64 vector
         pipe peak measured in this run; tensor-pipe (DMMA) work is reported against its own peak, never summed in."""
-        # with the helicity symmetry in use (library default; cfg 3, 5, 6, 7 have Gamma_t = 0) the kernels execute fewer operations
+        # with the helicity symmetry in use (library default; cfg 2, 3, 5, 6, 7 have Gamma_t = 0) the kernels execute fewer operations
         fpe = (F["flops_hsym"].get(cfg) if hsym else None) or F["flops"].get(cfg)
         if not fpe or not kernel_ms:
             return None
@@ -279,7 +279,7 @@ def main():
         T.trex_set_precision(precision)
         T.trex_set_helicity_symmetry(hsym)
         res = {"workload": w.name, "events": w.n, "steps": steps, "warmup": warm,
-               "helicity_symmetry": bool(hsym and w.theta_old[6] == 0.0 and w.theta_new[6] == 0.0 and cfg in (3, 5, 6, 7))}
+               "helicity_symmetry": bool(hsym and w.theta_old[6] == 0.0 and w.theta_new[6] == 0.0 and cfg in (2, 3, 5, 6, 7))}
         run = lambda: T.trex_run(keys, mom, w.theta_old, w.theta_new, win, w_out=wout, want_me2=False)  # noqa: E731
         if kernel_in_region:
             # the kernel is timed inside the timed region itself (the chain is launched directly, not as a graph replay:
@@ -402,7 +402,7 @@ def main():
         for cfg, warm, steps in ((1, 3, 20), (2, 3, 20), (3, 3, 10), (5, 3, 10), (6, 3, 10), (7, 3, 10)):
             configs["cfg%d" % cfg] = measure(cfg, warm, steps, with_e2e=(cfg != 1))
         # the same samples with every helicity configuration evaluated (trex_set_helicity_symmetry(0)): the round-1 arithmetic
-        for cfg, warm, steps in ((3, 3, 10), (5, 3, 10), (7, 3, 10)):
+        for cfg, warm, steps in ((2, 3, 20), (3, 3, 10), (5, 3, 10), (7, 3, 10)):
             configs["cfg%d_all_helicities" % cfg] = measure(cfg, warm, steps, hsym=False)
         configs["cfg4_mixed"] = measure(4, 3, 10, precision=1)
         configs["cfg4_fp32"] = measure(4, 3, 10, precision=2)

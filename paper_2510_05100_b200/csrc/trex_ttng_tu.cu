@@ -34,9 +34,11 @@ namespace trex {
 // two-gluon current and field-strength bracket once (J_21 = -J_12), walks the two orderings one after the other and
 // closes the 2 x 2 colour sum. Same recursion and the same operation order per amplitude as TTNGS<R, 2, 1, .>
 // (SURVEY.md C-4); parameter points with equal top mass and width only (otherwise the generic kernel runs).
-template <class R, class RC>
-__global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(const ReweightArgs a) {
-  constexpr int NW = TREX_GGTT_NW;                            // warps per block: 8 (one unit each) or 4 (two units each)
+// HS (helicity symmetry, R-21; Gamma_t = 0): only the four units with lambda_t = - are evaluated (and doubled):
+// four warps per block, one unit each, and twice as many blocks per SM.
+template <class R, class RC, bool HS = false>
+__global__ void __launch_bounds__(32 * (HS ? 4 : TREX_GGTT_NW), HS ? 2 * TREX_GGTT_MINB : TREX_GGTT_MINB) k_gg_tt(const ReweightArgs a) {
+  constexpr int NW = HS ? 4 : TREX_GGTT_NW;                   // warps per block: 8 (one unit each) or 4 (two units each; HS: one each)
   __shared__ double wf[8][8][32];
   __shared__ double red[2][NW][32];
   extern __shared__ __align__(16) double u1t_raw[];              // [8][16][32]: line state after ONE gluon, see phase A2
@@ -70,6 +72,7 @@ __global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(con
   // event where the 8 units x 2 orderings would form 16; one per warp, parked in shared memory
   for (int item = warp; item < 8; item += NW) {
     const int ga = item >> 2, ha = (item >> 1) & 1, lt = item & 1;
+    if (HS && lt) continue;                                    // only lambda_t = - is walked
     vec4<R> ea;
     spinor<R> ubar;
     rvec4<double> Ka, pt;
@@ -105,7 +108,8 @@ __global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(con
   __syncthreads();
   RC acc[2] = {RC(0), RC(0)};
 #pragma unroll 1
- for (int unit = warp; unit < 8; unit += NW) {
+ for (int uu = warp; uu < (HS ? 4 : 8); uu += NW) {
+  const int unit = HS ? 2 * uu : uu;
   const int gh = unit >> 1, lt = unit & 1;
   const int wsel[2] = {gh & 1, 2 + ((gh >> 1) & 1)};           // wavefunction slots of eps(g1), eps(g2) for this unit
   spinor<R> ubar;
@@ -210,7 +214,8 @@ __global__ void __launch_bounds__(32 * TREX_GGTT_NW, TREX_GGTT_MINB) k_gg_tt(con
     double s0 = 0.0, s1 = 0.0;
 #pragma unroll
     for (int w = 0; w < NW; ++w) { s0 += red[0][w][lane]; s1 += red[1][w][lane]; }
-    const double mo = s0 * a.T.pref[0], mn = s1 * a.T.pref[1];
+    const double hs = HS ? 2.0 : 1.0;
+    const double mo = s0 * (a.T.pref[0] * hs), mn = s1 * (a.T.pref[1] * hs);
     const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
     io.w_out[e] = io.w_in[e] * norm * mn;                        // evaluate + append_wgts
     if (io.me2_old) io.me2_old[e] = mo;
@@ -224,8 +229,13 @@ int TREX_TU_NAME(trex_tu_launch_n, TREX_TU_N, TREX_TU_MODE)(const ReweightArgs& 
   if (npass == 1) {                                   // equal top mass and width at both parameter points
     constexpr int kU1Bytes = 8 * 16 * 32 * (int)sizeof(double);
     static bool configured = false;
-    if (!configured) { cudaFuncSetAttribute(k_gg_tt<TuR, TuRC>, cudaFuncAttributeMaxDynamicSharedMemorySize, kU1Bytes); configured = true; }
-    k_gg_tt<TuR, TuRC><<<grid, 32 * TREX_GGTT_NW, kU1Bytes, s>>>(a);
+    if (!configured) {
+      cudaFuncSetAttribute(k_gg_tt<TuR, TuRC>, cudaFuncAttributeMaxDynamicSharedMemorySize, kU1Bytes);
+      cudaFuncSetAttribute(k_gg_tt<TuR, TuRC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kU1Bytes);
+      configured = true;
+    }
+    if (a.hsym && !a.dbg) k_gg_tt<TuR, TuRC, true><<<grid, 32 * 4, kU1Bytes, s>>>(a);
+    else k_gg_tt<TuR, TuRC><<<grid, 32 * TREX_GGTT_NW, kU1Bytes, s>>>(a);
     return (int)cudaGetLastError();
   }
 #endif
