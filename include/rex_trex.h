@@ -225,8 +225,8 @@ int trex_set_poly_multi(int on);         /* 1 (default): trex_run_multi may use 
 /* 1 (default): kernels may use the parity symmetry of the helicity sum. QCD and the chromomagnetic operator with a real
  * coefficient conserve parity: flipping every helicity conjugates the spinor products, so |M_{-h}|^2 = |M_h|^2 as long as
  * no propagator carries a width. When Gamma_t = 0 at BOTH parameter points a kernel that honours the switch evaluates one
- * helicity configuration of every pair {h, -h} and doubles the sum (g g > t t~, g g > t t~ g, g g > t t~ g g g and every quark channel do;
- * the other kernels evaluate every configuration regardless). With a width the symmetry is broken at the per-cent level
+ * helicity configuration of every pair {h, -h} and doubles the sum (every QCD channel does; g g > t t~ g g only
+ * when top mass and width also agree at the two points). With a width the symmetry is broken at the per-cent level
  * per helicity and every configuration is evaluated. 0: always evaluate every configuration. */
 int trex_set_helicity_symmetry(int on);
 const char* trex_last_error(void);

@@ -25,7 +25,7 @@ struct ReweightArgs {
   const DevPlan* plan;     // trex_run: device-resident bucket ranges; nullptr for trex_reweight
   int sid;
   int hsym;                // 1: sum one helicity configuration of every parity pair {h, -h} and double (valid for Gamma_t = 0 at
-                           // both parameter points: DESIGN.md R-21); honoured by k_gg_tt, k_table<3>, k_table<5>, k_qq and k_qq2
+                           // both parameter points: DESIGN.md R-21); honoured by k_gg_tt, k_table<3>, k_table4w<., ., 1>, k_table<5>, k_qq and k_qq2
   int qfamily;             // k_qq inside trex_run: one launch serves every quark-channel class of the plan
   const double* C120;
   ThetaPair T;

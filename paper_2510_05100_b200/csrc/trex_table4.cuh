@@ -288,8 +288,16 @@ template <class R> __device__ __forceinline__ void w4_leaf_term(cx<R>& a0, cx<R>
 
 // ---- top-line walk: task = (ordering, helicities of s1 s2 s3, lambda_t, pass); closes both helicities of s4 and both
 // antitop helicities from one line state U3 (see the "W form" section of trex_table.cuh)
-template <class R, class RC, int NPASS>
-__device__ __forceinline__ void w4_walk(const W4Ptr<R>& p, const typename W4<R, RC>::Small& sm, cx<RC>* __restrict__ xs, const ReweightArgs& a, int par, int tid) {
+// HS (helicity symmetry, R-21; one parameter-point pass, Gamma_t = 0): only the 192 tasks with lambda_t = - exist,
+// one per thread of warps 0-5, and they run BESIDE the level-4 entries (warps 6-11): the closed scalars of level 4 enter a
+// task only as the starting value of its sums, so the task keeps its sums (W4Held) and w4_walk_finish adds the scalars and
+// writes the X tile after the block barrier.
+template <class R> struct W4Held { cx<R> a0[4], a1[4]; int e4[4], colc[4], sg0, prank; };
+
+template <class R, class RC, int NPASS, bool HS = false>
+__device__ __forceinline__ void w4_walk(const W4Ptr<R>& p, const typename W4<R, RC>::Small& sm, cx<RC>* __restrict__ xs, const ReweightArgs& a, int par, int tid,
+                                        W4Held<R>* held = nullptr) {
+  static_assert(!HS || NPASS == 1, "the symmetric walk has one pass");
   using W = W4<R, RC>;
   using I = typename W::I;
   constexpr int TS = W::TS, XS = W::XS;
@@ -298,8 +306,8 @@ __device__ __forceinline__ void w4_walk(const W4Ptr<R>& p, const typename W4<R, 
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) pt.c[mu] = sm.pm[8 + mu];
   const R kq0 = R(a.T.kq[0]), kq1 = R(a.T.kq[1]);
-  for (int task = tid; task < 384 * NPASS; task += W::TB) {
-    const int pass = task / 384, r = task - pass * 384;
+  for (int task = tid; task < (HS ? 192 : 384 * NPASS); task += W::TB) {
+    const int pass = HS ? 0 : task / 384, r = HS ? 2 * task : task - pass * 384;
     const int prank = r >> 4, lt = r & 1;
     const unsigned hp = (unsigned)(r >> 1) & 7u;             // helicities of s1, s2, s3 (bit i: s_{i+1})
     // table references of this ordering (TabIdx::M_REC): no index arithmetic on the critical path of the loads
@@ -349,8 +357,11 @@ __device__ __forceinline__ void w4_walk(const W4Ptr<R>& p, const typename W4<R, 
       const unsigned h4 = (unsigned)c >> 1, hp4 = hp | (h4 << 3);
       const int ltb = c & 1;
       const int e4 = b4 + (int)(r4 ? I::bitrev(hp4, 4) : hp4);
-      a0[c] = tab_get<R>(p.tab, ((lt * 2 + ltb) * 2 + 0) * TS + e4, sg0);
-      a1[c] = tab_get<R>(p.tab, ((lt * 2 + ltb) * 2 + 1) * TS + e4, sg0);
+      if constexpr (HS) { a0[c] = cx<R>(R(0), R(0)); a1[c] = cx<R>(R(0), R(0)); held->e4[c] = e4; }
+      else {
+        a0[c] = tab_get<R>(p.tab, ((lt * 2 + ltb) * 2 + 0) * TS + e4, sg0);
+        a1[c] = tab_get<R>(p.tab, ((lt * 2 + ltb) * 2 + 1) * TS + e4, sg0);
+      }
       rec1[c] = (b1 + (int)(r1 ? I::bitrev(hp4 >> 1, 3) : hp4 >> 1)) * 2 + ltb;
       rec2[c] = (b2 + (int)(r2 ? I::bitrev(hp4 >> 2, 2) : hp4 >> 2) + poffw) * 2 + ltb;
       rec3[c] = (b3 + (int)h4 + poffw) * 2 + ltb;
@@ -374,6 +385,11 @@ __device__ __forceinline__ void w4_walk(const W4Ptr<R>& p, const typename W4<R, 
     close_with(U1, sg1, rec1);
     close_with(U2, sg2, rec2);
     close_with(U3, sg3, rec3);
+    if constexpr (HS) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) { held->a0[c] = a0[c]; held->a1[c] = a1[c]; held->colc[c] = colc[c]; }
+      held->sg0 = sg0; held->prank = prank;
+    } else
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
       if constexpr (NPASS == 1) {
@@ -386,6 +402,23 @@ __device__ __forceinline__ void w4_walk(const W4Ptr<R>& p, const typename W4<R, 
         xs[prank * XS + colc[c] + pass] = cx<RC>(RC(x.re), RC(x.im));
       }
     }
+  }
+}
+
+// second half of a symmetric walk task (after the level-4 entries are complete): lambda_t = -, combos c = 2 h4 + ltb
+template <class R, class RC>
+__device__ __forceinline__ void w4_walk_finish(const W4Ptr<R>& p, cx<RC>* __restrict__ xs, const ReweightArgs& a, const W4Held<R>& h) {
+  using W = W4<R, RC>;
+  const R kq0 = R(a.T.kq[0]), kq1 = R(a.T.kq[1]);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const int ltb = c & 1;
+    const cx<R> a0 = h.a0[c] + tab_get<R>(p.tab, (ltb * 2 + 0) * W::TS + h.e4[c], h.sg0);
+    const cx<R> a1 = h.a1[c] + tab_get<R>(p.tab, (ltb * 2 + 1) * W::TS + h.e4[c], h.sg0);
+    cx<R> x = a0; cfma(x, a1, kq0);
+    cx<R> y = a0; cfma(y, a1, kq1);
+    xs[h.prank * W::XS + h.colc[c]] = cx<RC>(RC(x.re), RC(x.im));
+    xs[h.prank * W::XS + h.colc[c] + 1] = cx<RC>(RC(y.re), RC(y.im));
   }
 }
 
@@ -425,8 +458,58 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
 #else
 #define W4_TICK(k) do { } while (0)
 #endif
+  // helicity symmetry (one pass, Gamma_t = 0): 192 walk tasks beside the level-4 entries; colour sum over the columns of
+  // lambda_t = - only; the sum is doubled in the epilogue
+  const bool hs = NPASS == 1 && a.hsym && !a.dbg;
+  const double hscale = hs ? 2.0 : 1.0;
+  const auto epilogue = [&](long ev) {                    // by one warp: fixed-order reduction of the partial sums (slot parity = theta)
+    double v = 0.0;
+    for (int i = lane; i < G::NCI; i += 32) { v += part[i]; part[i] = 0.0; }
+#pragma unroll
+    for (int o = 16; o >= 2; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    const double s1 = __shfl_sync(0xFFFFFFFFu, v, 1);
+    if (lane == 0) {
+      const double mo = v * (a.T.pref[0] * hscale), mn = s1 * (a.T.pref[1] * hscale);
+      const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
+      io.w_out[ev] = io.w_in[ev] * norm * mn;                      // evaluate + append_wgts
+      if (io.me2_old) io.me2_old[ev] = mo;
+      if (io.me2_new) io.me2_new[ev] = mn;
+    }
+  };
   for (long e = e_first; e < io.n; e += e_step, par ^= 1) {
     const bool more = e + e_step < io.n;
+    if constexpr (NPASS == 1) {
+      if (hs) {
+        // ---- phases B + C merged: walk tasks (warps 0-5) | level-4 entries (warps 6-11), then the epilogue of the previous
+        // event (warp 8)
+        W4Held<R> held;
+        if (wrp < 6) w4_walk<R, RC, 1, true>(p, small[par], xs, a, par, tid, &held);
+        else {
+          w4_top<R, RC>(p, small[par], W::E4 + tid - 192, par);
+          if (wrp == 8 && e != e_first) epilogue(e - e_step);
+        }
+        __syncthreads();
+        W4_TICK(0);
+        // the tasks add the level-4 scalars and write X (warps 0-5) | prep of the next event (warps 6, 7). (Measured: prep
+        // behind the level-4 entries on the same warps, or two level-4 entries per thread on fewer warps, make the merged
+        // phase longer than the walk tasks.)
+        if (wrp < 6) w4_walk_finish<R, RC>(p, xs, a, held);
+        else if (wrp < 8 && more) w4_prep<R, RC, NPASS>(p, small[par ^ 1], io, a, e + e_step, par ^ 1, wrp - 6, lane);
+        __syncthreads();
+        W4_TICK(1);
+        if constexpr (G::DMMA || G::TF32) {
+          if (wrp < W::NCW) colour_phase<R, RC, 4>(xs, Cs, part, tid, tid, W::NCW, true);
+          else if (more) w4_build3<R, RC, NPASS>(p, small[par ^ 1], a, par ^ 1, tid - 32 * W::NCW, W::TB - 32 * W::NCW);
+        } else {
+          colour_phase<R, RC, 4>(xs, Cs, part, tid, tid, 0, true);
+          if (more) w4_build3<R, RC, NPASS>(p, small[par ^ 1], a, par ^ 1, tid, W::TB);
+        }
+        __syncthreads();
+        W4_TICK(2);
+        if (!more && wrp == 8) epilogue(e);
+        continue;
+      }
+    }
     // ---- phase B: level-4 entries of this event | prep of the next one
     if (wrp < 6) w4_top<R, RC>(p, small[par], W::E4 + tid, par);
     else if (wrp < 8 && more) w4_prep<R, RC, NPASS>(p, small[par ^ 1], io, a, e + e_step, par ^ 1, wrp - 6, lane);
@@ -457,20 +540,7 @@ __global__ void __launch_bounds__(384, 1) k_table4w(const ReweightArgs a, const 
     W4_TICK(2);
     // ---- fixed-order reduction of the partial sums (slot parity = theta) + epilogue by warp 8, which has nothing to do
     // in phase B and clears what it has read; the other warps already work on the next event
-    if (wrp == 8) {
-      double v = 0.0;
-      for (int i = lane; i < G::NCI; i += 32) { v += part[i]; part[i] = 0.0; }
-#pragma unroll
-      for (int o = 16; o >= 2; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
-      const double s1 = __shfl_sync(0xFFFFFFFFu, v, 1);
-      if (lane == 0) {
-        const double mo = v * a.T.pref[0], mn = s1 * a.T.pref[1];
-        const double norm = (mo == 0.0) ? 0.0 : 1.0 / mo;          // procReweightor::initialise
-        io.w_out[e] = io.w_in[e] * norm * mn;                        // evaluate + append_wgts
-        if (io.me2_old) io.me2_old[e] = mo;
-        if (io.me2_new) io.me2_new[e] = mn;
-      }
-    }
+    if (wrp == 8) epilogue(e);
     W4_TICK(3);
   }
 #ifdef TREX_PHASE_CLOCKS

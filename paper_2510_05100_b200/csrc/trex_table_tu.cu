@@ -248,7 +248,9 @@ __device__ __forceinline__ void colour_phase(const cx<RC>* __restrict__ xs, cons
     // independent accumulator chains
     const int cstep = ncw > 0 ? ncw : GS / 32;
     if (wrp >= cstep) return;
-    for (int cb = wrp; cb < NCB; cb += cstep) {
+    // half_lt: the column blocks of lambda_t = + (odd ones) are not in use (helicity symmetry)
+    for (int kb = wrp; kb < (half_lt ? NCB / 2 : NCB); kb += cstep) {
+      const int cb = half_lt ? 2 * kb : kb;
       for (int J0 = 0; J0 < NB; J0 += 4) {
         double d[4][2];
 #pragma unroll
