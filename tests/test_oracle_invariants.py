@@ -140,3 +140,35 @@ def test_flavour_of_the_light_line_does_not_change_the_matrix_element():
         assert np.array_equal(O.me2(sp.sid, mom, th), want[kind]), sp.name
         seen += 1
     assert seen == 11
+
+
+# ---------------------------------------------------------------- parity of the helicity sum (R-21)
+@pytest.mark.parametrize("sid,cfg,engine", [(1, 2, 1), (2, 3, 1), (3, 4, 1), (5, 3, 2), (7, 3, 2), (8, 3, 2)])
+def test_flipping_every_helicity_is_a_symmetry_only_without_a_width(sid, cfg, engine):
+    """QCD and the chromomagnetic operator with a real coefficient conserve parity: flipping every helicity conjugates the
+    spinor products, so the three coefficients (A, B, D) of |M_h|^2 equal those of |M_{-h}|^2 -- as long as no propagator
+    carries a width (the width keeps its sign under the conjugation). The CUDA kernels use this when Gamma_t = 0; the oracle
+    never does, and this test pins both halves of the statement on single helicity configurations."""
+    w = make_config(cfg, n=8)
+    mom = np.ascontiguousarray(w.momenta[:, :, :2])
+    npar = mom.shape[0]
+    full = (1 << npar) - 1
+    th = default_theta()
+    th[TH_CTG] = 0.9
+    scale = O.abd(sid, mom, th, engine=engine)              # helicity-summed, for an absolute yardstick
+    checked = broken = 0
+    for h in list(range(0, full, 3))[:8]:
+        a = O.abd(sid, mom, th, engine=engine, hel_only=h)
+        b = O.abd(sid, mom, th, engine=engine, hel_only=full ^ h)
+        assert np.all(np.abs(a - b) <= 1e-12 * np.abs(scale)), (sid, bin(h), a, b)
+        if np.any(a != 0):
+            checked += 1
+        th_w = th.copy()
+        th_w[TH_GAMMAT] = 1.5
+        aw = O.abd(sid, mom, th_w, engine=engine, hel_only=h)
+        bw = O.abd(sid, mom, th_w, engine=engine, hel_only=full ^ h)
+        if np.any(np.abs(aw - bw) > 1e-6 * np.abs(scale)):
+            broken += 1
+    # the symmetry was tested on non-zero amplitudes, and a width breaks it (not visibly in the 2 -> 2 process, where the
+    # top propagators are far off shell in the t / u channels)
+    assert checked >= 2 and (broken >= 1 or npar == 4)
