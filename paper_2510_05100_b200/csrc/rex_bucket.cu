@@ -315,6 +315,16 @@ __global__ void __launch_bounds__(1024) k_bucket_small(const unsigned long long*
     res->keys[rank] = sk[s];
   }
   if (tid == 0) { res->nb = nb; res->err = bad ? 1 : 0; if (!bad && has_npos) res->keys[nd] = EMPTY; }
+  // trex_run on a sample of ONE known class: nothing has to move (no permutation is read when plan->single is set)
+  if (npar > 0 && !bad && nd == 1 && !has_npos && !force_gather) {              // uniform over the block
+    const unsigned long long the_key = sk[slots[0]];
+    const bool mine = tid < TREX_NSUBPROC && (int)sub[2 * tid + 1] == npar && sub[2 * tid] == the_key;
+    if (__syncthreads_or(mine ? 1 : 0)) {
+      if (tid < TREX_NSUBPROC) { plan->off[tid] = 0; plan->cnt[tid] = mine ? n : 0; }
+      if (tid == 0) { plan->single = 1; plan->nb = 1; res->offsets[0] = 0; res->offsets[1] = n; }
+      return;
+    }
+  }
   for (int i = lane; i <= NBMAX; i += 32) cnt[warp][i] = 0;
   __syncthreads();
   auto lookup = [&](unsigned long long key) -> int {
