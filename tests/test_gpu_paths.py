@@ -324,3 +324,47 @@ def test_host_entry_point_pipelines_chunks_without_changing_a_bit(T):
     ho = torch.empty(w4.n, dtype=torch.float64).pin_memory()
     assert T.trex_run_host(hk, hm, w4.theta_old, w4.theta_new, hw, ho) == 1
     assert np.array_equal(ho.numpy(), r4[0].cpu().numpy())
+
+
+def test_four_leg_sample_with_both_classes(T):
+    """A four-leg sample has two candidate classes (e- e+ > mu- mu+ and g g > t t~). A sample that really holds both (and a
+    sample of each alone) must give what per-class trex_reweight calls give, and those agree with the oracle."""
+    import torch
+    a, b = make_config(1, n=3000), make_config(2, n=5000)
+    rng = np.random.default_rng(8)
+    th_old, th_new = b.theta_old.copy(), b.theta_new.copy()
+    th_new[2] = a.theta_new[2]                                   # sin^2 theta_W moves as in cfg 1, c_tG as in cfg 2
+    keys = np.concatenate([a.keys, b.keys])
+    mom = np.concatenate([a.momenta, b.momenta], axis=2)
+    w_in = np.concatenate([a.w_in, b.w_in])
+    order = rng.permutation(len(keys))
+    keys, mom, w_in = keys[order], np.ascontiguousarray(mom[:, :, order]), w_in[order]
+    for sel_name, sel in (("both", np.arange(len(keys))), ("ee", np.where(keys == a.keys[0])[0]), ("gg", np.where(keys == b.keys[0])[0])):
+        k, m, w = keys[sel], np.ascontiguousarray(mom[:, :, sel]), w_in[sel]
+        l0 = T.trex_launch_count()
+        out = T.trex_run(dev(k), dev(m), th_old, th_new, dev(w))
+        torch.cuda.synchronize()
+        nl = T.trex_launch_count() - l0
+        got = [x.cpu().numpy() for x in out[:3]]
+        assert out[3] == (2 if sel_name == "both" else 1), sel_name
+        for sid, key in ((0, a.keys[0]), (1, b.keys[0])):
+            idx = np.where(k == key)[0]
+            if len(idx) == 0:
+                continue
+            r = T.trex_reweight(sid, dev(np.ascontiguousarray(m[:, :, idx])), th_old, th_new, dev(w[idx]))
+            for g, x in zip(got, r):
+                assert np.array_equal(g[idx], x.cpu().numpy()), (sel_name, sid)
+            j = idx[:5]
+            want = O.reweight(sid, np.ascontiguousarray(m[:, :, j]), th_old, th_new, w[j])
+            for g, x in zip(got, want):
+                assert rel(g[j], x).max() < RTOL64, (sel_name, sid)
+        assert nl <= 6, nl                                        # small sample: bucketing, gather, two candidate launches, scatter
+    # different top widths at the two points: the two-pass g g kernel runs
+    th2 = th_new.copy(); th2[6] = 1.4
+    out = T.trex_run(dev(keys), dev(mom), th_old, th2, dev(w_in))
+    idx = np.where(keys == a.keys[0])[0][:4]
+    want = O.reweight(0, np.ascontiguousarray(mom[:, :, idx]), th_old, th2, w_in[idx])
+    assert rel(out[0].cpu().numpy()[idx], want[0]).max() < RTOL64
+    idx = np.where(keys == b.keys[0])[0][:4]
+    want = O.reweight(1, np.ascontiguousarray(mom[:, :, idx]), th_old, th2, w_in[idx])
+    assert rel(out[0].cpu().numpy()[idx], want[0]).max() < RTOL64
